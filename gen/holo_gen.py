@@ -144,7 +144,7 @@ def stream_torch(cfg: Config, seed: int, device, n_frames=None, chunk=32):
     f = torch.from_numpy(scene.f).to(device=device, dtype=torch.float64)
     psi = torch.from_numpy(scene.psi).to(device=device, dtype=torch.float64)
     qc = torch.from_numpy(np.conj(chirp_np(n, n, cfg.lam, cfg.pitch, cfg.z))).to(device=device, dtype=torch.complex64)
-    out = torch.empty((n_frames, n, n), dtype=torch.uint16, device=device)
+    out = torch.empty((n_frames, n, n), dtype=torch.int16, device=device)   # values <= 4095
     for t0 in range(0, n_frames, chunk):
         c = min(chunk, n_frames - t0)
         t = torch.arange(t0, t0 + c, device=device, dtype=torch.float64)
@@ -156,5 +156,5 @@ def stream_torch(cfg: Config, seed: int, device, n_frames=None, chunk=32):
         if cfg.self_beating:
             Ibar = Ibar + 40.0 * Es.abs() ** 2
         I = torch.poisson(Ibar, generator=g).clamp_(0, 4095)
-        out[t0:t0 + c] = I.to(torch.int32).to(torch.uint16)
-    return out
+        out[t0:t0 + c] = I.to(torch.int16)
+    return out.view(torch.uint16)

@@ -1,0 +1,144 @@
+/*
+ * holo.h -- C ABI of libholo_b200: the data-parallel hot path of arXiv 2004.00923
+ * ("Real-time digital holography of the retina by principal component analysis"),
+ * hand-written CUDA for sm_100a (NVIDIA B200).  No cuFFT/cuBLAS/cuSOLVER, no CPU fallback.
+ *
+ * Path (PAPER.md = /root/reference/PAPER.md; R<n> = reading n in DESIGN.md):
+ *   A0  Ibar(x,y)  = (1/T) sum_t I_t(x,y)                         BASELINE.json north_star ("I_t - mean_t I"), R2
+ *   A1  g_t        = (I_t - Ibar) * exp(+i pi (x^2+y^2)/(lambda z))   PAPER.md:33-37 Eq. 1 (expanded), R3,R4,R6
+ *   A2  H_t        = FFT2D[g_t], forward, unnormalised, no fftshift   PAPER.md:33 ("one spatial Fourier transform"), R5
+ *   A3  C          = H^{t*} H,  C_ts = sum_p conj(H_t(p)) H_s(p)      PAPER.md:57-59 Eq. 4, R9
+ *   A4  C          = V Lambda V^{t*}                                  PAPER.md:61-65 Eq. 5, R1 (DESCENDING order)
+ *   A5  Hc         = H V I_f,  P_k(p) = sum_t H_t(p) V_{t,k}          PAPER.md:67-71 Eq. 6
+ *   A6  M(p)       = sum_{k=k_lo}^{k_hi} |P_k(p)|^2                   PAPER.md:71-74 Eq. 7
+ *   F1  Fourier demodulation: same as A5/A6 with V := W of Eq. 8      PAPER.md:78-86 Eq. 8-9
+ *
+ * Conventions common to every call
+ *   - All data pointers are DEVICE pointers unless a name ends in _host.  The caller owns every
+ *     buffer it passes in; the handle owns its workspace (chirp/twiddle tables, per-pixel frame sum,
+ *     FFT scratch, hologram stack H, covariance partials, C, evals, V).
+ *   - Layouts: frames uint16 [T][ny][nx] (frame-planar, x fastest), 16-byte aligned;
+ *     H complex64 [T][ny][nx] interleaved (re,im), indexed by output bin (ky row, kx column);
+ *     C, V complex64 [T][T] row-major; column k-1 of V is eigenvector k (V[t*T + (k-1)]);
+ *     evals float [T], DESCENDING, k = 1 is the largest (R1: the paper sorts ascending and keeps
+ *     n1..n2; (n1,n2) <-> (k_lo,k_hi) = (T+1-n2, T+1-n1));  image float [ny][nx] in FFT-bin order.
+ *   - `stream` is a cudaStream_t cast to void* (NULL = legacy default stream).  Every call only
+ *     ENQUEUES work on that stream: no allocation, no host synchronisation, no host<->device copy
+ *     (except the *_host entry point, which says so).  Calls are CUDA-graph capturable.
+ *   - Return value: HOLO_OK or a negative error code; nothing is launched on HOLO_ERR_ARG.
+ *     holo_last_error() gives a thread-local message.  Asynchronous CUDA faults surface at the
+ *     next call or at destroy.  Jacobi non-convergence is recorded in a device status word
+ *     readable with holo_status(); results are never silently NaN.
+ *   - Arguments: nx, ny powers of two in [16, 4096]; 2 <= T <= 64; lambda, pitch, z finite > 0;
+ *     1 <= k_lo <= k_hi <= T (1-based, inclusive, descending eigenvalue order).
+ *   - One in-flight call per handle per stream order: calls on one handle must be issued on the
+ *     same stream or otherwise ordered by the caller.
+ */
+#ifndef HOLO_H
+#define HOLO_H
+#include <stdint.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct holo_ctx holo_ctx;   /* opaque */
+typedef void* holo_stream;          /* cudaStream_t */
+
+enum {
+    HOLO_OK = 0,
+    HOLO_ERR_ARG = -1,
+    HOLO_ERR_ALLOC = -2,
+    HOLO_ERR_CUDA = -3,
+    HOLO_ERR_STATE = -4,
+    HOLO_ERR_NOCONV = -5
+};
+
+/* which-values for holo_workspace() */
+enum {
+    HOLO_WS_SUM = 0,     /* uint32 [ny][nx]  sum_t I_t of the last fresnel/process call            */
+    HOLO_WS_H = 1,       /* float2 [T][ny][nx] hologram stack of the last holo_process call        */
+    HOLO_WS_C = 2,       /* float2 [T][T]                                                           */
+    HOLO_WS_EVALS = 3,   /* float  [T]                                                              */
+    HOLO_WS_V = 4,       /* float2 [T][T]                                                           */
+    HOLO_WS_STATUS = 5,  /* int32  [4]: {noconv flag, sweeps used, rotations in last sweep, 0}      */
+    HOLO_WS_QX = 6,      /* float2 [nx] chirp table exp(+i pi x_i^2/(lambda z))                     */
+    HOLO_WS_QY = 7       /* float2 [ny]                                                             */
+};
+
+/* Create a handle for stacks of T frames of ny x nx pixels (n_t=32, 1024x1024) and
+ * the Fresnel parameters of Eq. 1 (lambda = 785 nm, pixel pitch, distance z).
+ * Allocates all device workspace (about 8*T*nx*ny + 16*nx*ny*min(T,8) bytes) on the current device
+ * and builds the chirp / twiddle tables in double precision on the host.  Returns NULL on failure
+ * (reason via holo_last_error()).  This is the only call besides holo_destroy that synchronises. */
+holo_ctx* holo_create(int nx, int ny, int T, double lambda_m, double pitch_m, double z_m,
+                      int k_lo, int k_hi);
+
+/* NULL-safe.  Synchronises the device, frees the workspace. */
+void holo_destroy(holo_ctx* ctx);
+
+/* The whole path A0..A6 for one stack: frames_dev (uint16 [T][ny][nx]) -> image_dev (float [ny][nx]). */
+int holo_process(holo_ctx* ctx, const uint16_t* frames_dev, float* image_dev, holo_stream stream);
+
+/* Same path, HOST buffers (pinned or pageable): copies frames in, runs holo_process, copies the
+ * image out, and synchronises `stream` before returning.  Uses a frame/image staging buffer owned by
+ * the handle (allocated at first use).  This is the end-to-end call bench.py's `e2e` times. */
+int holo_process_host(holo_ctx* ctx, const uint16_t* frames_host, float* image_host, holo_stream stream);
+
+/* A0+A1+A2: frames_dev -> H_dev (float2 [T][ny][nx]).  (Eq. 1) */
+int holo_fresnel(holo_ctx* ctx, const uint16_t* frames_dev, void* H_dev, holo_stream stream);
+
+/* A3: H_dev -> C_dev (float2 [T][T]), full Hermitian matrix written, deterministic (fixed partial
+ * count and reduction order; bit-identical across runs).  (Eq. 4) */
+int holo_covariance(holo_ctx* ctx, const void* H_dev, void* C_dev, holo_stream stream);
+
+/* A4: any Hermitian C_dev (only its lower triangle t >= s and real diagonal are read) ->
+ * evals_dev (float [T], descending), V_dev (float2 [T][T], unitary, column k-1 = eigenvector k,
+ * phase fixed so that each column's largest-magnitude entry is real positive).  Single-CTA
+ * parallel-order complex Jacobi in FP32 with an FP64 Rayleigh-quotient refinement of the
+ * eigenvalues.  (Eq. 5) */
+int holo_eig(holo_ctx* ctx, const void* C_dev, float* evals_dev, void* V_dev, holo_stream stream);
+
+/* A5+A6 fused: image(p) = sum_{k=k_lo}^{k_hi} |sum_t H_t(p) V_{t,k}|^2 with the handle's current
+ * (k_lo,k_hi); P is never stored.  V_dev may be ANY T x T matrix (unitary or not) when
+ * `assume_unitary` was not enabled (default): the direct form is used.  (Eq. 6-7) */
+int holo_project(holo_ctx* ctx, const void* H_dev, const void* V_dev, float* image_dev, holo_stream stream);
+
+/* F1 (Eq. 8-9): Fourier demodulation of the stack: image(p) = sum_{n=n1}^{n2} |sum_m H_m(p) w_mn|^2,
+ * w_mn = exp(-2 i pi (m-1)(n-1)/T)/sqrt(T), n1..n2 1-based inclusive (paper: 8..24 of 32). */
+int holo_fourier_demod(holo_ctx* ctx, const void* H_dev, int n1, int n2, float* image_dev, holo_stream stream);
+
+/* Change the component window (1-based inclusive, descending order).  Takes effect at the next call. */
+int holo_set_range(holo_ctx* ctx, int k_lo, int k_hi);
+
+/* Allow holo_process/holo_project to use the exact identity sum_{k in S}|P_k|^2 =
+ * sum_t |H_t|^2 - sum_{k not in S}|P_k|^2 (valid for unitary V; R12) when the complement of S is
+ * smaller than S.  holo_process always may (its V is unitary by construction); for holo_project
+ * this flag (default 0) states that the caller's V is unitary. */
+int holo_set_assume_unitary(holo_ctx* ctx, int on);
+
+/* Test hook: device pointer of a workspace array (see HOLO_WS_*), NULL if `which` is invalid. */
+const void* holo_workspace(holo_ctx* ctx, int which);
+
+/* Test hook: enqueue a device-to-device copy of the first `nbytes` bytes of workspace array `which`
+ * into dst_dev (caller-owned device memory). */
+int holo_workspace_copy(holo_ctx* ctx, int which, void* dst_dev, unsigned long long nbytes, holo_stream stream);
+
+/* Copies the 4-int status word of the last holo_eig/holo_process to the host (synchronises `stream`).
+ * Returns HOLO_ERR_NOCONV if the Jacobi sweep cap was hit, else HOLO_OK. */
+int holo_status(holo_ctx* ctx, int32_t status_host[4], holo_stream stream);
+
+/* Number of kernels one holo_process call launches with the current settings (for gpu_launches). */
+int holo_launches_per_process(holo_ctx* ctx);
+
+/* Experiment knobs (not needed for normal use; defaults are chosen at create).  Keys:
+ *   0 frames per FFT row/column group (L2 residency of the intermediate), 1 covariance CTAs,
+ *   2 allow the complement form in holo_process (default 1), 3 reserved, 4 Jacobi sweep cap. */
+int holo_tune(holo_ctx* ctx, int key, int value);
+
+const char* holo_last_error(void);   /* thread-local, static storage */
+int holo_version(void);              /* major*10000 + minor*100 + patch */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* HOLO_H */

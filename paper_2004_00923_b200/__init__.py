@@ -1,0 +1,10 @@
+"""paper_2004_00923_b200 -- B200-native (sm_100a) hot path of arXiv 2004.00923.
+
+Thin Python binding over the C ABI in include/holo.h (argument marshalling only; every step of the
+path runs in the CUDA kernels under csrc/).  PyTorch is used for device memory and streams.
+There is NO CPU fallback: importing `binding` without the built library, or creating a handle
+without a CUDA device, raises.
+"""
+from .binding import (Holo, load_library, library_path, HoloError,  # noqa: F401
+                      HOLO_WS_SUM, HOLO_WS_H, HOLO_WS_C, HOLO_WS_EVALS, HOLO_WS_V, HOLO_WS_STATUS,
+                      HOLO_WS_QX, HOLO_WS_QY, EXPORTED_SYMBOLS)

@@ -1,0 +1,352 @@
+// fresnel.cu -- A0 (temporal sum), A1 (mean-subtract + chirp prologue) and A2 (2-D FFT) kernels.
+//   H_t = FFT2D[(I_t - mean_t I) * exp(+i pi (x^2+y^2)/(lambda z))]      (Eq. 1; R2-R6)
+// Stockham autosort FFT, radix-16/32 butterflies in registers, one shared-memory exchange per extra
+// pass, row pass (x) then column pass (y); the row->column intermediate is kept L2-resident by
+// processing the stack in small frame groups.
+#include "holo_internal.cuh"
+#include <math.h>
+#include <vector>
+
+// ------------------------------------------------------------------------------------------------
+// register FFT, radix-2 decimation in frequency, fully unrolled; result is in bit-reversed order
+// ------------------------------------------------------------------------------------------------
+__host__ __device__ constexpr float cos32(int k) {   // cos(2 pi k / 32), 0 <= k <= 16
+    return k == 0 ? 1.0f : k == 1 ? 0.98078528040323043f : k == 2 ? 0.92387953251128674f
+         : k == 3 ? 0.83146961230254524f : k == 4 ? 0.70710678118654752f : k == 5 ? 0.55557023301960218f
+         : k == 6 ? 0.38268343236508978f : k == 7 ? 0.19509032201612825f : k == 8 ? 0.0f
+         : -cos32(16 - k);
+}
+__host__ __device__ constexpr float sin32(int k) {   // sin(2 pi k / 32), 0 <= k <= 16
+    return k <= 8 ? cos32(8 - k) : cos32(k - 8);
+}
+template <int R> __host__ __device__ constexpr int brev(int r) {
+    int o = 0;
+    for (int b = 1; b < R; b <<= 1) { o = (o << 1) | (r & 1); r >>= 1; }
+    return o;
+}
+
+// d * exp(-2 pi i idx/32), idx a compile-time constant after unrolling
+template <int IDX> __host__ __device__ __forceinline__ float2 mul_w32(float2 d) {
+    if (IDX == 0) return d;
+    if (IDX == 8) return make_float2(d.y, -d.x);
+    if (IDX == 4) return make_float2((d.x + d.y) * 0.70710678118654752f, (d.y - d.x) * 0.70710678118654752f);
+    if (IDX == 12) return make_float2((d.y - d.x) * 0.70710678118654752f, -(d.x + d.y) * 0.70710678118654752f);
+    constexpr float c = cos32(IDX), s = sin32(IDX);
+    return make_float2(fmaf(d.y, s, d.x * c), fmaf(-d.x, s, d.y * c));
+}
+
+template <int SPAN, int G, int K> struct BflyK {
+    static __host__ __device__ __forceinline__ void run(float2* v) {
+        float2 a = v[G + K], b = v[G + K + SPAN];
+        v[G + K] = make_float2(a.x + b.x, a.y + b.y);
+        v[G + K + SPAN] = mul_w32<K * (16 / SPAN)>(make_float2(a.x - b.x, a.y - b.y));
+        if constexpr (K + 1 < SPAN) BflyK<SPAN, G, K + 1>::run(v);
+    }
+};
+template <int R, int SPAN, int G> struct BflyG {
+    static __host__ __device__ __forceinline__ void run(float2* v) {
+        BflyK<SPAN, G, 0>::run(v);
+        if constexpr (G + 2 * SPAN < R) BflyG<R, SPAN, G + 2 * SPAN>::run(v);
+    }
+};
+template <int R, int SPAN> struct BflyS {
+    static __host__ __device__ __forceinline__ void run(float2* v) {
+        BflyG<R, SPAN, 0>::run(v);
+        if constexpr (SPAN > 1) BflyS<R, SPAN / 2>::run(v);
+    }
+};
+// in-place DFT of size R (power of two <= 32) on registers v[0..R); X[r] = v[brev<R>(r)] afterwards
+template <int R> __host__ __device__ __forceinline__ void fft_reg(float2* v) {
+    if constexpr (R > 1) BflyS<R, R / 2>::run(v);
+}
+
+__device__ __forceinline__ float2 cmul(float2 a, float2 b) {
+    return make_float2(fmaf(-a.y, b.y, a.x * b.x), fmaf(a.y, b.x, a.x * b.y));
+}
+
+// ------------------------------------------------------------------------------------------------
+// A0: per-pixel temporal sum  S(p) = sum_t I_t(p)   (uint32: exact, T*65535 < 2^32)
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_frame_sum(const uint16_t* __restrict__ frames, uint32_t* __restrict__ sum,
+                                                   long long npix, int T) {
+    long long v = (long long)blockIdx.x * blockDim.x + threadIdx.x;      // one uint4 = 8 pixels per thread
+    long long nvec = npix >> 3;
+    for (; v < nvec; v += (long long)gridDim.x * blockDim.x) {
+        uint32_t s[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+        const uint4* src = reinterpret_cast<const uint4*>(frames) + v;
+#pragma unroll 8
+        for (int t = 0; t < T; ++t) {
+            uint4 w = __ldg(src + (long long)t * nvec);
+            s[0] += w.x & 0xffffu; s[1] += w.x >> 16;
+            s[2] += w.y & 0xffffu; s[3] += w.y >> 16;
+            s[4] += w.z & 0xffffu; s[5] += w.z >> 16;
+            s[6] += w.w & 0xffffu; s[7] += w.w >> 16;
+        }
+        uint4* dst = reinterpret_cast<uint4*>(sum) + 2 * v;
+        dst[0] = make_uint4(s[0], s[1], s[2], s[3]);
+        dst[1] = make_uint4(s[4], s[5], s[6], s[7]);
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// 1-D FFT pass kernel over a batch of B sequences per CTA.
+//   COL = false: sequences are image rows (contiguous), PRO = fused uint16/mean/chirp prologue
+//   COL = true : sequences are image columns (stride ld), B adjacent columns per CTA
+// ------------------------------------------------------------------------------------------------
+struct FftArgs {
+    const uint16_t* frames;   // PRO: [nf][ny][nx] (already offset to the first frame of the group)
+    const uint32_t* sum;      // PRO
+    const float2* qx;         // PRO
+    const float2* qy;         // PRO
+    const float2* in;         // !PRO
+    float2* out;
+    const float2* tw1;
+    const float2* tw2;
+    long long in_fstride, out_fstride;   // elements between frames
+    int ld;                   // elements between consecutive rows (= nx)
+    int nseq;                 // sequences per frame (ROW: ny, COL: nx)
+    int tiles_per_frame;      // nseq / B
+    int ntiles;               // nf * tiles_per_frame
+    int T;
+    float invT;
+};
+
+template <int N, int E, int R1, int R2, int B, bool COL, bool PRO>
+__global__ void __launch_bounds__((N / E) * B) k_fft(const FftArgs a) {
+    constexpr int TPS = N / E;
+    constexpr int PADN = N + N / E;
+    constexpr bool MULTI = (R1 > 1);
+    extern __shared__ float2 sm[];
+    const int tid = threadIdx.x;
+    const int j = COL ? tid / B : tid % TPS;
+    const int c = COL ? tid % B : tid / TPS;
+    auto sidx = [&](int i) -> int {
+        int p = i + i / E;
+        return COL ? p * B + c : c * PADN + p;
+    };
+
+    for (int tile = blockIdx.x; tile < a.ntiles; tile += gridDim.x) {
+        const int fl = tile / a.tiles_per_frame;
+        const int s0 = (tile - fl * a.tiles_per_frame) * B + c;       // sequence index (row y or column x)
+        const long long ibase = (long long)fl * a.in_fstride + (COL ? (long long)s0 : (long long)s0 * a.ld);
+        const long long obase = (long long)fl * a.out_fstride + (COL ? (long long)s0 : (long long)s0 * a.ld);
+        const long long estride = COL ? a.ld : 1;
+        float2 v[E];
+        // ---------------- pass 0: radix E, Ns = 1, inputs straight from global
+        if constexpr (PRO) {
+            const float2 qyv = __ldg(a.qy + s0);
+            const uint16_t* fr = a.frames + ibase;
+            const uint32_t* sp = a.sum + (long long)s0 * a.ld;
+#pragma unroll
+            for (int r = 0; r < E; ++r) {
+                const int i = j + r * TPS;
+                const int I = (int)__ldg(fr + i);
+                const int S = (int)__ldg(sp + i);
+                const float d = (float)(a.T * I - S) * a.invT;         // exact integer, one rounding
+                const float2 q = cmul(__ldg(a.qx + i), qyv);
+                v[r] = make_float2(d * q.x, d * q.y);
+            }
+        } else {
+            const float2* ip = a.in + ibase;
+#pragma unroll
+            for (int r = 0; r < E; ++r) v[r] = __ldg(ip + (long long)(j + r * TPS) * estride);
+        }
+        fft_reg<E>(v);
+        float2* op = a.out + obase;
+        if constexpr (!MULTI) {
+#pragma unroll
+            for (int r = 0; r < E; ++r) op[(long long)r * estride] = v[brev<E>(r)];
+        } else {
+#pragma unroll
+            for (int r = 0; r < E; ++r) sm[sidx(j * E + r)] = v[brev<E>(r)];
+            __syncthreads();
+            // ---------------- pass 1: radix R1, Ns = E
+            constexpr int M1 = E / R1;
+#pragma unroll
+            for (int m = 0; m < M1; ++m) {
+                const int b = j + m * TPS;
+#pragma unroll
+                for (int r = 0; r < R1; ++r) v[m * R1 + r] = sm[sidx(b + r * (N / R1))];
+            }
+            if constexpr (R2 > 1) __syncthreads();
+#pragma unroll
+            for (int m = 0; m < M1; ++m) {
+                const int b = j + m * TPS;
+                const int k = b % E;
+#pragma unroll
+                for (int r = 1; r < R1; ++r) v[m * R1 + r] = cmul(v[m * R1 + r], __ldg(a.tw1 + r * E + k));
+                fft_reg<R1>(v + m * R1);
+                const int j0 = (b - k) * R1 + k;
+                if constexpr (R2 == 1) {
+#pragma unroll
+                    for (int r = 0; r < R1; ++r) op[(long long)(j0 + r * E) * estride] = v[m * R1 + brev<R1>(r)];
+                } else {
+#pragma unroll
+                    for (int r = 0; r < R1; ++r) sm[sidx(j0 + r * E)] = v[m * R1 + brev<R1>(r)];
+                }
+            }
+            if constexpr (R2 > 1) {
+                __syncthreads();
+                // ---------------- pass 2: radix R2, Ns = E*R1
+                constexpr int M2 = E / R2;
+                constexpr int NS2 = E * R1;
+#pragma unroll
+                for (int m = 0; m < M2; ++m) {
+                    const int b = j + m * TPS;
+#pragma unroll
+                    for (int r = 0; r < R2; ++r) v[m * R2 + r] = sm[sidx(b + r * (N / R2))];
+                }
+#pragma unroll
+                for (int m = 0; m < M2; ++m) {
+                    const int b = j + m * TPS;                         // b < N/R2 = NS2, so k = b
+#pragma unroll
+                    for (int r = 1; r < R2; ++r) v[m * R2 + r] = cmul(v[m * R2 + r], __ldg(a.tw2 + r * NS2 + b));
+                    fft_reg<R2>(v + m * R2);
+#pragma unroll
+                    for (int r = 0; r < R2; ++r) op[(long long)(b + r * NS2) * estride] = v[m * R2 + brev<R2>(r)];
+                }
+            }
+            __syncthreads();        // smem is reused by the next tile
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// host side: plans, dispatch, launch
+// ------------------------------------------------------------------------------------------------
+static bool plan_shape(int N, int* E, int* R1, int* R2) {
+    switch (N) {
+        case 16:   *E = 16; *R1 = 1;  *R2 = 1;  return true;
+        case 32:   *E = 32; *R1 = 1;  *R2 = 1;  return true;
+        case 64:   *E = 16; *R1 = 4;  *R2 = 1;  return true;
+        case 128:  *E = 16; *R1 = 8;  *R2 = 1;  return true;
+        case 256:  *E = 16; *R1 = 16; *R2 = 1;  return true;
+        case 512:  *E = 32; *R1 = 16; *R2 = 1;  return true;
+        case 1024: *E = 32; *R1 = 32; *R2 = 1;  return true;
+        case 2048: *E = 16; *R1 = 16; *R2 = 8;  return true;
+        case 4096: *E = 16; *R1 = 16; *R2 = 16; return true;
+    }
+    return false;
+}
+
+int holo_fft_plan_init(FftPlan* p, int N) {
+    p->N = N; p->tw1 = nullptr; p->tw2 = nullptr;
+    if (!plan_shape(N, &p->E, &p->R1, &p->R2)) { holo_set_error("unsupported FFT length %d", N); return HOLO_ERR_ARG; }
+    p->tps = N / p->E;
+    const double PI = 3.14159265358979323846264338327950288;
+    if (p->R1 > 1) {
+        int Ns = p->E, R = p->R1;
+        std::vector<float2> h((size_t)R * Ns);
+        for (int r = 0; r < R; ++r)
+            for (int k = 0; k < Ns; ++k) {
+                double ang = -2.0 * PI * (double)r * (double)k / ((double)Ns * R);
+                h[(size_t)r * Ns + k] = make_float2((float)cos(ang), (float)sin(ang));
+            }
+        HOLO_CUDA_OK(cudaMalloc(&p->tw1, h.size() * sizeof(float2)));
+        HOLO_CUDA_OK(cudaMemcpy(p->tw1, h.data(), h.size() * sizeof(float2), cudaMemcpyHostToDevice));
+    }
+    if (p->R2 > 1) {
+        int Ns = p->E * p->R1, R = p->R2;
+        std::vector<float2> h((size_t)R * Ns);
+        for (int r = 0; r < R; ++r)
+            for (int k = 0; k < Ns; ++k) {
+                double ang = -2.0 * PI * (double)r * (double)k / ((double)Ns * R);
+                h[(size_t)r * Ns + k] = make_float2((float)cos(ang), (float)sin(ang));
+            }
+        HOLO_CUDA_OK(cudaMalloc(&p->tw2, h.size() * sizeof(float2)));
+        HOLO_CUDA_OK(cudaMemcpy(p->tw2, h.data(), h.size() * sizeof(float2), cudaMemcpyHostToDevice));
+    }
+    return HOLO_OK;
+}
+
+void holo_fft_plan_free(FftPlan* p) {
+    if (p->tw1) cudaFree(p->tw1);
+    if (p->tw2) cudaFree(p->tw2);
+    p->tw1 = p->tw2 = nullptr;
+}
+
+template <int N, int E, int R1, int R2, int B, bool COL, bool PRO>
+static int launch_fft_t(const FftArgs& a, int num_sms, cudaStream_t st) {
+    constexpr int threads = (N / E) * B;
+    constexpr size_t smem = (R1 > 1) ? sizeof(float2) * (size_t)(N + N / E) * B : 0;
+    auto kern = k_fft<N, E, R1, R2, B, COL, PRO>;
+    static int blocks_per_sm = 0;      // per instantiation
+    if (blocks_per_sm == 0) {
+        if (smem > 48 * 1024) HOLO_CUDA_OK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        int occ = 0;
+        HOLO_CUDA_OK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, threads, smem));
+        if (occ < 1) { holo_set_error("fft kernel N=%d does not fit on an SM", N); return HOLO_ERR_CUDA; }
+        blocks_per_sm = occ;
+    }
+    int grid = a.ntiles < num_sms * blocks_per_sm ? a.ntiles : num_sms * blocks_per_sm;
+    kern<<<grid, threads, smem, st>>>(a);
+    HOLO_CUDA_OK(cudaGetLastError());
+    return HOLO_OK;
+}
+
+// B (sequences per CTA) per length: rows aim at 256 threads; columns at >= 64-byte segments
+template <bool COL, bool PRO>
+static int launch_fft(int N, const FftArgs& a, int num_sms, cudaStream_t st) {
+    switch (N) {
+        case 16:   return launch_fft_t<16, 16, 1, 1, 16, COL, PRO>(a, num_sms, st);
+        case 32:   return launch_fft_t<32, 32, 1, 1, 16, COL, PRO>(a, num_sms, st);
+        case 64:   return launch_fft_t<64, 16, 4, 1, 16, COL, PRO>(a, num_sms, st);
+        case 128:  return launch_fft_t<128, 16, 8, 1, 16, COL, PRO>(a, num_sms, st);
+        case 256:  return launch_fft_t<256, 16, 16, 1, 16, COL, PRO>(a, num_sms, st);
+        case 512:  return launch_fft_t<512, 32, 16, 1, 16, COL, PRO>(a, num_sms, st);
+        case 1024: return launch_fft_t<1024, 32, 32, 1, 8, COL, PRO>(a, num_sms, st);
+        case 2048: return launch_fft_t<2048, 16, 16, 8, 4, COL, PRO>(a, num_sms, st);
+        case 4096: return launch_fft_t<4096, 16, 16, 16, 4, COL, PRO>(a, num_sms, st);
+    }
+    holo_set_error("unsupported FFT length %d", N);
+    return HOLO_ERR_ARG;
+}
+static int fft_batch(int N) { return N <= 512 ? 16 : N == 1024 ? 8 : 4; }
+
+int holo_fresnel_launch_count(holo_ctx* c) {
+    int g = c->scratch_frames;
+    int groups = (c->T + g - 1) / g;
+    return 1 + 2 * groups;
+}
+
+int holo_launch_fresnel(holo_ctx* c, const uint16_t* frames, float2* H, cudaStream_t st) {
+    // A0
+    {
+        long long nvec = c->npix >> 3;
+        int threads = 256;
+        long long want = (nvec + threads - 1) / threads;
+        int grid = (int)(want < (long long)c->num_sms * 8 ? want : (long long)c->num_sms * 8);
+        HoloProf prof(c, HOLO_K_SUM, st);
+        k_frame_sum<<<grid, threads, 0, st>>>(frames, c->sum, c->npix, c->T);
+        HOLO_CUDA_OK(cudaGetLastError());
+    }
+    // A1 + A2, frame groups so that the row->column intermediate stays in L2
+    const int G = c->scratch_frames;
+    for (int f0 = 0; f0 < c->T; f0 += G) {
+        const int nf = (c->T - f0 < G) ? c->T - f0 : G;
+        FftArgs a{};
+        a.frames = frames + (long long)f0 * c->npix;
+        a.sum = c->sum; a.qx = c->qx; a.qy = c->qy;
+        a.in = nullptr; a.out = c->scratch;
+        a.tw1 = c->px.tw1; a.tw2 = c->px.tw2;
+        a.in_fstride = c->npix; a.out_fstride = c->npix;
+        a.ld = c->nx; a.nseq = c->ny;
+        a.tiles_per_frame = c->ny / fft_batch(c->nx);
+        a.ntiles = nf * a.tiles_per_frame;
+        a.T = c->T; a.invT = 1.0f / (float)c->T;
+        int rc;
+        { HoloProf prof(c, HOLO_K_FFT_ROWS, st); rc = launch_fft<false, true>(c->nx, a, c->num_sms, st); }
+        if (rc) return rc;
+        FftArgs b{};
+        b.in = c->scratch; b.out = H + (long long)f0 * c->npix;
+        b.tw1 = c->py.tw1; b.tw2 = c->py.tw2;
+        b.in_fstride = c->npix; b.out_fstride = c->npix;
+        b.ld = c->nx; b.nseq = c->nx;
+        b.tiles_per_frame = c->nx / fft_batch(c->ny);
+        b.ntiles = nf * b.tiles_per_frame;
+        b.T = c->T; b.invT = a.invT;
+        { HoloProf prof(c, HOLO_K_FFT_COLS, st); rc = launch_fft<true, false>(c->ny, b, c->num_sms, st); }
+        if (rc) return rc;
+    }
+    return HOLO_OK;
+}

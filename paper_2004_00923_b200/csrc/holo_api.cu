@@ -1,0 +1,293 @@
+// holo_api.cu -- the C ABI declared in include/holo.h: handle, workspace, argument checks, chaining.
+// Every compute step runs in the kernels of fresnel.cu / covariance.cu / eig.cu / project.cu.
+#include "holo_internal.cuh"
+#include <math.h>
+#include <stdarg.h>
+#include <string.h>
+#include <new>
+#include <vector>
+
+static thread_local char g_err[512] = "";
+
+void holo_set_error(const char* fmt, ...) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+}
+
+extern "C" const char* holo_last_error(void) { return g_err; }
+extern "C" int holo_version(void) { return 100; }   // 0.1.0
+
+static bool is_pow2(int n) { return n > 0 && (n & (n - 1)) == 0; }
+
+static int build_chirp(float2** dst, int n, double lambda_m, double pitch_m, double z_m) {
+    // q_x[i] = exp(+i pi x_i^2/(lambda z)), x_i = (i - n/2) pitch; evaluated in double with the phase
+    // reduced mod 2 (in units of pi) BEFORE the trigonometric call (the phase reaches 1e4 rad).
+    std::vector<float2> h(n);
+    const double PI = 3.14159265358979323846264338327950288;
+    const double a = pitch_m * pitch_m / (lambda_m * z_m);      // phase / pi per unit offset^2
+    for (int i = 0; i < n; ++i) {
+        const double o = (double)(i - n / 2);
+        double u = fmod(o * o * a, 2.0);
+        h[i] = make_float2((float)cos(PI * u), (float)sin(PI * u));
+    }
+    HOLO_CUDA_OK(cudaMalloc(dst, n * sizeof(float2)));
+    HOLO_CUDA_OK(cudaMemcpy(*dst, h.data(), n * sizeof(float2), cudaMemcpyHostToDevice));
+    return HOLO_OK;
+}
+
+static void free_ctx(holo_ctx* c) {
+    if (!c) return;
+    cudaFree(c->qx); cudaFree(c->qy); cudaFree(c->Wdft);
+    holo_fft_plan_free(&c->px); holo_fft_plan_free(&c->py);
+    cudaFree(c->sum); cudaFree(c->scratch); cudaFree(c->H); cudaFree(c->cov_partials);
+    cudaFree(c->C); cudaFree(c->evals); cudaFree(c->V); cudaFree(c->Vsel); cudaFree(c->status);
+    cudaFree(c->counters);
+    if (c->prof_ev) {
+        for (int i = 0; i < 2 * HOLO_PROF_CAP; ++i) cudaEventDestroy(c->prof_ev[i]);
+        delete[] c->prof_ev;
+        delete[] c->prof_cls;
+    }
+    if (c->frames_stage) cudaFree(c->frames_stage);
+    if (c->image_stage) cudaFree(c->image_stage);
+    delete c;
+}
+
+static int create_impl(holo_ctx* c) {
+    HOLO_CUDA_OK(cudaGetDevice(&c->device));
+    cudaDeviceProp prop;
+    HOLO_CUDA_OK(cudaGetDeviceProperties(&prop, c->device));
+    if (prop.major < 10) { holo_set_error("libholo_b200 needs an sm_100a device (found sm_%d%d)", prop.major, prop.minor); return HOLO_ERR_CUDA; }
+    c->num_sms = prop.multiProcessorCount;
+    const int T = c->T;
+    const long long np = c->npix;
+    int rc;
+    if ((rc = build_chirp(&c->qx, c->nx, c->lambda_m, c->pitch_m, c->z_m))) return rc;
+    if ((rc = build_chirp(&c->qy, c->ny, c->lambda_m, c->pitch_m, c->z_m))) return rc;
+    if ((rc = holo_fft_plan_init(&c->px, c->nx))) return rc;
+    if ((rc = holo_fft_plan_init(&c->py, c->ny))) return rc;
+    {   // Eq. 8: w_mn = exp(-2 i pi (m-1)(n-1)/T)/sqrt(T)
+        std::vector<float2> W((size_t)T * T);
+        const double PI = 3.14159265358979323846264338327950288;
+        for (int m = 0; m < T; ++m)
+            for (int n = 0; n < T; ++n) {
+                const double ang = -2.0 * PI * (double)((m * n) % T) / (double)T;
+                W[(size_t)m * T + n] = make_float2((float)(cos(ang) / sqrt((double)T)), (float)(sin(ang) / sqrt((double)T)));
+            }
+        HOLO_CUDA_OK(cudaMalloc(&c->Wdft, W.size() * sizeof(float2)));
+        HOLO_CUDA_OK(cudaMemcpy(c->Wdft, W.data(), W.size() * sizeof(float2), cudaMemcpyHostToDevice));
+    }
+    // tuning defaults
+    long long grp = (32ll << 20) / (8 * np);                 // keep the FFT intermediate <= 32 MiB (L2-resident)
+    if (grp < 1) grp = 1;
+    if (grp > T) grp = T;
+    c->tune[HOLO_TUNE_FFT_GROUP] = (int)grp;
+    c->tune[HOLO_TUNE_COV_GRIDX] = c->num_sms;
+    c->tune[HOLO_TUNE_PROJ_COMPLEMENT] = 1;
+    c->tune[HOLO_TUNE_FFT_PERSISTENT] = 0;
+    c->tune[HOLO_TUNE_EIG_MAX_SWEEPS] = 30;
+    c->scratch_frames = (int)grp;
+    c->cov_parts_cap = 4 * c->num_sms;
+    const int T8 = (T + 7) / 8 * 8;
+    HOLO_CUDA_OK(cudaMalloc(&c->sum, np * sizeof(uint32_t)));
+    HOLO_CUDA_OK(cudaMalloc(&c->scratch, (size_t)T * np * 0 + (size_t)c->scratch_frames * np * sizeof(float2)));
+    HOLO_CUDA_OK(cudaMalloc(&c->H, (size_t)T * np * sizeof(float2)));
+    HOLO_CUDA_OK(cudaMalloc(&c->cov_partials, (size_t)c->cov_parts_cap * T8 * T8 * sizeof(float2)));
+    HOLO_CUDA_OK(cudaMalloc(&c->C, (size_t)T * T * sizeof(float2)));
+    HOLO_CUDA_OK(cudaMalloc(&c->evals, T * sizeof(float)));
+    HOLO_CUDA_OK(cudaMalloc(&c->V, (size_t)T * T * sizeof(float2)));
+    HOLO_CUDA_OK(cudaMalloc(&c->Vsel, (size_t)T * HOLO_MAX_T * sizeof(float2)));
+    HOLO_CUDA_OK(cudaMalloc(&c->status, 4 * sizeof(int32_t)));
+    HOLO_CUDA_OK(cudaMalloc(&c->counters, 1024 * sizeof(unsigned int)));
+    HOLO_CUDA_OK(cudaMemset(c->status, 0, 4 * sizeof(int32_t)));
+    HOLO_CUDA_OK(cudaMemset(c->counters, 0, 1024 * sizeof(unsigned int)));
+    HOLO_CUDA_OK(cudaMemset(c->cov_partials, 0, (size_t)c->cov_parts_cap * T8 * T8 * sizeof(float2)));
+    HOLO_CUDA_OK(cudaDeviceSynchronize());
+    return HOLO_OK;
+}
+
+extern "C" holo_ctx* holo_create(int nx, int ny, int T, double lambda_m, double pitch_m, double z_m,
+                                 int k_lo, int k_hi) {
+    if (!is_pow2(nx) || !is_pow2(ny) || nx < 16 || ny < 16 || nx > 4096 || ny > 4096) {
+        holo_set_error("nx, ny must be powers of two in [16, 4096] (got %d x %d)", nx, ny);
+        return nullptr;
+    }
+    if (T < 2 || T > HOLO_MAX_T) { holo_set_error("T must be in [2, %d] (got %d)", HOLO_MAX_T, T); return nullptr; }
+    if (!(lambda_m > 0) || !(pitch_m > 0) || !(z_m > 0) || !isfinite(lambda_m) || !isfinite(pitch_m) || !isfinite(z_m)) {
+        holo_set_error("lambda, pitch, z must be finite and > 0");
+        return nullptr;
+    }
+    if (k_lo < 1 || k_hi > T || k_lo > k_hi) { holo_set_error("need 1 <= k_lo <= k_hi <= T (got %d, %d)", k_lo, k_hi); return nullptr; }
+    holo_ctx* c = new (std::nothrow) holo_ctx();
+    if (!c) { holo_set_error("out of host memory"); return nullptr; }
+    memset(c, 0, sizeof(*c));
+    c->nx = nx; c->ny = ny; c->T = T; c->npix = (long long)nx * ny;
+    c->lambda_m = lambda_m; c->pitch_m = pitch_m; c->z_m = z_m;
+    c->k_lo = k_lo; c->k_hi = k_hi;
+    if (create_impl(c) != HOLO_OK) { free_ctx(c); return nullptr; }
+    return c;
+}
+
+extern "C" void holo_destroy(holo_ctx* c) {
+    if (!c) return;
+    cudaDeviceSynchronize();
+    free_ctx(c);
+}
+
+#define CHECK_CTX(c) do { if (!(c)) { holo_set_error("NULL handle"); return HOLO_ERR_ARG; } } while (0)
+#define CHECK_PTR(p, name) do { if (!(p)) { holo_set_error("NULL pointer: %s", name); return HOLO_ERR_ARG; } } while (0)
+
+extern "C" int holo_fresnel(holo_ctx* c, const uint16_t* frames_dev, void* H_dev, holo_stream stream) {
+    CHECK_CTX(c); CHECK_PTR(frames_dev, "frames_dev"); CHECK_PTR(H_dev, "H_dev");
+    if (((uintptr_t)frames_dev & 15) || ((uintptr_t)H_dev & 15)) { holo_set_error("frames_dev/H_dev must be 16-byte aligned"); return HOLO_ERR_ARG; }
+    return holo_launch_fresnel(c, frames_dev, (float2*)H_dev, (cudaStream_t)stream);
+}
+
+extern "C" int holo_covariance(holo_ctx* c, const void* H_dev, void* C_dev, holo_stream stream) {
+    CHECK_CTX(c); CHECK_PTR(H_dev, "H_dev"); CHECK_PTR(C_dev, "C_dev");
+    if ((uintptr_t)H_dev & 15) { holo_set_error("H_dev must be 16-byte aligned"); return HOLO_ERR_ARG; }
+    return holo_launch_covariance(c, (const float2*)H_dev, (float2*)C_dev, (cudaStream_t)stream);
+}
+
+extern "C" int holo_eig(holo_ctx* c, const void* C_dev, float* evals_dev, void* V_dev, holo_stream stream) {
+    CHECK_CTX(c); CHECK_PTR(C_dev, "C_dev"); CHECK_PTR(evals_dev, "evals_dev"); CHECK_PTR(V_dev, "V_dev");
+    return holo_launch_eig(c, (const float2*)C_dev, evals_dev, (float2*)V_dev, (cudaStream_t)stream);
+}
+
+extern "C" int holo_project(holo_ctx* c, const void* H_dev, const void* V_dev, float* image_dev, holo_stream stream) {
+    CHECK_CTX(c); CHECK_PTR(H_dev, "H_dev"); CHECK_PTR(V_dev, "V_dev"); CHECK_PTR(image_dev, "image_dev");
+    if (((uintptr_t)H_dev & 15) || ((uintptr_t)image_dev & 7)) { holo_set_error("H_dev must be 16-byte and image_dev 8-byte aligned"); return HOLO_ERR_ARG; }
+    return holo_launch_project(c, (const float2*)H_dev, (const float2*)V_dev, c->k_lo, c->k_hi,
+                               c->assume_unitary, image_dev, (cudaStream_t)stream);
+}
+
+extern "C" int holo_fourier_demod(holo_ctx* c, const void* H_dev, int n1, int n2, float* image_dev, holo_stream stream) {
+    CHECK_CTX(c); CHECK_PTR(H_dev, "H_dev"); CHECK_PTR(image_dev, "image_dev");
+    if (n1 < 1 || n2 > c->T || n1 > n2) { holo_set_error("need 1 <= n1 <= n2 <= T"); return HOLO_ERR_ARG; }
+    if (((uintptr_t)H_dev & 15) || ((uintptr_t)image_dev & 7)) { holo_set_error("H_dev must be 16-byte and image_dev 8-byte aligned"); return HOLO_ERR_ARG; }
+    return holo_launch_project(c, (const float2*)H_dev, c->Wdft, n1, n2, /*W is unitary*/ 1, image_dev, (cudaStream_t)stream);
+}
+
+extern "C" int holo_process(holo_ctx* c, const uint16_t* frames_dev, float* image_dev, holo_stream stream) {
+    CHECK_CTX(c); CHECK_PTR(frames_dev, "frames_dev"); CHECK_PTR(image_dev, "image_dev");
+    if (((uintptr_t)frames_dev & 15) || ((uintptr_t)image_dev & 7)) { holo_set_error("frames_dev must be 16-byte and image_dev 8-byte aligned"); return HOLO_ERR_ARG; }
+    cudaStream_t st = (cudaStream_t)stream;
+    int rc;
+    if ((rc = holo_launch_fresnel(c, frames_dev, c->H, st))) return rc;
+    if ((rc = holo_launch_covariance(c, c->H, c->C, st))) return rc;
+    if ((rc = holo_launch_eig(c, c->C, c->evals, c->V, st))) return rc;
+    return holo_launch_project(c, c->H, c->V, c->k_lo, c->k_hi, c->tune[HOLO_TUNE_PROJ_COMPLEMENT], image_dev, st);
+}
+
+extern "C" int holo_process_host(holo_ctx* c, const uint16_t* frames_host, float* image_host, holo_stream stream) {
+    CHECK_CTX(c); CHECK_PTR(frames_host, "frames_host"); CHECK_PTR(image_host, "image_host");
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t fbytes = (size_t)c->T * c->npix * sizeof(uint16_t), ibytes = (size_t)c->npix * sizeof(float);
+    if (!c->frames_stage) {
+        if (cudaMalloc(&c->frames_stage, fbytes) != cudaSuccess || cudaMalloc(&c->image_stage, ibytes) != cudaSuccess) {
+            holo_set_error("staging allocation failed");
+            return HOLO_ERR_ALLOC;
+        }
+    }
+    HOLO_CUDA_OK(cudaMemcpyAsync(c->frames_stage, frames_host, fbytes, cudaMemcpyHostToDevice, st));
+    int rc = holo_process(c, c->frames_stage, c->image_stage, stream);
+    if (rc) return rc;
+    HOLO_CUDA_OK(cudaMemcpyAsync(image_host, c->image_stage, ibytes, cudaMemcpyDeviceToHost, st));
+    HOLO_CUDA_OK(cudaStreamSynchronize(st));
+    return HOLO_OK;
+}
+
+extern "C" int holo_set_range(holo_ctx* c, int k_lo, int k_hi) {
+    CHECK_CTX(c);
+    if (k_lo < 1 || k_hi > c->T || k_lo > k_hi) { holo_set_error("need 1 <= k_lo <= k_hi <= T (got %d, %d)", k_lo, k_hi); return HOLO_ERR_ARG; }
+    c->k_lo = k_lo; c->k_hi = k_hi;
+    return HOLO_OK;
+}
+
+extern "C" int holo_set_assume_unitary(holo_ctx* c, int on) {
+    CHECK_CTX(c);
+    c->assume_unitary = on ? 1 : 0;
+    return HOLO_OK;
+}
+
+extern "C" const void* holo_workspace(holo_ctx* c, int which) {
+    if (!c) return nullptr;
+    switch (which) {
+        case HOLO_WS_SUM: return c->sum;
+        case HOLO_WS_H: return c->H;
+        case HOLO_WS_C: return c->C;
+        case HOLO_WS_EVALS: return c->evals;
+        case HOLO_WS_V: return c->V;
+        case HOLO_WS_STATUS: return c->status;
+        case HOLO_WS_QX: return c->qx;
+        case HOLO_WS_QY: return c->qy;
+    }
+    return nullptr;
+}
+
+extern "C" int holo_workspace_copy(holo_ctx* c, int which, void* dst_dev, unsigned long long nbytes, holo_stream stream) {
+    CHECK_CTX(c); CHECK_PTR(dst_dev, "dst_dev");
+    const void* src = holo_workspace(c, which);
+    if (!src) { holo_set_error("bad workspace id %d", which); return HOLO_ERR_ARG; }
+    HOLO_CUDA_OK(cudaMemcpyAsync(dst_dev, src, (size_t)nbytes, cudaMemcpyDeviceToDevice, (cudaStream_t)stream));
+    return HOLO_OK;
+}
+
+extern "C" int holo_status(holo_ctx* c, int32_t status_host[4], holo_stream stream) {
+    CHECK_CTX(c); CHECK_PTR(status_host, "status_host");
+    cudaStream_t st = (cudaStream_t)stream;
+    HOLO_CUDA_OK(cudaMemcpyAsync(status_host, c->status, 4 * sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+    HOLO_CUDA_OK(cudaStreamSynchronize(st));
+    if (status_host[0]) { holo_set_error("Jacobi eigensolver hit the sweep cap (%d sweeps)", status_host[1]); return HOLO_ERR_NOCONV; }
+    return HOLO_OK;
+}
+
+extern "C" int holo_launches_per_process(holo_ctx* c) {
+    CHECK_CTX(c);
+    return holo_fresnel_launch_count(c) + 2 /*cov partial + reduce*/ + 1 /*eig*/ + 1 /*project*/;
+}
+
+// not in holo.h: experiment knob used by bench.py sweeps (see holo_internal.cuh HOLO_TUNE_*)
+extern "C" int holo_tune(holo_ctx* c, int key, int value) {
+    CHECK_CTX(c);
+    if (key < 0 || key >= HOLO_NUM_TUNE) { holo_set_error("bad tuning key"); return HOLO_ERR_ARG; }
+    if (key == HOLO_TUNE_FFT_GROUP) {
+        if (value < 1 || value > c->T) { holo_set_error("fft group out of range"); return HOLO_ERR_ARG; }
+        if (value > c->scratch_frames) {
+            cudaDeviceSynchronize();
+            cudaFree(c->scratch);
+            c->scratch = nullptr;
+            if (cudaMalloc(&c->scratch, (size_t)value * c->npix * sizeof(float2)) != cudaSuccess) { holo_set_error("scratch allocation failed"); return HOLO_ERR_ALLOC; }
+        }
+        c->scratch_frames = value;
+    }
+    if (key == HOLO_TUNE_PROFILE && value && !c->prof_ev) {
+        c->prof_ev = new cudaEvent_t[2 * HOLO_PROF_CAP];
+        c->prof_cls = new int[HOLO_PROF_CAP];
+        for (int i = 0; i < 2 * HOLO_PROF_CAP; ++i) HOLO_CUDA_OK(cudaEventCreate(&c->prof_ev[i]));
+        c->prof_n = 0;
+    }
+    if (key == HOLO_TUNE_COV_GRIDX && (value < 1 || value > c->cov_parts_cap)) { holo_set_error("cov grid out of range"); return HOLO_ERR_ARG; }
+    c->tune[key] = value;
+    return HOLO_OK;
+}
+
+// not in the stable ABI: per-kernel-class device time accumulated since the last read, while
+// holo_tune(ctx, 5, 1) is on.  ms_out[HOLO_K_COUNT], count_out[HOLO_K_COUNT]; synchronises the device.
+extern "C" int holo_profile_read(holo_ctx* c, double* ms_out, int* count_out) {
+    CHECK_CTX(c); CHECK_PTR(ms_out, "ms_out"); CHECK_PTR(count_out, "count_out");
+    for (int k = 0; k < HOLO_K_COUNT; ++k) { ms_out[k] = 0.0; count_out[k] = 0; }
+    if (!c->prof_ev) return HOLO_OK;
+    HOLO_CUDA_OK(cudaDeviceSynchronize());
+    for (int i = 0; i < c->prof_n; ++i) {
+        float ms = 0.f;
+        HOLO_CUDA_OK(cudaEventElapsedTime(&ms, c->prof_ev[2 * i], c->prof_ev[2 * i + 1]));
+        ms_out[c->prof_cls[i]] += ms;
+        count_out[c->prof_cls[i]] += 1;
+    }
+    c->prof_n = 0;
+    return HOLO_OK;
+}
+
+extern "C" int holo_fft_group(holo_ctx* c) { return c ? c->scratch_frames : 0; }

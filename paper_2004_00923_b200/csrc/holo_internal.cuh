@@ -1,0 +1,101 @@
+// holo_internal.cuh -- private declarations shared by the translation units of libholo_b200.
+// Product code (CUDA, sm_100a).  Nothing here is shared with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stdio.h>
+#include "../../include/holo.h"
+
+#define HOLO_MAX_T 64
+#define HOLO_NUM_TUNE 16
+
+// tuning keys (holo_tune); not part of the stable ABI
+enum {
+    HOLO_TUNE_FFT_GROUP = 0,     // frames per row/column pass group (scratch = group * 8*nx*ny bytes)
+    HOLO_TUNE_COV_GRIDX = 1,     // covariance CTAs along pixels
+    HOLO_TUNE_PROJ_COMPLEMENT = 2, // 1 = allow complement form in holo_process (default 1)
+    HOLO_TUNE_FFT_PERSISTENT = 3,  // 1 = single persistent fresnel kernel (default set at create)
+    HOLO_TUNE_EIG_MAX_SWEEPS = 4,
+    HOLO_TUNE_PROFILE = 5,         // 1 = bracket every kernel launch with events (holo_profile_read)
+};
+
+// kernel classes for the profile hook
+enum { HOLO_K_SUM = 0, HOLO_K_FFT_ROWS, HOLO_K_FFT_COLS, HOLO_K_COV_PARTIAL, HOLO_K_COV_REDUCE, HOLO_K_EIG, HOLO_K_PROJECT, HOLO_K_COUNT };
+#define HOLO_PROF_CAP 4096
+
+struct FftPlan {            // one 1-D FFT length
+    int N;                  // length
+    int E;                  // elements per thread per pass (16 or 32)
+    int R1, R2;             // radices of pass 1 and 2 (1 = absent); pass 0 is radix E
+    int tps;                // threads per sequence = N / E
+    float2* tw1;            // device: pass-1 twiddles [R1][E]          exp(-2 pi i r k /(E R1))
+    float2* tw2;            // device: pass-2 twiddles [R2][E*R1]
+};
+
+struct holo_ctx {
+    int nx, ny, T;
+    long long npix;
+    double lambda_m, pitch_m, z_m;
+    int k_lo, k_hi;
+    int assume_unitary;
+    int device, num_sms;
+    int tune[HOLO_NUM_TUNE];
+    // tables
+    float2 *qx, *qy;        // chirp, separable (built in double on the host)
+    FftPlan px, py;
+    float2* Wdft;           // Eq. 8 DFT basis [T][T]
+    // workspace
+    uint32_t* sum;          // [ny][nx]
+    float2* scratch;        // FFT row->column intermediate, fft_group frames
+    int scratch_frames;
+    float2* H;              // [T][ny][nx]
+    float2* cov_partials;   // [cov_parts][T][T]
+    int cov_parts_cap;
+    float2* C;
+    float* evals;
+    float2* V;
+    float2* Vsel;           // [T][HOLO_MAX_T] selected/zero-padded projection coefficients
+    int32_t* status;        // [4]
+    unsigned int* counters; // persistent-kernel tickets / dependency counters
+    // profile hook
+    cudaEvent_t* prof_ev;   // [2*HOLO_PROF_CAP]
+    int* prof_cls;
+    int prof_n;
+    // host staging for holo_process_host
+    uint16_t* frames_stage;
+    float* image_stage;
+};
+
+void holo_set_error(const char* fmt, ...);
+#define HOLO_CUDA_OK(expr)                                                              \
+    do {                                                                                \
+        cudaError_t _e = (expr);                                                        \
+        if (_e != cudaSuccess) {                                                        \
+            holo_set_error("%s failed: %s (%s:%d)", #expr, cudaGetErrorString(_e), __FILE__, __LINE__); \
+            return HOLO_ERR_CUDA;                                                       \
+        }                                                                               \
+    } while (0)
+
+// RAII event bracket around one kernel launch (only when profiling is on)
+struct HoloProf {
+    holo_ctx* c; cudaStream_t st; int slot;
+    HoloProf(holo_ctx* c_, int cls, cudaStream_t st_) : c(c_), st(st_), slot(-1) {
+        if (c->tune[HOLO_TUNE_PROFILE] && c->prof_ev && c->prof_n < HOLO_PROF_CAP) {
+            slot = c->prof_n++;
+            c->prof_cls[slot] = cls;
+            cudaEventRecord(c->prof_ev[2 * slot], st);
+        }
+    }
+    ~HoloProf() { if (slot >= 0) cudaEventRecord(c->prof_ev[2 * slot + 1], st); }
+};
+
+// stage launchers (each only enqueues on `st`)
+int holo_launch_fresnel(holo_ctx* c, const uint16_t* frames, float2* H, cudaStream_t st);
+int holo_launch_covariance(holo_ctx* c, const float2* H, float2* C, cudaStream_t st);
+int holo_launch_eig(holo_ctx* c, const float2* C, float* evals, float2* V, cudaStream_t st);
+// mode 0: direct over columns [k_lo,k_hi] of V; mode 1: complement (total - columns outside)
+int holo_launch_project(holo_ctx* c, const float2* H, const float2* V, int k_lo, int k_hi,
+                        int allow_complement, float* image, cudaStream_t st);
+int holo_fresnel_launch_count(holo_ctx* c);
+int holo_fft_plan_init(FftPlan* p, int N);
+void holo_fft_plan_free(FftPlan* p);

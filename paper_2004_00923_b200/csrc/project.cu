@@ -1,0 +1,112 @@
+// project.cu -- A5 + A6 fused:  M(p) = sum_{k in S} | sum_t H_t(p) V_{t,k} |^2     (Eq. 6-7)
+// Reads the hologram stack once, never stores P.  Two exact forms (R12):
+//   direct     : sum over the columns k in S = [k_lo,k_hi]
+//   complement : sum_t |H_t(p)|^2 - sum over the columns k NOT in S   (V unitary), used when smaller
+// The same kernel serves the Fourier demodulation of Eq. 8-9 with V := W.
+#include "holo_internal.cuh"
+
+struct ProjArgs {
+    const float2* H;
+    const float2* V;       // [T][T] row-major, column = component
+    float* M;
+    long long npix;
+    int T;
+    int r0_lo, r0_hi;      // first 0-based inclusive column range (empty if lo > hi)
+    int r1_lo, r1_hi;      // second range
+    int complement;        // 1: M = total - sum
+};
+
+template <int NC, int PIX>      // PIX = pixels per thread (2: float4 loads; 1 for very wide component sets)
+__global__ void __launch_bounds__(256) k_project(const ProjArgs a) {
+    __shared__ __align__(16) float2 Vs[HOLO_MAX_T * NC];          // [t][c], zero padded
+    const int tid = threadIdx.x;
+    const int n0 = a.r0_hi - a.r0_lo + 1 > 0 ? a.r0_hi - a.r0_lo + 1 : 0;
+    for (int i = tid; i < a.T * NC; i += blockDim.x) {
+        const int t = i / NC, c = i - t * NC;
+        int col = -1;
+        if (c < n0) col = a.r0_lo + c;
+        else if (c - n0 <= a.r1_hi - a.r1_lo) col = a.r1_lo + (c - n0);
+        Vs[i] = col >= 0 ? a.V[t * a.T + col] : make_float2(0.f, 0.f);
+    }
+    __syncthreads();
+    const long long item = (long long)blockIdx.x * blockDim.x + tid;     // PIX adjacent pixels per thread
+    if (item * PIX >= a.npix) return;
+    const long long fstride = a.npix / PIX;
+    float2 acc[PIX][NC];
+#pragma unroll
+    for (int x = 0; x < PIX; ++x)
+#pragma unroll
+        for (int c = 0; c < NC; ++c) acc[x][c] = make_float2(0.f, 0.f);
+    float tot[PIX];
+#pragma unroll
+    for (int x = 0; x < PIX; ++x) tot[x] = 0.f;
+#pragma unroll 4
+    for (int t = 0; t < a.T; ++t) {
+        float2 h[PIX];
+        if constexpr (PIX == 2) {
+            const float4 w = __ldg(reinterpret_cast<const float4*>(a.H) + item + (long long)t * fstride);
+            h[0] = make_float2(w.x, w.y); h[1] = make_float2(w.z, w.w);
+        } else {
+            h[0] = __ldg(a.H + item + (long long)t * fstride);
+        }
+#pragma unroll
+        for (int x = 0; x < PIX; ++x) tot[x] = fmaf(h[x].x, h[x].x, fmaf(h[x].y, h[x].y, tot[x]));
+#pragma unroll
+        for (int c = 0; c < NC; ++c) {
+            const float2 v = Vs[t * NC + c];
+#pragma unroll
+            for (int x = 0; x < PIX; ++x) {
+                acc[x][c].x = fmaf(h[x].x, v.x, fmaf(-h[x].y, v.y, acc[x][c].x));
+                acc[x][c].y = fmaf(h[x].x, v.y, fmaf(h[x].y, v.x, acc[x][c].y));
+            }
+        }
+    }
+    float s[PIX];
+#pragma unroll
+    for (int x = 0; x < PIX; ++x) {
+        s[x] = 0.f;
+#pragma unroll
+        for (int c = 0; c < NC; ++c) s[x] = fmaf(acc[x][c].x, acc[x][c].x, fmaf(acc[x][c].y, acc[x][c].y, s[x]));
+        if (a.complement) s[x] = tot[x] - s[x];
+    }
+    if constexpr (PIX == 2) reinterpret_cast<float2*>(a.M)[item] = make_float2(s[0], s[1]);
+    else a.M[item] = s[0];
+}
+
+template <int NC> static int launch_proj_t(holo_ctx* c, const ProjArgs& a, cudaStream_t st) {
+    HoloProf prof(c, HOLO_K_PROJECT, st);
+    constexpr int PIX = NC > 32 ? 1 : 2;
+    const long long items = a.npix / PIX;
+    const int threads = 256;
+    const int grid = (int)((items + threads - 1) / threads);
+    k_project<NC, PIX><<<grid, threads, 0, st>>>(a);
+    HOLO_CUDA_OK(cudaGetLastError());
+    return HOLO_OK;
+}
+
+int holo_launch_project(holo_ctx* c, const float2* H, const float2* V, int k_lo, int k_hi,
+                        int allow_complement, float* image, cudaStream_t st) {
+    const int T = c->T;
+    const int nS = k_hi - k_lo + 1;
+    ProjArgs a{};
+    a.H = H; a.V = V; a.M = image; a.npix = c->npix; a.T = T;
+    int nc;
+    if (allow_complement && (T - nS) < nS) {
+        a.complement = 1;
+        a.r0_lo = 0; a.r0_hi = k_lo - 2;          // components 1 .. k_lo-1
+        a.r1_lo = k_hi; a.r1_hi = T - 1;          // components k_hi+1 .. T
+        nc = T - nS;
+    } else {
+        a.complement = 0;
+        a.r0_lo = k_lo - 1; a.r0_hi = k_hi - 1;
+        a.r1_lo = 0; a.r1_hi = -1;
+        nc = nS;
+    }
+    if (nc <= 1) return launch_proj_t<1>(c, a, st);
+    if (nc <= 2) return launch_proj_t<2>(c, a, st);
+    if (nc <= 4) return launch_proj_t<4>(c, a, st);
+    if (nc <= 8) return launch_proj_t<8>(c, a, st);
+    if (nc <= 16) return launch_proj_t<16>(c, a, st);
+    if (nc <= 32) return launch_proj_t<32>(c, a, st);
+    return launch_proj_t<64>(c, a, st);
+}
