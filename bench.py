@@ -157,6 +157,9 @@ def run_ours(args, cfg):
     frames = G.stream_torch(cfg, 1000 + rank, dev, n_frames=n_stacks * T)
     torch.cuda.synchronize()
     h = Holo(n, n, T, cfg.lam, cfg.pitch, cfg.z, cfg.k_lo, cfg.k_hi)
+    for kv in args.tune:
+        k, v = kv.split("=")
+        h.tune(int(k), int(v))
     images = torch.empty((4, n, n), dtype=torch.float32, device=dev)
     st = torch.cuda.Stream(device=dev)
     fbytes = T * n * n * 2
@@ -311,6 +314,7 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=24)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--tune", action="append", default=[], help="experiment knob key=value (holo_tune), repeatable")
     args = ap.parse_args()
     from gen import holo_gen as G
     cfg = G.CONFIGS[args.config]

@@ -111,8 +111,8 @@ int holo_fourier_demod(holo_ctx* ctx, const void* H_dev, int n1, int n2, float* 
 int holo_set_range(holo_ctx* ctx, int k_lo, int k_hi);
 
 /* Allow holo_process/holo_project to use the exact identity sum_{k in S}|P_k|^2 =
- * sum_t |H_t|^2 - sum_{k not in S}|P_k|^2 (valid for unitary V; R12) when the complement of S is
- * smaller than S.  holo_process always may (its V is unitary by construction); for holo_project
+ * sum_t |H_t|^2 - sum_{k not in S}|P_k|^2 (valid for unitary V; R12), evaluated without cancellation
+ * as sum_t |H_t - sum_{k not in S} P_k conj(V_tk)|^2, when the complement of S is at most half of S.  holo_process always may (its V is unitary by construction); for holo_project
  * this flag (default 0) states that the caller's V is unitary. */
 int holo_set_assume_unitary(holo_ctx* ctx, int on);
 

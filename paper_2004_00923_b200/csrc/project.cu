@@ -1,7 +1,10 @@
 // project.cu -- A5 + A6 fused:  M(p) = sum_{k in S} | sum_t H_t(p) V_{t,k} |^2     (Eq. 6-7)
 // Reads the hologram stack once, never stores P.  Two exact forms (R12):
 //   direct     : sum over the columns k in S = [k_lo,k_hi]
-//   complement : sum_t |H_t(p)|^2 - sum over the columns k NOT in S   (V unitary), used when smaller
+//   complement : (V unitary) deflation  H'_t = H_t - sum_{k not in S} P_k conj(V_tk),  M = sum_t |H'_t|^2,
+//                used when the complement of S is smaller than S.  Algebraically equal to
+//                sum_t|H_t|^2 - sum_{k not in S}|P_k|^2, but without the catastrophic cancellation of that
+//                subtraction when the rejected clutter carries almost all of the energy (the method's use case).
 // The same kernel serves the Fourier demodulation of Eq. 8-9 with V := W.
 #include "holo_internal.cuh"
 
@@ -73,6 +76,86 @@ __global__ void __launch_bounds__(256) k_project(const ProjArgs a) {
     else a.M[item] = s[0];
 }
 
+// complement (deflation) form; the T holograms of the thread's pixel(s) stay in registers and the
+// rejected components are removed one after the other (modified Gram-Schmidt order):
+//   for k not in S:  P = sum_t h_t V_tk ;  h_t -= P conj(V_tk)        then  M = sum_t |h_t|^2
+template <int TMAX, int PIX>
+__global__ void __launch_bounds__(256) k_project_deflate(const ProjArgs a, int nc) {
+    extern __shared__ __align__(16) float2 Vd[];            // [c][TMAX], zero padded in t
+    const int tid = threadIdx.x;
+    const int n0 = a.r0_hi - a.r0_lo + 1 > 0 ? a.r0_hi - a.r0_lo + 1 : 0;
+    for (int i = tid; i < nc * TMAX; i += blockDim.x) {
+        const int c = i / TMAX, t = i - c * TMAX;
+        const int col = c < n0 ? a.r0_lo + c : a.r1_lo + (c - n0);
+        Vd[i] = t < a.T ? a.V[t * a.T + col] : make_float2(0.f, 0.f);
+    }
+    __syncthreads();
+    const long long item = (long long)blockIdx.x * blockDim.x + tid;
+    if (item * PIX >= a.npix) return;
+    const long long fstride = a.npix / PIX;
+    float2 h[TMAX][PIX];
+#pragma unroll
+    for (int t = 0; t < TMAX; ++t) {
+        if (t < a.T) {
+            if constexpr (PIX == 2) {
+                const float4 w = __ldg(reinterpret_cast<const float4*>(a.H) + item + (long long)t * fstride);
+                h[t][0] = make_float2(w.x, w.y); h[t][1] = make_float2(w.z, w.w);
+            } else {
+                h[t][0] = __ldg(a.H + item + (long long)t * fstride);
+            }
+        } else {
+#pragma unroll
+            for (int x = 0; x < PIX; ++x) h[t][x] = make_float2(0.f, 0.f);
+        }
+    }
+#pragma unroll 1
+    for (int c = 0; c < nc; ++c) {
+        const float2* v = Vd + c * TMAX;
+        float2 P[PIX];
+#pragma unroll
+        for (int x = 0; x < PIX; ++x) P[x] = make_float2(0.f, 0.f);
+#pragma unroll
+        for (int t = 0; t < TMAX; ++t) {
+            const float2 w = v[t];
+#pragma unroll
+            for (int x = 0; x < PIX; ++x) {                       // P += h_t * v_t
+                P[x].x = fmaf(h[t][x].x, w.x, fmaf(-h[t][x].y, w.y, P[x].x));
+                P[x].y = fmaf(h[t][x].x, w.y, fmaf(h[t][x].y, w.x, P[x].y));
+            }
+        }
+#pragma unroll
+        for (int t = 0; t < TMAX; ++t) {
+            const float2 w = v[t];
+#pragma unroll
+            for (int x = 0; x < PIX; ++x) {                       // h_t -= P * conj(v_t)
+                h[t][x].x = fmaf(-P[x].x, w.x, fmaf(-P[x].y, w.y, h[t][x].x));
+                h[t][x].y = fmaf(-P[x].y, w.x, fmaf(P[x].x, w.y, h[t][x].y));
+            }
+        }
+    }
+    float s[PIX];
+#pragma unroll
+    for (int x = 0; x < PIX; ++x) s[x] = 0.f;
+#pragma unroll
+    for (int t = 0; t < TMAX; ++t)
+#pragma unroll
+        for (int x = 0; x < PIX; ++x) s[x] = fmaf(h[t][x].x, h[t][x].x, fmaf(h[t][x].y, h[t][x].y, s[x]));
+    if constexpr (PIX == 2) reinterpret_cast<float2*>(a.M)[item] = make_float2(s[0], s[1]);
+    else a.M[item] = s[0];
+}
+
+template <int TMAX> static int launch_deflate(holo_ctx* c, const ProjArgs& a, int nc, cudaStream_t st) {
+    HoloProf prof(c, HOLO_K_PROJECT, st);
+    constexpr int PIX = TMAX <= 32 ? 2 : 1;
+    const long long items = a.npix / PIX;
+    const int threads = 256;
+    const int grid = (int)((items + threads - 1) / threads);
+    const size_t smem = (size_t)(nc > 0 ? nc : 1) * TMAX * sizeof(float2);
+    k_project_deflate<TMAX, PIX><<<grid, threads, smem, st>>>(a, nc);
+    HOLO_CUDA_OK(cudaGetLastError());
+    return HOLO_OK;
+}
+
 template <int NC> static int launch_proj_t(holo_ctx* c, const ProjArgs& a, cudaStream_t st) {
     HoloProf prof(c, HOLO_K_PROJECT, st);
     constexpr int PIX = NC > 32 ? 1 : 2;
@@ -91,7 +174,7 @@ int holo_launch_project(holo_ctx* c, const float2* H, const float2* V, int k_lo,
     ProjArgs a{};
     a.H = H; a.V = V; a.M = image; a.npix = c->npix; a.T = T;
     int nc;
-    if (allow_complement && (T - nS) < nS) {
+    if (allow_complement && 2 * (T - nS) <= nS) {          // deflating costs 2 passes per rejected component
         a.complement = 1;
         a.r0_lo = 0; a.r0_hi = k_lo - 2;          // components 1 .. k_lo-1
         a.r1_lo = k_hi; a.r1_hi = T - 1;          // components k_hi+1 .. T
@@ -101,6 +184,12 @@ int holo_launch_project(holo_ctx* c, const float2* H, const float2* V, int k_lo,
         a.r0_lo = k_lo - 1; a.r0_hi = k_hi - 1;
         a.r1_lo = 0; a.r1_hi = -1;
         nc = nS;
+    }
+    if (a.complement) {
+        if (T <= 8) return launch_deflate<8>(c, a, nc, st);
+        if (T <= 16) return launch_deflate<16>(c, a, nc, st);
+        if (T <= 32) return launch_deflate<32>(c, a, nc, st);
+        return launch_deflate<64>(c, a, nc, st);
     }
     if (nc <= 1) return launch_proj_t<1>(c, a, st);
     if (nc <= 2) return launch_proj_t<2>(c, a, st);

@@ -1,0 +1,100 @@
+#include <cstdio>
+#include <cuda_runtime.h>
+#include <cstdint>
+#define CK(x) do{cudaError_t e=(x); if(e!=cudaSuccess){printf("ERR %s line %d\n",cudaGetErrorString(e),__LINE__); return 1;}}while(0)
+template<int NACC>
+__global__ void k_ffma(float* out, float a, float b, int iters){
+  float acc[NACC];
+  #pragma unroll
+  for(int i=0;i<NACC;i++) acc[i]=threadIdx.x*0.001f+i;
+  for(int it=0; it<iters; ++it){
+    #pragma unroll
+    for(int i=0;i<NACC;i++) acc[i]=fmaf(acc[i],a,b);
+  }
+  float s=0; 
+  #pragma unroll
+  for(int i=0;i<NACC;i++) s+=acc[i];
+  out[blockIdx.x*blockDim.x+threadIdx.x]=s;
+}
+// outer-product style: 8x8 acc, 8 a + 8 b regs (3 distinct regs per FFMA)
+__global__ void k_ffma_outer(float* out, const float* in, int iters){
+  float acc[8][8]; float a[8], b[8];
+  #pragma unroll
+  for(int i=0;i<8;i++){a[i]=in[threadIdx.x+i*32]; b[i]=in[threadIdx.x+i*32+256];}
+  #pragma unroll
+  for(int i=0;i<8;i++)
+  #pragma unroll
+  for(int j=0;j<8;j++) acc[i][j]=0;
+  for(int it=0; it<iters; ++it){
+    #pragma unroll
+    for(int i=0;i<8;i++)
+    #pragma unroll
+    for(int j=0;j<8;j++) acc[i][j]=fmaf(a[i],b[j],acc[i][j]);
+    #pragma unroll
+    for(int i=0;i<8;i++){a[i]+=1e-9f;}
+  }
+  float s=0;
+  #pragma unroll
+  for(int i=0;i<8;i++)
+  #pragma unroll
+  for(int j=0;j<8;j++) s+=acc[i][j];
+  out[blockIdx.x*blockDim.x+threadIdx.x]=s;
+}
+template<int NACC>
+__global__ void k_ffma2(float* out, float a, float b, int iters){
+  unsigned long long acc[NACC];
+  unsigned long long A, B;
+  asm("mov.b64 %0, {%1,%2};":"=l"(A):"f"(a),"f"(a));
+  asm("mov.b64 %0, {%1,%2};":"=l"(B):"f"(b),"f"(b));
+  #pragma unroll
+  for(int i=0;i<NACC;i++){ float x=threadIdx.x*0.001f+i; asm("mov.b64 %0, {%1,%2};":"=l"(acc[i]):"f"(x),"f"(x+0.5f)); }
+  for(int it=0; it<iters; ++it){
+    #pragma unroll
+    for(int i=0;i<NACC;i++) asm volatile("fma.rn.f32x2 %0, %0, %1, %2;":"+l"(acc[i]):"l"(A),"l"(B));
+  }
+  float s=0;
+  #pragma unroll
+  for(int i=0;i<NACC;i++){ float x,y; asm("mov.b64 {%0,%1}, %2;":"=f"(x),"=f"(y):"l"(acc[i])); s+=x+y; }
+  out[blockIdx.x*blockDim.x+threadIdx.x]=s;
+}
+__global__ void k_read(const uint4* __restrict__ in, size_t n, uint4* out){
+  size_t i=(size_t)blockIdx.x*blockDim.x+threadIdx.x; size_t stride=(size_t)gridDim.x*blockDim.x;
+  uint4 s=make_uint4(0,0,0,0);
+  for(; i+3*stride<n; i+=4*stride){ uint4 a=in[i],b=in[i+stride],c=in[i+2*stride],d=in[i+3*stride]; s.x^=a.x^b.x^c.x^d.x; s.y^=a.y^b.y^c.y^d.y; s.z^=a.z^b.z^c.z^d.z; s.w^=a.w^b.w^c.w^d.w;}
+  if(s.x==0x12345678u) out[0]=s;
+}
+__global__ void k_copy(const uint4* __restrict__ in, uint4* __restrict__ out, size_t n){
+  size_t i=(size_t)blockIdx.x*blockDim.x+threadIdx.x; size_t stride=(size_t)gridDim.x*blockDim.x;
+  for(; i<n; i+=stride) out[i]=in[i];
+}
+int main(){
+  int sms; cudaDeviceGetAttribute(&sms,cudaDevAttrMultiProcessorCount,0);
+  float* out; CK(cudaMalloc(&out, 148*8*1024*4)); float* in; CK(cudaMalloc(&in,4096*4)); CK(cudaMemset(in,0,4096*4));
+  cudaEvent_t e0,e1; cudaEventCreate(&e0); cudaEventCreate(&e1); float ms;
+  int iters=20000;
+  for(int thr: {256,512,1024}) for(int bps: {1,2,4}){
+    if(thr*bps>2048) continue;
+    k_ffma<16><<<sms*bps,thr>>>(out,1.0001f,0.5f,100); cudaDeviceSynchronize();
+    cudaEventRecord(e0); k_ffma<16><<<sms*bps,thr>>>(out,1.0001f,0.5f,iters); cudaEventRecord(e1); CK(cudaEventSynchronize(e1)); cudaEventElapsedTime(&ms,e0,e1);
+    printf("FFMA  thr=%4d bps=%d: %.2f TFLOPS\n",thr,bps, 2.0*16*iters*(double)sms*bps*thr/ms/1e9);
+    k_ffma2<16><<<sms*bps,thr>>>(out,1.0001f,0.5f,100); cudaDeviceSynchronize();
+    cudaEventRecord(e0); k_ffma2<16><<<sms*bps,thr>>>(out,1.0001f,0.5f,iters); cudaEventRecord(e1); CK(cudaEventSynchronize(e1)); cudaEventElapsedTime(&ms,e0,e1);
+    printf("FFMA2 thr=%4d bps=%d: %.2f TFLOPS\n",thr,bps, 4.0*16*iters*(double)sms*bps*thr/ms/1e9);
+  }
+  for(int thr: {128,256,320}){
+    k_ffma_outer<<<sms,thr>>>(out,in,100); cudaDeviceSynchronize();
+    cudaEventRecord(e0); k_ffma_outer<<<sms,thr>>>(out,in,iters); cudaEventRecord(e1); CK(cudaEventSynchronize(e1)); cudaEventElapsedTime(&ms,e0,e1);
+    printf("FFMA outer8x8 thr=%d: %.2f TFLOPS\n",thr, 2.0*64*iters*(double)sms*thr/ms/1e9);
+  }
+  size_t bytes=(size_t)4<<30; uint4 *a,*b; CK(cudaMalloc(&a,bytes)); CK(cudaMalloc(&b,bytes)); CK(cudaMemset(a,1,bytes)); CK(cudaMemset(b,0,bytes));
+  size_t n=bytes/16;
+  for(int rep=0;rep<3;rep++){
+    cudaEventRecord(e0); k_read<<<sms*8,512>>>(a,n,b); cudaEventRecord(e1); CK(cudaEventSynchronize(e1)); cudaEventElapsedTime(&ms,e0,e1);
+    printf("read  4GiB: %.1f GB/s\n", bytes/ms/1e6);
+    cudaEventRecord(e0); k_copy<<<sms*8,512>>>(a,b,n); cudaEventRecord(e1); CK(cudaEventSynchronize(e1)); cudaEventElapsedTime(&ms,e0,e1);
+    printf("copy  4GiB: %.1f GB/s (r+w)\n", 2.0*bytes/ms/1e6);
+    cudaEventRecord(e0); cudaMemsetAsync(b,0,bytes); cudaEventRecord(e1); CK(cudaEventSynchronize(e1)); cudaEventElapsedTime(&ms,e0,e1);
+    printf("memset 4GiB: %.1f GB/s\n", bytes/ms/1e6);
+  }
+  return 0;
+}
