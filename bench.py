@@ -295,6 +295,7 @@ def run_ours(args, cfg):
             "roofline": roof, "roofline_end_to_end": {"bound": "hbm", "achieved": round(e2e_gbps, 1), "peak": hbm_peak, "unit": "GB/s",
                                                       "frac": round(e2e_gbps / hbm_peak, 4), "bytes_per_step": sb["total"], "peak_source": peak_src},
             "stages": stages, "cpu_baseline": cpu, "eig_status": status,
+            "eig_cycles": h.workspace_tensor(5).cpu().tolist()[4:7],
             "paper_context": {"images_per_s": PAPER_IMAGES_PER_S, "input_frames_per_s": 500, "hardware": "NVIDIA Titan RTX (PAPER.md:96)"},
         }
         print(json.dumps(line))

@@ -60,7 +60,8 @@ enum {
     HOLO_WS_C = 2,       /* float2 [T][T]                                                           */
     HOLO_WS_EVALS = 3,   /* float  [T]                                                              */
     HOLO_WS_V = 4,       /* float2 [T][T]                                                           */
-    HOLO_WS_STATUS = 5,  /* int32  [4]: {noconv flag, sweeps used, rotations in last sweep, 0}      */
+    HOLO_WS_STATUS = 5,  /* int32  [8]: {noconv flag, sweeps used, rotations in last sweep, 0,
+                          *              SM cycles of load / sweeps / refinement, 0}                        */
     HOLO_WS_QX = 6,      /* float2 [nx] chirp table exp(+i pi x_i^2/(lambda z))                     */
     HOLO_WS_QY = 7       /* float2 [ny]                                                             */
 };

@@ -158,7 +158,7 @@ class Holo:
         T, ny, nx = self.T, self.ny, self.nx
         shapes = {HOLO_WS_SUM: ((ny, nx), torch.int32), HOLO_WS_H: ((T, ny, nx), torch.complex64),
                   HOLO_WS_C: ((T, T), torch.complex64), HOLO_WS_EVALS: ((T,), torch.float32),
-                  HOLO_WS_V: ((T, T), torch.complex64), HOLO_WS_STATUS: ((4,), torch.int32),
+                  HOLO_WS_V: ((T, T), torch.complex64), HOLO_WS_STATUS: ((8,), torch.int32),
                   HOLO_WS_QX: ((nx,), torch.complex64), HOLO_WS_QY: ((ny,), torch.complex64)}
         shape, dtype = shapes[which]
         out = torch.empty(shape, dtype=dtype, device="cuda")

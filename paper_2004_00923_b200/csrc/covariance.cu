@@ -112,25 +112,33 @@ k_cov_partial(const float2* __restrict__ H, float2* __restrict__ partials, long 
     }
 }
 
-// fixed-order FP64 reduction over the partials; writes the full Hermitian C (both triangles),
-// diagonal imaginary parts forced to 0.
-__global__ void k_cov_reduce(const float2* __restrict__ partials, int nparts, int T, int T8, float2* __restrict__ C) {
-    const int idx = blockIdx.x * blockDim.x + threadIdx.x;
-    if (idx >= T * T) return;
-    const int t = idx / T, s = idx - t * T;
+// fixed-order FP64 reduction over the partials: one warp per lower-triangle entry, lane l sums parts
+// l, l+32, ... in order, then a fixed shuffle tree (deterministic).  Writes the full Hermitian C (both
+// triangles), diagonal imaginary parts forced to 0.
+__global__ void __launch_bounds__(256) k_cov_reduce(const float2* __restrict__ partials, int nparts, int T, int T8, float2* __restrict__ C) {
+    const int w = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+    if (w >= T * T) return;
+    const int t = w / T, s = w - t * T;
     if (s > t) return;
     double re = 0.0, im = 0.0;
     const float2* p = partials + t * T8 + s;
-    for (int k = 0; k < nparts; ++k) {
-        float2 v = p[(size_t)k * T8 * T8];
+    for (int k = lane; k < nparts; k += 32) {
+        const float2 v = p[(size_t)k * T8 * T8];
         re += (double)v.x;
         im += (double)v.y;
     }
-    if (s == t) {
-        C[t * T + t] = make_float2((float)re, 0.f);
-    } else {
-        C[t * T + s] = make_float2((float)re, (float)im);
-        C[s * T + t] = make_float2((float)re, (float)-im);
+#pragma unroll
+    for (int o = 16; o >= 1; o >>= 1) {
+        re += __shfl_xor_sync(0xffffffffu, re, o);
+        im += __shfl_xor_sync(0xffffffffu, im, o);
+    }
+    if (lane == 0) {
+        if (s == t) {
+            C[t * T + t] = make_float2((float)re, 0.f);
+        } else {
+            C[t * T + s] = make_float2((float)re, (float)im);
+            C[s * T + t] = make_float2((float)re, (float)-im);
+        }
     }
 }
 
@@ -157,7 +165,7 @@ static int launch_cov_t(holo_ctx* c, const float2* H, float2* C, cudaStream_t st
     HOLO_CUDA_OK(cudaGetLastError());
     int n = c->T * c->T;
     HoloProf prof(c, HOLO_K_COV_REDUCE, st);
-    k_cov_reduce<<<(n + 255) / 256, 256, 0, st>>>(c->cov_partials, gx, c->T, T8, C);
+    k_cov_reduce<<<(n * 32 + 255) / 256, 256, 0, st>>>(c->cov_partials, gx, c->T, T8, C);
     HOLO_CUDA_OK(cudaGetLastError());
     return HOLO_OK;
 }

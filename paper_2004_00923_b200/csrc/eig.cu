@@ -26,114 +26,139 @@ __device__ float block_sum(float v, float* red) {       // all threads must call
     return s;
 }
 
-__global__ void __launch_bounds__(512, 1)
+// rotation that annihilates the pivot of a Hermitian 2x2 block [[app, apq],[conj(apq), aqq]]:
+// J = [[c, se],[-conj(se), c]], se = s e^{i phi}; identity when the pivot is below thr2 (or padding).
+__device__ __forceinline__ bool jacobi_rot(float app, float aqq, float2 apq, float thr2, bool valid, float& c, float2& se) {
+    c = 1.f; se = make_float2(0.f, 0.f);
+    const float mag2 = fmaf(apq.x, apq.x, apq.y * apq.y);
+    if (!valid || !(mag2 > thr2)) return false;
+    const float inv_mag = rsqrtf(mag2);
+    const float m2 = 2.f * mag2 * inv_mag;                  // 2|apq|
+    const float d = aqq - app;
+    const float t = copysignf(m2, d) / (fabsf(d) + sqrtf(fmaf(d, d, m2 * m2)));   // sgn(tau)/(|tau|+sqrt(1+tau^2))
+    c = rsqrtf(fmaf(t, t, 1.f));
+    const float s = t * c * inv_mag;
+    se = make_float2(apq.x * s, apq.y * s);
+    return true;
+}
+
+template <int TP>
+__global__ void __launch_bounds__((TP / 2) * (TP / 2) < 32 ? 32 : (TP / 2) * (TP / 2), 1)
 k_eig(const float2* __restrict__ C, int T, float* __restrict__ evals, float2* __restrict__ Vout,
       int32_t* __restrict__ status, int max_sweeps) {
     extern __shared__ __align__(16) unsigned char raw[];
-    const int Tp = (T + 1) & ~1;
-    const int LD = Tp + 1;
-    float2* A = reinterpret_cast<float2*>(raw);
-    float2* V = A + Tp * LD;
-    float2* rot_se = V + Tp * LD;                 // [Tp/2] s*e^{i phi}
-    float* rot_c = reinterpret_cast<float*>(rot_se + Tp / 2);       // [Tp/2]
-    int* rot_p = reinterpret_cast<int*>(rot_c + Tp / 2);
-    int* rot_q = rot_p + Tp / 2;
-    float* red = reinterpret_cast<float*>(rot_q + Tp / 2);          // [32]
-    int* cnt = reinterpret_cast<int*>(red + 32);                    // [2]
-    size_t off = (size_t)((unsigned char*)(cnt + 2) - raw);
+    constexpr int Tp = TP, LD = TP + 1, half = TP / 2, m = TP - 1;
+    float2* A0 = reinterpret_cast<float2*>(raw);
+    float2* A1 = A0 + Tp * LD;
+    float2* V = A1 + Tp * LD;
+    float* red = reinterpret_cast<float*>(V + Tp * LD);             // [32]
+    size_t off = (size_t)((unsigned char*)(red + 32) - raw);
     off = (off + 15) & ~(size_t)15;
     double* dscr = reinterpret_cast<double*>(raw + off);            // [T*T] partial Rayleigh terms
     double* lam = dscr + (size_t)T * T;                             // [T]
     int* rank = reinterpret_cast<int*>(lam + T);                    // [T]
 
     const int tid = threadIdx.x, nt = blockDim.x;
-    const int half = Tp / 2, m = Tp - 1;
+    const long long clk0 = clock64();
 
-    // ---- load: lower triangle of C -> full Hermitian A; V = I
+    // ---- load: lower triangle of C -> full Hermitian A (scaled by a power of two so that max|diag| <= 1); V = I
+    float dmax = 0.f;
+    for (int i = tid; i < T; i += nt) dmax = fmaxf(dmax, fabsf(C[i * T + i].x));
+    for (int i = tid; i < T * T; i += nt) { const int r = i / T, c = i - r * T; if (c < r) { const float2 a = C[i]; dmax = fmaxf(dmax, fmaxf(fabsf(a.x), fabsf(a.y))); } }
+#pragma unroll
+    for (int o = 16; o >= 1; o >>= 1) dmax = fmaxf(dmax, __shfl_xor_sync(0xffffffffu, dmax, o));
+    if ((tid & 31) == 0) red[tid >> 5] = dmax;
+    __syncthreads();
+    dmax = 0.f;
+    for (int w = 0; w < (nt >> 5); ++w) dmax = fmaxf(dmax, red[w]);
+    int ex = 0;
+    if (dmax > 0.f && dmax < 3.0e38f) frexpf(dmax, &ex);
+    const float scale = ldexpf(1.f, -ex);
     for (int i = tid; i < Tp * Tp; i += nt) {
-        int r = i / Tp, c = i - r * Tp;
+        const int r = i / Tp, c = i - r * Tp;
         float2 a = make_float2(0.f, 0.f);
         if (r < T && c < T) {
             if (c < r) a = C[r * T + c];
             else if (c > r) { a = C[c * T + r]; a.y = -a.y; }
             else a = make_float2(C[r * T + r].x, 0.f);
+            a.x *= scale; a.y *= scale;
         }
-        A[r * LD + c] = a;
+        A0[r * LD + c] = a;
         V[r * LD + c] = make_float2(r == c ? 1.f : 0.f, 0.f);
     }
-    if (tid == 0) { cnt[0] = 0; cnt[1] = 0; }
     __syncthreads();
     float n2 = 0.f;
-    for (int i = tid; i < Tp * Tp; i += nt) { float2 a = A[(i / Tp) * LD + (i % Tp)]; n2 += a.x * a.x + a.y * a.y; }
+    for (int i = tid; i < Tp * Tp; i += nt) { const float2 a = A0[(i / Tp) * LD + (i % Tp)]; n2 += a.x * a.x + a.y * a.y; }
     const float normF2 = block_sum(n2, red);
     const float eps = 5.96e-8f;
     const float thr2 = (0.25f * eps * eps / (float)(T * T)) * normF2;   // skip pivots below (eps/2T)*||A||_F
     const float tol2 = (float)(T * T) * eps * eps * normF2;             // stop at off-norm <= T*eps*||A||_F
 
+    // one thread per 2x2 block (pair bi, pair bj) of A; the same thread rotates rows 2bi, 2bi+1 of V by J_bj
+    const int bi = tid / half, bj = tid % half;
+    const bool worker = tid < half * half;
+    float2* Ac = A0;
+    float2* An = A1;
     int sweeps = 0, converged = 0, last_rot = 0;
+    const long long clk1 = clock64();
     for (; sweeps < max_sweeps; ++sweeps) {
-        if (tid == 0) cnt[0] = 0;            // ordered before the pivots' atomicAdd by block_sum's barriers
         float o2 = 0.f;
         for (int i = tid; i < Tp * Tp; i += nt) {
-            int r = i / Tp, c = i - r * Tp;
-            if (r != c) { float2 a = A[r * LD + c]; o2 += a.x * a.x + a.y * a.y; }
+            const int r = i / Tp, c = i - r * Tp;
+            if (r != c) { const float2 a = Ac[r * LD + c]; o2 += a.x * a.x + a.y * a.y; }
         }
         const float off2 = block_sum(o2, red);
         if (off2 <= tol2) { converged = 1; break; }
+        int rot_count = 0;
+#pragma unroll 1
         for (int step = 0; step < m; ++step) {
-            // ---- 1. rotations for the Tp/2 disjoint pivots of this step
-            if (tid < half) {
-                int p, q;
-                if (tid == 0) { p = step; q = m; }
-                else { int a = (step + tid) % m, b = (step - tid + m) % m; p = a < b ? a : b; q = a < b ? b : a; }
-                float c = 1.f; float2 se = make_float2(0.f, 0.f);
-                if (q < T) {
-                    const float2 apq = A[p * LD + q];
-                    const float mag2 = apq.x * apq.x + apq.y * apq.y;
-                    if (mag2 > thr2 && mag2 > 0.f) {
-                        const float app = A[p * LD + p].x, aqq = A[q * LD + q].x;
-                        const float mag = sqrtf(mag2);
-                        const float tau = (aqq - app) / (2.f * mag);
-                        const float t = copysignf(1.f, tau) / (fabsf(tau) + sqrtf(fmaf(tau, tau, 1.f)));
-                        c = 1.f / sqrtf(fmaf(t, t, 1.f));
-                        const float s = t * c, inv = s / mag;
-                        se = make_float2(apq.x * inv, apq.y * inv);
-                        atomicAdd(&cnt[0], 1);
-                    }
+            int applied = 0;
+            if (worker) {
+                int pi, qi, pj, qj;
+                if (bi == 0) { pi = step; qi = m; } else { const int a = (step + bi) % m, b = (step - bi + m) % m; pi = min(a, b); qi = max(a, b); }
+                if (bj == 0) { pj = step; qj = m; } else { const int a = (step + bj) % m, b = (step - bj + m) % m; pj = min(a, b); qj = max(a, b); }
+                float ci, cj; float2 sei, sej;
+                const bool ri = jacobi_rot(Ac[pi * LD + pi].x, Ac[qi * LD + qi].x, Ac[pi * LD + qi], thr2, qi < T, ci, sei);
+                jacobi_rot(Ac[pj * LD + pj].x, Ac[qj * LD + qj].x, Ac[pj * LD + qj], thr2, qj < T, cj, sej);
+                applied = (bi == bj) && ri;
+                // B' = J_i^H B J_j
+                const float2 b00 = Ac[pi * LD + pj], b01 = Ac[pi * LD + qj], b10 = Ac[qi * LD + pj], b11 = Ac[qi * LD + qj];
+                float2 t1, t2;
+                t1 = cmulcf(b01, sej); t2 = cmulf(b00, sej);
+                const float2 x00 = make_float2(fmaf(cj, b00.x, -t1.x), fmaf(cj, b00.y, -t1.y));
+                const float2 x01 = make_float2(fmaf(cj, b01.x, t2.x), fmaf(cj, b01.y, t2.y));
+                t1 = cmulcf(b11, sej); t2 = cmulf(b10, sej);
+                const float2 x10 = make_float2(fmaf(cj, b10.x, -t1.x), fmaf(cj, b10.y, -t1.y));
+                const float2 x11 = make_float2(fmaf(cj, b11.x, t2.x), fmaf(cj, b11.y, t2.y));
+                t1 = cmulf(x10, sei); t2 = cmulcf(x00, sei);
+                float2 y00 = make_float2(fmaf(ci, x00.x, -t1.x), fmaf(ci, x00.y, -t1.y));
+                float2 y10 = make_float2(fmaf(ci, x10.x, t2.x), fmaf(ci, x10.y, t2.y));
+                t1 = cmulf(x11, sei); t2 = cmulcf(x01, sei);
+                float2 y01 = make_float2(fmaf(ci, x01.x, -t1.x), fmaf(ci, x01.y, -t1.y));
+                float2 y11 = make_float2(fmaf(ci, x11.x, t2.x), fmaf(ci, x11.y, t2.y));
+                if (bi == bj) {                      // the pivot block: exactly diagonal and real afterwards
+                    y00.y = 0.f; y11.y = 0.f;
+                    if (ri) { y01 = make_float2(0.f, 0.f); y10 = make_float2(0.f, 0.f); }
                 }
-                rot_c[tid] = c; rot_se[tid] = se; rot_p[tid] = p; rot_q[tid] = q;
+                An[pi * LD + pj] = y00; An[pi * LD + qj] = y01; An[qi * LD + pj] = y10; An[qi * LD + qj] = y11;
+                // V <- V J_j on rows 2bi, 2bi+1 (in place: nobody else touches these elements this step)
+#pragma unroll
+                for (int rr = 0; rr < 2; ++rr) {
+                    const int r = 2 * bi + rr;
+                    const float2 vp = V[r * LD + pj], vq = V[r * LD + qj];
+                    t1 = cmulcf(vq, sej); t2 = cmulf(vp, sej);
+                    V[r * LD + pj] = make_float2(fmaf(cj, vp.x, -t1.x), fmaf(cj, vp.y, -t1.y));
+                    V[r * LD + qj] = make_float2(fmaf(cj, vq.x, t2.x), fmaf(cj, vq.y, t2.y));
+                }
             }
-            __syncthreads();
-            // ---- 2. A <- A J, V <- V J   (columns p,q; lanes run over rows: stride LD is odd -> no conflicts)
-            for (int i = tid; i < 2 * half * Tp; i += nt) {
-                const int row = i % Tp, pr = (i / Tp) % half, which = i / (Tp * half);
-                float2* M = which ? V : A;
-                const int p = rot_p[pr], q = rot_q[pr];
-                const float c = rot_c[pr]; const float2 se = rot_se[pr];
-                const float2 ap = M[row * LD + p], aq = M[row * LD + q];
-                const float2 t1 = cmulcf(aq, se);          // aq * s e^{-i phi}
-                const float2 t2 = cmulf(ap, se);           // ap * s e^{+i phi}
-                M[row * LD + p] = make_float2(fmaf(c, ap.x, -t1.x), fmaf(c, ap.y, -t1.y));
-                M[row * LD + q] = make_float2(fmaf(c, aq.x, t2.x), fmaf(c, aq.y, t2.y));
-            }
-            __syncthreads();
-            // ---- 3. A <- J^H A   (rows p,q; lanes run over columns)
-            for (int i = tid; i < half * Tp; i += nt) {
-                const int col = i % Tp, pr = i / Tp;
-                const int p = rot_p[pr], q = rot_q[pr];
-                const float c = rot_c[pr]; const float2 se = rot_se[pr];
-                const float2 ap = A[p * LD + col], aq = A[q * LD + col];
-                const float2 t1 = cmulf(aq, se);           // s e^{+i phi} aq
-                const float2 t2 = cmulcf(ap, se);          // s e^{-i phi} ap
-                A[p * LD + col] = make_float2(fmaf(c, ap.x, -t1.x), fmaf(c, ap.y, -t1.y));
-                A[q * LD + col] = make_float2(fmaf(c, aq.x, t2.x), fmaf(c, aq.y, t2.y));
-            }
-            __syncthreads();
+            rot_count += __syncthreads_count(applied);
+            float2* tmp = Ac; Ac = An; An = tmp;
         }
-        last_rot = cnt[0];
+        last_rot = rot_count;
         if (last_rot == 0) { converged = 1; ++sweeps; break; }
-        __syncthreads();
     }
+    __syncthreads();
+    const long long clk2 = clock64();
 
     // ---- FP64 Rayleigh quotients against the original C (Hermitian from its lower triangle)
     for (int i = tid; i < T * T; i += nt) {
@@ -181,28 +206,38 @@ k_eig(const float2* __restrict__ C, int T, float* __restrict__ evals, float2* __
         status[1] = sweeps;
         status[2] = last_rot;
         status[3] = 0;
+        status[4] = (int)(clk1 - clk0);          // cycles: load + scale
+        status[5] = (int)(clk2 - clk1);          // cycles: Jacobi sweeps
+        status[6] = (int)(clock64() - clk2);     // cycles: Rayleigh refinement, sort, phase fix
+        status[7] = 0;
     }
 }
 
-static size_t eig_smem_bytes(int T) {
-    const int Tp = (T + 1) & ~1, LD = Tp + 1, half = Tp / 2;
-    size_t b = (size_t)2 * Tp * LD * sizeof(float2) + half * (sizeof(float2) + sizeof(float) + 2 * sizeof(int)) +
-               32 * sizeof(float) + 2 * sizeof(int);
-    b = (b + 15) & ~(size_t)15;
-    b += (size_t)T * T * sizeof(double) + T * sizeof(double) + T * sizeof(int);
-    return b + 16;
+template <int TP>
+static int launch_eig_t(holo_ctx* c, const float2* C, float* evals, float2* V, cudaStream_t st) {
+    const int T = c->T;
+    constexpr int LD = TP + 1;
+    size_t smem = (size_t)3 * TP * LD * sizeof(float2) + 32 * sizeof(float);
+    smem = (smem + 15) & ~(size_t)15;
+    smem += (size_t)T * T * sizeof(double) + T * sizeof(double) + T * sizeof(int) + 16;
+    static bool attr = false;
+    if (!attr) {
+        const size_t worst = (size_t)3 * TP * LD * sizeof(float2) + 256 + (size_t)TP * TP * 8 + TP * 12 + 32;
+        HOLO_CUDA_OK(cudaFuncSetAttribute(k_eig<TP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)worst));
+        attr = true;
+    }
+    constexpr int threads = (TP / 2) * (TP / 2) < 32 ? 32 : (TP / 2) * (TP / 2);
+    HoloProf prof(c, HOLO_K_EIG, st);
+    k_eig<TP><<<1, threads, smem, st>>>(C, T, evals, V, c->status, c->tune[HOLO_TUNE_EIG_MAX_SWEEPS]);
+    HOLO_CUDA_OK(cudaGetLastError());
+    return HOLO_OK;
 }
 
 int holo_launch_eig(holo_ctx* c, const float2* C, float* evals, float2* V, cudaStream_t st) {
-    const size_t smem = eig_smem_bytes(c->T);
-    static size_t attr_set = 0;
-    if (smem > attr_set) {
-        HOLO_CUDA_OK(cudaFuncSetAttribute(k_eig, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        attr_set = smem;
-    }
-    const int threads = c->T <= 32 ? 256 : 512;
-    HoloProf prof(c, HOLO_K_EIG, st);
-    k_eig<<<1, threads, smem, st>>>(C, c->T, evals, V, c->status, c->tune[HOLO_TUNE_EIG_MAX_SWEEPS]);
-    HOLO_CUDA_OK(cudaGetLastError());
-    return HOLO_OK;
+    const int T = c->T;
+    if (T <= 4) return launch_eig_t<4>(c, C, evals, V, st);
+    if (T <= 8) return launch_eig_t<8>(c, C, evals, V, st);
+    if (T <= 16) return launch_eig_t<16>(c, C, evals, V, st);
+    if (T <= 32) return launch_eig_t<32>(c, C, evals, V, st);
+    return launch_eig_t<64>(c, C, evals, V, st);
 }

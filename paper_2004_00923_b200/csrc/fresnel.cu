@@ -68,7 +68,8 @@ __device__ __forceinline__ float2 cmul(float2 a, float2 b) {
 // A0: per-pixel temporal sum  S(p) = sum_t I_t(p)   (uint32: exact, T*65535 < 2^32)
 // ------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256) k_frame_sum(const uint16_t* __restrict__ frames, uint32_t* __restrict__ sum,
-                                                   long long npix, int T) {
+                                                   long long npix, int T, unsigned int* __restrict__ counters) {
+    if (blockIdx.x == 0 && threadIdx.x < 2 * T + 1) counters[threadIdx.x] = 0u;   // tickets of the fused Fresnel kernel
     long long v = (long long)blockIdx.x * blockDim.x + threadIdx.x;      // one uint4 = 8 pixels per thread
     long long nvec = npix >> 3;
     for (; v < nvec; v += (long long)gridDim.x * blockDim.x) {
@@ -111,12 +112,12 @@ struct FftArgs {
     float invT;
 };
 
+// one tile = B sequences of one frame; in_foff / out_foff = element offset of the frame in a.in(frames) / a.out
 template <int N, int E, int R1, int R2, int B, bool COL, bool PRO>
-__global__ void __launch_bounds__((N / E) * B) k_fft(const FftArgs a) {
+__device__ __forceinline__ void fft_tile(const FftArgs& a, long long in_foff, long long out_foff, int tile_in_frame, float2* sm) {
     constexpr int TPS = N / E;
     constexpr int PADN = N + N / E;
     constexpr bool MULTI = (R1 > 1);
-    extern __shared__ float2 sm[];
     const int tid = threadIdx.x;
     const int j = COL ? tid / B : tid % TPS;
     const int c = COL ? tid % B : tid / TPS;
@@ -124,13 +125,11 @@ __global__ void __launch_bounds__((N / E) * B) k_fft(const FftArgs a) {
         int p = i + i / E;
         return COL ? p * B + c : c * PADN + p;
     };
-
-    for (int tile = blockIdx.x; tile < a.ntiles; tile += gridDim.x) {
-        const int fl = tile / a.tiles_per_frame;
-        const int s0 = (tile - fl * a.tiles_per_frame) * B + c;       // sequence index (row y or column x)
-        const long long ibase = (long long)fl * a.in_fstride + (COL ? (long long)s0 : (long long)s0 * a.ld);
-        const long long obase = (long long)fl * a.out_fstride + (COL ? (long long)s0 : (long long)s0 * a.ld);
-        const long long estride = COL ? a.ld : 1;
+    {
+        const int s0 = tile_in_frame * B + c;                          // sequence index (row y or column x)
+        const long long ibase = in_foff + (COL ? (long long)s0 : (long long)s0 * a.ld);
+        const long long obase = out_foff + (COL ? (long long)s0 : (long long)s0 * a.ld);
+        const int estride = COL ? a.ld : 1;
         float2 v[E];
         // ---------------- pass 0: radix E, Ns = 1, inputs straight from global
         if constexpr (PRO) {
@@ -149,13 +148,13 @@ __global__ void __launch_bounds__((N / E) * B) k_fft(const FftArgs a) {
         } else {
             const float2* ip = a.in + ibase;
 #pragma unroll
-            for (int r = 0; r < E; ++r) v[r] = __ldg(ip + (long long)(j + r * TPS) * estride);
+            for (int r = 0; r < E; ++r) v[r] = __ldcg(ip + (j + r * TPS) * estride);   // L2-coherent: written earlier in this kernel
         }
         fft_reg<E>(v);
         float2* op = a.out + obase;
         if constexpr (!MULTI) {
 #pragma unroll
-            for (int r = 0; r < E; ++r) op[(long long)r * estride] = v[brev<E>(r)];
+            for (int r = 0; r < E; ++r) op[r * estride] = v[brev<E>(r)];
         } else {
 #pragma unroll
             for (int r = 0; r < E; ++r) sm[sidx(j * E + r)] = v[brev<E>(r)];
@@ -179,7 +178,7 @@ __global__ void __launch_bounds__((N / E) * B) k_fft(const FftArgs a) {
                 const int j0 = (b - k) * R1 + k;
                 if constexpr (R2 == 1) {
 #pragma unroll
-                    for (int r = 0; r < R1; ++r) op[(long long)(j0 + r * E) * estride] = v[m * R1 + brev<R1>(r)];
+                    for (int r = 0; r < R1; ++r) op[(j0 + r * E) * estride] = v[m * R1 + brev<R1>(r)];
                 } else {
 #pragma unroll
                     for (int r = 0; r < R1; ++r) sm[sidx(j0 + r * E)] = v[m * R1 + brev<R1>(r)];
@@ -203,11 +202,76 @@ __global__ void __launch_bounds__((N / E) * B) k_fft(const FftArgs a) {
                     for (int r = 1; r < R2; ++r) v[m * R2 + r] = cmul(v[m * R2 + r], __ldg(a.tw2 + r * NS2 + b));
                     fft_reg<R2>(v + m * R2);
 #pragma unroll
-                    for (int r = 0; r < R2; ++r) op[(long long)(b + r * NS2) * estride] = v[m * R2 + brev<R2>(r)];
+                    for (int r = 0; r < R2; ++r) op[(b + r * NS2) * estride] = v[m * R2 + brev<R2>(r)];
                 }
             }
             __syncthreads();        // smem is reused by the next tile
         }
+    }
+}
+
+template <int N, int E, int R1, int R2, int B, bool COL, bool PRO>
+__global__ void __launch_bounds__((N / E) * B) k_fft(const FftArgs a) {
+    extern __shared__ float2 sm[];
+    for (int tile = blockIdx.x; tile < a.ntiles; tile += gridDim.x) {
+        const int fl = tile / a.tiles_per_frame;
+        fft_tile<N, E, R1, R2, B, COL, PRO>(a, (long long)fl * a.in_fstride, (long long)fl * a.out_fstride,
+                                            tile - fl * a.tiles_per_frame, sm);
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// Persistent fused Fresnel kernel (square frames): ONE launch does the row pass and the column pass of
+// all T frames.  CTAs draw tiles from a global ticket in the order
+//   rows(0), [rows(f), cols(f-1)] for f = 1..T-1, cols(T-1)
+// so a column tile almost never waits; the row->column intermediate is a ring of R frames that stays
+// in L2.  cols(f) waits for rows_done[f] == RT; rows(f) waits for cols_done[f-R] == CT (ring reuse).
+// All CTAs are co-resident (grid <= occupancy x SMs) and tickets are served in order, so the tile with
+// the smallest unfinished ticket can always run: no deadlock.
+// ------------------------------------------------------------------------------------------------
+struct FresnelArgs {
+    FftArgs rows, cols;         // rows.out = cols.in = scratch ring; frame offsets are computed here
+    unsigned int* counters;     // [0] ticket, [1..T] rows_done, [1+T..2T] cols_done (zeroed by k_frame_sum)
+    long long npix;
+    int T, R, RT, CT;
+};
+
+__device__ __forceinline__ unsigned int ld_acquire(const unsigned int* p) {
+    unsigned int v;
+    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+
+template <int N, int E, int R1, int R2, int B>
+__global__ void __launch_bounds__((N / E) * B, ((N / E) * B <= 256) ? 2 : 1) k_fresnel(const FresnelArgs p) {
+    extern __shared__ float2 sm[];
+    __shared__ unsigned int s_ticket;
+    const unsigned int per = (unsigned int)(p.RT + p.CT);
+    const unsigned int total = (unsigned int)p.T * per;
+    for (;;) {
+        if (threadIdx.x == 0) s_ticket = atomicAdd(p.counters, 1u);
+        __syncthreads();
+        const unsigned int tk = s_ticket;
+        if (tk >= total) break;
+        int f, w; bool is_col;
+        if (tk < (unsigned int)p.RT) { f = 0; w = (int)tk; is_col = false; }
+        else {
+            const unsigned int u = tk - (unsigned int)p.RT;
+            const int seg = (int)(u / per), r = (int)(u - (unsigned int)seg * per);
+            if (seg < p.T - 1) { if (r < p.RT) { f = seg + 1; w = r; is_col = false; } else { f = seg; w = r - p.RT; is_col = true; } }
+            else { f = p.T - 1; w = r; is_col = true; }
+        }
+        if (threadIdx.x == 0) {                      // dependency wait (rare by construction of the order)
+            if (is_col) { while (ld_acquire(p.counters + 1 + f) < (unsigned int)p.RT) __nanosleep(64); }
+            else if (f >= p.R) { while (ld_acquire(p.counters + 1 + p.T + (f - p.R)) < (unsigned int)p.CT) __nanosleep(64); }
+        }
+        __syncthreads();
+        const long long slot = (long long)(f % p.R) * p.npix;
+        if (!is_col) fft_tile<N, E, R1, R2, B, false, true>(p.rows, (long long)f * p.npix, slot, w, sm);
+        else         fft_tile<N, E, R1, R2, B, true, false>(p.cols, slot, (long long)f * p.npix, w, sm);
+        __threadfence();
+        __syncthreads();
+        if (threadIdx.x == 0) atomicAdd(p.counters + 1 + (is_col ? p.T + f : f), 1u);
     }
 }
 
@@ -303,7 +367,49 @@ static int launch_fft(int N, const FftArgs& a, int num_sms, cudaStream_t st) {
 }
 static int fft_batch(int N) { return N <= 512 ? 16 : N == 1024 ? 8 : 4; }
 
+template <int N, int E, int R1, int R2, int B>
+static int launch_fresnel_t(const FresnelArgs& p, int num_sms, cudaStream_t st) {
+    constexpr int threads = (N / E) * B;
+    constexpr size_t smem = (R1 > 1) ? sizeof(float2) * (size_t)(N + N / E) * B : 0;
+    auto kern = k_fresnel<N, E, R1, R2, B>;
+    static int blocks_per_sm = 0;
+    if (blocks_per_sm == 0) {
+        if (smem > 48 * 1024) HOLO_CUDA_OK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        int occ = 0;
+        HOLO_CUDA_OK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, threads, smem));
+        if (occ < 1) { holo_set_error("fused fresnel kernel N=%d does not fit on an SM", N); return HOLO_ERR_CUDA; }
+        blocks_per_sm = occ;
+    }
+    const long long total = (long long)p.T * (p.RT + p.CT);
+    long long grid = (long long)num_sms * blocks_per_sm;      // all CTAs co-resident (required by the dependency waits)
+    if (grid > total) grid = total;
+    kern<<<(int)grid, threads, smem, st>>>(p);
+    HOLO_CUDA_OK(cudaGetLastError());
+    return HOLO_OK;
+}
+
+static int launch_fresnel_fused(int N, const FresnelArgs& p, int num_sms, cudaStream_t st) {
+    switch (N) {
+        case 16:   return launch_fresnel_t<16, 16, 1, 1, 16>(p, num_sms, st);
+        case 32:   return launch_fresnel_t<32, 32, 1, 1, 16>(p, num_sms, st);
+        case 64:   return launch_fresnel_t<64, 16, 4, 1, 16>(p, num_sms, st);
+        case 128:  return launch_fresnel_t<128, 16, 8, 1, 16>(p, num_sms, st);
+        case 256:  return launch_fresnel_t<256, 16, 16, 1, 16>(p, num_sms, st);
+        case 512:  return launch_fresnel_t<512, 32, 16, 1, 16>(p, num_sms, st);
+        case 1024: return launch_fresnel_t<1024, 32, 32, 1, 8>(p, num_sms, st);
+        case 2048: return launch_fresnel_t<2048, 16, 16, 8, 4>(p, num_sms, st);
+        case 4096: return launch_fresnel_t<4096, 16, 16, 16, 4>(p, num_sms, st);
+    }
+    holo_set_error("unsupported FFT length %d", N);
+    return HOLO_ERR_ARG;
+}
+
+static bool use_fused(const holo_ctx* c) {
+    return c->nx == c->ny && c->tune[HOLO_TUNE_FFT_PERSISTENT] && c->scratch_frames >= 2 && 2 * c->T + 1 <= 256;
+}
+
 int holo_fresnel_launch_count(holo_ctx* c) {
+    if (use_fused(c)) return 2;
     int g = c->scratch_frames;
     int groups = (c->T + g - 1) / g;
     return 1 + 2 * groups;
@@ -317,8 +423,21 @@ int holo_launch_fresnel(holo_ctx* c, const uint16_t* frames, float2* H, cudaStre
         long long want = (nvec + threads - 1) / threads;
         int grid = (int)(want < (long long)c->num_sms * 8 ? want : (long long)c->num_sms * 8);
         HoloProf prof(c, HOLO_K_SUM, st);
-        k_frame_sum<<<grid, threads, 0, st>>>(frames, c->sum, c->npix, c->T);
+        k_frame_sum<<<grid, threads, 0, st>>>(frames, c->sum, c->npix, c->T, c->counters);
         HOLO_CUDA_OK(cudaGetLastError());
+    }
+    if (use_fused(c)) {
+        FresnelArgs p{};
+        const int Bq = fft_batch(c->nx);
+        FftArgs& a = p.rows;
+        a.frames = frames; a.sum = c->sum; a.qx = c->qx; a.qy = c->qy; a.in = nullptr; a.out = c->scratch;
+        a.tw1 = c->px.tw1; a.tw2 = c->px.tw2; a.ld = c->nx; a.nseq = c->ny; a.T = c->T; a.invT = 1.0f / (float)c->T;
+        FftArgs& b = p.cols;
+        b.in = c->scratch; b.out = H; b.tw1 = c->py.tw1; b.tw2 = c->py.tw2; b.ld = c->nx; b.nseq = c->nx; b.T = c->T; b.invT = a.invT;
+        p.counters = c->counters; p.npix = c->npix; p.T = c->T; p.R = c->scratch_frames;
+        p.RT = c->ny / Bq; p.CT = c->nx / Bq;
+        HoloProf prof(c, HOLO_K_FFT_ROWS, st);
+        return launch_fresnel_fused(c->nx, p, c->num_sms, st);
     }
     // A1 + A2, frame groups so that the row->column intermediate stays in L2
     const int G = c->scratch_frames;

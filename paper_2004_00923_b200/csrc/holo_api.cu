@@ -80,12 +80,12 @@ static int create_impl(holo_ctx* c) {
     }
     // tuning defaults
     long long grp = (32ll << 20) / (8 * np);                 // keep the FFT intermediate <= 32 MiB (L2-resident)
-    if (grp < 1) grp = 1;
+    if (grp < 2) grp = 2;                                    // the fused kernel needs a ring of >= 2 frames
     if (grp > T) grp = T;
     c->tune[HOLO_TUNE_FFT_GROUP] = (int)grp;
     c->tune[HOLO_TUNE_COV_GRIDX] = c->num_sms;
     c->tune[HOLO_TUNE_PROJ_COMPLEMENT] = 1;
-    c->tune[HOLO_TUNE_FFT_PERSISTENT] = 0;
+    c->tune[HOLO_TUNE_FFT_PERSISTENT] = 1;
     c->tune[HOLO_TUNE_EIG_MAX_SWEEPS] = 30;
     c->scratch_frames = (int)grp;
     c->cov_parts_cap = 4 * c->num_sms;
@@ -98,9 +98,9 @@ static int create_impl(holo_ctx* c) {
     HOLO_CUDA_OK(cudaMalloc(&c->evals, T * sizeof(float)));
     HOLO_CUDA_OK(cudaMalloc(&c->V, (size_t)T * T * sizeof(float2)));
     HOLO_CUDA_OK(cudaMalloc(&c->Vsel, (size_t)T * HOLO_MAX_T * sizeof(float2)));
-    HOLO_CUDA_OK(cudaMalloc(&c->status, 4 * sizeof(int32_t)));
+    HOLO_CUDA_OK(cudaMalloc(&c->status, 8 * sizeof(int32_t)));
     HOLO_CUDA_OK(cudaMalloc(&c->counters, 1024 * sizeof(unsigned int)));
-    HOLO_CUDA_OK(cudaMemset(c->status, 0, 4 * sizeof(int32_t)));
+    HOLO_CUDA_OK(cudaMemset(c->status, 0, 8 * sizeof(int32_t)));
     HOLO_CUDA_OK(cudaMemset(c->counters, 0, 1024 * sizeof(unsigned int)));
     HOLO_CUDA_OK(cudaMemset(c->cov_partials, 0, (size_t)c->cov_parts_cap * T8 * T8 * sizeof(float2)));
     HOLO_CUDA_OK(cudaDeviceSynchronize());
