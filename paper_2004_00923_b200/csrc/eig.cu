@@ -2,9 +2,14 @@
 //
 // Single-CTA two-sided complex Hermitian Jacobi in FP32, parallel (round-robin tournament) ordering:
 // each of the Tp-1 steps of a sweep annihilates Tp/2 disjoint pivots at once.  A and V live in
-// shared memory.  After convergence the eigenvalues are refined as FP64 Rayleigh quotients
-// v_k^H C v_k of the ORIGINAL matrix, sorted descending, and every eigenvector is normalised and
-// phase-fixed (largest-magnitude entry real positive, ties -> lowest index).
+// shared memory in SYSTOLIC (Brent-Luk) arrangement: the pivot pairs of every step are the
+// positions (2b, 2b+1); after the rotations each row/column is written to the position it takes in
+// the next step (a fixed permutation), so a thread's read and write addresses never change and
+// the step body carries no index arithmetic -- the kernel is bound by the latency of one step
+// (shared-memory round trip + rotation parameters + 2x2 update + one barrier), not by throughput.
+// After convergence the eigenvalues are refined as FP64 Rayleigh quotients v_k^H C v_k of the
+// ORIGINAL matrix, sorted descending, and every eigenvector is normalised and phase-fixed
+// (largest-magnitude entry real positive, ties -> lowest index).
 #include "holo_internal.cuh"
 
 __device__ __forceinline__ float2 cmulf(float2 a, float2 b) {
@@ -13,6 +18,8 @@ __device__ __forceinline__ float2 cmulf(float2 a, float2 b) {
 __device__ __forceinline__ float2 cmulcf(float2 a, float2 b) {      // a * conj(b)
     return make_float2(fmaf(a.y, b.y, a.x * b.x), fmaf(a.y, b.x, -a.x * b.y));
 }
+__device__ __forceinline__ float rsqrt_fast(float x) { float y; asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+__device__ __forceinline__ float rcp_fast(float x) { float y; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
 
 __device__ float block_sum(float v, float* red) {       // all threads must call; result broadcast
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nw = blockDim.x >> 5;
@@ -27,19 +34,29 @@ __device__ float block_sum(float v, float* red) {       // all threads must call
 }
 
 // rotation that annihilates the pivot of a Hermitian 2x2 block [[app, apq],[conj(apq), aqq]]:
-// J = [[c, se],[-conj(se), c]], se = s e^{i phi}; identity when the pivot is below thr2 (or padding).
-__device__ __forceinline__ bool jacobi_rot(float app, float aqq, float2 apq, float thr2, bool valid, float& c, float2& se) {
-    c = 1.f; se = make_float2(0.f, 0.f);
+// J = [[c, se],[-conj(se), c]], se = s e^{i phi}; identity when the pivot is below thr2 (zero padding too).
+// With d = aqq - app:  t = sgn(d) 2|apq| / (|d| + sqrt(d^2 + 4|apq|^2)),  c = 1/sqrt(1+t^2),  se = apq (t/|apq|) c.
+// Branch-free and written so that |apq| itself is never needed; the approximate rsqrt / rcp keep the
+// dependent chain short.  c^2 + |se|^2 = 1 up to the rounding of one rsqrt, i.e. J is a unitary times
+// (1 + O(eps)); the columns of V are renormalised at the end.
+__device__ __forceinline__ bool jacobi_rot(float app, float aqq, float2 apq, float thr2, float& c, float2& se) {
     const float mag2 = fmaf(apq.x, apq.x, apq.y * apq.y);
-    if (!valid || !(mag2 > thr2)) return false;
-    const float inv_mag = rsqrtf(mag2);
-    const float m2 = 2.f * mag2 * inv_mag;                  // 2|apq|
+    const bool rot = mag2 > thr2;
     const float d = aqq - app;
-    const float t = copysignf(m2, d) / (fabsf(d) + sqrtf(fmaf(d, d, m2 * m2)));   // sgn(tau)/(|tau|+sqrt(1+tau^2))
-    c = rsqrtf(fmaf(t, t, 1.f));
-    const float s = t * c * inv_mag;
-    se = make_float2(apq.x * s, apq.y * s);
-    return true;
+    const float x = fmaxf(fmaf(d, d, 4.f * mag2), 1e-36f);
+    const float root = x * rsqrt_fast(x);
+    const float u = copysignf(2.f, d) * rcp_fast(fabsf(d) + root);      // t / |apq|
+    const float cc = rsqrt_fast(fmaf(u * u, mag2, 1.f));
+    const float uc = rot ? u * cc : 0.f;
+    c = rot ? cc : 1.f;
+    se = make_float2(apq.x * uc, apq.y * uc);
+    return rot;
+}
+
+// position taken in the next step by the row/column now at position pos (round-robin "chairs":
+// top row = even positions, bottom row = odd positions, position 0 fixed)
+__host__ __device__ constexpr int rr_next(int pos, int Tp) {
+    return pos == 0 ? 0 : pos == 1 ? (Tp > 2 ? 2 : 1) : (pos & 1) ? pos - 2 : (pos == Tp - 2 ? Tp - 1 : pos + 2);
 }
 
 template <int TP>
@@ -47,24 +64,30 @@ __global__ void __launch_bounds__((TP / 2) * (TP / 2) < 32 ? 32 : (TP / 2) * (TP
 k_eig(const float2* __restrict__ C, int T, float* __restrict__ evals, float2* __restrict__ Vout,
       int32_t* __restrict__ status, int max_sweeps) {
     extern __shared__ __align__(16) unsigned char raw[];
-    constexpr int Tp = TP, LD = TP + 1, half = TP / 2, m = TP - 1;
+    constexpr int Tp = TP, LD = TP + 2, half = TP / 2, m = TP - 1;   // LD even: rows 16-byte aligned for LDS.128
     float2* A0 = reinterpret_cast<float2*>(raw);
     float2* A1 = A0 + Tp * LD;
-    float2* V = A1 + Tp * LD;
-    float* red = reinterpret_cast<float*>(V + Tp * LD);             // [32]
-    size_t off = (size_t)((unsigned char*)(red + 32) - raw);
-    off = (off + 15) & ~(size_t)15;
-    double* dscr = reinterpret_cast<double*>(raw + off);            // [T*T] partial Rayleigh terms
-    double* lam = dscr + (size_t)T * T;                             // [T]
-    int* rank = reinterpret_cast<int*>(lam + T);                    // [T]
+    float2* V0 = A1 + Tp * LD;
+    float2* V1 = V0 + Tp * LD;
+    float2* Cs = V1 + Tp * LD;                                      // [T][T] full Hermitian copy of the input
+    float* red = reinterpret_cast<float*>(Cs + Tp * Tp);            // [32]
+    double* lam = reinterpret_cast<double*>(red + 32);              // [Tp]
+    double* dscr = reinterpret_cast<double*>(raw);                  // [T*T], aliases A0/A1 after the sweeps
 
     const int tid = threadIdx.x, nt = blockDim.x;
     const long long clk0 = clock64();
 
-    // ---- load: lower triangle of C -> full Hermitian A (scaled by a power of two so that max|diag| <= 1); V = I
+    // ---- load: lower triangle of C -> full Hermitian Cs; A = Cs scaled by a power of two (max|entry| <= 1); V = I
     float dmax = 0.f;
-    for (int i = tid; i < T; i += nt) dmax = fmaxf(dmax, fabsf(C[i * T + i].x));
-    for (int i = tid; i < T * T; i += nt) { const int r = i / T, c = i - r * T; if (c < r) { const float2 a = C[i]; dmax = fmaxf(dmax, fmaxf(fabsf(a.x), fabsf(a.y))); } }
+    for (int i = tid; i < T * T; i += nt) {
+        const int r = i / T, c = i - r * T;
+        float2 a;
+        if (c < r) a = C[i];
+        else if (c > r) { a = C[c * T + r]; a.y = -a.y; }
+        else a = make_float2(C[i].x, 0.f);
+        Cs[i] = a;
+        dmax = fmaxf(dmax, fmaxf(fabsf(a.x), fabsf(a.y)));
+    }
 #pragma unroll
     for (int o = 16; o >= 1; o >>= 1) dmax = fmaxf(dmax, __shfl_xor_sync(0xffffffffu, dmax, o));
     if ((tid & 31) == 0) red[tid >> 5] = dmax;
@@ -74,21 +97,15 @@ k_eig(const float2* __restrict__ C, int T, float* __restrict__ evals, float2* __
     int ex = 0;
     if (dmax > 0.f && dmax < 3.0e38f) frexpf(dmax, &ex);
     const float scale = ldexpf(1.f, -ex);
+    float n2 = 0.f;
     for (int i = tid; i < Tp * Tp; i += nt) {
         const int r = i / Tp, c = i - r * Tp;
         float2 a = make_float2(0.f, 0.f);
-        if (r < T && c < T) {
-            if (c < r) a = C[r * T + c];
-            else if (c > r) { a = C[c * T + r]; a.y = -a.y; }
-            else a = make_float2(C[r * T + r].x, 0.f);
-            a.x *= scale; a.y *= scale;
-        }
+        if (r < T && c < T) { a = Cs[r * T + c]; a.x *= scale; a.y *= scale; }
         A0[r * LD + c] = a;
-        V[r * LD + c] = make_float2(r == c ? 1.f : 0.f, 0.f);
+        V0[r * LD + c] = make_float2(r == c ? 1.f : 0.f, 0.f);
+        n2 = fmaf(a.x, a.x, fmaf(a.y, a.y, n2));
     }
-    __syncthreads();
-    float n2 = 0.f;
-    for (int i = tid; i < Tp * Tp; i += nt) { const float2 a = A0[(i / Tp) * LD + (i % Tp)]; n2 += a.x * a.x + a.y * a.y; }
     const float normF2 = block_sum(n2, red);
     const float eps = 5.96e-8f;
     const float thr2 = (0.25f * eps * eps / (float)(T * T)) * normF2;   // skip pivots below (eps/2T)*||A||_F
@@ -97,32 +114,44 @@ k_eig(const float2* __restrict__ C, int T, float* __restrict__ evals, float2* __
     // one thread per 2x2 block (pair bi, pair bj) of A; the same thread rotates rows 2bi, 2bi+1 of V by J_bj
     const int bi = tid / half, bj = tid % half;
     const bool worker = tid < half * half;
-    float2* Ac = A0;
-    float2* An = A1;
+    const int r0 = 2 * bi, c0 = 2 * bj;
+    const int rd0 = rr_next(r0, Tp), rd1 = rr_next(r0 + 1, Tp), cd0 = rr_next(c0, Tp), cd1 = rr_next(c0 + 1, Tp);
+    // element offsets (fixed for the whole solve)
+    const int oB0 = r0 * LD + c0, oB1 = oB0 + LD;            // block rows (reads, 16-byte vectors)
+    const int oDi = r0 * LD + r0, oDj = c0 * LD + c0;        // pivot blocks of pair i and pair j
+    const int w00 = rd0 * LD + cd0, w01 = rd0 * LD + cd1, w10 = rd1 * LD + cd0, w11 = rd1 * LD + cd1;
+    const int wv00 = r0 * LD + cd0, wv01 = r0 * LD + cd1, wv10 = wv00 + LD, wv11 = wv01 + LD;
+    float2 *Ac = A0, *An = A1, *Vc = V0, *Vn = V1;
     int sweeps = 0, converged = 0, last_rot = 0;
     const long long clk1 = clock64();
     for (; sweeps < max_sweeps; ++sweeps) {
         float o2 = 0.f;
         for (int i = tid; i < Tp * Tp; i += nt) {
             const int r = i / Tp, c = i - r * Tp;
-            if (r != c) { const float2 a = Ac[r * LD + c]; o2 += a.x * a.x + a.y * a.y; }
+            if (r != c) { const float2 a = Ac[r * LD + c]; o2 = fmaf(a.x, a.x, fmaf(a.y, a.y, o2)); }
         }
         const float off2 = block_sum(o2, red);
         if (off2 <= tol2) { converged = 1; break; }
-        int rot_count = 0;
+        int applied = 0;
 #pragma unroll 1
         for (int step = 0; step < m; ++step) {
-            int applied = 0;
             if (worker) {
-                int pi, qi, pj, qj;
-                if (bi == 0) { pi = step; qi = m; } else { const int a = (step + bi) % m, b = (step - bi + m) % m; pi = min(a, b); qi = max(a, b); }
-                if (bj == 0) { pj = step; qj = m; } else { const int a = (step + bj) % m, b = (step - bj + m) % m; pj = min(a, b); qj = max(a, b); }
+                // all shared-memory reads of the step are issued before the first use
+                const float4 di = *reinterpret_cast<const float4*>(Ac + oDi);       // [app, apq]
+                const float aqqi = Ac[oDi + LD + 1].x;
+                const float4 dj = *reinterpret_cast<const float4*>(Ac + oDj);
+                const float aqqj = Ac[oDj + LD + 1].x;
+                const float4 B0 = *reinterpret_cast<const float4*>(Ac + oB0);       // [b00, b01]
+                const float4 B1 = *reinterpret_cast<const float4*>(Ac + oB1);       // [b10, b11]
+                const float4 U0 = *reinterpret_cast<const float4*>(Vc + oB0);       // V rows r0, r0+1, columns c0, c0+1
+                const float4 U1 = *reinterpret_cast<const float4*>(Vc + oB1);
                 float ci, cj; float2 sei, sej;
-                const bool ri = jacobi_rot(Ac[pi * LD + pi].x, Ac[qi * LD + qi].x, Ac[pi * LD + qi], thr2, qi < T, ci, sei);
-                jacobi_rot(Ac[pj * LD + pj].x, Ac[qj * LD + qj].x, Ac[pj * LD + qj], thr2, qj < T, cj, sej);
-                applied = (bi == bj) && ri;
+                const bool ri = jacobi_rot(di.x, aqqi, make_float2(di.z, di.w), thr2, ci, sei);
+                jacobi_rot(dj.x, aqqj, make_float2(dj.z, dj.w), thr2, cj, sej);
+                applied += (bi == bj) && ri;
+                const float2 b00 = make_float2(B0.x, B0.y), b01 = make_float2(B0.z, B0.w);
+                const float2 b10 = make_float2(B1.x, B1.y), b11 = make_float2(B1.z, B1.w);
                 // B' = J_i^H B J_j
-                const float2 b00 = Ac[pi * LD + pj], b01 = Ac[pi * LD + qj], b10 = Ac[qi * LD + pj], b11 = Ac[qi * LD + qj];
                 float2 t1, t2;
                 t1 = cmulcf(b01, sej); t2 = cmulf(b00, sej);
                 const float2 x00 = make_float2(fmaf(cj, b00.x, -t1.x), fmaf(cj, b00.y, -t1.y));
@@ -140,41 +169,56 @@ k_eig(const float2* __restrict__ C, int T, float* __restrict__ evals, float2* __
                     y00.y = 0.f; y11.y = 0.f;
                     if (ri) { y01 = make_float2(0.f, 0.f); y10 = make_float2(0.f, 0.f); }
                 }
-                An[pi * LD + pj] = y00; An[pi * LD + qj] = y01; An[qi * LD + pj] = y10; An[qi * LD + qj] = y11;
-                // V <- V J_j on rows 2bi, 2bi+1 (in place: nobody else touches these elements this step)
-#pragma unroll
-                for (int rr = 0; rr < 2; ++rr) {
-                    const int r = 2 * bi + rr;
-                    const float2 vp = V[r * LD + pj], vq = V[r * LD + qj];
-                    t1 = cmulcf(vq, sej); t2 = cmulf(vp, sej);
-                    V[r * LD + pj] = make_float2(fmaf(cj, vp.x, -t1.x), fmaf(cj, vp.y, -t1.y));
-                    V[r * LD + qj] = make_float2(fmaf(cj, vq.x, t2.x), fmaf(cj, vq.y, t2.y));
-                }
+                An[w00] = y00; An[w01] = y01; An[w10] = y10; An[w11] = y11;
+                // V <- V J_j on rows r0, r0+1
+                const float2 v0p = make_float2(U0.x, U0.y), v0q = make_float2(U0.z, U0.w);
+                const float2 v1p = make_float2(U1.x, U1.y), v1q = make_float2(U1.z, U1.w);
+                t1 = cmulcf(v0q, sej); t2 = cmulf(v0p, sej);
+                Vn[wv00] = make_float2(fmaf(cj, v0p.x, -t1.x), fmaf(cj, v0p.y, -t1.y));
+                Vn[wv01] = make_float2(fmaf(cj, v0q.x, t2.x), fmaf(cj, v0q.y, t2.y));
+                t1 = cmulcf(v1q, sej); t2 = cmulf(v1p, sej);
+                Vn[wv10] = make_float2(fmaf(cj, v1p.x, -t1.x), fmaf(cj, v1p.y, -t1.y));
+                Vn[wv11] = make_float2(fmaf(cj, v1q.x, t2.x), fmaf(cj, v1q.y, t2.y));
             }
-            rot_count += __syncthreads_count(applied);
+            __syncthreads();
             float2* tmp = Ac; Ac = An; An = tmp;
+            tmp = Vc; Vc = Vn; Vn = tmp;
         }
-        last_rot = rot_count;
+        last_rot = (int)(block_sum((float)applied, red) + 0.5f);      // rotations applied in this sweep (<= Tp^2/2: exact)
         if (last_rot == 0) { converged = 1; ++sweeps; break; }
     }
     __syncthreads();
     const long long clk2 = clock64();
+    // m steps of the chair permutation are the identity, so after whole sweeps position == original index
+    const float2* V = Vc;
 
-    // ---- FP64 Rayleigh quotients against the original C (Hermitian from its lower triangle)
-    for (int i = tid; i < T * T; i += nt) {
-        const int t = i / T, k = i - t * T;
-        double wr = 0.0, wi = 0.0;
-        for (int s = 0; s < T; ++s) {
-            float2 cf;
-            if (s < t) cf = C[t * T + s];
-            else if (s > t) { cf = C[s * T + t]; cf.y = -cf.y; }
-            else cf = make_float2(C[t * T + t].x, 0.f);
-            const float2 v = V[s * LD + k];
-            wr += (double)cf.x * v.x - (double)cf.y * v.y;
-            wi += (double)cf.x * v.y + (double)cf.y * v.x;
+    // ---- FP64 Rayleigh quotients against the original C (shared-memory copy), FP32 vectors
+    // (A0/A1 are dead: dscr aliases them; V0/V1/Cs are not touched)
+    // thread = (column k, row group); RB rows of C share every load of v_sk
+    {
+        constexpr int RB = 4;
+        const int k = tid % T, g = tid / T, ng = nt / T > 0 ? nt / T : 1;
+        for (int tb = g * RB; tb < T && tid < ng * T; tb += ng * RB) {
+            double wr[RB], wi[RB];
+#pragma unroll
+            for (int j = 0; j < RB; ++j) { wr[j] = 0.0; wi[j] = 0.0; }
+            for (int s = 0; s < T; ++s) {
+                const float2 v = V[s * LD + k];
+                const double vx = (double)v.x, vy = (double)v.y;
+#pragma unroll
+                for (int j = 0; j < RB; ++j) {
+                    const int t = min(tb + j, T - 1);
+                    const float2 cf = Cs[t * T + s];
+                    wr[j] += (double)cf.x * vx - (double)cf.y * vy;
+                    wi[j] += (double)cf.x * vy + (double)cf.y * vx;
+                }
+            }
+#pragma unroll
+            for (int j = 0; j < RB; ++j) {
+                const int t = tb + j;
+                if (t < T) { const float2 vt = V[t * LD + k]; dscr[t * T + k] = (double)vt.x * wr[j] + (double)vt.y * wi[j]; }   // Re(conj(v_tk) w_tk)
+            }
         }
-        const float2 vt = V[t * LD + k];
-        dscr[i] = (double)vt.x * wr + (double)vt.y * wi;          // Re(conj(v_tk) w_tk)
     }
     __syncthreads();
     if (tid < T) {
@@ -187,7 +231,6 @@ k_eig(const float2* __restrict__ C, int T, float* __restrict__ evals, float2* __
         const double l = lam[tid];
         int r = 0;
         for (int j = 0; j < T; ++j) { const double lj = lam[j]; r += (lj > l) || (lj == l && j < tid); }
-        rank[tid] = r;
         // normalise + canonical phase
         float best = -1.f; float2 bv = make_float2(1.f, 0.f); float nn = 0.f;
         for (int t = 0; t < T; ++t) {
@@ -216,14 +259,13 @@ k_eig(const float2* __restrict__ C, int T, float* __restrict__ evals, float2* __
 template <int TP>
 static int launch_eig_t(holo_ctx* c, const float2* C, float* evals, float2* V, cudaStream_t st) {
     const int T = c->T;
-    constexpr int LD = TP + 1;
-    size_t smem = (size_t)3 * TP * LD * sizeof(float2) + 32 * sizeof(float);
-    smem = (smem + 15) & ~(size_t)15;
-    smem += (size_t)T * T * sizeof(double) + T * sizeof(double) + T * sizeof(int) + 16;
+    constexpr int LD = TP + 2;
+    // A0, A1, V0, V1 [TP][LD] + Cs [TP][TP] float2, red[32] float, lam[TP] double
+    constexpr size_t smem = (size_t)4 * TP * LD * sizeof(float2) + (size_t)TP * TP * sizeof(float2) + 32 * sizeof(float)
+                          + TP * sizeof(double);
     static bool attr = false;
     if (!attr) {
-        const size_t worst = (size_t)3 * TP * LD * sizeof(float2) + 256 + (size_t)TP * TP * 8 + TP * 12 + 32;
-        HOLO_CUDA_OK(cudaFuncSetAttribute(k_eig<TP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)worst));
+        HOLO_CUDA_OK(cudaFuncSetAttribute(k_eig<TP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         attr = true;
     }
     constexpr int threads = (TP / 2) * (TP / 2) < 32 ? 32 : (TP / 2) * (TP / 2);
