@@ -1,114 +1,217 @@
 // covariance.cu -- A3: C = H^{t*} H, C_ts = sum_p conj(H_t(p)) H_s(p)   (Eq. 4; R9)
 //
-// FP32 FFMA Gram of a tall-skinny matrix (N_p x T, T <= 64).  The Hermitian lower half of C is cut
-// into 8x8 complex blocks ("jobs"); one warp owns one job and keeps its 64 complex accumulators in
-// registers; the 32 lanes split the pixels of a staged chunk (shared memory, cp.async double
-// buffer), so the only reduction is a once-per-CTA shuffle tree.  Each CTA writes one partial;
-// a second kernel sums the partials in a FIXED order in FP64 (deterministic, bit-identical runs).
+// FP32 FFMA Gram of a tall-skinny matrix (N_p x T, T <= 64); FP32-ALU bound at T >= 32.
+// The Hermitian lower half of C is cut into 8x8 complex blocks.  One warp owns either one off-diagonal
+// block (64 complex accumulators) or a PAIR of diagonal blocks (2 x 36 entries, real diagonal): both cost
+// 256 FFMA per pixel, so the eight consumer warps of a CTA (two per SM sub-partition) are exactly balanced
+// and no redundant upper-triangle work is done.  The 32 lanes of a warp split the pixels of a staged
+// chunk, so the only reduction is a once-per-CTA shuffle tree.  Warp 0 doubles as the producer: before
+// each of its chunks it streams the chunk NS-2 ahead into a multi-stage shared-memory ring with 2-D TMA
+// tensor copies (cp.async.bulk.tensor.2d + mbarrier complete_tx; one [8 rows x 128 pixels] box per row
+// block -- 1-D bulk copies of single 1 KB rows were measured TMA-issue bound at 1.5 TB/s); rows t >= T of
+// the last row block are zero-filled by the TMA unit (out-of-bounds fill).  The warps release a stage with
+// one mbarrier arrive each: no __syncthreads and no per-thread copy loops in the steady state
+// (256 threads, so every thread may hold the full 255 registers).
+// Each CTA writes one partial; a second kernel sums the partials in a FIXED order in FP64
+// (deterministic, bit-identical runs).  For T > 32 the blocks are split over gridDim.y CTA groups, each
+// staging only the row blocks its jobs touch.
 #include "holo_internal.cuh"
+#include <string.h>
+#include <cuda.h>
 
-#define COV_P 128            // pixels per staged chunk
-#define COV_MAXW 10          // jobs (warps) per CTA
+#define COV_P 128            // pixels per stage (1 KB per row)
+#define COV_NW 8             // consumer warps per CTA
+#define COV_MAX_SLOTS 8      // row blocks (of 8 rows) staged per CTA group
+#define COV_MAX_GROUPS 4
+#define COV_MAX_STAGES 8
+#define COV_SMEM_BUDGET (200 * 1024)
 
-__device__ __forceinline__ void cp_async16(void* smem, const void* gmem) {
-    unsigned s = (unsigned)__cvta_generic_to_shared(smem);
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(s), "l"(gmem));
+struct CovJob {              // one consumer warp
+    int kind;                // 0 idle, 1 off-diagonal block (ra > rb), 2 pair of diagonal blocks (rb < 0: single)
+    int sa, sb;              // stage slots of the two row blocks
+    int ra, rb;              // global row-block indexes (output position)
+};
+struct CovGroup {
+    int nslots, njobs;
+    int rowblk[COV_MAX_SLOTS];
+    CovJob job[COV_NW];
+};
+struct CovPlan {
+    int ngroups;
+    CovGroup g[COV_MAX_GROUPS];
+};
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
 }
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::); }
-template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N)); }
-
-// job index -> (block row bi, block col bj), bj <= bi, row-major over the lower triangle
-__device__ __forceinline__ void job_to_blocks(int job, int& bi, int& bj) {
-    bi = 0;
-    while ((bi + 1) * (bi + 2) / 2 <= job) ++bi;
-    bj = job - bi * (bi + 1) / 2;
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+    const uint32_t a = smem_u32(bar);
+    uint32_t ok;
+    do {
+        asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                     : "=r"(ok) : "r"(a), "r"(parity) : "memory");
+    } while (!ok);
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t* bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void tma_2d_g2s(void* dst_smem, const CUtensorMap* tm, int c0, int c1, uint64_t* bar) {
+    asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
+                 ::"r"(smem_u32(dst_smem)), "l"(tm), "r"(c0), "r"(c1), "r"(smem_u32(bar)) : "memory");
 }
 
-// partials layout: [part][T8][T8] float2 (T8 = T rounded up to 8), only blocks bj <= bi are written
-template <int T8>
-__global__ void __launch_bounds__(COV_MAXW * 32, 1)
-k_cov_partial(const float2* __restrict__ H, float2* __restrict__ partials, long long npix, int T,
-              int njobs, int jobs_per_cta) {
-    extern __shared__ __align__(16) float2 smem[];          // [2][T8][COV_P]
+__device__ __forceinline__ float warp_sum(float x) {
+#pragma unroll
+    for (int o = 16; o >= 1; o >>= 1) x += __shfl_xor_sync(0xffffffffu, x, o);
+    return x;
+}
+
+// acc += conj(a) * b
+__device__ __forceinline__ void cmac_conj(float2& acc, const float2 a, const float2 b) {
+    acc.x = fmaf(a.x, b.x, acc.x);
+    acc.x = fmaf(a.y, b.y, acc.x);
+    acc.y = fmaf(a.x, b.y, acc.y);
+    acc.y = fmaf(-a.y, b.x, acc.y);
+}
+
+// partials layout: [part][T8][T8] float2 (T8 = T rounded up to 8), only entries s <= t are written
+__global__ void __launch_bounds__(COV_NW * 32, 1)
+k_cov_partial(const __grid_constant__ CUtensorMap tmH, float2* __restrict__ partials, long long npix, int T, int T8,
+              int nstages, const CovPlan plan) {
+    extern __shared__ __align__(128) unsigned char smraw[];
+    uint64_t* full = reinterpret_cast<uint64_t*>(smraw);
+    uint64_t* empty = full + COV_MAX_STAGES;
+    float2* ring = reinterpret_cast<float2*>(smraw + 128);
+    const CovGroup& g = plan.g[blockIdx.y];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int nthreads = blockDim.x;
-    const int job = blockIdx.y * jobs_per_cta + warp;
-    const bool active = (warp < jobs_per_cta) && (job < njobs);
-    int bi = 0, bj = 0;
-    if (active) job_to_blocks(job, bi, bj);
-
-    // zero the padding rows t >= T of both buffers once
-    for (int i = tid; i < 2 * T8 * COV_P; i += nthreads) {
-        int row = (i / COV_P) % T8;
-        if (row >= T) smem[i] = make_float2(0.f, 0.f);
-    }
+    const int nslots = g.nslots;
+    const int stage_elems = nslots * 8 * COV_P;
     const long long nchunks = npix / COV_P;
-    const int vec_per_row = COV_P / 2;                       // 16-byte pieces per row
-    auto stage = [&](int buf, long long chunk) {
-        float2* dst = smem + (size_t)buf * T8 * COV_P;
-        const float2* src = H + chunk * COV_P;
-        for (int i = tid; i < T * vec_per_row; i += nthreads) {
-            int t = i / vec_per_row, v = i - t * vec_per_row;
-            cp_async16(dst + t * COV_P + 2 * v, src + (long long)t * npix + 2 * v);
-        }
+
+    if (tid == 0) {
+        for (int s = 0; s < nstages; ++s) { mbar_init(full + s, 1); mbar_init(empty + s, (uint32_t)g.njobs); }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+
+    // ---------------------------------------------------- producer state (used by warp 0 only)
+    int ps = 0; uint32_t pph = 0;
+    long long pchunk = blockIdx.x;
+    auto issue = [&]() {
+        if (pchunk >= nchunks) return;
+        mbar_wait(empty + ps, pph ^ 1u);
+        if (lane == 0) mbar_arrive_expect_tx(full + ps, (uint32_t)stage_elems * (uint32_t)sizeof(float2));
+        __syncwarp();
+        if (lane < nslots)      // one [8 rows x COV_P pixels] box per row block; coordinates in floats / rows
+            tma_2d_g2s(ring + (size_t)ps * stage_elems + lane * 8 * COV_P, &tmH, (int)(pchunk * (2 * COV_P)), 8 * g.rowblk[lane], full + ps);
+        pchunk += gridDim.x;
+        if (++ps == nstages) { ps = 0; pph ^= 1u; }
     };
-
-    float2 acc[8][8];
+    if (warp == 0)
+        for (int d = 0; d < nstages - 2; ++d) issue();
+    // ---------------------------------------------------- consumer warps
+    const CovJob job = g.job[warp];
+    if (job.kind == 0) return;
+    float2* out = partials + (size_t)blockIdx.x * T8 * T8;
+    int s = 0; uint32_t ph = 0;
+    if (job.kind == 1) {
+        float2 acc[8][8];
 #pragma unroll
-    for (int i = 0; i < 8; ++i)
+        for (int i = 0; i < 8; ++i)
 #pragma unroll
-        for (int j = 0; j < 8; ++j) acc[i][j] = make_float2(0.f, 0.f);
-
-    long long chunk = blockIdx.x;
-    int buf = 0;
-    if (chunk < nchunks) stage(0, chunk);
-    cp_async_commit();
-    for (; chunk < nchunks; chunk += gridDim.x) {
-        long long next = chunk + gridDim.x;
-        if (next < nchunks) stage(buf ^ 1, next);
-        cp_async_commit();
-        cp_async_wait<1>();
-        __syncthreads();
-        if (active) {
-            const float2* A = smem + (size_t)buf * T8 * COV_P + (bi * 8) * COV_P;
-            const float2* Bm = smem + (size_t)buf * T8 * COV_P + (bj * 8) * COV_P;
-#pragma unroll 2
-            for (int pp = 0; pp < COV_P / 32; ++pp) {
-                const int p = pp * 32 + lane;
-                float2 a[8], b[8];
+            for (int j = 0; j < 8; ++j) acc[i][j] = make_float2(0.f, 0.f);
+        for (long long chunk = blockIdx.x; chunk < nchunks; chunk += gridDim.x) {
+            if (warp == 0) issue();
+            mbar_wait(full + s, ph);
+            const float4* A = reinterpret_cast<const float4*>(ring + (size_t)s * stage_elems + job.sa * 8 * COV_P) + lane;
+            const float4* B = reinterpret_cast<const float4*>(ring + (size_t)s * stage_elems + job.sb * 8 * COV_P) + lane;
 #pragma unroll
-                for (int i = 0; i < 8; ++i) a[i] = A[i * COV_P + p];
+            for (int it = 0; it < COV_P / 64; ++it) {                 // 2 adjacent pixels per lane per load
+                float4 a[8], b[8];
 #pragma unroll
-                for (int j = 0; j < 8; ++j) b[j] = Bm[j * COV_P + p];
+                for (int i = 0; i < 8; ++i) a[i] = A[i * (COV_P / 2) + it * 32];
+#pragma unroll
+                for (int j = 0; j < 8; ++j) b[j] = B[j * (COV_P / 2) + it * 32];
 #pragma unroll
                 for (int i = 0; i < 8; ++i)
 #pragma unroll
-                    for (int j = 0; j < 8; ++j) {            // acc += conj(a_i) * b_j
-                        acc[i][j].x = fmaf(a[i].x, b[j].x, acc[i][j].x);
-                        acc[i][j].x = fmaf(a[i].y, b[j].y, acc[i][j].x);
-                        acc[i][j].y = fmaf(a[i].x, b[j].y, acc[i][j].y);
-                        acc[i][j].y = fmaf(-a[i].y, b[j].x, acc[i][j].y);
+                    for (int j = 0; j < 8; ++j) {
+                        cmac_conj(acc[i][j], make_float2(a[i].x, a[i].y), make_float2(b[j].x, b[j].y));
+                        cmac_conj(acc[i][j], make_float2(a[i].z, a[i].w), make_float2(b[j].z, b[j].w));
                     }
             }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(empty + s);
+            if (++s == nstages) { s = 0; ph ^= 1u; }
         }
-        __syncthreads();
-        buf ^= 1;
-    }
-    cp_async_wait<0>();
-    if (active) {
-        float2* out = partials + (size_t)blockIdx.x * T8 * T8;
 #pragma unroll
         for (int i = 0; i < 8; ++i)
 #pragma unroll
             for (int j = 0; j < 8; ++j) {
-                float x = acc[i][j].x, y = acc[i][j].y;
-#pragma unroll
-                for (int o = 16; o >= 1; o >>= 1) {
-                    x += __shfl_xor_sync(0xffffffffu, x, o);
-                    y += __shfl_xor_sync(0xffffffffu, y, o);
-                }
-                if (lane == 0) out[(bi * 8 + i) * T8 + (bj * 8 + j)] = make_float2(x, y);
+                const float x = warp_sum(acc[i][j].x), y = warp_sum(acc[i][j].y);
+                if (lane == 0) out[(job.ra * 8 + i) * T8 + (job.rb * 8 + j)] = make_float2(x, y);
             }
+    } else {
+        // two diagonal blocks: entries i > j complex, i == j real
+        float2 lo[2][28];
+        float dg[2][8];
+#pragma unroll
+        for (int d = 0; d < 2; ++d) {
+#pragma unroll
+            for (int e = 0; e < 28; ++e) lo[d][e] = make_float2(0.f, 0.f);
+#pragma unroll
+            for (int i = 0; i < 8; ++i) dg[d][i] = 0.f;
+        }
+        const bool two = job.rb >= 0;
+        for (long long chunk = blockIdx.x; chunk < nchunks; chunk += gridDim.x) {
+            if (warp == 0) issue();
+            mbar_wait(full + s, ph);
+#pragma unroll
+            for (int d = 0; d < 2; ++d) {
+                if (d == 1 && !two) continue;
+                const float4* A = reinterpret_cast<const float4*>(ring + (size_t)s * stage_elems + (d == 0 ? job.sa : job.sb) * 8 * COV_P) + lane;
+#pragma unroll
+                for (int it = 0; it < COV_P / 64; ++it) {
+                    float4 a[8];
+#pragma unroll
+                    for (int i = 0; i < 8; ++i) a[i] = A[i * (COV_P / 2) + it * 32];
+#pragma unroll
+                    for (int i = 0; i < 8; ++i) {
+                        dg[d][i] = fmaf(a[i].x, a[i].x, dg[d][i]);
+                        dg[d][i] = fmaf(a[i].y, a[i].y, dg[d][i]);
+                        dg[d][i] = fmaf(a[i].z, a[i].z, dg[d][i]);
+                        dg[d][i] = fmaf(a[i].w, a[i].w, dg[d][i]);
+#pragma unroll
+                        for (int j = 0; j < i; ++j) {
+                            cmac_conj(lo[d][i * (i - 1) / 2 + j], make_float2(a[i].x, a[i].y), make_float2(a[j].x, a[j].y));
+                            cmac_conj(lo[d][i * (i - 1) / 2 + j], make_float2(a[i].z, a[i].w), make_float2(a[j].z, a[j].w));
+                        }
+                    }
+                }
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(empty + s);
+            if (++s == nstages) { s = 0; ph ^= 1u; }
+        }
+#pragma unroll
+        for (int d = 0; d < 2; ++d) {
+            if (d == 1 && !two) continue;
+            const int r = (d == 0 ? job.ra : job.rb) * 8;
+#pragma unroll
+            for (int i = 0; i < 8; ++i) {
+                const float x = warp_sum(dg[d][i]);
+                if (lane == 0) out[(r + i) * T8 + (r + i)] = make_float2(x, 0.f);
+#pragma unroll
+                for (int j = 0; j < i; ++j) {
+                    const float lx = warp_sum(lo[d][i * (i - 1) / 2 + j].x), ly = warp_sum(lo[d][i * (i - 1) / 2 + j].y);
+                    if (lane == 0) out[(r + i) * T8 + (r + j)] = make_float2(lx, ly);
+                }
+            }
+        }
     }
 }
 
@@ -142,46 +245,96 @@ __global__ void __launch_bounds__(256) k_cov_reduce(const float2* __restrict__ p
     }
 }
 
-template <int T8>
-static int launch_cov_t(holo_ctx* c, const float2* H, float2* C, cudaStream_t st) {
-    const int nb = T8 / 8, njobs = nb * (nb + 1) / 2;
-    const int jobs_per_cta = njobs < COV_MAXW ? njobs : (njobs == 36 ? 9 : COV_MAXW);
-    const int gy = (njobs + jobs_per_cta - 1) / jobs_per_cta;
-    const size_t smem = (size_t)2 * T8 * COV_P * sizeof(float2);
-    auto kern = k_cov_partial<T8>;
-    static bool attr = false;
-    if (!attr) {
-        HOLO_CUDA_OK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        attr = true;
+// ---- host: split the block lower triangle into CTA groups of <= COV_NW warp jobs
+static int slot_of(CovGroup& g, int rb) {
+    for (int k = 0; k < g.nslots; ++k) if (g.rowblk[k] == rb) return k;
+    g.rowblk[g.nslots] = rb;
+    return g.nslots++;
+}
+static void add_off(CovGroup& g, int bi, int bj) {
+    CovJob& j = g.job[g.njobs++];
+    j.kind = 1; j.ra = bi; j.rb = bj; j.sa = slot_of(g, bi); j.sb = slot_of(g, bj);
+}
+static void add_diag(CovGroup& g, int b0, int b1) {
+    CovJob& j = g.job[g.njobs++];
+    j.kind = 2; j.ra = b0; j.rb = b1; j.sa = slot_of(g, b0); j.sb = b1 >= 0 ? slot_of(g, b1) : 0;
+}
+// all jobs inside the row-block range [lo, hi) (hi - lo <= 4): <= 6 off-diagonal + 2 diagonal pairs
+static void add_triangle(CovGroup& g, int lo, int hi) {
+    for (int bi = lo; bi < hi; ++bi)
+        for (int bj = lo; bj < bi; ++bj) add_off(g, bi, bj);
+    for (int b = lo; b < hi; b += 2) add_diag(g, b, b + 1 < hi ? b + 1 : -1);
+}
+static void make_plan(int nb, CovPlan* p) {
+    memset(p, 0, sizeof(*p));
+    if (nb <= 4) { p->ngroups = 1; add_triangle(p->g[0], 0, nb); return; }
+    // nb in 5..8: A = [0,4), B = [4,nb): triangle(A), triangle(B), rectangle B x A in strips of two block rows
+    add_triangle(p->g[0], 0, 4);
+    add_triangle(p->g[1], 4, nb);
+    p->ngroups = 2;
+    for (int b0 = 4; b0 < nb; b0 += 2) {
+        CovGroup& g = p->g[p->ngroups++];
+        for (int bi = b0; bi < b0 + 2 && bi < nb; ++bi)
+            for (int bj = 0; bj < 4; ++bj) add_off(g, bi, bj);
     }
-    long long nchunks = c->npix / COV_P;
-    int gx = c->tune[HOLO_TUNE_COV_GRIDX];
-    if (gx > c->cov_parts_cap) gx = c->cov_parts_cap;
-    if ((long long)gx > nchunks) gx = (int)nchunks;
-    {
-        HoloProf prof(c, HOLO_K_COV_PARTIAL, st);
-        kern<<<dim3(gx, gy), jobs_per_cta * 32, smem, st>>>(H, c->cov_partials, c->npix, c->T, njobs, jobs_per_cta);
+}
+
+// H viewed as a 2-D float tensor [T rows][2*npix floats]; box = [8 rows][2*COV_P floats]
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+static int make_tensor_map(CUtensorMap* tm, const float2* H, long long npix, int T) {
+    static EncodeTiledFn encode = nullptr;
+    if (!encode) {
+        void* fn = nullptr;
+        cudaDriverEntryPointQueryResult qres;
+        HOLO_CUDA_OK(cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres));
+        if (!fn || qres != cudaDriverEntryPointSuccess) { holo_set_error("cuTensorMapEncodeTiled not available"); return HOLO_ERR_CUDA; }
+        encode = (EncodeTiledFn)fn;
     }
-    HOLO_CUDA_OK(cudaGetLastError());
-    int n = c->T * c->T;
-    HoloProf prof(c, HOLO_K_COV_REDUCE, st);
-    k_cov_reduce<<<(n * 32 + 255) / 256, 256, 0, st>>>(c->cov_partials, gx, c->T, T8, C);
-    HOLO_CUDA_OK(cudaGetLastError());
+    const cuuint64_t gdim[2] = {(cuuint64_t)(2 * npix), (cuuint64_t)T};
+    const cuuint64_t gstr[1] = {(cuuint64_t)npix * sizeof(float2)};
+    const cuuint32_t box[2] = {2 * COV_P, 8};
+    const cuuint32_t estr[2] = {1, 1};
+    const CUresult r = encode(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, const_cast<float2*>(H), gdim, gstr, box, estr,
+                              CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                              CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) { holo_set_error("cuTensorMapEncodeTiled failed (%d)", (int)r); return HOLO_ERR_CUDA; }
     return HOLO_OK;
 }
 
 int holo_launch_covariance(holo_ctx* c, const float2* H, float2* C, cudaStream_t st) {
-    const int T8 = (c->T + 7) / 8 * 8;
-    switch (T8) {
-        case 8:  return launch_cov_t<8>(c, H, C, st);
-        case 16: return launch_cov_t<16>(c, H, C, st);
-        case 24: return launch_cov_t<24>(c, H, C, st);
-        case 32: return launch_cov_t<32>(c, H, C, st);
-        case 40: return launch_cov_t<40>(c, H, C, st);
-        case 48: return launch_cov_t<48>(c, H, C, st);
-        case 56: return launch_cov_t<56>(c, H, C, st);
-        case 64: return launch_cov_t<64>(c, H, C, st);
+    const int T = c->T, T8 = (T + 7) / 8 * 8, nb = T8 / 8;
+    if (nb < 1 || nb > 8) { holo_set_error("T out of range"); return HOLO_ERR_ARG; }
+    CovPlan plan;
+    make_plan(nb, &plan);
+    int max_slots = 0;
+    for (int k = 0; k < plan.ngroups; ++k) max_slots = plan.g[k].nslots > max_slots ? plan.g[k].nslots : max_slots;
+    const size_t stage_bytes = (size_t)max_slots * 8 * COV_P * sizeof(float2);
+    int nstages = (int)(COV_SMEM_BUDGET / stage_bytes);
+    if (nstages > COV_MAX_STAGES) nstages = COV_MAX_STAGES;
+    if (nstages < 3) { holo_set_error("covariance stage ring does not fit"); return HOLO_ERR_STATE; }
+    const size_t smem = 128 + (size_t)nstages * stage_bytes;
+    static bool attr = false;
+    if (!attr) {
+        HOLO_CUDA_OK(cudaFuncSetAttribute(k_cov_partial, cudaFuncAttributeMaxDynamicSharedMemorySize, COV_SMEM_BUDGET + 128));
+        attr = true;
     }
-    holo_set_error("T out of range");
-    return HOLO_ERR_ARG;
+    const long long nchunks = c->npix / COV_P;
+    int gx = c->tune[HOLO_TUNE_COV_GRIDX] / plan.ngroups;          // all CTAs co-resident: one per SM
+    if (gx < 1) gx = 1;
+    if (gx > c->cov_parts_cap) gx = c->cov_parts_cap;
+    if ((long long)gx > nchunks) gx = (int)nchunks;
+    alignas(64) CUtensorMap tmH;
+    { const int rc = make_tensor_map(&tmH, H, c->npix, T); if (rc) return rc; }
+    {
+        HoloProf prof(c, HOLO_K_COV_PARTIAL, st);
+        k_cov_partial<<<dim3(gx, plan.ngroups), COV_NW * 32, smem, st>>>(tmH, c->cov_partials, c->npix, T, T8, nstages, plan);
+    }
+    HOLO_CUDA_OK(cudaGetLastError());
+    const int n = T * T;
+    HoloProf prof(c, HOLO_K_COV_REDUCE, st);
+    k_cov_reduce<<<(n * 32 + 255) / 256, 256, 0, st>>>(c->cov_partials, gx, T, T8, C);
+    HOLO_CUDA_OK(cudaGetLastError());
+    return HOLO_OK;
 }
