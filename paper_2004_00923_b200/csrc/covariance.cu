@@ -70,13 +70,31 @@ __device__ __forceinline__ float warp_sum(float x) {
     return x;
 }
 
-// acc += conj(a) * b
-__device__ __forceinline__ void cmac_conj(float2& acc, const float2 a, const float2 b) {
-    acc.x = fmaf(a.x, b.x, acc.x);
-    acc.x = fmaf(a.y, b.y, acc.x);
-    acc.y = fmaf(a.x, b.y, acc.y);
-    acc.y = fmaf(-a.y, b.x, acc.y);
+#ifndef COV_SCALAR
+#define COV_SCALAR 1
+#endif
+#if COV_SCALAR
+typedef float2 pair_t;
+__device__ __forceinline__ pair_t pack2(float lo, float hi) { return make_float2(lo, hi); }
+__device__ __forceinline__ void unpack2(pair_t v, float& lo, float& hi) { lo = v.x; hi = v.y; }
+__device__ __forceinline__ void ffma2(pair_t& acc, pair_t a, pair_t b) { acc.x = fmaf(a.x, b.x, acc.x); acc.y = fmaf(a.y, b.y, acc.y); }
+__device__ __forceinline__ pair_t pzero() { return make_float2(0.f, 0.f); }
+#else
+typedef unsigned long long pair_t;
+__device__ __forceinline__ pair_t pzero() { return 0ull; }
+__device__ __forceinline__ unsigned long long pack2(float lo, float hi) {
+    unsigned long long r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+    return r;
 }
+__device__ __forceinline__ void unpack2(unsigned long long v, float& lo, float& hi) {
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+}
+// acc = a * b + acc on both FP32 halves (IEEE round-to-nearest each)
+__device__ __forceinline__ void ffma2(unsigned long long& acc, unsigned long long a, unsigned long long b) {
+    asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(acc) : "l"(a), "l"(b));
+}
+#endif
 
 // partials layout: [part][T8][T8] float2 (T8 = T rounded up to 8), only entries s <= t are written
 __global__ void __launch_bounds__(COV_NW * 32, 1)
@@ -114,35 +132,36 @@ k_cov_partial(const __grid_constant__ CUtensorMap tmH, float2* __restrict__ part
     if (warp == 0)
         for (int d = 0; d < nstages - 2; ++d) issue();
     // ---------------------------------------------------- consumer warps
-    const CovJob job = g.job[warp];
+    // One pixel per lane per trip: 16 LDS.64 + 256 FFMA, a 4.5 KB loop body.  An accumulator is the pair
+    // (re, im);  acc += conj(a) b  =  (ax,ax)*(bx,by) + (ay,-ay)*(by,bx)  (pair_t / ffma2 below).
+    // Measured alternatives (profiles/r01c.md): two pixels per trip with LDS.128 (same speed, twice the code),
+    // the packed fma.rn.f32x2 form (COV_SCALAR 0: 16 % slower -- the operand-pair moves land on the FMA pipe).
+    const CovJob job = g.job[warp];      // make_plan orders the jobs so that one SM sub-partition (warp & 3) runs one kind
     if (job.kind == 0) return;
     float2* out = partials + (size_t)blockIdx.x * T8 * T8;
     int s = 0; uint32_t ph = 0;
     if (job.kind == 1) {
-        float2 acc[8][8];
+        pair_t acc[8][8];
 #pragma unroll
         for (int i = 0; i < 8; ++i)
 #pragma unroll
-            for (int j = 0; j < 8; ++j) acc[i][j] = make_float2(0.f, 0.f);
+            for (int j = 0; j < 8; ++j) acc[i][j] = pzero();
         for (long long chunk = blockIdx.x; chunk < nchunks; chunk += gridDim.x) {
             if (warp == 0) issue();
             mbar_wait(full + s, ph);
-            const float4* A = reinterpret_cast<const float4*>(ring + (size_t)s * stage_elems + job.sa * 8 * COV_P) + lane;
-            const float4* B = reinterpret_cast<const float4*>(ring + (size_t)s * stage_elems + job.sb * 8 * COV_P) + lane;
+            const float2* A = ring + (size_t)s * stage_elems + job.sa * 8 * COV_P + lane;
+            const float2* B = ring + (size_t)s * stage_elems + job.sb * 8 * COV_P + lane;
+#pragma unroll 1
+            for (int it = 0; it < COV_P / 32; ++it) {
+                pair_t a1[8], a2[8], b1[8], b2[8];
 #pragma unroll
-            for (int it = 0; it < COV_P / 64; ++it) {                 // 2 adjacent pixels per lane per load
-                float4 a[8], b[8];
+                for (int i = 0; i < 8; ++i) { const float2 a = A[i * COV_P + it * 32]; a1[i] = pack2(a.x, a.x); a2[i] = pack2(a.y, -a.y); }
 #pragma unroll
-                for (int i = 0; i < 8; ++i) a[i] = A[i * (COV_P / 2) + it * 32];
-#pragma unroll
-                for (int j = 0; j < 8; ++j) b[j] = B[j * (COV_P / 2) + it * 32];
+                for (int j = 0; j < 8; ++j) { const float2 b = B[j * COV_P + it * 32]; b1[j] = pack2(b.x, b.y); b2[j] = pack2(b.y, b.x); }
 #pragma unroll
                 for (int i = 0; i < 8; ++i)
 #pragma unroll
-                    for (int j = 0; j < 8; ++j) {
-                        cmac_conj(acc[i][j], make_float2(a[i].x, a[i].y), make_float2(b[j].x, b[j].y));
-                        cmac_conj(acc[i][j], make_float2(a[i].z, a[i].w), make_float2(b[j].z, b[j].w));
-                    }
+                    for (int j = 0; j < 8; ++j) { ffma2(acc[i][j], a1[i], b1[j]); ffma2(acc[i][j], a2[i], b2[j]); }
             }
             __syncwarp();
             if (lane == 0) mbar_arrive(empty + s);
@@ -152,44 +171,44 @@ k_cov_partial(const __grid_constant__ CUtensorMap tmH, float2* __restrict__ part
         for (int i = 0; i < 8; ++i)
 #pragma unroll
             for (int j = 0; j < 8; ++j) {
-                const float x = warp_sum(acc[i][j].x), y = warp_sum(acc[i][j].y);
+                float x, y;
+                unpack2(acc[i][j], x, y);
+                x = warp_sum(x); y = warp_sum(y);
                 if (lane == 0) out[(job.ra * 8 + i) * T8 + (job.rb * 8 + j)] = make_float2(x, y);
             }
     } else {
-        // two diagonal blocks: entries i > j complex, i == j real
-        float2 lo[2][28];
-        float dg[2][8];
+        // two diagonal blocks: entries i > j complex; i == j real, accumulated as the pair (sum ax^2, sum ay^2)
+        pair_t lo[2][28], dg[2][8];
 #pragma unroll
         for (int d = 0; d < 2; ++d) {
 #pragma unroll
-            for (int e = 0; e < 28; ++e) lo[d][e] = make_float2(0.f, 0.f);
+            for (int e = 0; e < 28; ++e) lo[d][e] = pzero();
 #pragma unroll
-            for (int i = 0; i < 8; ++i) dg[d][i] = 0.f;
+            for (int i = 0; i < 8; ++i) dg[d][i] = pzero();
         }
         const bool two = job.rb >= 0;
         for (long long chunk = blockIdx.x; chunk < nchunks; chunk += gridDim.x) {
             if (warp == 0) issue();
             mbar_wait(full + s, ph);
+            const float2* A0 = ring + (size_t)s * stage_elems + job.sa * 8 * COV_P + lane;
+            const float2* A1 = ring + (size_t)s * stage_elems + job.sb * 8 * COV_P + lane;
+#pragma unroll 1
+            for (int it = 0; it < COV_P / 32; ++it) {
 #pragma unroll
-            for (int d = 0; d < 2; ++d) {
-                if (d == 1 && !two) continue;
-                const float4* A = reinterpret_cast<const float4*>(ring + (size_t)s * stage_elems + (d == 0 ? job.sa : job.sb) * 8 * COV_P) + lane;
-#pragma unroll
-                for (int it = 0; it < COV_P / 64; ++it) {
-                    float4 a[8];
-#pragma unroll
-                    for (int i = 0; i < 8; ++i) a[i] = A[i * (COV_P / 2) + it * 32];
+                for (int d = 0; d < 2; ++d) {
+                    if (d == 1 && !two) continue;
+                    const float2* A = d == 0 ? A0 : A1;
+                    pair_t a1[8], a2[8], b1[8], b2[8];
 #pragma unroll
                     for (int i = 0; i < 8; ++i) {
-                        dg[d][i] = fmaf(a[i].x, a[i].x, dg[d][i]);
-                        dg[d][i] = fmaf(a[i].y, a[i].y, dg[d][i]);
-                        dg[d][i] = fmaf(a[i].z, a[i].z, dg[d][i]);
-                        dg[d][i] = fmaf(a[i].w, a[i].w, dg[d][i]);
+                        const float2 a = A[i * COV_P + it * 32];
+                        a1[i] = pack2(a.x, a.x); a2[i] = pack2(a.y, -a.y); b1[i] = pack2(a.x, a.y); b2[i] = pack2(a.y, a.x);
+                    }
 #pragma unroll
-                        for (int j = 0; j < i; ++j) {
-                            cmac_conj(lo[d][i * (i - 1) / 2 + j], make_float2(a[i].x, a[i].y), make_float2(a[j].x, a[j].y));
-                            cmac_conj(lo[d][i * (i - 1) / 2 + j], make_float2(a[i].z, a[i].w), make_float2(a[j].z, a[j].w));
-                        }
+                    for (int i = 0; i < 8; ++i) {
+                        ffma2(dg[d][i], b1[i], b1[i]);
+#pragma unroll
+                        for (int j = 0; j < i; ++j) { ffma2(lo[d][i * (i - 1) / 2 + j], a1[i], b1[j]); ffma2(lo[d][i * (i - 1) / 2 + j], a2[i], b2[j]); }
                     }
                 }
             }
@@ -203,12 +222,15 @@ k_cov_partial(const __grid_constant__ CUtensorMap tmH, float2* __restrict__ part
             const int r = (d == 0 ? job.ra : job.rb) * 8;
 #pragma unroll
             for (int i = 0; i < 8; ++i) {
-                const float x = warp_sum(dg[d][i]);
+                float x, y;
+                unpack2(dg[d][i], x, y);
+                x = warp_sum(x + y);
                 if (lane == 0) out[(r + i) * T8 + (r + i)] = make_float2(x, 0.f);
 #pragma unroll
                 for (int j = 0; j < i; ++j) {
-                    const float lx = warp_sum(lo[d][i * (i - 1) / 2 + j].x), ly = warp_sum(lo[d][i * (i - 1) / 2 + j].y);
-                    if (lane == 0) out[(r + i) * T8 + (r + j)] = make_float2(lx, ly);
+                    unpack2(lo[d][i * (i - 1) / 2 + j], x, y);
+                    x = warp_sum(x); y = warp_sum(y);
+                    if (lane == 0) out[(r + i) * T8 + (r + j)] = make_float2(x, y);
                 }
             }
         }
@@ -265,7 +287,24 @@ static void add_triangle(CovGroup& g, int lo, int hi) {
         for (int bj = lo; bj < bi; ++bj) add_off(g, bi, bj);
     for (int b = lo; b < hi; b += 2) add_diag(g, b, b + 1 < hi ? b + 1 : -1);
 }
+// warps w and w+4 share an SM sub-partition: put the diagonal-pair jobs on sub-partition 3 so that every
+// sub-partition runs a single loop body (instruction-cache footprint)
+static void order_jobs(CovGroup& g) {
+    CovJob off[COV_NW], dia[COV_NW];
+    int no = 0, nd = 0;
+    for (int k = 0; k < g.njobs; ++k) (g.job[k].kind == 1 ? off[no++] : dia[nd++]) = g.job[k];
+    int io = 0, id = 0;
+    for (int w = 0; w < g.njobs; ++w) {
+        const bool want_diag = (w & 3) == 3 || io == no;
+        g.job[w] = (want_diag && id < nd) ? dia[id++] : off[io++];
+    }
+}
+static void make_plan_groups(int nb, CovPlan* p);
 static void make_plan(int nb, CovPlan* p) {
+    make_plan_groups(nb, p);
+    for (int k = 0; k < p->ngroups; ++k) order_jobs(p->g[k]);
+}
+static void make_plan_groups(int nb, CovPlan* p) {
     memset(p, 0, sizeof(*p));
     if (nb <= 4) { p->ngroups = 1; add_triangle(p->g[0], 0, nb); return; }
     // nb in 5..8: A = [0,4), B = [4,nb): triangle(A), triangle(B), rectangle B x A in strips of two block rows
