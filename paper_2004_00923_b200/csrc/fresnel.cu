@@ -1,6 +1,6 @@
 // fresnel.cu -- A0 (temporal sum), A1 (mean-subtract + chirp prologue) and A2 (2-D FFT) kernels.
 //   H_t = FFT2D[(I_t - mean_t I) * exp(+i pi (x^2+y^2)/(lambda z))]      (Eq. 1; R2-R6)
-// Stockham autosort FFT, radix-16/32 butterflies in registers, one shared-memory exchange per extra
+// Stockham autosort FFT, radix-16/32 butterflies in registers (FMA-fused DIT), one shared-memory exchange per extra
 // pass, row pass (x) then column pass (y); the row->column intermediate is kept L2-resident by
 // processing the stack in small frame groups.
 #include "holo_internal.cuh"
@@ -8,16 +8,20 @@
 #include <vector>
 
 // ------------------------------------------------------------------------------------------------
-// register FFT, radix-2 decimation in frequency, fully unrolled; result is in bit-reversed order
+// register FFT, radix-2 decimation in time, natural-order input, fully unrolled; the result is in
+// bit-reversed order.  Stage s (s = 0 .. log2 R - 1) works in place on pairs at distance R/2^(s+1);
+// the pairs of group g share the twiddle W_{2^(s+1)}^{rev_s(g)}.  A butterfly with a non-trivial
+// twiddle costs 6 FMA-class instructions (tangent form: w b = wr (b_r - c b_i, b_i + c b_r), c = wi/wr,
+// or the cotangent form when |wi| > |wr|) instead of 4 adds + 4 for the complex product.
 // ------------------------------------------------------------------------------------------------
-__host__ __device__ constexpr float cos32(int k) {   // cos(2 pi k / 32), 0 <= k <= 16
-    return k == 0 ? 1.0f : k == 1 ? 0.98078528040323043f : k == 2 ? 0.92387953251128674f
-         : k == 3 ? 0.83146961230254524f : k == 4 ? 0.70710678118654752f : k == 5 ? 0.55557023301960218f
-         : k == 6 ? 0.38268343236508978f : k == 7 ? 0.19509032201612825f : k == 8 ? 0.0f
-         : -cos32(16 - k);
+__host__ __device__ constexpr double cos32d(int k) {   // cos(2 pi k / 32), 0 <= k <= 16
+    return k == 0 ? 1.0 : k == 1 ? 0.98078528040323044913 : k == 2 ? 0.92387953251128675613
+         : k == 3 ? 0.83146961230254523708 : k == 4 ? 0.70710678118654752440 : k == 5 ? 0.55557023301960222474
+         : k == 6 ? 0.38268343236508977173 : k == 7 ? 0.19509032201612826785 : k == 8 ? 0.0
+         : -cos32d(16 - k);
 }
-__host__ __device__ constexpr float sin32(int k) {   // sin(2 pi k / 32), 0 <= k <= 16
-    return k <= 8 ? cos32(8 - k) : cos32(k - 8);
+__host__ __device__ constexpr double sin32d(int k) {   // sin(2 pi k / 32), 0 <= k <= 16
+    return k <= 8 ? cos32d(8 - k) : cos32d(k - 8);
 }
 template <int R> __host__ __device__ constexpr int brev(int r) {
     int o = 0;
@@ -25,39 +29,57 @@ template <int R> __host__ __device__ constexpr int brev(int r) {
     return o;
 }
 
-// d * exp(-2 pi i idx/32), idx a compile-time constant after unrolling
-template <int IDX> __host__ __device__ __forceinline__ float2 mul_w32(float2 d) {
-    if (IDX == 0) return d;
-    if (IDX == 8) return make_float2(d.y, -d.x);
-    if (IDX == 4) return make_float2((d.x + d.y) * 0.70710678118654752f, (d.y - d.x) * 0.70710678118654752f);
-    if (IDX == 12) return make_float2((d.y - d.x) * 0.70710678118654752f, -(d.x + d.y) * 0.70710678118654752f);
-    constexpr float c = cos32(IDX), s = sin32(IDX);
-    return make_float2(fmaf(d.y, s, d.x * c), fmaf(-d.x, s, d.y * c));
+// (a, b) <- (a + w b, a - w b),  w = exp(-2 pi i E32 / 32), 0 <= E32 < 16
+template <int E32> __host__ __device__ __forceinline__ void bfly_dit(float2& a, float2& b) {
+    if constexpr (E32 == 0) {
+        const float2 t = b;
+        b = make_float2(a.x - t.x, a.y - t.y);
+        a = make_float2(a.x + t.x, a.y + t.y);
+    } else if constexpr (E32 == 8) {                      // w = -i: w b = (b_i, -b_r)
+        const float2 t = b;
+        b = make_float2(a.x - t.y, a.y + t.x);
+        a = make_float2(a.x + t.y, a.y - t.x);
+    } else {
+        constexpr double wr = cos32d(E32), wi = -sin32d(E32);
+        constexpr bool tanform = (wr < 0 ? -wr : wr) >= (wi < 0 ? -wi : wi);
+        float tr, ti, sc;
+        if constexpr (E32 == 4) { tr = b.x + b.y; ti = b.y - b.x; sc = (float)wr; }            // c = wi/wr = -1
+        else if constexpr (E32 == 12) { tr = b.x - b.y; ti = b.y + b.x; sc = (float)wr; }      // c = +1
+        else if constexpr (tanform) {
+            constexpr float c = (float)(wi / wr);
+            tr = fmaf(-c, b.y, b.x); ti = fmaf(c, b.x, b.y); sc = (float)wr;
+        } else {
+            constexpr float c = (float)(wr / wi);
+            tr = fmaf(c, b.x, -b.y); ti = fmaf(c, b.y, b.x); sc = (float)wi;
+        }
+        b = make_float2(fmaf(-sc, tr, a.x), fmaf(-sc, ti, a.y));
+        a = make_float2(fmaf(sc, tr, a.x), fmaf(sc, ti, a.y));
+    }
 }
 
-template <int SPAN, int G, int K> struct BflyK {
+template <int R, int S, int G, int M> struct DitM {      // pair M of group G in stage S
     static __host__ __device__ __forceinline__ void run(float2* v) {
-        float2 a = v[G + K], b = v[G + K + SPAN];
-        v[G + K] = make_float2(a.x + b.x, a.y + b.y);
-        v[G + K + SPAN] = mul_w32<K * (16 / SPAN)>(make_float2(a.x - b.x, a.y - b.y));
-        if constexpr (K + 1 < SPAN) BflyK<SPAN, G, K + 1>::run(v);
+        constexpr int span = R >> (S + 1);
+        constexpr int e32 = brev<(1 << S)>(G) * (16 >> S);           // W_{2^(S+1)}^{rev_S(G)} as a 32nd root
+        bfly_dit<e32>(v[2 * span * G + M], v[2 * span * G + M + span]);
+        if constexpr (M + 1 < span) DitM<R, S, G, M + 1>::run(v);
     }
 };
-template <int R, int SPAN, int G> struct BflyG {
+template <int R, int S, int G> struct DitG {
     static __host__ __device__ __forceinline__ void run(float2* v) {
-        BflyK<SPAN, G, 0>::run(v);
-        if constexpr (G + 2 * SPAN < R) BflyG<R, SPAN, G + 2 * SPAN>::run(v);
+        DitM<R, S, G, 0>::run(v);
+        if constexpr (G + 1 < (1 << S)) DitG<R, S, G + 1>::run(v);
     }
 };
-template <int R, int SPAN> struct BflyS {
+template <int R, int S> struct DitS {
     static __host__ __device__ __forceinline__ void run(float2* v) {
-        BflyG<R, SPAN, 0>::run(v);
-        if constexpr (SPAN > 1) BflyS<R, SPAN / 2>::run(v);
+        DitG<R, S, 0>::run(v);
+        if constexpr ((2 << S) < R) DitS<R, S + 1>::run(v);
     }
 };
 // in-place DFT of size R (power of two <= 32) on registers v[0..R); X[r] = v[brev<R>(r)] afterwards
 template <int R> __host__ __device__ __forceinline__ void fft_reg(float2* v) {
-    if constexpr (R > 1) BflyS<R, R / 2>::run(v);
+    if constexpr (R > 1) DitS<R, 0>::run(v);
 }
 
 __device__ __forceinline__ float2 cmul(float2 a, float2 b) {
@@ -69,7 +91,7 @@ __device__ __forceinline__ float2 cmul(float2 a, float2 b) {
 // ------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256) k_frame_sum(const uint16_t* __restrict__ frames, uint32_t* __restrict__ sum,
                                                    long long npix, int T, unsigned int* __restrict__ counters) {
-    if (blockIdx.x == 0 && threadIdx.x < 2 * T + 1) counters[threadIdx.x] = 0u;   // tickets of the fused Fresnel kernel
+    if (blockIdx.x == 0 && threadIdx.x < 2 * T + 1) counters[threadIdx.x] = 0u;   // ticket / completion counters of the fused Fresnel kernel
     long long v = (long long)blockIdx.x * blockDim.x + threadIdx.x;      // one uint4 = 8 pixels per thread
     long long nvec = npix >> 3;
     for (; v < nvec; v += (long long)gridDim.x * blockDim.x) {
@@ -113,8 +135,13 @@ struct FftArgs {
 };
 
 // one tile = B sequences of one frame; in_foff / out_foff = element offset of the frame in a.in(frames) / a.out
-template <int N, int E, int R1, int R2, int B, bool COL, bool PRO>
-__device__ __forceinline__ void fft_tile(const FftArgs& a, long long in_foff, long long out_foff, int tile_in_frame, float2* sm) {
+struct NoHook { __device__ __forceinline__ void operator()() const {} };
+
+// `mid` is called once by every thread in the middle of the tile (after the pass-0 butterflies; the fused
+// kernel does its scheduling work there, when the stores of the previous tile have long drained)
+template <int N, int E, int R1, int R2, int B, bool COL, bool PRO, class Mid = NoHook>
+__device__ __forceinline__ void fft_tile(const FftArgs& a, long long in_foff, long long out_foff, int tile_in_frame, float2* sm,
+                                         Mid mid = Mid()) {
     constexpr int TPS = N / E;
     constexpr int PADN = N + N / E;
     constexpr bool MULTI = (R1 > 1);
@@ -141,7 +168,7 @@ __device__ __forceinline__ void fft_tile(const FftArgs& a, long long in_foff, lo
                 const int i = j + r * TPS;
                 const int I = (int)__ldg(fr + i);
                 const int S = (int)__ldg(sp + i);
-                const float d = (float)(a.T * I - S) * a.invT;         // exact integer, one rounding
+                const float d = (float)(a.T * I - S);                  // exact integer; the 1/T lives in the qx table
                 const float2 q = cmul(__ldg(a.qx + i), qyv);
                 v[r] = make_float2(d * q.x, d * q.y);
             }
@@ -153,12 +180,14 @@ __device__ __forceinline__ void fft_tile(const FftArgs& a, long long in_foff, lo
         fft_reg<E>(v);
         float2* op = a.out + obase;
         if constexpr (!MULTI) {
+            mid();
 #pragma unroll
             for (int r = 0; r < E; ++r) op[r * estride] = v[brev<E>(r)];
         } else {
 #pragma unroll
             for (int r = 0; r < E; ++r) sm[sidx(j * E + r)] = v[brev<E>(r)];
             __syncthreads();
+            mid();
             // ---------------- pass 1: radix R1, Ns = E
             constexpr int M1 = E / R1;
 #pragma unroll
@@ -222,18 +251,20 @@ __global__ void __launch_bounds__((N / E) * B) k_fft(const FftArgs a) {
 
 // ------------------------------------------------------------------------------------------------
 // Persistent fused Fresnel kernel (square frames): ONE launch does the row pass and the column pass of
-// all T frames.  CTAs draw tiles from a global ticket in the order
-//   rows(0), [rows(f), cols(f-1)] for f = 1..T-1, cols(T-1)
-// so a column tile almost never waits; the row->column intermediate is a ring of R frames that stays
-// in L2.  cols(f) waits for rows_done[f] == RT; rows(f) waits for cols_done[f-R] == CT (ring reuse).
-// All CTAs are co-resident (grid <= occupancy x SMs) and tickets are served in order, so the tile with
-// the smallest unfinished ticket can always run: no deadlock.
+// all T frames.  CTAs draw tiles from a global ticket (atomicAdd: a compare-and-swap claim of "ready" tiles
+// was measured to serialise at one claim per L2 round trip, 4.5 ms) in the order
+//   rows(0..L-1), [rows(f), cols(f-L)] for f = L..T-1, cols(T-L..T-1)
+// The lag L (frames) is chosen so that the tickets in flight (one or two per resident CTA) span fewer
+// tiles than separate rows(f) from cols(f): a column tile then almost never waits for its row pass.
+// The row->column intermediate is a ring of R > L frames that stays in L2: cols(f) waits for
+// rows_done[f] == RT, rows(f) waits for cols_done[f-R] == CT (ring reuse).  Tickets are served in order and
+// every dependency of a ticket has a smaller ticket, so the smallest unfinished ticket can always run.
 // ------------------------------------------------------------------------------------------------
 struct FresnelArgs {
     FftArgs rows, cols;         // rows.out = cols.in = scratch ring; frame offsets are computed here
     unsigned int* counters;     // [0] ticket, [1..T] rows_done, [1+T..2T] cols_done (zeroed by k_frame_sum)
     long long npix;
-    int T, R, RT, CT;
+    int T, R, L, RT, CT;
 };
 
 __device__ __forceinline__ unsigned int ld_acquire(const unsigned int* p) {
@@ -241,38 +272,84 @@ __device__ __forceinline__ unsigned int ld_acquire(const unsigned int* p) {
     asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
     return v;
 }
+__device__ __forceinline__ void red_release_add(unsigned int* p, unsigned int v) {
+    asm volatile("red.release.gpu.global.add.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+
+// ticket -> (frame, tile in frame, row/column pass)
+__device__ __forceinline__ void fresnel_decode(const FresnelArgs& p, unsigned int tk, int& f, int& w, bool& is_col) {
+    const unsigned int per = (unsigned int)(p.RT + p.CT);
+    const unsigned int head = (unsigned int)(p.L * p.RT);                    // rows(0..L-1)
+    const unsigned int body = head + (unsigned int)(p.T - p.L) * per;        // + [rows(f), cols(f-L)]
+    if (tk < head) { f = (int)(tk / (unsigned int)p.RT); w = (int)tk - f * p.RT; is_col = false; }
+    else if (tk < body) {
+        const unsigned int u = tk - head;
+        const int seg = (int)(u / per), r = (int)(u - (unsigned int)seg * per);
+        if (r < p.RT) { f = seg + p.L; w = r; is_col = false; } else { f = seg; w = r - p.RT; is_col = true; }
+    } else {
+        const unsigned int u = tk - body;
+        const int g = (int)(u / (unsigned int)p.CT);
+        f = p.T - p.L + g; w = (int)u - g * p.CT; is_col = true;
+    }
+}
+// counter a tile depends on (nullptr: none) and the value it must reach
+__device__ __forceinline__ const unsigned int* fresnel_dep(const FresnelArgs& p, int f, bool is_col, unsigned int& need) {
+    if (is_col) { need = (unsigned int)p.RT; return p.counters + 1 + f; }
+    if (f >= p.R) { need = (unsigned int)p.CT; return p.counters + 1 + p.T + (f - p.R); }
+    need = 0u;
+    return nullptr;
+}
 
 template <int N, int E, int R1, int R2, int B>
 __global__ void __launch_bounds__((N / E) * B, ((N / E) * B <= 256) ? 2 : 1) k_fresnel(const FresnelArgs p) {
     extern __shared__ float2 sm[];
-    __shared__ unsigned int s_ticket;
-    const unsigned int per = (unsigned int)(p.RT + p.CT);
-    const unsigned int total = (unsigned int)p.T * per;
-    for (;;) {
-        if (threadIdx.x == 0) s_ticket = atomicAdd(p.counters, 1u);
-        __syncthreads();
-        const unsigned int tk = s_ticket;
+    __shared__ unsigned int s_ticket[2];
+    __shared__ int s_ready[2];
+    const unsigned int total = (unsigned int)p.T * (unsigned int)(p.RT + p.CT);
+    if (threadIdx.x == 0) { s_ticket[0] = atomicAdd(p.counters, 1u); s_ready[0] = 0; }
+    __syncthreads();
+    int pending = -1;            // thread 0: completion counter of the previous tile, not yet published
+    for (int it = 0;; ++it) {
+        const unsigned int tk = s_ticket[it & 1];
+        const int ready = s_ready[it & 1];
         if (tk >= total) break;
         int f, w; bool is_col;
-        if (tk < (unsigned int)p.RT) { f = 0; w = (int)tk; is_col = false; }
-        else {
-            const unsigned int u = tk - (unsigned int)p.RT;
-            const int seg = (int)(u / per), r = (int)(u - (unsigned int)seg * per);
-            if (seg < p.T - 1) { if (r < p.RT) { f = seg + 1; w = r; is_col = false; } else { f = seg; w = r - p.RT; is_col = true; } }
-            else { f = p.T - 1; w = r; is_col = true; }
+        fresnel_decode(p, tk, f, w, is_col);
+        if (!ready) {                                // rare: the dependency was not complete when the ticket was drawn
+            if (threadIdx.x == 0) {
+                if (pending >= 0) { red_release_add(p.counters + pending, 1u); pending = -1; }   // never wait while holding a signal
+                unsigned int need;
+                const unsigned int* dep = fresnel_dep(p, f, is_col, need);
+                if (dep) while (ld_acquire(dep) < need) __nanosleep(32);
+            }
+            __syncthreads();
         }
-        if (threadIdx.x == 0) {                      // dependency wait (rare by construction of the order)
-            if (is_col) { while (ld_acquire(p.counters + 1 + f) < (unsigned int)p.RT) __nanosleep(64); }
-            else if (f >= p.R) { while (ld_acquire(p.counters + 1 + p.T + (f - p.R)) < (unsigned int)p.CT) __nanosleep(64); }
-        }
-        __syncthreads();
+        // the next ticket is drawn now; its value is first used in the middle of the tile, so the round trip is hidden
+        unsigned int nt = 0u;
+        if (threadIdx.x == 0) nt = atomicAdd(p.counters, 1u);
+        auto mid = [&]() {
+            if (threadIdx.x == 0) {
+                // the stores of the previous tile drained long ago, so this release does not stall on them; every
+                // thread's stores / scratch reads of that tile were ordered before its closing barrier (cumulativity)
+                if (pending >= 0) { red_release_add(p.counters + pending, 1u); pending = -1; }
+                int rdy = 1;
+                if (nt < total) {
+                    int nf, nw; bool ncol; unsigned int need;
+                    fresnel_decode(p, nt, nf, nw, ncol);
+                    const unsigned int* dep = fresnel_dep(p, nf, ncol, need);
+                    if (dep) rdy = ld_acquire(dep) >= need;
+                }
+                s_ticket[(it + 1) & 1] = nt;
+                s_ready[(it + 1) & 1] = rdy;
+            }
+        };
         const long long slot = (long long)(f % p.R) * p.npix;
-        if (!is_col) fft_tile<N, E, R1, R2, B, false, true>(p.rows, (long long)f * p.npix, slot, w, sm);
-        else         fft_tile<N, E, R1, R2, B, true, false>(p.cols, slot, (long long)f * p.npix, w, sm);
-        __threadfence();
-        __syncthreads();
-        if (threadIdx.x == 0) atomicAdd(p.counters + 1 + (is_col ? p.T + f : f), 1u);
+        if (!is_col) fft_tile<N, E, R1, R2, B, false, true>(p.rows, (long long)f * p.npix, slot, w, sm, mid);
+        else         fft_tile<N, E, R1, R2, B, true, false>(p.cols, slot, (long long)f * p.npix, w, sm, mid);
+        if constexpr (R1 == 1) __syncthreads();      // single-pass tiles have no closing barrier of their own
+        pending = 1 + (is_col ? p.T + f : f);
     }
+    if (threadIdx.x == 0 && pending >= 0) red_release_add(p.counters + pending, 1u);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -381,7 +458,7 @@ static int launch_fresnel_t(const FresnelArgs& p, int num_sms, cudaStream_t st) 
         blocks_per_sm = occ;
     }
     const long long total = (long long)p.T * (p.RT + p.CT);
-    long long grid = (long long)num_sms * blocks_per_sm;      // all CTAs co-resident (required by the dependency waits)
+    long long grid = (long long)num_sms * blocks_per_sm;      // one wave of persistent CTAs
     if (grid > total) grid = total;
     kern<<<(int)grid, threads, smem, st>>>(p);
     HOLO_CUDA_OK(cudaGetLastError());
@@ -430,11 +507,15 @@ int holo_launch_fresnel(holo_ctx* c, const uint16_t* frames, float2* H, cudaStre
         FresnelArgs p{};
         const int Bq = fft_batch(c->nx);
         FftArgs& a = p.rows;
-        a.frames = frames; a.sum = c->sum; a.qx = c->qx; a.qy = c->qy; a.in = nullptr; a.out = c->scratch;
+        a.frames = frames; a.sum = c->sum; a.qx = c->qxs; a.qy = c->qy; a.in = nullptr; a.out = c->scratch;
         a.tw1 = c->px.tw1; a.tw2 = c->px.tw2; a.ld = c->nx; a.nseq = c->ny; a.T = c->T; a.invT = 1.0f / (float)c->T;
         FftArgs& b = p.cols;
         b.in = c->scratch; b.out = H; b.tw1 = c->py.tw1; b.tw2 = c->py.tw2; b.ld = c->nx; b.nseq = c->nx; b.T = c->T; b.invT = a.invT;
         p.counters = c->counters; p.npix = c->npix; p.T = c->T; p.R = c->scratch_frames;
+        p.L = c->tune[HOLO_TUNE_FFT_LAG] > 0 ? c->tune[HOLO_TUNE_FFT_LAG] : p.R / 2;
+        if (p.L > p.R - 1) p.L = p.R - 1;
+        if (p.L > p.T) p.L = p.T;
+        if (p.L < 1) p.L = 1;
         p.RT = c->ny / Bq; p.CT = c->nx / Bq;
         HoloProf prof(c, HOLO_K_FFT_ROWS, st);
         return launch_fresnel_fused(c->nx, p, c->num_sms, st);
@@ -445,7 +526,7 @@ int holo_launch_fresnel(holo_ctx* c, const uint16_t* frames, float2* H, cudaStre
         const int nf = (c->T - f0 < G) ? c->T - f0 : G;
         FftArgs a{};
         a.frames = frames + (long long)f0 * c->npix;
-        a.sum = c->sum; a.qx = c->qx; a.qy = c->qy;
+        a.sum = c->sum; a.qx = c->qxs; a.qy = c->qy;
         a.in = nullptr; a.out = c->scratch;
         a.tw1 = c->px.tw1; a.tw2 = c->px.tw2;
         a.in_fstride = c->npix; a.out_fstride = c->npix;

@@ -21,7 +21,7 @@ extern "C" int holo_version(void) { return 100; }   // 0.1.0
 
 static bool is_pow2(int n) { return n > 0 && (n & (n - 1)) == 0; }
 
-static int build_chirp(float2** dst, int n, double lambda_m, double pitch_m, double z_m) {
+static int build_chirp(float2** dst, int n, double lambda_m, double pitch_m, double z_m, double scale) {
     // q_x[i] = exp(+i pi x_i^2/(lambda z)), x_i = (i - n/2) pitch; evaluated in double with the phase
     // reduced mod 2 (in units of pi) BEFORE the trigonometric call (the phase reaches 1e4 rad).
     std::vector<float2> h(n);
@@ -30,7 +30,7 @@ static int build_chirp(float2** dst, int n, double lambda_m, double pitch_m, dou
     for (int i = 0; i < n; ++i) {
         const double o = (double)(i - n / 2);
         double u = fmod(o * o * a, 2.0);
-        h[i] = make_float2((float)cos(PI * u), (float)sin(PI * u));
+        h[i] = make_float2((float)(scale * cos(PI * u)), (float)(scale * sin(PI * u)));
     }
     HOLO_CUDA_OK(cudaMalloc(dst, n * sizeof(float2)));
     HOLO_CUDA_OK(cudaMemcpy(*dst, h.data(), n * sizeof(float2), cudaMemcpyHostToDevice));
@@ -39,7 +39,7 @@ static int build_chirp(float2** dst, int n, double lambda_m, double pitch_m, dou
 
 static void free_ctx(holo_ctx* c) {
     if (!c) return;
-    cudaFree(c->qx); cudaFree(c->qy); cudaFree(c->Wdft);
+    cudaFree(c->qx); cudaFree(c->qy); cudaFree(c->qxs); cudaFree(c->Wdft);
     holo_fft_plan_free(&c->px); holo_fft_plan_free(&c->py);
     cudaFree(c->sum); cudaFree(c->scratch); cudaFree(c->H); cudaFree(c->cov_partials);
     cudaFree(c->C); cudaFree(c->evals); cudaFree(c->V); cudaFree(c->Vsel); cudaFree(c->status);
@@ -63,8 +63,9 @@ static int create_impl(holo_ctx* c) {
     const int T = c->T;
     const long long np = c->npix;
     int rc;
-    if ((rc = build_chirp(&c->qx, c->nx, c->lambda_m, c->pitch_m, c->z_m))) return rc;
-    if ((rc = build_chirp(&c->qy, c->ny, c->lambda_m, c->pitch_m, c->z_m))) return rc;
+    if ((rc = build_chirp(&c->qx, c->nx, c->lambda_m, c->pitch_m, c->z_m, 1.0))) return rc;
+    if ((rc = build_chirp(&c->qy, c->ny, c->lambda_m, c->pitch_m, c->z_m, 1.0))) return rc;
+    if ((rc = build_chirp(&c->qxs, c->nx, c->lambda_m, c->pitch_m, c->z_m, 1.0 / (double)c->T))) return rc;
     if ((rc = holo_fft_plan_init(&c->px, c->nx))) return rc;
     if ((rc = holo_fft_plan_init(&c->py, c->ny))) return rc;
     {   // Eq. 8: w_mn = exp(-2 i pi (m-1)(n-1)/T)/sqrt(T)
@@ -79,7 +80,7 @@ static int create_impl(holo_ctx* c) {
         HOLO_CUDA_OK(cudaMemcpy(c->Wdft, W.data(), W.size() * sizeof(float2), cudaMemcpyHostToDevice));
     }
     // tuning defaults
-    long long grp = (32ll << 20) / (8 * np);                 // keep the FFT intermediate <= 32 MiB (L2-resident)
+    long long grp = (48ll << 20) / (8 * np);                 // keep the FFT intermediate <= 48 MiB (L2-resident)
     if (grp < 2) grp = 2;                                    // the fused kernel needs a ring of >= 2 frames
     if (grp > T) grp = T;
     c->tune[HOLO_TUNE_FFT_GROUP] = (int)grp;

@@ -16,7 +16,8 @@ enum {
     HOLO_TUNE_PROJ_COMPLEMENT = 2, // 1 = allow complement form in holo_process (default 1)
     HOLO_TUNE_FFT_PERSISTENT = 3,  // 1 = single persistent fresnel kernel (default set at create)
     HOLO_TUNE_EIG_MAX_SWEEPS = 4,
-    HOLO_TUNE_PROFILE = 5,         // 1 = bracket every kernel launch with events (holo_profile_read)
+    HOLO_TUNE_PROFILE = 5,
+    HOLO_TUNE_FFT_LAG = 6,         // frames between the row pass and the column pass in the fused kernel (0 = auto)         // 1 = bracket every kernel launch with events (holo_profile_read)
 };
 
 // kernel classes for the profile hook
@@ -42,6 +43,7 @@ struct holo_ctx {
     int tune[HOLO_NUM_TUNE];
     // tables
     float2 *qx, *qy;        // chirp, separable (built in double on the host)
+    float2* qxs;            // qx / T (the mean-subtraction scale folded into the row-pass prologue)
     FftPlan px, py;
     float2* Wdft;           // Eq. 8 DFT basis [T][T]
     // workspace
