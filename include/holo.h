@@ -80,6 +80,18 @@ void holo_destroy(holo_ctx* ctx);
 /* The whole path A0..A6 for one stack: frames_dev (uint16 [T][ny][nx]) -> image_dev (float [ny][nx]). */
 int holo_process(holo_ctx* ctx, const uint16_t* frames_dev, float* image_dev, holo_stream stream);
 
+/* Streaming form of holo_process for a SEQUENCE of stacks (the paper's use: a continuous camera stream,
+ * PAPER.md:13,31).  Same arithmetic, same kernels, software-pipelined by one stack: holo_submit(i)
+ * enqueues on `stream` the Fresnel stage of stack i, then the projection of stack i-1 into the image_dev
+ * given to submit(i-1), then the covariance of stack i, and forks the single-CTA eigensolver of stack i
+ * to a side stream owned by the handle, where it runs under the Fresnel kernels of stack i+1.
+ * Contract: the image passed to submit(i) is complete, in `stream` order, after the NEXT holo_submit or
+ * after holo_flush; frames_dev may be reused as soon as `stream` has passed the submit.  The handle
+ * allocates a second hologram stack (8*T*nx*ny bytes) at the first call.  holo_process / holo_flush
+ * deliver an owed image first.  Use one stream per handle for a submit sequence. */
+int holo_submit(holo_ctx* ctx, const uint16_t* frames_dev, float* image_dev, holo_stream stream);
+int holo_flush(holo_ctx* ctx, holo_stream stream);
+
 /* Same path, HOST buffers (pinned or pageable): copies frames in, runs holo_process, copies the
  * image out, and synchronises `stream` before returning.  Uses a frame/image staging buffer owned by
  * the handle (allocated at first use).  This is the end-to-end call bench.py's `e2e` times. */

@@ -49,6 +49,11 @@ static void free_ctx(holo_ctx* c) {
         delete[] c->prof_ev;
         delete[] c->prof_cls;
     }
+    cudaFree(c->H1); cudaFree(c->C1); cudaFree(c->evals1); cudaFree(c->V1); cudaFree(c->status1);
+    if (c->side) {
+        cudaStreamDestroy(c->side);
+        for (int i = 0; i < 2; ++i) { cudaEventDestroy(c->ev_cov[i]); cudaEventDestroy(c->ev_eig[i]); }
+    }
     if (c->frames_stage) cudaFree(c->frames_stage);
     if (c->image_stage) cudaFree(c->image_stage);
     delete c;
@@ -170,15 +175,81 @@ extern "C" int holo_fourier_demod(holo_ctx* c, const void* H_dev, int n1, int n2
     return holo_launch_project(c, (const float2*)H_dev, c->Wdft, n1, n2, /*W is unitary*/ 1, image_dev, (cudaStream_t)stream);
 }
 
+static int project_pending(holo_ctx* c, cudaStream_t st);
+
 extern "C" int holo_process(holo_ctx* c, const uint16_t* frames_dev, float* image_dev, holo_stream stream) {
     CHECK_CTX(c); CHECK_PTR(frames_dev, "frames_dev"); CHECK_PTR(image_dev, "image_dev");
     if (((uintptr_t)frames_dev & 15) || ((uintptr_t)image_dev & 7)) { holo_set_error("frames_dev must be 16-byte and image_dev 8-byte aligned"); return HOLO_ERR_ARG; }
     cudaStream_t st = (cudaStream_t)stream;
     int rc;
+    if ((rc = project_pending(c, st))) return rc;          // a holo_submit still owes its image: deliver it first
+    c->nsubmit = 0;                                        // the next holo_submit starts again with slot 0
     if ((rc = holo_launch_fresnel(c, frames_dev, c->H, st))) return rc;
     if ((rc = holo_launch_covariance(c, c->H, c->C, st))) return rc;
     if ((rc = holo_launch_eig(c, c->C, c->evals, c->V, st))) return rc;
     return holo_launch_project(c, c->H, c->V, c->k_lo, c->k_hi, c->tune[HOLO_TUNE_PROJ_COMPLEMENT], image_dev, st);
+}
+
+// ---- streaming form: software pipeline over consecutive stacks -------------------------------------
+// submit(i) enqueues on `stream`:  A0+A1+A2 of stack i  ->  [join eig(i-1)] A5+A6 of stack i-1  ->  A3 of
+// stack i  ->  fork: A4 of stack i on the handle's side stream.  The single-CTA eigensolver of stack i thus
+// runs under the Fresnel kernels of stack i+1 instead of idling 147 SMs; everything else keeps stream order.
+static int submit_init(holo_ctx* c) {
+    if (c->side) return HOLO_OK;
+    const size_t T = (size_t)c->T;
+    HOLO_CUDA_OK(cudaMalloc(&c->H1, T * c->npix * sizeof(float2)));
+    HOLO_CUDA_OK(cudaMalloc(&c->C1, T * T * sizeof(float2)));
+    HOLO_CUDA_OK(cudaMalloc(&c->evals1, T * sizeof(float)));
+    HOLO_CUDA_OK(cudaMalloc(&c->V1, T * T * sizeof(float2)));
+    HOLO_CUDA_OK(cudaMalloc(&c->status1, 8 * sizeof(int32_t)));
+    HOLO_CUDA_OK(cudaMemset(c->status1, 0, 8 * sizeof(int32_t)));
+    int lo = 0, hi = 0;
+    HOLO_CUDA_OK(cudaDeviceGetStreamPriorityRange(&lo, &hi));
+    HOLO_CUDA_OK(cudaStreamCreateWithPriority(&c->side, cudaStreamNonBlocking, hi));
+    for (int i = 0; i < 2; ++i) {
+        HOLO_CUDA_OK(cudaEventCreateWithFlags(&c->ev_cov[i], cudaEventDisableTiming));
+        HOLO_CUDA_OK(cudaEventCreateWithFlags(&c->ev_eig[i], cudaEventDisableTiming));
+    }
+    return HOLO_OK;
+}
+
+static int project_pending(holo_ctx* c, cudaStream_t st) {
+    if (!c->pend_image) return HOLO_OK;
+    const int s = c->pend_slot;
+    HOLO_CUDA_OK(cudaStreamWaitEvent(st, c->ev_eig[s], 0));
+    const int rc = holo_launch_project(c, s ? c->H1 : c->H, s ? c->V1 : c->V, c->k_lo, c->k_hi,
+                                       c->tune[HOLO_TUNE_PROJ_COMPLEMENT], c->pend_image, st);
+    c->pend_image = nullptr;
+    return rc;
+}
+
+extern "C" int holo_submit(holo_ctx* c, const uint16_t* frames_dev, float* image_dev, holo_stream stream) {
+    CHECK_CTX(c); CHECK_PTR(frames_dev, "frames_dev"); CHECK_PTR(image_dev, "image_dev");
+    if (((uintptr_t)frames_dev & 15) || ((uintptr_t)image_dev & 7)) { holo_set_error("frames_dev must be 16-byte and image_dev 8-byte aligned"); return HOLO_ERR_ARG; }
+    cudaStream_t st = (cudaStream_t)stream;
+    int rc;
+    if ((rc = submit_init(c))) return rc;
+    const int s = (int)(c->nsubmit & 1);
+    float2* H = s ? c->H1 : c->H;
+    float2* C = s ? c->C1 : c->C;
+    if ((rc = holo_launch_fresnel(c, frames_dev, H, st))) return rc;
+    if ((rc = project_pending(c, st))) return rc;
+    if ((rc = holo_launch_covariance(c, H, C, st))) return rc;
+    HOLO_CUDA_OK(cudaEventRecord(c->ev_cov[s], st));
+    HOLO_CUDA_OK(cudaStreamWaitEvent(c->side, c->ev_cov[s], 0));
+    int32_t* status_main = c->status;
+    if (s) c->status = c->status1;
+    rc = holo_launch_eig(c, C, s ? c->evals1 : c->evals, s ? c->V1 : c->V, c->side);
+    c->status = status_main;
+    if (rc) return rc;
+    HOLO_CUDA_OK(cudaEventRecord(c->ev_eig[s], c->side));
+    c->pend_image = image_dev; c->pend_slot = s; c->nsubmit++;
+    return HOLO_OK;
+}
+
+extern "C" int holo_flush(holo_ctx* c, holo_stream stream) {
+    CHECK_CTX(c);
+    return project_pending(c, (cudaStream_t)stream);
 }
 
 extern "C" int holo_process_host(holo_ctx* c, const uint16_t* frames_host, float* image_host, holo_stream stream) {

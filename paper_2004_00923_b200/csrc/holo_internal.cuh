@@ -63,6 +63,13 @@ struct holo_ctx {
     cudaEvent_t* prof_ev;   // [2*HOLO_PROF_CAP]
     int* prof_cls;
     int prof_n;
+    // streaming form (holo_submit / holo_flush): second workspace slot, side stream for the eigensolver
+    float2* H1; float2* C1; float* evals1; float2* V1; int32_t* status1;
+    cudaStream_t side;
+    cudaEvent_t ev_cov[2], ev_eig[2];
+    float* pend_image;      // image of the stack whose projection is still owed (nullptr: none)
+    int pend_slot;
+    long long nsubmit;
     // host staging for holo_process_host
     uint16_t* frames_stage;
     float* image_stage;
