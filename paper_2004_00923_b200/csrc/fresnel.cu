@@ -86,6 +86,30 @@ __device__ __forceinline__ float2 cmul(float2 a, float2 b) {
     return make_float2(fmaf(-a.y, b.y, a.x * b.x), fmaf(a.y, b.x, a.x * b.y));
 }
 
+// L2 residency hints (createpolicy + ld/st .L2::cache_hint): the uint16 stack (64 MB at 1024^2 x 32) is kept
+// in L2 between the sum kernel and the row pass, the row->column ring is kept until it is overwritten,
+// and the hologram stores stream through (they are next read after 256 MB more have been written).
+__device__ __forceinline__ uint64_t l2_evict_first() { uint64_t p; asm("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p)); return p; }
+__device__ __forceinline__ uint64_t l2_evict_last() { uint64_t p; asm("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p)); return p; }
+__device__ __forceinline__ float2 ldcg_hint(const float2* p, uint64_t pol) {
+    float2 v;
+    asm volatile("ld.global.cg.L2::cache_hint.v2.f32 {%0,%1}, [%2], %3;" : "=f"(v.x), "=f"(v.y) : "l"(p), "l"(pol) : "memory");
+    return v;
+}
+__device__ __forceinline__ void st_hint(float2* p, float2 v, uint64_t pol) {
+    asm volatile("st.global.L2::cache_hint.v2.f32 [%0], {%1,%2}, %3;" ::"l"(p), "f"(v.x), "f"(v.y), "l"(pol) : "memory");
+}
+__device__ __forceinline__ int ldnc_u16_hint(const uint16_t* p, uint64_t pol) {
+    unsigned short u;
+    asm volatile("ld.global.nc.L2::cache_hint.u16 %0, [%1], %2;" : "=h"(u) : "l"(p), "l"(pol));
+    return (int)u;
+}
+__device__ __forceinline__ uint4 ldnc_v4_hint(const uint4* p, uint64_t pol) {
+    uint4 w;
+    asm volatile("ld.global.nc.L2::cache_hint.v4.u32 {%0,%1,%2,%3}, [%4], %5;" : "=r"(w.x), "=r"(w.y), "=r"(w.z), "=r"(w.w) : "l"(p), "l"(pol));
+    return w;
+}
+
 // ------------------------------------------------------------------------------------------------
 // A0: per-pixel temporal sum  S(p) = sum_t I_t(p)   (uint32: exact, T*65535 < 2^32)
 // ------------------------------------------------------------------------------------------------
@@ -139,12 +163,17 @@ struct NoHook { __device__ __forceinline__ void operator()() const {} };
 
 // `mid` is called once by every thread in the middle of the tile (after the pass-0 butterflies; the fused
 // kernel does its scheduling work there, when the stores of the previous tile have long drained)
-template <int N, int E, int R1, int R2, int B, bool COL, bool PRO, class Mid = NoHook>
+// LDC: row pitch in elements known at compile time (0: use a.ld) -- turns every address into base + immediate
+template <int N, int E, int R1, int R2, int B, bool COL, bool PRO, int LDC = 0, class Mid = NoHook>
 __device__ __forceinline__ void fft_tile(const FftArgs& a, long long in_foff, long long out_foff, int tile_in_frame, float2* sm,
                                          Mid mid = Mid()) {
     constexpr int TPS = N / E;
     constexpr int PADN = N + N / E;
     constexpr bool MULTI = (R1 > 1);
+    // a row whose N/E threads are exactly one warp is exchanged through that warp's private slice of the buffer:
+    // warp-level synchronisation only (the eight warps of a row tile then run freely against each other)
+    constexpr bool WARP_SEQ = !COL && (N / E == 32);
+    auto sync_tile = [&]() { if constexpr (WARP_SEQ) __syncwarp(); else __syncthreads(); };
     const int tid = threadIdx.x;
     const int j = COL ? tid / B : tid % TPS;
     const int c = COL ? tid % B : tid / TPS;
@@ -154,19 +183,24 @@ __device__ __forceinline__ void fft_tile(const FftArgs& a, long long in_foff, lo
     };
     {
         const int s0 = tile_in_frame * B + c;                          // sequence index (row y or column x)
-        const long long ibase = in_foff + (COL ? (long long)s0 : (long long)s0 * a.ld);
-        const long long obase = out_foff + (COL ? (long long)s0 : (long long)s0 * a.ld);
-        const int estride = COL ? a.ld : 1;
+        const int ld = LDC ? LDC : a.ld;
+        const long long ibase = in_foff + (COL ? (long long)s0 : (long long)s0 * ld);
+        const long long obase = out_foff + (COL ? (long long)s0 : (long long)s0 * ld);
+        const int estride = COL ? ld : 1;
+        constexpr bool FUSED = LDC != 0;                 // fused persistent kernel: rows write / columns read the L2 ring
+        const uint64_t pol_in = (FUSED && COL) ? l2_evict_last() : l2_evict_first();
+        const uint64_t pol_out = (FUSED && !COL) ? l2_evict_last() : l2_evict_first();
+        auto store = [&](float2* q, float2 val) { if constexpr (FUSED) st_hint(q, val, pol_out); else *q = val; };
         float2 v[E];
         // ---------------- pass 0: radix E, Ns = 1, inputs straight from global
         if constexpr (PRO) {
             const float2 qyv = __ldg(a.qy + s0);
             const uint16_t* fr = a.frames + ibase;
-            const uint32_t* sp = a.sum + (long long)s0 * a.ld;
+            const uint32_t* sp = a.sum + (long long)s0 * ld;
 #pragma unroll
             for (int r = 0; r < E; ++r) {
                 const int i = j + r * TPS;
-                const int I = (int)__ldg(fr + i);
+                const int I = FUSED ? ldnc_u16_hint(fr + i, pol_in) : (int)__ldg(fr + i);
                 const int S = (int)__ldg(sp + i);
                 const float d = (float)(a.T * I - S);                  // exact integer; the 1/T lives in the qx table
                 const float2 q = cmul(__ldg(a.qx + i), qyv);
@@ -175,18 +209,18 @@ __device__ __forceinline__ void fft_tile(const FftArgs& a, long long in_foff, lo
         } else {
             const float2* ip = a.in + ibase;
 #pragma unroll
-            for (int r = 0; r < E; ++r) v[r] = __ldcg(ip + (j + r * TPS) * estride);   // L2-coherent: written earlier in this kernel
+            for (int r = 0; r < E; ++r) v[r] = FUSED ? ldcg_hint(ip + (j + r * TPS) * estride, pol_in) : __ldcg(ip + (j + r * TPS) * estride);   // L2-coherent: written earlier in this kernel
         }
         fft_reg<E>(v);
         float2* op = a.out + obase;
         if constexpr (!MULTI) {
             mid();
 #pragma unroll
-            for (int r = 0; r < E; ++r) op[r * estride] = v[brev<E>(r)];
+            for (int r = 0; r < E; ++r) store(op + r * estride, v[brev<E>(r)]);
         } else {
 #pragma unroll
             for (int r = 0; r < E; ++r) sm[sidx(j * E + r)] = v[brev<E>(r)];
-            __syncthreads();
+            sync_tile();
             mid();
             // ---------------- pass 1: radix R1, Ns = E
             constexpr int M1 = E / R1;
@@ -196,7 +230,7 @@ __device__ __forceinline__ void fft_tile(const FftArgs& a, long long in_foff, lo
 #pragma unroll
                 for (int r = 0; r < R1; ++r) v[m * R1 + r] = sm[sidx(b + r * (N / R1))];
             }
-            if constexpr (R2 > 1) __syncthreads();
+            if constexpr (R2 > 1) sync_tile();
 #pragma unroll
             for (int m = 0; m < M1; ++m) {
                 const int b = j + m * TPS;
@@ -207,14 +241,14 @@ __device__ __forceinline__ void fft_tile(const FftArgs& a, long long in_foff, lo
                 const int j0 = (b - k) * R1 + k;
                 if constexpr (R2 == 1) {
 #pragma unroll
-                    for (int r = 0; r < R1; ++r) op[(j0 + r * E) * estride] = v[m * R1 + brev<R1>(r)];
+                    for (int r = 0; r < R1; ++r) store(op + (j0 + r * E) * estride, v[m * R1 + brev<R1>(r)]);
                 } else {
 #pragma unroll
                     for (int r = 0; r < R1; ++r) sm[sidx(j0 + r * E)] = v[m * R1 + brev<R1>(r)];
                 }
             }
             if constexpr (R2 > 1) {
-                __syncthreads();
+                sync_tile();
                 // ---------------- pass 2: radix R2, Ns = E*R1
                 constexpr int M2 = E / R2;
                 constexpr int NS2 = E * R1;
@@ -231,7 +265,7 @@ __device__ __forceinline__ void fft_tile(const FftArgs& a, long long in_foff, lo
                     for (int r = 1; r < R2; ++r) v[m * R2 + r] = cmul(v[m * R2 + r], __ldg(a.tw2 + r * NS2 + b));
                     fft_reg<R2>(v + m * R2);
 #pragma unroll
-                    for (int r = 0; r < R2; ++r) op[(b + r * NS2) * estride] = v[m * R2 + brev<R2>(r)];
+                    for (int r = 0; r < R2; ++r) store(op + (b + r * NS2) * estride, v[m * R2 + brev<R2>(r)]);
                 }
             }
             __syncthreads();        // smem is reused by the next tile
@@ -301,7 +335,7 @@ __device__ __forceinline__ const unsigned int* fresnel_dep(const FresnelArgs& p,
 }
 
 template <int N, int E, int R1, int R2, int B>
-__global__ void __launch_bounds__((N / E) * B, ((N / E) * B <= 256) ? 2 : 1) k_fresnel(const FresnelArgs p) {
+__global__ void __launch_bounds__((N / E) * B, 512 / ((N / E) * B) > 0 ? 512 / ((N / E) * B) : 1) k_fresnel(const FresnelArgs p) {
     extern __shared__ float2 sm[];
     __shared__ unsigned int s_ticket[2];
     __shared__ int s_ready[2];
@@ -344,9 +378,11 @@ __global__ void __launch_bounds__((N / E) * B, ((N / E) * B <= 256) ? 2 : 1) k_f
             }
         };
         const long long slot = (long long)(f % p.R) * p.npix;
-        if (!is_col) fft_tile<N, E, R1, R2, B, false, true>(p.rows, (long long)f * p.npix, slot, w, sm, mid);
-        else         fft_tile<N, E, R1, R2, B, true, false>(p.cols, slot, (long long)f * p.npix, w, sm, mid);
-        if constexpr (R1 == 1) __syncthreads();      // single-pass tiles have no closing barrier of their own
+        {
+            if (!is_col) fft_tile<N, E, R1, R2, B, false, true, N>(p.rows, (long long)f * p.npix, slot, w, sm, mid);
+            else         fft_tile<N, E, R1, R2, B, true, false, N>(p.cols, slot, (long long)f * p.npix, w, sm, mid);
+            if constexpr (R1 == 1) __syncthreads();      // single-pass tiles have no closing barrier of their own
+        }
         pending = 1 + (is_col ? p.T + f : f);
     }
     if (threadIdx.x == 0 && pending >= 0) red_release_add(p.counters + pending, 1u);
@@ -442,6 +478,9 @@ static int launch_fft(int N, const FftArgs& a, int num_sms, cudaStream_t st) {
     holo_set_error("unsupported FFT length %d", N);
     return HOLO_ERR_ARG;
 }
+#ifndef FUSED_B1024
+#define FUSED_B1024 8          // sequences per CTA of the fused kernel at N = 1024 (4 = four 128-thread CTAs per SM was measured 8 % slower)
+#endif
 static int fft_batch(int N) { return N <= 512 ? 16 : N == 1024 ? 8 : 4; }
 
 template <int N, int E, int R1, int R2, int B>
@@ -473,7 +512,7 @@ static int launch_fresnel_fused(int N, const FresnelArgs& p, int num_sms, cudaSt
         case 128:  return launch_fresnel_t<128, 16, 8, 1, 16>(p, num_sms, st);
         case 256:  return launch_fresnel_t<256, 16, 16, 1, 16>(p, num_sms, st);
         case 512:  return launch_fresnel_t<512, 32, 16, 1, 16>(p, num_sms, st);
-        case 1024: return launch_fresnel_t<1024, 32, 32, 1, 8>(p, num_sms, st);
+        case 1024: return launch_fresnel_t<1024, 32, 32, 1, FUSED_B1024>(p, num_sms, st);
         case 2048: return launch_fresnel_t<2048, 16, 16, 8, 4>(p, num_sms, st);
         case 4096: return launch_fresnel_t<4096, 16, 16, 16, 4>(p, num_sms, st);
     }
@@ -505,7 +544,7 @@ int holo_launch_fresnel(holo_ctx* c, const uint16_t* frames, float2* H, cudaStre
     }
     if (use_fused(c)) {
         FresnelArgs p{};
-        const int Bq = fft_batch(c->nx);
+        const int Bq = c->nx == 1024 ? FUSED_B1024 : fft_batch(c->nx);
         FftArgs& a = p.rows;
         a.frames = frames; a.sum = c->sum; a.qx = c->qxs; a.qy = c->qy; a.in = nullptr; a.out = c->scratch;
         a.tw1 = c->px.tw1; a.tw2 = c->px.tw2; a.ld = c->nx; a.nseq = c->ny; a.T = c->T; a.invT = 1.0f / (float)c->T;
