@@ -15,7 +15,7 @@ FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std
 def _stale(obj, src):
     if not os.path.exists(obj):
         return True
-    deps = [src, os.path.join(CSRC, "holo_internal.cuh"), os.path.join(HERE, "..", "include", "holo.h")]
+    deps = [src, os.path.join(CSRC, "holo_internal.cuh"), os.path.join(CSRC, "tma.cuh"), os.path.join(HERE, "..", "include", "holo.h")]
     return os.path.getmtime(obj) < max(os.path.getmtime(d) for d in deps)
 
 

@@ -17,7 +17,7 @@
 // staging only the row blocks its jobs touch.
 #include "holo_internal.cuh"
 #include <string.h>
-#include <cuda.h>
+#include "tma.cuh"
 
 #define COV_P 128            // pixels per stage (1 KB per row)
 #define COV_NW 8             // consumer warps per CTA
@@ -40,29 +40,6 @@ struct CovPlan {
     int ngroups;
     CovGroup g[COV_MAX_GROUPS];
 };
-
-__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
-}
-__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
-    const uint32_t a = smem_u32(bar);
-    uint32_t ok;
-    do {
-        asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
-                     : "=r"(ok) : "r"(a), "r"(parity) : "memory");
-    } while (!ok);
-}
-__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t* bar, uint32_t bytes) {
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void tma_2d_g2s(void* dst_smem, const CUtensorMap* tm, int c0, int c1, uint64_t* bar) {
-    asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
-                 ::"r"(smem_u32(dst_smem)), "l"(tm), "r"(c0), "r"(c1), "r"(smem_u32(bar)) : "memory");
-}
 
 __device__ __forceinline__ float warp_sum(float x) {
 #pragma unroll
@@ -318,30 +295,6 @@ static void make_plan_groups(int nb, CovPlan* p) {
     }
 }
 
-// H viewed as a 2-D float tensor [T rows][2*npix floats]; box = [8 rows][2*COV_P floats]
-typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
-                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
-                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-static int make_tensor_map(CUtensorMap* tm, const float2* H, long long npix, int T) {
-    static EncodeTiledFn encode = nullptr;
-    if (!encode) {
-        void* fn = nullptr;
-        cudaDriverEntryPointQueryResult qres;
-        HOLO_CUDA_OK(cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres));
-        if (!fn || qres != cudaDriverEntryPointSuccess) { holo_set_error("cuTensorMapEncodeTiled not available"); return HOLO_ERR_CUDA; }
-        encode = (EncodeTiledFn)fn;
-    }
-    const cuuint64_t gdim[2] = {(cuuint64_t)(2 * npix), (cuuint64_t)T};
-    const cuuint64_t gstr[1] = {(cuuint64_t)npix * sizeof(float2)};
-    const cuuint32_t box[2] = {2 * COV_P, 8};
-    const cuuint32_t estr[2] = {1, 1};
-    const CUresult r = encode(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, const_cast<float2*>(H), gdim, gstr, box, estr,
-                              CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
-                              CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-    if (r != CUDA_SUCCESS) { holo_set_error("cuTensorMapEncodeTiled failed (%d)", (int)r); return HOLO_ERR_CUDA; }
-    return HOLO_OK;
-}
-
 int holo_launch_covariance(holo_ctx* c, const float2* H, float2* C, cudaStream_t st) {
     const int T = c->T, T8 = (T + 7) / 8 * 8, nb = T8 / 8;
     if (nb < 1 || nb > 8) { holo_set_error("T out of range"); return HOLO_ERR_ARG; }
@@ -365,7 +318,7 @@ int holo_launch_covariance(holo_ctx* c, const float2* H, float2* C, cudaStream_t
     if (gx > c->cov_parts_cap) gx = c->cov_parts_cap;
     if ((long long)gx > nchunks) gx = (int)nchunks;
     alignas(64) CUtensorMap tmH;
-    { const int rc = make_tensor_map(&tmH, H, c->npix, T); if (rc) return rc; }
+    { const int rc = holo_make_tensor_map(&tmH, H, c->npix, T, COV_P); if (rc) return rc; }
     {
         HoloProf prof(c, HOLO_K_COV_PARTIAL, st);
         k_cov_partial<<<dim3(gx, plan.ngroups), COV_NW * 32, smem, st>>>(tmH, c->cov_partials, c->npix, T, T8, nstages, plan);

@@ -92,6 +92,7 @@ static int create_impl(holo_ctx* c) {
     c->tune[HOLO_TUNE_COV_GRIDX] = c->num_sms;
     c->tune[HOLO_TUNE_PROJ_COMPLEMENT] = 1;
     c->tune[HOLO_TUNE_FFT_PERSISTENT] = 1;
+    c->tune[HOLO_TUNE_PROJ_TMA] = 1;
     c->tune[HOLO_TUNE_EIG_MAX_SWEEPS] = 30;
     c->scratch_frames = (int)grp;
     c->cov_parts_cap = 4 * c->num_sms;

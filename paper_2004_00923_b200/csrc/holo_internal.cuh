@@ -17,6 +17,7 @@ enum {
     HOLO_TUNE_FFT_PERSISTENT = 3,  // 1 = single persistent fresnel kernel (default set at create)
     HOLO_TUNE_EIG_MAX_SWEEPS = 4,
     HOLO_TUNE_PROFILE = 5,
+    HOLO_TUNE_PROJ_TMA = 7,        // 1 = deflation projection fed by a TMA ring (default), 0 = register-streaming kernel
     HOLO_TUNE_FFT_LAG = 6,         // frames between the row pass and the column pass in the fused kernel (0 = auto)         // 1 = bracket every kernel launch with events (holo_profile_read)
 };
 
