@@ -256,15 +256,26 @@ def run_ours(args, cfg):
         n_host = 2
         host_frames = torch.empty((n_host, T, n, n), dtype=torch.int16).pin_memory()
         host_frames.copy_(frames[:n_host * T].view(torch.int16).reshape(n_host, T, n, n).cpu())
-        host_img = torch.empty((n, n), dtype=torch.float32).pin_memory()
+        host_img = torch.empty((2, n, n), dtype=torch.float32).pin_memory()
         k2 = max(3, min(args.e2e_steps, steps))
+
+        def e2e_step(i):
+            if streaming:
+                h.submit_host(host_frames[i % n_host], host_img[i % 2], st)
+            else:
+                h.process_host(host_frames[i % n_host], host_img[i % 2], st)
+
         for i in range(3):
-            h.process_host(host_frames[i % n_host], host_img, st)
+            e2e_step(i)
+        if streaming:
+            h.flush_host(st)
         barrier()
         a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         a0.record(st)
         for i in range(k2):
-            h.process_host(host_frames[i % n_host], host_img, st)
+            e2e_step(i)
+        if streaming:
+            h.flush_host(st)                 # the last image reaches the host inside the timed region
         a1.record(st)
         barrier()
         ms2 = a0.elapsed_time(a1)
@@ -274,7 +285,8 @@ def run_ours(args, cfg):
             ms2 = float(t.item())
         e2e = {"value": world * k2 / (ms2 * 1e-3), "unit": "images/s", "h2d_bytes_per_step": fbytes,
                "d2h_bytes_per_step": n * n * 4, "steps": k2, "ms_per_step": ms2 / k2,
-               "api": "holo_process_host (pinned host frames -> host image, synchronous)"}
+               "api": ("holo_submit_host/holo_flush_host (pinned host frames -> host images; the H2D copy of stack i runs under "
+                       "the kernels of stack i-1)") if streaming else "holo_process_host (pinned host frames -> host image, synchronous)"}
 
     # ---- CPU oracle on the box's host cores (rank 0, N = 1 only): a reported baseline, not the target
     cpu = None

@@ -92,9 +92,18 @@ int holo_process(holo_ctx* ctx, const uint16_t* frames_dev, float* image_dev, ho
 int holo_submit(holo_ctx* ctx, const uint16_t* frames_dev, float* image_dev, holo_stream stream);
 int holo_flush(holo_ctx* ctx, holo_stream stream);
 
+/* Streaming form with HOST buffers: holo_submit_host copies stack i host -> device on a copy stream owned
+ * by the handle (double-buffered staging, so the copy runs under the kernels of stack i-1), enqueues
+ * holo_submit on `stream`, and enqueues the device -> host copy of the image of stack i-1.  It returns when
+ * the frames have been copied (frames_host may then be reused); every image_host passed so far is complete
+ * only after holo_flush_host returns (it synchronises `stream`).  Pinned host memory is needed for the
+ * copies to overlap.  This is the end-to-end call bench.py's `e2e` times. */
+int holo_submit_host(holo_ctx* ctx, const uint16_t* frames_host, float* image_host, holo_stream stream);
+int holo_flush_host(holo_ctx* ctx, holo_stream stream);
+
 /* Same path, HOST buffers (pinned or pageable): copies frames in, runs holo_process, copies the
  * image out, and synchronises `stream` before returning.  Uses a frame/image staging buffer owned by
- * the handle (allocated at first use).  This is the end-to-end call bench.py's `e2e` times. */
+ * the handle (allocated at first use).  Serial: one stack per call. */
 int holo_process_host(holo_ctx* ctx, const uint16_t* frames_host, float* image_host, holo_stream stream);
 
 /* A0+A1+A2: frames_dev -> H_dev (float2 [T][ny][nx]).  (Eq. 1) */

@@ -54,6 +54,10 @@ static void free_ctx(holo_ctx* c) {
         cudaStreamDestroy(c->side);
         for (int i = 0; i < 2; ++i) { cudaEventDestroy(c->ev_cov[i]); cudaEventDestroy(c->ev_eig[i]); }
     }
+    if (c->copy) {
+        cudaStreamDestroy(c->copy);
+        for (int i = 0; i < 2; ++i) { cudaFree(c->fstage[i]); cudaFree(c->istage[i]); cudaEventDestroy(c->ev_h2d[i]); cudaEventDestroy(c->ev_free[i]); }
+    }
     if (c->frames_stage) cudaFree(c->frames_stage);
     if (c->image_stage) cudaFree(c->image_stage);
     delete c;
@@ -251,6 +255,56 @@ extern "C" int holo_submit(holo_ctx* c, const uint16_t* frames_dev, float* image
 extern "C" int holo_flush(holo_ctx* c, holo_stream stream) {
     CHECK_CTX(c);
     return project_pending(c, (cudaStream_t)stream);
+}
+
+// ---- streaming host entry: H2D of stack i (copy stream) runs under the kernels of stack i-1 ----------
+static int host_init(holo_ctx* c) {
+    if (c->copy) return HOLO_OK;
+    const size_t fbytes = (size_t)c->T * c->npix * sizeof(uint16_t), ibytes = (size_t)c->npix * sizeof(float);
+    for (int i = 0; i < 2; ++i) {
+        HOLO_CUDA_OK(cudaMalloc(&c->fstage[i], fbytes));
+        HOLO_CUDA_OK(cudaMalloc(&c->istage[i], ibytes));
+        HOLO_CUDA_OK(cudaEventCreateWithFlags(&c->ev_h2d[i], cudaEventDisableTiming));
+        HOLO_CUDA_OK(cudaEventCreateWithFlags(&c->ev_free[i], cudaEventDisableTiming));
+    }
+    HOLO_CUDA_OK(cudaStreamCreateWithFlags(&c->copy, cudaStreamNonBlocking));
+    return HOLO_OK;
+}
+
+static int deliver_host(holo_ctx* c, cudaStream_t st) {      // D2H of the image whose projection was just enqueued
+    if (!c->pend_image_host) return HOLO_OK;
+    HOLO_CUDA_OK(cudaMemcpyAsync(c->pend_image_host, c->istage[c->pend_islot], (size_t)c->npix * sizeof(float), cudaMemcpyDeviceToHost, st));
+    c->pend_image_host = nullptr;
+    return HOLO_OK;
+}
+
+extern "C" int holo_submit_host(holo_ctx* c, const uint16_t* frames_host, float* image_host, holo_stream stream) {
+    CHECK_CTX(c); CHECK_PTR(frames_host, "frames_host"); CHECK_PTR(image_host, "image_host");
+    cudaStream_t st = (cudaStream_t)stream;
+    int rc;
+    if ((rc = host_init(c))) return rc;
+    const int s = (int)(c->nsubmit_host & 1);
+    const size_t fbytes = (size_t)c->T * c->npix * sizeof(uint16_t);
+    if (c->nsubmit_host >= 2) HOLO_CUDA_OK(cudaStreamWaitEvent(c->copy, c->ev_free[s], 0));   // stage s was read by stack i-2
+    HOLO_CUDA_OK(cudaMemcpyAsync(c->fstage[s], frames_host, fbytes, cudaMemcpyHostToDevice, c->copy));
+    HOLO_CUDA_OK(cudaEventRecord(c->ev_h2d[s], c->copy));
+    HOLO_CUDA_OK(cudaStreamWaitEvent(st, c->ev_h2d[s], 0));
+    if ((rc = holo_submit(c, c->fstage[s], c->istage[s], stream))) return rc;   // enqueues the projection of stack i-1
+    HOLO_CUDA_OK(cudaEventRecord(c->ev_free[s], st));
+    if ((rc = deliver_host(c, st))) return rc;
+    c->pend_image_host = image_host; c->pend_islot = s; c->nsubmit_host++;
+    HOLO_CUDA_OK(cudaEventSynchronize(c->ev_h2d[s]));        // frames_host may be reused on return
+    return HOLO_OK;
+}
+
+extern "C" int holo_flush_host(holo_ctx* c, holo_stream stream) {
+    CHECK_CTX(c);
+    cudaStream_t st = (cudaStream_t)stream;
+    int rc;
+    if ((rc = holo_flush(c, stream))) return rc;
+    if ((rc = deliver_host(c, st))) return rc;
+    HOLO_CUDA_OK(cudaStreamSynchronize(st));
+    return HOLO_OK;
 }
 
 extern "C" int holo_process_host(holo_ctx* c, const uint16_t* frames_host, float* image_host, holo_stream stream) {

@@ -74,6 +74,12 @@ struct holo_ctx {
     // host staging for holo_process_host
     uint16_t* frames_stage;
     float* image_stage;
+    // streaming host entry (holo_submit_host / holo_flush_host): double-buffered staging + copy stream
+    uint16_t* fstage[2]; float* istage[2];
+    cudaStream_t copy;
+    cudaEvent_t ev_h2d[2], ev_free[2];
+    float* pend_image_host; int pend_islot;
+    long long nsubmit_host;
 };
 
 void holo_set_error(const char* fmt, ...);

@@ -325,6 +325,14 @@ def test_submit_stream_matches_process(torch_cuda):
     assert torch.equal(A, ref[3]) and torch.equal(B, ref[1]) and torch.equal(C2, ref[4])
     rc, status = h.status(st)
     assert rc == 0
+    # host streaming entry: same images, delivered to pinned host buffers by holo_flush_host
+    fh = [torch.from_numpy(G.stack_np(cfg, 20 + i).view(np.int16)).pin_memory() for i in range(5)]
+    oh = [torch.zeros((128, 128), dtype=torch.float32).pin_memory() for _ in range(5)]
+    for f, o in zip(fh, oh):
+        h.submit_host(f, o, st)
+    h.flush_host(st)
+    for o, b in zip(oh, ref):
+        assert torch.equal(o, b.cpu())
     h.close()
 
 
