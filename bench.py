@@ -237,9 +237,12 @@ def run_ours(args, cfg):
         stages["cov_partial"]["TFLOPs_fp32"] = round(cov_flops / (stages["cov_partial"]["us_per_launch"] * 1e-6) / 1e12, 2)
     dom = max(stages, key=lambda k: stages[k]["share"])
     traffic = None
-    tpath = os.path.join(ROOT, "profiles", "traffic.json")
-    if os.path.exists(tpath):
-        traffic = json.load(open(tpath)).get(dom)
+    tpath = os.path.join(ROOT, "profiles", "r01c_traffic.csv")     # dram__bytes_read.sum + dram__bytes_write.sum, one ncu --set full capture
+    if os.path.exists(tpath) and cfg.name.startswith("cfg3"):
+        for ln in open(tpath).read().splitlines()[1:]:
+            k, v = ln.split(",")
+            if k == dom:
+                traffic = int(v)
     if dom == "cov_partial" and cov_flops / sb["cov"] > fp32_peak_tflops * 1e12 / (hbm_peak * 1e9):
         roof = {"kernel": dom, "bound": "alu", "achieved": stages[dom]["TFLOPs_fp32"], "peak": round(fp32_peak_tflops, 1),
                 "unit": "TFLOP/s", "frac": round(stages[dom]["TFLOPs_fp32"] / fp32_peak_tflops, 4), "traffic": traffic,
