@@ -214,6 +214,121 @@ k_cov_partial(const __grid_constant__ CUtensorMap tmH, float2* __restrict__ part
     }
 }
 
+// ------------------------------------------------------------------------------------------------
+// Real part only, for the hologram stacks of holo_process / holo_submit (T <= 32).  There H_t = F[q d_t] with d_t
+// real, q unimodular and F unitary up to nx ny, so C_ts = nx ny sum_x d_t d_s is REAL in exact arithmetic
+// (R8, R21): the imaginary part the complex kernel would compute is rounding noise and half the
+// FFMA work.  Re C_ts = sum_p (re_t re_s + im_t im_s): a real Gram over 2 N_p samples.  Jobs (one real
+// accumulator per entry): "off" = rows [16,32) x one 8-row block of [0,16) (128 entries, 24 loads per pixel),
+// "diag16" = lower triangle of a 16-row block (136 entries, 16 loads).  Four jobs cover T <= 32; warps w and
+// w+4 run the same job on alternate 128-pixel chunks (two partials per CTA).  T <= 16: one diag16 job,
+// four warps take every fourth chunk each.  Same TMA ring / mbarrier protocol as k_cov_partial.
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(COV_NW * 32, 1)
+k_cov_partial_real(const __grid_constant__ CUtensorMap tmH, float2* __restrict__ partials, long long npix, int T8,
+                   int nstages, int nslots, int njobs) {
+    extern __shared__ __align__(128) unsigned char smraw[];
+    uint64_t* full = reinterpret_cast<uint64_t*>(smraw);
+    uint64_t* empty = full + COV_MAX_STAGES;
+    float2* ring = reinterpret_cast<float2*>(smraw + 128);
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int stage_elems = nslots * 8 * COV_P;
+    const long long nchunks = npix / COV_P;
+    const int ngroups = njobs == 4 ? 2 : 4;              // warp groups: group g owns the CTA's chunks k = g (mod ngroups)
+    const int nactive = njobs * ngroups;                 // 8 or 4 warps
+    if (tid == 0) {
+        for (int s = 0; s < nstages; ++s) { mbar_init(full + s, 1); mbar_init(empty + s, (uint32_t)njobs); }   // nstages is a multiple of ngroups: a stage always serves the same group
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    int ps = 0; uint32_t pph = 0;
+    long long pchunk = blockIdx.x;
+    auto issue = [&]() {
+        if (pchunk >= nchunks) return;
+        mbar_wait(empty + ps, pph ^ 1u);
+        if (lane == 0) mbar_arrive_expect_tx(full + ps, (uint32_t)stage_elems * (uint32_t)sizeof(float2));
+        __syncwarp();
+        if (lane < nslots) tma_2d_g2s(ring + (size_t)ps * stage_elems + lane * 8 * COV_P, &tmH, (int)(pchunk * (2 * COV_P)), 8 * lane, full + ps);
+        pchunk += gridDim.x;
+        if (++ps == nstages) { ps = 0; pph ^= 1u; }
+    };
+    if (warp == 0)
+        for (int d = 0; d < nstages - 2; ++d) issue();
+    if (warp >= nactive) return;
+    const int job = warp % njobs, group = warp / njobs;
+    float2* out = partials + ((size_t)blockIdx.x * ngroups + group) * T8 * T8;
+    int s = 0; uint32_t ph = 0;
+    if (njobs == 4 && job < 2) {
+        float acc[16][8];
+#pragma unroll
+        for (int i = 0; i < 16; ++i)
+#pragma unroll
+            for (int j = 0; j < 8; ++j) acc[i][j] = 0.f;
+        int k = 0;
+        for (long long chunk = blockIdx.x; chunk < nchunks; chunk += gridDim.x, ++k) {
+            if (warp == 0) issue();
+            if (k % ngroups != group) { if (++s == nstages) { s = 0; ph ^= 1u; } continue; }
+            mbar_wait(full + s, ph);
+            const float2* A = ring + (size_t)s * stage_elems + 16 * COV_P + lane;
+            const float2* B = ring + (size_t)s * stage_elems + job * 8 * COV_P + lane;
+#pragma unroll 1
+            for (int it = 0; it < COV_P / 32; ++it) {
+                float2 a[16], b[8];
+#pragma unroll
+                for (int i = 0; i < 16; ++i) a[i] = A[i * COV_P + it * 32];
+#pragma unroll
+                for (int j = 0; j < 8; ++j) b[j] = B[j * COV_P + it * 32];
+#pragma unroll
+                for (int i = 0; i < 16; ++i)
+#pragma unroll
+                    for (int j = 0; j < 8; ++j) acc[i][j] = fmaf(a[i].y, b[j].y, fmaf(a[i].x, b[j].x, acc[i][j]));
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(empty + s);
+            if (++s == nstages) { s = 0; ph ^= 1u; }
+        }
+#pragma unroll
+        for (int i = 0; i < 16; ++i)
+#pragma unroll
+            for (int j = 0; j < 8; ++j) {
+                const float x = warp_sum(acc[i][j]);
+                if (lane == 0 && 16 + i < T8) out[(16 + i) * T8 + (job * 8 + j)] = make_float2(x, 0.f);
+            }
+    } else {
+        const int r0 = (njobs == 4 && job == 3) ? 16 : 0;
+        float acc[136];
+#pragma unroll
+        for (int e = 0; e < 136; ++e) acc[e] = 0.f;
+        int k = 0;
+        for (long long chunk = blockIdx.x; chunk < nchunks; chunk += gridDim.x, ++k) {
+            if (warp == 0) issue();
+            if (k % ngroups != group) { if (++s == nstages) { s = 0; ph ^= 1u; } continue; }
+            mbar_wait(full + s, ph);
+            const float2* A = ring + (size_t)s * stage_elems + r0 * COV_P + lane;
+#pragma unroll 1
+            for (int it = 0; it < COV_P / 32; ++it) {
+                float2 a[16];
+#pragma unroll
+                for (int i = 0; i < 16; ++i) a[i] = A[i * COV_P + it * 32];
+#pragma unroll
+                for (int i = 0; i < 16; ++i)
+#pragma unroll
+                    for (int j = 0; j <= i; ++j) acc[i * (i + 1) / 2 + j] = fmaf(a[i].y, a[j].y, fmaf(a[i].x, a[j].x, acc[i * (i + 1) / 2 + j]));
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(empty + s);
+            if (++s == nstages) { s = 0; ph ^= 1u; }
+        }
+#pragma unroll
+        for (int i = 0; i < 16; ++i)
+#pragma unroll
+            for (int j = 0; j <= i; ++j) {
+                const float x = warp_sum(acc[i * (i + 1) / 2 + j]);
+                if (lane == 0 && r0 + i < T8) out[(r0 + i) * T8 + (r0 + j)] = make_float2(x, 0.f);
+            }
+    }
+}
+
 // fixed-order FP64 reduction over the partials: one warp per lower-triangle entry, lane l sums parts
 // l, l+32, ... in order, then a fixed shuffle tree (deterministic).  Writes the full Hermitian C (both
 // triangles), diagonal imaginary parts forced to 0.
@@ -295,9 +410,42 @@ static void make_plan_groups(int nb, CovPlan* p) {
     }
 }
 
-int holo_launch_covariance(holo_ctx* c, const float2* H, float2* C, cudaStream_t st) {
+static int launch_cov_real(holo_ctx* c, const float2* H, float2* C, cudaStream_t st) {
+    const int T = c->T, T8 = (T + 7) / 8 * 8;
+    const int njobs = T8 > 16 ? 4 : 1, nslots = njobs == 4 ? 4 : 2, ngroups = njobs == 4 ? 2 : 4;
+    const size_t stage_bytes = (size_t)nslots * 8 * COV_P * sizeof(float2);
+    int nstages = (int)(COV_SMEM_BUDGET / stage_bytes);
+    if (nstages > COV_MAX_STAGES) nstages = COV_MAX_STAGES;
+    nstages -= nstages % ngroups;                          // a stage always serves the same warp group
+    const size_t smem = 128 + (size_t)nstages * stage_bytes;
+    static bool attr = false;
+    if (!attr) {
+        HOLO_CUDA_OK(cudaFuncSetAttribute(k_cov_partial_real, cudaFuncAttributeMaxDynamicSharedMemorySize, COV_SMEM_BUDGET + 128));
+        attr = true;
+    }
+    const long long nchunks = c->npix / COV_P;
+    int gx = c->tune[HOLO_TUNE_COV_GRIDX];
+    if (gx * ngroups > c->cov_parts_cap) gx = c->cov_parts_cap / ngroups;
+    if ((long long)gx > nchunks) gx = (int)nchunks;
+    alignas(64) CUtensorMap tmH;
+    { const int rc = holo_make_tensor_map(&tmH, H, c->npix, T, COV_P); if (rc) return rc; }
+    {
+        HoloProf prof(c, HOLO_K_COV_PARTIAL, st);
+        k_cov_partial_real<<<gx, COV_NW * 32, smem, st>>>(tmH, c->cov_partials, c->npix, T8, nstages, nslots, njobs);
+    }
+    HOLO_CUDA_OK(cudaGetLastError());
+    const int n = T * T;
+    HoloProf prof(c, HOLO_K_COV_REDUCE, st);
+    k_cov_reduce<<<(n * 32 + 255) / 256, 256, 0, st>>>(c->cov_partials, gx * ngroups, T, T8, C);
+    HOLO_CUDA_OK(cudaGetLastError());
+    return HOLO_OK;
+}
+
+// real_only: the caller guarantees that C is real in exact arithmetic (holograms produced by holo_fresnel)
+int holo_launch_covariance(holo_ctx* c, const float2* H, float2* C, cudaStream_t st, bool real_only) {
     const int T = c->T, T8 = (T + 7) / 8 * 8, nb = T8 / 8;
     if (nb < 1 || nb > 8) { holo_set_error("T out of range"); return HOLO_ERR_ARG; }
+    if (real_only && T8 <= 32 && c->tune[HOLO_TUNE_COV_REAL]) return launch_cov_real(c, H, C, st);
     CovPlan plan;
     make_plan(nb, &plan);
     int max_slots = 0;

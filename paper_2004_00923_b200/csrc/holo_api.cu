@@ -97,6 +97,7 @@ static int create_impl(holo_ctx* c) {
     c->tune[HOLO_TUNE_PROJ_COMPLEMENT] = 1;
     c->tune[HOLO_TUNE_FFT_PERSISTENT] = 1;
     c->tune[HOLO_TUNE_PROJ_TMA] = 1;
+    c->tune[HOLO_TUNE_COV_REAL] = 1;
     c->tune[HOLO_TUNE_EIG_MAX_SWEEPS] = 30;
     c->scratch_frames = (int)grp;
     c->cov_parts_cap = 4 * c->num_sms;
@@ -190,7 +191,7 @@ extern "C" int holo_process(holo_ctx* c, const uint16_t* frames_dev, float* imag
     if ((rc = project_pending(c, st))) return rc;          // a holo_submit still owes its image: deliver it first
     c->nsubmit = 0;                                        // the next holo_submit starts again with slot 0
     if ((rc = holo_launch_fresnel(c, frames_dev, c->H, st))) return rc;
-    if ((rc = holo_launch_covariance(c, c->H, c->C, st))) return rc;
+    if ((rc = holo_launch_covariance(c, c->H, c->C, st, /*real_only=*/true))) return rc;
     if ((rc = holo_launch_eig(c, c->C, c->evals, c->V, st))) return rc;
     return holo_launch_project(c, c->H, c->V, c->k_lo, c->k_hi, c->tune[HOLO_TUNE_PROJ_COMPLEMENT], image_dev, st);
 }
@@ -239,7 +240,7 @@ extern "C" int holo_submit(holo_ctx* c, const uint16_t* frames_dev, float* image
     float2* C = s ? c->C1 : c->C;
     if ((rc = holo_launch_fresnel(c, frames_dev, H, st))) return rc;
     if ((rc = project_pending(c, st))) return rc;
-    if ((rc = holo_launch_covariance(c, H, C, st))) return rc;
+    if ((rc = holo_launch_covariance(c, H, C, st, /*real_only=*/true))) return rc;
     HOLO_CUDA_OK(cudaEventRecord(c->ev_cov[s], st));
     HOLO_CUDA_OK(cudaStreamWaitEvent(c->side, c->ev_cov[s], 0));
     int32_t* status_main = c->status;

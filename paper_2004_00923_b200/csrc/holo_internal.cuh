@@ -18,6 +18,7 @@ enum {
     HOLO_TUNE_EIG_MAX_SWEEPS = 4,
     HOLO_TUNE_PROFILE = 5,
     HOLO_TUNE_PROJ_TMA = 7,        // 1 = deflation projection fed by a TMA ring (default), 0 = register-streaming kernel
+    HOLO_TUNE_COV_REAL = 8,        // 1 = holo_process / holo_submit compute Re C only (C is real there, R21); default 1
     HOLO_TUNE_FFT_LAG = 6,         // frames between the row pass and the column pass in the fused kernel (0 = auto)         // 1 = bracket every kernel launch with events (holo_profile_read)
 };
 
@@ -107,7 +108,7 @@ struct HoloProf {
 
 // stage launchers (each only enqueues on `st`)
 int holo_launch_fresnel(holo_ctx* c, const uint16_t* frames, float2* H, cudaStream_t st);
-int holo_launch_covariance(holo_ctx* c, const float2* H, float2* C, cudaStream_t st);
+int holo_launch_covariance(holo_ctx* c, const float2* H, float2* C, cudaStream_t st, bool real_only = false);
 int holo_launch_eig(holo_ctx* c, const float2* C, float* evals, float2* V, cudaStream_t st);
 // mode 0: direct over columns [k_lo,k_hi] of V; mode 1: complement (total - columns outside)
 int holo_launch_project(holo_ctx* c, const float2* H, const float2* V, int k_lo, int k_hi,
