@@ -400,7 +400,7 @@ static bool plan_shape(int N, int* E, int* R1, int* R2) {
         case 256:  *E = 16; *R1 = 16; *R2 = 1;  return true;
         case 512:  *E = 32; *R1 = 16; *R2 = 1;  return true;
         case 1024: *E = 32; *R1 = 32; *R2 = 1;  return true;
-        case 2048: *E = 16; *R1 = 16; *R2 = 8;  return true;
+        case 2048: *E = 32; *R1 = 32; *R2 = 2;  return true;
         case 4096: *E = 16; *R1 = 16; *R2 = 16; return true;
     }
     return false;
@@ -472,7 +472,7 @@ static int launch_fft(int N, const FftArgs& a, int num_sms, cudaStream_t st) {
         case 256:  return launch_fft_t<256, 16, 16, 1, 16, COL, PRO>(a, num_sms, st);
         case 512:  return launch_fft_t<512, 32, 16, 1, 16, COL, PRO>(a, num_sms, st);
         case 1024: return launch_fft_t<1024, 32, 32, 1, 8, COL, PRO>(a, num_sms, st);
-        case 2048: return launch_fft_t<2048, 16, 16, 8, 4, COL, PRO>(a, num_sms, st);
+        case 2048: return launch_fft_t<2048, 32, 32, 2, 4, COL, PRO>(a, num_sms, st);
         case 4096: return launch_fft_t<4096, 16, 16, 16, 4, COL, PRO>(a, num_sms, st);
     }
     holo_set_error("unsupported FFT length %d", N);
@@ -513,7 +513,7 @@ static int launch_fresnel_fused(int N, const FresnelArgs& p, int num_sms, cudaSt
         case 256:  return launch_fresnel_t<256, 16, 16, 1, 16>(p, num_sms, st);
         case 512:  return launch_fresnel_t<512, 32, 16, 1, 16>(p, num_sms, st);
         case 1024: return launch_fresnel_t<1024, 32, 32, 1, FUSED_B1024>(p, num_sms, st);
-        case 2048: return launch_fresnel_t<2048, 16, 16, 8, 4>(p, num_sms, st);
+        case 2048: return launch_fresnel_t<2048, 32, 32, 2, 4>(p, num_sms, st);
         case 4096: return launch_fresnel_t<4096, 16, 16, 16, 4>(p, num_sms, st);
     }
     holo_set_error("unsupported FFT length %d", N);

@@ -150,13 +150,10 @@ __global__ void __launch_bounds__(256) k_project_deflate(const ProjArgs a, int n
 // elected producer lane, 5-6 stages in flight) instead of T dependent 16-byte loads per thread.  Four
 // consumer warps, one pixel per lane; a lane reads its pixel of every frame from shared memory (conflict
 // free: 32 consecutive float2).  Bound by HBM; measured 4.7 -> see profiles/ TB/s.
-#ifndef PROJ_P
-#define PROJ_P 256                 // pixels per stage
-#endif
-#define PROJ_NW (PROJ_P / 32)       // consumer warps (32 pixels each)
+// PROJ_P pixels per stage (256 up to T = 32, 128 above so that >= 2 stages fit); PROJ_P / 32 consumer warps
 #define PROJ_MAX_STAGES 8
-template <int TMAX>
-__global__ void __launch_bounds__(PROJ_NW * 32, 1)
+template <int TMAX, int PROJ_P>
+__global__ void __launch_bounds__(PROJ_P, 1)
 k_project_deflate_tma(const __grid_constant__ CUtensorMap tmH, const ProjArgs a, int nc, int nstages) {
     extern __shared__ __align__(128) unsigned char smraw[];
     uint64_t* full = reinterpret_cast<uint64_t*>(smraw);
@@ -174,7 +171,7 @@ k_project_deflate_tma(const __grid_constant__ CUtensorMap tmH, const ProjArgs a,
         Vd[i] = t < a.T ? a.V[t * a.T + col] : make_float2(0.f, 0.f);
     }
     if (tid == 0) {
-        for (int s = 0; s < nstages; ++s) { mbar_init(full + s, 1); mbar_init(empty + s, PROJ_NW); }
+        for (int s = 0; s < nstages; ++s) { mbar_init(full + s, 1); mbar_init(empty + s, PROJ_P / 32); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
@@ -233,6 +230,7 @@ k_project_deflate_tma(const __grid_constant__ CUtensorMap tmH, const ProjArgs a,
 }
 
 template <int TMAX> static int launch_deflate(holo_ctx* c, const ProjArgs& a, int nc, cudaStream_t st) {
+    constexpr int PROJ_P = TMAX <= 32 ? 256 : 128;
     const int vbytes = ((nc > 0 ? nc : 1) * TMAX * (int)sizeof(float2) + 127) & ~127;
     const size_t stage_bytes = (size_t)TMAX * PROJ_P * sizeof(float2);
     int nstages = (int)((200 * 1024 - vbytes) / stage_bytes);
@@ -241,7 +239,7 @@ template <int TMAX> static int launch_deflate(holo_ctx* c, const ProjArgs& a, in
         const size_t smem = 128 + vbytes + (size_t)nstages * stage_bytes;
         static bool attr = false;
         if (!attr) {
-            HOLO_CUDA_OK(cudaFuncSetAttribute(k_project_deflate_tma<TMAX>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024 + 128));
+            HOLO_CUDA_OK(cudaFuncSetAttribute(k_project_deflate_tma<TMAX, PROJ_P>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024 + 128));
             attr = true;
         }
         alignas(64) CUtensorMap tmH;
@@ -249,7 +247,7 @@ template <int TMAX> static int launch_deflate(holo_ctx* c, const ProjArgs& a, in
         const long long nchunks = a.npix / PROJ_P;
         const int grid = (int)(nchunks < c->num_sms ? nchunks : c->num_sms);
         HoloProf prof(c, HOLO_K_PROJECT, st);
-        k_project_deflate_tma<TMAX><<<grid, PROJ_NW * 32, smem, st>>>(tmH, a, nc, nstages);
+        k_project_deflate_tma<TMAX, PROJ_P><<<grid, PROJ_P, smem, st>>>(tmH, a, nc, nstages);
         HOLO_CUDA_OK(cudaGetLastError());
         return HOLO_OK;
     }

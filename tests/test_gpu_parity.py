@@ -336,6 +336,30 @@ def test_submit_stream_matches_process(torch_cuda):
     h.close()
 
 
+def test_process_real_covariance_identity(torch_cuda):
+    """DESIGN.md R21: holo_process accumulates Re C only (C is real for holograms of real frames).  Its C must have
+    a zero imaginary part and agree with the complex Gram of holo_covariance on the same H; M must agree too."""
+    torch = torch_cuda
+    cfg = G.small_config(n=128, T=32)
+    d = _to_dev(torch, G.stack_np(cfg, 31))
+    h = _holo(128, 128, 32, 2, 32)
+    M1 = torch.empty((128, 128), dtype=torch.float32, device="cuda")
+    h.process(d, M1)
+    C_real = h.workspace_tensor(2).cpu().numpy()
+    H = h.workspace_tensor(1)
+    Cc = torch.empty((32, 32), dtype=torch.complex64, device="cuda")
+    h.covariance(H, Cc)
+    Cc = Cc.cpu().numpy()
+    assert np.all(C_real.imag == 0)
+    assert rel_l2(C_real, Cc) <= 5e-6
+    assert np.linalg.norm(Cc.imag) <= 1e-5 * np.linalg.norm(Cc.real)
+    h.tune(8, 0)                                  # complex Gram inside holo_process
+    M2 = torch.empty_like(M1)
+    h.process(d, M2)
+    assert rel_l2(M2.cpu().numpy(), M1.cpu().numpy()) <= 2e-5
+    h.close()
+
+
 def test_bad_arguments(torch_cuda):
     from paper_2004_00923_b200 import Holo, HoloError
     for args in [(100, 64, 8, LAM, PITCH, Z, 2, 8), (64, 8, 8, LAM, PITCH, Z, 2, 8), (64, 64, 1, LAM, PITCH, Z, 1, 1),
