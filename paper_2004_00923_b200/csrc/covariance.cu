@@ -329,40 +329,32 @@ k_cov_partial_real(const __grid_constant__ CUtensorMap tmH, float2* __restrict__
     }
 }
 
-// fixed-order FP64 reduction over the partials.  CTA = (row t, block of 32 columns s): lane = s, warp g sums the
-// parts g, g+8, g+16, ... in that order (every load is a coalesced row segment of one partial, eight in flight),
-// then the eight warp sums are added in the order g = 0..7 (deterministic).  Writes the full Hermitian C (both
+// fixed-order FP64 reduction over the partials: one warp per lower-triangle entry, lane l sums parts
+// l, l+32, ... in order, then a fixed shuffle tree (deterministic).  Writes the full Hermitian C (both
 // triangles), diagonal imaginary parts forced to 0.
 __global__ void __launch_bounds__(256) k_cov_reduce(const float2* __restrict__ partials, int nparts, int T, int T8, float2* __restrict__ C) {
-    __shared__ double sre[8][32], sim[8][32];
-    const int lane = threadIdx.x & 31, g = threadIdx.x >> 5;
-    const int t = blockIdx.x, sidx = blockIdx.y * 32 + lane;
-    const bool ok = sidx <= t && sidx < T;
+    const int w = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+    if (w >= T * T) return;
+    const int t = w / T, s = w - t * T;
+    if (s > t) return;
     double re = 0.0, im = 0.0;
-    if (ok) {
-        const float2* p = partials + t * T8 + sidx;
-        const size_t pstride = (size_t)T8 * T8;
-        int k = g;
-        for (; k + 56 < nparts; k += 64) {
-            float2 v[8];
-#pragma unroll
-            for (int q = 0; q < 8; ++q) v[q] = p[(size_t)(k + 8 * q) * pstride];
-#pragma unroll
-            for (int q = 0; q < 8; ++q) { re += (double)v[q].x; im += (double)v[q].y; }
-        }
-        for (; k < nparts; k += 8) { const float2 v = p[(size_t)k * pstride]; re += (double)v.x; im += (double)v.y; }
+    const float2* p = partials + t * T8 + s;
+    for (int k = lane; k < nparts; k += 32) {
+        const float2 v = p[(size_t)k * T8 * T8];
+        re += (double)v.x;
+        im += (double)v.y;
     }
-    sre[g][lane] = re; sim[g][lane] = im;
-    __syncthreads();
-    if (g == 0 && ok) {
-        re = 0.0; im = 0.0;
 #pragma unroll
-        for (int q = 0; q < 8; ++q) { re += sre[q][lane]; im += sim[q][lane]; }
-        if (sidx == t) {
+    for (int o = 16; o >= 1; o >>= 1) {
+        re += __shfl_xor_sync(0xffffffffu, re, o);
+        im += __shfl_xor_sync(0xffffffffu, im, o);
+    }
+    if (lane == 0) {
+        if (s == t) {
             C[t * T + t] = make_float2((float)re, 0.f);
         } else {
-            C[t * T + sidx] = make_float2((float)re, (float)im);
-            C[sidx * T + t] = make_float2((float)re, (float)-im);
+            C[t * T + s] = make_float2((float)re, (float)im);
+            C[s * T + t] = make_float2((float)re, (float)-im);
         }
     }
 }
@@ -444,7 +436,7 @@ static int launch_cov_real(holo_ctx* c, const float2* H, float2* C, cudaStream_t
     HOLO_CUDA_OK(cudaGetLastError());
     const int n = T * T;
     HoloProf prof(c, HOLO_K_COV_REDUCE, st);
-    k_cov_reduce<<<dim3(T, (T + 31) / 32), 256, 0, st>>>(c->cov_partials, gx * ngroups, T, T8, C);
+    k_cov_reduce<<<(n * 32 + 255) / 256, 256, 0, st>>>(c->cov_partials, gx * ngroups, T, T8, C);
     HOLO_CUDA_OK(cudaGetLastError());
     return HOLO_OK;
 }
@@ -482,7 +474,7 @@ int holo_launch_covariance(holo_ctx* c, const float2* H, float2* C, cudaStream_t
     HOLO_CUDA_OK(cudaGetLastError());
     const int n = T * T;
     HoloProf prof(c, HOLO_K_COV_REDUCE, st);
-    k_cov_reduce<<<dim3(T, (T + 31) / 32), 256, 0, st>>>(c->cov_partials, gx, T, T8, C);
+    k_cov_reduce<<<(n * 32 + 255) / 256, 256, 0, st>>>(c->cov_partials, gx, T, T8, C);
     HOLO_CUDA_OK(cudaGetLastError());
     return HOLO_OK;
 }
