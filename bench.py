@@ -235,8 +235,8 @@ def run_ours(args, cfg):
         us = ms_k / cnt * 1e3
         stages[name] = {"us_per_launch": round(us, 2), "launches_per_step": cnt / prof_steps, "share": round(ms_k / tot_ms, 4),
                         "GBps": round(per_launch_bytes[name] / (us * 1e-6) / 1e9, 1)}
-    # holo_process / holo_submit compute Re C only at T <= 32 (C is real there, R21): half the complex Gram
-    cov_real = T <= 32 and "8=0" not in args.tune
+    # holo_process / holo_submit compute Re C only (C is real there, R21): half the complex Gram
+    cov_real = "8=0" not in args.tune
     cov_flops = (2 if cov_real else 4) * T * (T + 1) * npix
     if "cov_partial" in stages:
         stages["cov_partial"]["form"] = "real part (2T(T+1) flop/pixel)" if cov_real else "complex Hermitian half (4T(T+1) flop/pixel)"

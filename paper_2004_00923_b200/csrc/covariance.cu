@@ -214,19 +214,23 @@ k_cov_partial(const __grid_constant__ CUtensorMap tmH, float2* __restrict__ part
     }
 }
 
+struct RealJob { int kind, a16, b8; };        // kind 0: rows [16 a16, +16) x rows [8 b8, +8);  kind 1: lower triangle of rows [16 a16, +16)
+struct RealPlan { int njobs[2]; RealJob job[2][COV_NW]; };
+
 // ------------------------------------------------------------------------------------------------
-// Real part only, for the hologram stacks of holo_process / holo_submit (T <= 32).  There H_t = F[q d_t] with d_t
+// Real part only, for the hologram stacks of holo_process / holo_submit.  There H_t = F[q d_t] with d_t
 // real, q unimodular and F unitary up to nx ny, so C_ts = nx ny sum_x d_t d_s is REAL in exact arithmetic
 // (R8, R21): the imaginary part the complex kernel would compute is rounding noise and half the
 // FFMA work.  Re C_ts = sum_p (re_t re_s + im_t im_s): a real Gram over 2 N_p samples.  Jobs (one real
 // accumulator per entry): "off" = rows [16,32) x one 8-row block of [0,16) (128 entries, 24 loads per pixel),
 // "diag16" = lower triangle of a 16-row block (136 entries, 16 loads).  Four jobs cover T <= 32; warps w and
 // w+4 run the same job on alternate 128-pixel chunks (two partials per CTA).  T <= 16: one diag16 job,
-// four warps take every fourth chunk each.  Same TMA ring / mbarrier protocol as k_cov_partial.
+// four warps take every fourth chunk each.  32 < T <= 64: nine or sixteen jobs over two CTA groups (gridDim.y),
+// every CTA stages all T rows.  Same TMA ring / mbarrier protocol as k_cov_partial.
 // ------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(COV_NW * 32, 1)
 k_cov_partial_real(const __grid_constant__ CUtensorMap tmH, float2* __restrict__ partials, long long npix, int T8,
-                   int nstages, int nslots, int njobs) {
+                   int nstages, int nslots, int ngroups, int ahead, const RealPlan plan) {
     extern __shared__ __align__(128) unsigned char smraw[];
     uint64_t* full = reinterpret_cast<uint64_t*>(smraw);
     uint64_t* empty = full + COV_MAX_STAGES;
@@ -234,8 +238,9 @@ k_cov_partial_real(const __grid_constant__ CUtensorMap tmH, float2* __restrict__
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int stage_elems = nslots * 8 * COV_P;
     const long long nchunks = npix / COV_P;
-    const int ngroups = njobs == 4 ? 2 : 4;              // warp groups: group g owns the CTA's chunks k = g (mod ngroups)
-    const int nactive = njobs * ngroups;                 // 8 or 4 warps
+    // ngroups warp groups: group g owns the CTA's chunks k = g (mod ngroups); the jobs come from plan.job[blockIdx.y]
+    const int njobs = plan.njobs[blockIdx.y];
+    const int nactive = njobs * ngroups;                 // <= 8 warps
     if (tid == 0) {
         for (int s = 0; s < nstages; ++s) { mbar_init(full + s, 1); mbar_init(empty + s, (uint32_t)njobs); }   // nstages is a multiple of ngroups: a stage always serves the same group
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -253,12 +258,13 @@ k_cov_partial_real(const __grid_constant__ CUtensorMap tmH, float2* __restrict__
         if (++ps == nstages) { ps = 0; pph ^= 1u; }
     };
     if (warp == 0)
-        for (int d = 0; d < nstages - 2; ++d) issue();
+        for (int d = 0; d < ahead; ++d) issue();
     if (warp >= nactive) return;
-    const int job = warp % njobs, group = warp / njobs;
+    const int group = warp / njobs;
+    const RealJob job = plan.job[blockIdx.y][warp % njobs];
     float2* out = partials + ((size_t)blockIdx.x * ngroups + group) * T8 * T8;
     int s = 0; uint32_t ph = 0;
-    if (njobs == 4 && job < 2) {
+    if (job.kind == 0) {
         float acc[16][8];
 #pragma unroll
         for (int i = 0; i < 16; ++i)
@@ -269,8 +275,8 @@ k_cov_partial_real(const __grid_constant__ CUtensorMap tmH, float2* __restrict__
             if (warp == 0) issue();
             if (k % ngroups != group) { if (++s == nstages) { s = 0; ph ^= 1u; } continue; }
             mbar_wait(full + s, ph);
-            const float2* A = ring + (size_t)s * stage_elems + 16 * COV_P + lane;
-            const float2* B = ring + (size_t)s * stage_elems + job * 8 * COV_P + lane;
+            const float2* A = ring + (size_t)s * stage_elems + job.a16 * 16 * COV_P + lane;
+            const float2* B = ring + (size_t)s * stage_elems + job.b8 * 8 * COV_P + lane;
 #pragma unroll 1
             for (int it = 0; it < COV_P / 32; ++it) {
                 float2 a[16], b[8];
@@ -292,10 +298,10 @@ k_cov_partial_real(const __grid_constant__ CUtensorMap tmH, float2* __restrict__
 #pragma unroll
             for (int j = 0; j < 8; ++j) {
                 const float x = warp_sum(acc[i][j]);
-                if (lane == 0 && 16 + i < T8) out[(16 + i) * T8 + (job * 8 + j)] = make_float2(x, 0.f);
+                if (lane == 0 && job.a16 * 16 + i < T8) out[(job.a16 * 16 + i) * T8 + (job.b8 * 8 + j)] = make_float2(x, 0.f);
             }
     } else {
-        const int r0 = (njobs == 4 && job == 3) ? 16 : 0;
+        const int r0 = job.a16 * 16;
         float acc[136];
 #pragma unroll
         for (int e = 0; e < 136; ++e) acc[e] = 0.f;
@@ -411,12 +417,24 @@ static void make_plan_groups(int nb, CovPlan* p) {
 }
 
 static int launch_cov_real(holo_ctx* c, const float2* H, float2* C, cudaStream_t st) {
-    const int T = c->T, T8 = (T + 7) / 8 * 8;
-    const int njobs = T8 > 16 ? 4 : 1, nslots = njobs == 4 ? 4 : 2, ngroups = njobs == 4 ? 2 : 4;
+    const int T = c->T, T8 = (T + 7) / 8 * 8, nb16 = (T8 + 15) / 16;
+    // jobs: one diag16 per 16-row block, two [16 x 8] rectangles per pair of 16-row blocks
+    RealPlan plan;
+    memset(&plan, 0, sizeof(plan));
+    RealJob all[16];
+    int n = 0;
+    for (int a = 1; a < nb16; ++a)
+        for (int b = 0; b < a; ++b) { all[n++] = RealJob{0, a, 2 * b}; all[n++] = RealJob{0, a, 2 * b + 1}; }
+    for (int a = 0; a < nb16; ++a) all[n++] = RealJob{1, a, 0};
+    const int gy = n > COV_NW ? 2 : 1;
+    for (int k = 0; k < n; ++k) { const int g = gy == 2 ? (k & 1) : 0; plan.job[g][plan.njobs[g]++] = all[k]; }
+    const int ngroups = n == 4 ? 2 : n == 1 ? 4 : 1;       // spare warps take alternate chunks
+    const int nslots = nb16 * 2;
     const size_t stage_bytes = (size_t)nslots * 8 * COV_P * sizeof(float2);
     int nstages = (int)(COV_SMEM_BUDGET / stage_bytes);
     if (nstages > COV_MAX_STAGES) nstages = COV_MAX_STAGES;
     nstages -= nstages % ngroups;                          // a stage always serves the same warp group
+    const int ahead = nstages > 3 ? nstages - 2 : nstages - 1;
     const size_t smem = 128 + (size_t)nstages * stage_bytes;
     static bool attr = false;
     if (!attr) {
@@ -424,19 +442,20 @@ static int launch_cov_real(holo_ctx* c, const float2* H, float2* C, cudaStream_t
         attr = true;
     }
     const long long nchunks = c->npix / COV_P;
-    int gx = c->tune[HOLO_TUNE_COV_GRIDX];
+    int gx = c->tune[HOLO_TUNE_COV_GRIDX] / gy;            // all CTAs co-resident: one per SM
+    if (gx < 1) gx = 1;
     if (gx * ngroups > c->cov_parts_cap) gx = c->cov_parts_cap / ngroups;
     if ((long long)gx > nchunks) gx = (int)nchunks;
     alignas(64) CUtensorMap tmH;
     { const int rc = holo_make_tensor_map(&tmH, H, c->npix, T, COV_P); if (rc) return rc; }
     {
         HoloProf prof(c, HOLO_K_COV_PARTIAL, st);
-        k_cov_partial_real<<<gx, COV_NW * 32, smem, st>>>(tmH, c->cov_partials, c->npix, T8, nstages, nslots, njobs);
+        k_cov_partial_real<<<dim3(gx, gy), COV_NW * 32, smem, st>>>(tmH, c->cov_partials, c->npix, T8, nstages, nslots, ngroups, ahead, plan);
     }
     HOLO_CUDA_OK(cudaGetLastError());
-    const int n = T * T;
+    const int nn = T * T;
     HoloProf prof(c, HOLO_K_COV_REDUCE, st);
-    k_cov_reduce<<<(n * 32 + 255) / 256, 256, 0, st>>>(c->cov_partials, gx * ngroups, T, T8, C);
+    k_cov_reduce<<<(nn * 32 + 255) / 256, 256, 0, st>>>(c->cov_partials, gx * ngroups, T, T8, C);
     HOLO_CUDA_OK(cudaGetLastError());
     return HOLO_OK;
 }
@@ -445,7 +464,7 @@ static int launch_cov_real(holo_ctx* c, const float2* H, float2* C, cudaStream_t
 int holo_launch_covariance(holo_ctx* c, const float2* H, float2* C, cudaStream_t st, bool real_only) {
     const int T = c->T, T8 = (T + 7) / 8 * 8, nb = T8 / 8;
     if (nb < 1 || nb > 8) { holo_set_error("T out of range"); return HOLO_ERR_ARG; }
-    if (real_only && T8 <= 32 && c->tune[HOLO_TUNE_COV_REAL]) return launch_cov_real(c, H, C, st);
+    if (real_only && c->tune[HOLO_TUNE_COV_REAL]) return launch_cov_real(c, H, C, st);
     CovPlan plan;
     make_plan(nb, &plan);
     int max_slots = 0;
