@@ -481,6 +481,9 @@ static int launch_fft(int N, const FftArgs& a, int num_sms, cudaStream_t st) {
 #ifndef FUSED_B1024
 #define FUSED_B1024 8          // sequences per CTA of the fused kernel at N = 1024 (4 = four 128-thread CTAs per SM was measured 8 % slower)
 #endif
+#ifndef FUSED_B2048
+#define FUSED_B2048 4          // 2048: 8 (one 512-thread CTA per SM, 64-byte column segments) measured 8 % slower
+#endif
 static int fft_batch(int N) { return N <= 512 ? 16 : N == 1024 ? 8 : 4; }
 
 template <int N, int E, int R1, int R2, int B>
@@ -513,7 +516,7 @@ static int launch_fresnel_fused(int N, const FresnelArgs& p, int num_sms, cudaSt
         case 256:  return launch_fresnel_t<256, 16, 16, 1, 16>(p, num_sms, st);
         case 512:  return launch_fresnel_t<512, 32, 16, 1, 16>(p, num_sms, st);
         case 1024: return launch_fresnel_t<1024, 32, 32, 1, FUSED_B1024>(p, num_sms, st);
-        case 2048: return launch_fresnel_t<2048, 32, 32, 2, 4>(p, num_sms, st);
+        case 2048: return launch_fresnel_t<2048, 32, 32, 2, FUSED_B2048>(p, num_sms, st);
         case 4096: return launch_fresnel_t<4096, 16, 16, 16, 4>(p, num_sms, st);
     }
     holo_set_error("unsupported FFT length %d", N);
@@ -544,7 +547,7 @@ int holo_launch_fresnel(holo_ctx* c, const uint16_t* frames, float2* H, cudaStre
     }
     if (use_fused(c)) {
         FresnelArgs p{};
-        const int Bq = c->nx == 1024 ? FUSED_B1024 : fft_batch(c->nx);
+        const int Bq = c->nx == 1024 ? FUSED_B1024 : c->nx == 2048 ? FUSED_B2048 : fft_batch(c->nx);
         FftArgs& a = p.rows;
         a.frames = frames; a.sum = c->sum; a.qx = c->qxs; a.qy = c->qy; a.in = nullptr; a.out = c->scratch;
         a.tw1 = c->px.tw1; a.tw2 = c->px.tw2; a.ld = c->nx; a.nseq = c->ny; a.T = c->T; a.invT = 1.0f / (float)c->T;
