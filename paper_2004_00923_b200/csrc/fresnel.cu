@@ -168,6 +168,7 @@ template <int N, int E, int R1, int R2, int B, bool COL, bool PRO, int LDC = 0, 
 __device__ __forceinline__ void fft_tile(const FftArgs& a, long long in_foff, long long out_foff, int tile_in_frame, float2* sm,
                                          Mid mid = Mid()) {
     constexpr int TPS = N / E;
+    constexpr int PADN = N + N / E;
     constexpr bool MULTI = (R1 > 1);
     // a row whose N/E threads are exactly one warp is exchanged through that warp's private slice of the buffer:
     // warp-level synchronisation only (the eight warps of a row tile then run freely against each other)
@@ -176,11 +177,9 @@ __device__ __forceinline__ void fft_tile(const FftArgs& a, long long in_foff, lo
     const int tid = threadIdx.x;
     const int j = COL ? tid / B : tid % TPS;
     const int c = COL ? tid % B : tid / TPS;
-    // exchange-buffer index of element i: XOR swizzle of the low digit with the next digit (no padding, conflict free
-    // for the "thread writes E consecutive elements / reads stride-E elements" pattern of the Stockham passes)
     auto sidx = [&](int i) -> int {
-        const int p = (i & ~(E - 1)) | ((i ^ (i / E)) & (E - 1));
-        return COL ? p * B + c : c * N + p;
+        int p = i + i / E;
+        return COL ? p * B + c : c * PADN + p;
     };
     {
         const int s0 = tile_in_frame * B + c;                          // sequence index (row y or column x)
@@ -446,7 +445,7 @@ void holo_fft_plan_free(FftPlan* p) {
 template <int N, int E, int R1, int R2, int B, bool COL, bool PRO>
 static int launch_fft_t(const FftArgs& a, int num_sms, cudaStream_t st) {
     constexpr int threads = (N / E) * B;
-    constexpr size_t smem = (R1 > 1) ? sizeof(float2) * (size_t)N * B : 0;
+    constexpr size_t smem = (R1 > 1) ? sizeof(float2) * (size_t)(N + N / E) * B : 0;
     auto kern = k_fft<N, E, R1, R2, B, COL, PRO>;
     static int blocks_per_sm = 0;      // per instantiation
     if (blocks_per_sm == 0) {
@@ -490,7 +489,7 @@ static int fft_batch(int N) { return N <= 512 ? 16 : N == 1024 ? 8 : 4; }
 template <int N, int E, int R1, int R2, int B>
 static int launch_fresnel_t(const FresnelArgs& p, int num_sms, cudaStream_t st) {
     constexpr int threads = (N / E) * B;
-    constexpr size_t smem = (R1 > 1) ? sizeof(float2) * (size_t)N * B : 0;
+    constexpr size_t smem = (R1 > 1) ? sizeof(float2) * (size_t)(N + N / E) * B : 0;
     auto kern = k_fresnel<N, E, R1, R2, B>;
     static int blocks_per_sm = 0;
     if (blocks_per_sm == 0) {
