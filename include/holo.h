@@ -153,8 +153,12 @@ int holo_status(holo_ctx* ctx, int32_t status_host[4], holo_stream stream);
 int holo_launches_per_process(holo_ctx* ctx);
 
 /* Experiment knobs (not needed for normal use; defaults are chosen at create).  Keys:
- *   0 frames per FFT row/column group (L2 residency of the intermediate), 1 covariance CTAs,
- *   2 allow the complement form in holo_process (default 1), 3 reserved, 4 Jacobi sweep cap. */
+ *   0 frames in the FFT row->column ring (L2 residency of the intermediate), 1 covariance CTAs,
+ *   2 allow the complement (deflation) form in holo_process (default 1), 3 fused persistent Fresnel kernel
+ *   (default 1; 0 = separate row / column launches per frame group), 4 Jacobi sweep cap, 5 per-kernel event
+ *   brackets (holo_profile_read), 6 lag in frames between row and column pass in the fused kernel (0 = ring/2),
+ *   7 TMA-fed projection (default 1), 8 real-part covariance in holo_process / holo_submit (default 1; the
+ *   covariance of holograms of real frames is real in exact arithmetic, R21). */
 int holo_tune(holo_ctx* ctx, int key, int value);
 
 const char* holo_last_error(void);   /* thread-local, static storage */
