@@ -85,8 +85,10 @@ int holo_process(holo_ctx* ctx, const uint16_t* frames_dev, float* image_dev, ho
  * enqueues on `stream` the Fresnel stage of stack i, then the projection of stack i-1 into the image_dev
  * given to submit(i-1), then the covariance of stack i, and forks the single-CTA eigensolver of stack i
  * to a side stream owned by the handle, where it runs under the Fresnel kernels of stack i+1.
- * Contract: the image passed to submit(i) is complete, in `stream` order, after the NEXT holo_submit or
- * after holo_flush; frames_dev may be reused as soon as `stream` has passed the submit.  The handle
+ * By default (T <= 32) the projection of stack i follows its eigensolver on the side stream and runs on about a
+ * quarter of the SMs, next to the (ALU-bound) covariance of stack i+1 on the others.
+ * Contract: the image passed to submit(i) is complete, in `stream` order, after holo_flush, or after the
+ * holo_submit after next (i+2); frames_dev may be reused as soon as `stream` has passed the submit.  The handle
  * allocates a second hologram stack (8*T*nx*ny bytes) at the first call.  holo_process / holo_flush
  * deliver an owed image first.  Use one stream per handle for a submit sequence. */
 int holo_submit(holo_ctx* ctx, const uint16_t* frames_dev, float* image_dev, holo_stream stream);
@@ -158,7 +160,8 @@ int holo_launches_per_process(holo_ctx* ctx);
  *   (default 1; 0 = separate row / column launches per frame group), 4 Jacobi sweep cap, 5 per-kernel event
  *   brackets (holo_profile_read), 6 lag in frames between row and column pass in the fused kernel (0 = ring/2),
  *   7 TMA-fed projection (default 1), 8 real-part covariance in holo_process / holo_submit (default 1; the
- *   covariance of holograms of real frames is real in exact arithmetic, R21). */
+ *   covariance of holograms of real frames is real in exact arithmetic, R21), 9 SMs given to the
+ *   side-stream projection in holo_submit (0 = projection in stream order after the next Fresnel stage). */
 int holo_tune(holo_ctx* ctx, int key, int value);
 
 const char* holo_last_error(void);   /* thread-local, static storage */

@@ -442,7 +442,7 @@ static int launch_cov_real(holo_ctx* c, const float2* H, float2* C, cudaStream_t
         attr = true;
     }
     const long long nchunks = c->npix / COV_P;
-    int gx = c->tune[HOLO_TUNE_COV_GRIDX] / gy;            // all CTAs co-resident: one per SM
+    int gx = (c->cov_grid_cap > 0 ? c->cov_grid_cap : c->tune[HOLO_TUNE_COV_GRIDX]) / gy;   // all CTAs co-resident: one per SM
     if (gx < 1) gx = 1;
     if (gx * ngroups > c->cov_parts_cap) gx = c->cov_parts_cap / ngroups;
     if ((long long)gx > nchunks) gx = (int)nchunks;

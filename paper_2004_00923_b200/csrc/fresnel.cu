@@ -534,17 +534,21 @@ int holo_fresnel_launch_count(holo_ctx* c) {
     return 1 + 2 * groups;
 }
 
-int holo_launch_fresnel(holo_ctx* c, const uint16_t* frames, float2* H, cudaStream_t st) {
-    // A0
-    {
-        long long nvec = c->npix >> 3;
-        int threads = 256;
-        long long want = (nvec + threads - 1) / threads;
-        int grid = (int)(want < (long long)c->num_sms * 8 ? want : (long long)c->num_sms * 8);
-        HoloProf prof(c, HOLO_K_SUM, st);
-        k_frame_sum<<<grid, threads, 0, st>>>(frames, c->sum, c->npix, c->T, c->counters);
-        HOLO_CUDA_OK(cudaGetLastError());
-    }
+// A0 alone (also zeroes the counters of the fused Fresnel kernel)
+int holo_launch_sum(holo_ctx* c, const uint16_t* frames, cudaStream_t st) {
+    long long nvec = c->npix >> 3;
+    int threads = 256;
+    long long want = (nvec + threads - 1) / threads;
+    int grid = (int)(want < (long long)c->num_sms * 8 ? want : (long long)c->num_sms * 8);
+    HoloProf prof(c, HOLO_K_SUM, st);
+    k_frame_sum<<<grid, threads, 0, st>>>(frames, c->sum, c->npix, c->T, c->counters);
+    HOLO_CUDA_OK(cudaGetLastError());
+    return HOLO_OK;
+}
+
+// with_sum = false: the caller has already run holo_launch_sum for these frames (ordered before `st`)
+int holo_launch_fresnel(holo_ctx* c, const uint16_t* frames, float2* H, cudaStream_t st, bool with_sum) {
+    if (with_sum) { const int rc = holo_launch_sum(c, frames, st); if (rc) return rc; }
     if (use_fused(c)) {
         FresnelArgs p{};
         const int Bq = c->nx == 1024 ? FUSED_B1024 : c->nx == 2048 ? FUSED_B2048 : fft_batch(c->nx);

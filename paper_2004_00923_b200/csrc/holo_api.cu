@@ -52,7 +52,7 @@ static void free_ctx(holo_ctx* c) {
     cudaFree(c->H1); cudaFree(c->C1); cudaFree(c->evals1); cudaFree(c->V1); cudaFree(c->status1);
     if (c->side) {
         cudaStreamDestroy(c->side);
-        for (int i = 0; i < 2; ++i) { cudaEventDestroy(c->ev_cov[i]); cudaEventDestroy(c->ev_eig[i]); }
+        for (int i = 0; i < 2; ++i) { cudaEventDestroy(c->ev_cov[i]); cudaEventDestroy(c->ev_eig[i]); cudaEventDestroy(c->ev_proj[i]); }
     }
     if (c->copy) {
         cudaStreamDestroy(c->copy);
@@ -98,6 +98,9 @@ static int create_impl(holo_ctx* c) {
     c->tune[HOLO_TUNE_FFT_PERSISTENT] = 1;
     c->tune[HOLO_TUNE_PROJ_TMA] = 1;
     c->tune[HOLO_TUNE_COV_REAL] = 1;
+    // 40 of 148 SMs: measured optimum at 1024^2 x 32 (354 -> 320 us per stack); at T = 64 the projection is too slow
+    // per SM (64 holograms in registers) and the split loses (3.87 -> 4.30 ms), so it is off there
+    c->tune[HOLO_TUNE_SPLIT_SMS] = T <= 32 ? (c->num_sms * 27 + 50) / 100 : 0;
     c->tune[HOLO_TUNE_EIG_MAX_SWEEPS] = 30;
     c->scratch_frames = (int)grp;
     c->cov_parts_cap = 4 * c->num_sms;
@@ -182,12 +185,14 @@ extern "C" int holo_fourier_demod(holo_ctx* c, const void* H_dev, int n1, int n2
 }
 
 static int project_pending(holo_ctx* c, cudaStream_t st);
+static int join_side(holo_ctx* c, cudaStream_t st, int slot);
 
 extern "C" int holo_process(holo_ctx* c, const uint16_t* frames_dev, float* image_dev, holo_stream stream) {
     CHECK_CTX(c); CHECK_PTR(frames_dev, "frames_dev"); CHECK_PTR(image_dev, "image_dev");
     if (((uintptr_t)frames_dev & 15) || ((uintptr_t)image_dev & 7)) { holo_set_error("frames_dev must be 16-byte and image_dev 8-byte aligned"); return HOLO_ERR_ARG; }
     cudaStream_t st = (cudaStream_t)stream;
     int rc;
+    if ((rc = join_side(c, st, -1))) return rc;
     if ((rc = project_pending(c, st))) return rc;          // a holo_submit still owes its image: deliver it first
     c->nsubmit = 0;                                        // the next holo_submit starts again with slot 0
     if ((rc = holo_launch_fresnel(c, frames_dev, c->H, st))) return rc;
@@ -215,7 +220,18 @@ static int submit_init(holo_ctx* c) {
     for (int i = 0; i < 2; ++i) {
         HOLO_CUDA_OK(cudaEventCreateWithFlags(&c->ev_cov[i], cudaEventDisableTiming));
         HOLO_CUDA_OK(cudaEventCreateWithFlags(&c->ev_eig[i], cudaEventDisableTiming));
+        HOLO_CUDA_OK(cudaEventCreateWithFlags(&c->ev_proj[i], cudaEventDisableTiming));
     }
+    return HOLO_OK;
+}
+
+// SM-split mode: make `st` wait for the projections that were enqueued on the side stream
+static int join_side(holo_ctx* c, cudaStream_t st, int slot /* -1: both */) {
+    for (int s = 0; s < 2; ++s)
+        if ((slot < 0 || slot == s) && c->proj_recorded[s]) {
+            HOLO_CUDA_OK(cudaStreamWaitEvent(st, c->ev_proj[s], 0));
+            if (slot < 0) c->proj_recorded[s] = 0;
+        }
     return HOLO_OK;
 }
 
@@ -238,9 +254,14 @@ extern "C" int holo_submit(holo_ctx* c, const uint16_t* frames_dev, float* image
     const int s = (int)(c->nsubmit & 1);
     float2* H = s ? c->H1 : c->H;
     float2* C = s ? c->C1 : c->C;
+    const int split = c->tune[HOLO_TUNE_SPLIT_SMS];
+    if (split > 0) { if ((rc = join_side(c, st, s))) return rc; }      // H / V of slot s are free once the projection of stack i-2 is done
     if ((rc = holo_launch_fresnel(c, frames_dev, H, st))) return rc;
     if ((rc = project_pending(c, st))) return rc;
-    if ((rc = holo_launch_covariance(c, H, C, st, /*real_only=*/true))) return rc;
+    c->cov_grid_cap = split > 0 ? c->num_sms - split : 0;
+    rc = holo_launch_covariance(c, H, C, st, /*real_only=*/true);
+    c->cov_grid_cap = 0;
+    if (rc) return rc;
     HOLO_CUDA_OK(cudaEventRecord(c->ev_cov[s], st));
     HOLO_CUDA_OK(cudaStreamWaitEvent(c->side, c->ev_cov[s], 0));
     int32_t* status_main = c->status;
@@ -249,12 +270,26 @@ extern "C" int holo_submit(holo_ctx* c, const uint16_t* frames_dev, float* image
     c->status = status_main;
     if (rc) return rc;
     HOLO_CUDA_OK(cudaEventRecord(c->ev_eig[s], c->side));
+    if (split > 0) {
+        // the projection follows the eigensolver on the side stream and runs on `split` SMs next to the covariance
+        // of the next stack; the image is complete after the submit after next, or after holo_flush
+        c->proj_grid_cap = split;
+        rc = holo_launch_project(c, H, s ? c->V1 : c->V, c->k_lo, c->k_hi, c->tune[HOLO_TUNE_PROJ_COMPLEMENT], image_dev, c->side);
+        c->proj_grid_cap = 0;
+        if (rc) return rc;
+        HOLO_CUDA_OK(cudaEventRecord(c->ev_proj[s], c->side));
+        c->proj_recorded[s] = 1;
+        c->nsubmit++;
+        return HOLO_OK;
+    }
     c->pend_image = image_dev; c->pend_slot = s; c->nsubmit++;
     return HOLO_OK;
 }
 
 extern "C" int holo_flush(holo_ctx* c, holo_stream stream) {
     CHECK_CTX(c);
+    const int rc = join_side(c, (cudaStream_t)stream, -1);
+    if (rc) return rc;
     return project_pending(c, (cudaStream_t)stream);
 }
 
@@ -290,6 +325,20 @@ extern "C" int holo_submit_host(holo_ctx* c, const uint16_t* frames_host, float*
     HOLO_CUDA_OK(cudaMemcpyAsync(c->fstage[s], frames_host, fbytes, cudaMemcpyHostToDevice, c->copy));
     HOLO_CUDA_OK(cudaEventRecord(c->ev_h2d[s], c->copy));
     HOLO_CUDA_OK(cudaStreamWaitEvent(st, c->ev_h2d[s], 0));
+    if (c->tune[HOLO_TUNE_SPLIT_SMS] > 0) {
+        // SM-split mode: the projection of stack i-2 (same slot) is joined first and its image copied out BEFORE
+        // anything of stack i is enqueued, so the copy is ordered before the projection of stack i reuses the slot
+        if ((rc = join_side(c, st, s))) return rc;
+        if (c->pend_host_slot[s]) {
+            HOLO_CUDA_OK(cudaMemcpyAsync(c->pend_host_slot[s], c->istage[s], (size_t)c->npix * sizeof(float), cudaMemcpyDeviceToHost, st));
+            c->pend_host_slot[s] = nullptr;
+        }
+        if ((rc = holo_submit(c, c->fstage[s], c->istage[s], stream))) return rc;
+        HOLO_CUDA_OK(cudaEventRecord(c->ev_free[s], st));
+        c->pend_host_slot[s] = image_host; c->nsubmit_host++;
+        HOLO_CUDA_OK(cudaEventSynchronize(c->ev_h2d[s]));
+        return HOLO_OK;
+    }
     if ((rc = holo_submit(c, c->fstage[s], c->istage[s], stream))) return rc;   // enqueues the projection of stack i-1
     HOLO_CUDA_OK(cudaEventRecord(c->ev_free[s], st));
     if ((rc = deliver_host(c, st))) return rc;
@@ -304,6 +353,13 @@ extern "C" int holo_flush_host(holo_ctx* c, holo_stream stream) {
     int rc;
     if ((rc = holo_flush(c, stream))) return rc;
     if ((rc = deliver_host(c, st))) return rc;
+    for (int k = 0; k < 2; ++k) {                       // SM-split mode: up to two images are still owed
+        const int s = (int)((c->nsubmit_host + k) & 1);  // older slot first
+        if (c->pend_host_slot[s]) {
+            HOLO_CUDA_OK(cudaMemcpyAsync(c->pend_host_slot[s], c->istage[s], (size_t)c->npix * sizeof(float), cudaMemcpyDeviceToHost, st));
+            c->pend_host_slot[s] = nullptr;
+        }
+    }
     HOLO_CUDA_OK(cudaStreamSynchronize(st));
     return HOLO_OK;
 }

@@ -19,6 +19,8 @@ enum {
     HOLO_TUNE_PROFILE = 5,
     HOLO_TUNE_PROJ_TMA = 7,        // 1 = deflation projection fed by a TMA ring (default), 0 = register-streaming kernel
     HOLO_TUNE_COV_REAL = 8,        // 1 = holo_process / holo_submit compute Re C only (C is real there, R21); default 1
+    HOLO_TUNE_SPLIT_SMS = 9,       // holo_submit: k > 0 = projection on the side stream on k SMs, concurrent with the
+                                   // next covariance on the other SMs (memory-bound next to ALU-bound); 0 = in stream order
     HOLO_TUNE_FFT_LAG = 6,         // frames between the row pass and the column pass in the fused kernel (0 = auto)         // 1 = bracket every kernel launch with events (holo_profile_read)
 };
 
@@ -72,6 +74,8 @@ struct holo_ctx {
     float* pend_image;      // image of the stack whose projection is still owed (nullptr: none)
     int pend_slot;
     long long nsubmit;
+    cudaEvent_t ev_proj[2]; int proj_recorded[2];
+    int cov_grid_cap, proj_grid_cap;   // CTA caps used by the SM-split mode of holo_submit (0 = none)
     // host staging for holo_process_host
     uint16_t* frames_stage;
     float* image_stage;
@@ -80,6 +84,7 @@ struct holo_ctx {
     cudaStream_t copy;
     cudaEvent_t ev_h2d[2], ev_free[2];
     float* pend_image_host; int pend_islot;
+    float* pend_host_slot[2];          // SM-split mode: host image owed per staging slot
     long long nsubmit_host;
 };
 
@@ -107,7 +112,8 @@ struct HoloProf {
 };
 
 // stage launchers (each only enqueues on `st`)
-int holo_launch_fresnel(holo_ctx* c, const uint16_t* frames, float2* H, cudaStream_t st);
+int holo_launch_sum(holo_ctx* c, const uint16_t* frames, cudaStream_t st);
+int holo_launch_fresnel(holo_ctx* c, const uint16_t* frames, float2* H, cudaStream_t st, bool with_sum = true);
 int holo_launch_covariance(holo_ctx* c, const float2* H, float2* C, cudaStream_t st, bool real_only = false);
 int holo_launch_eig(holo_ctx* c, const float2* C, float* evals, float2* V, cudaStream_t st);
 // mode 0: direct over columns [k_lo,k_hi] of V; mode 1: complement (total - columns outside)

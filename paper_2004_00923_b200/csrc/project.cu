@@ -245,7 +245,8 @@ template <int TMAX> static int launch_deflate(holo_ctx* c, const ProjArgs& a, in
         alignas(64) CUtensorMap tmH;
         { const int rc = holo_make_tensor_map(&tmH, a.H, a.npix, a.T, 128); if (rc) return rc; }
         const long long nchunks = a.npix / PROJ_P;
-        const int grid = (int)(nchunks < c->num_sms ? nchunks : c->num_sms);
+        const int cap = c->proj_grid_cap > 0 ? c->proj_grid_cap : c->num_sms;
+        const int grid = (int)(nchunks < cap ? nchunks : cap);
         HoloProf prof(c, HOLO_K_PROJECT, st);
         k_project_deflate_tma<TMAX, PROJ_P><<<grid, PROJ_P, smem, st>>>(tmH, a, nc, nstages);
         HOLO_CUDA_OK(cudaGetLastError());

@@ -294,13 +294,16 @@ def test_process_determinism_and_host_entry(torch_cuda):
     h.close()
 
 
-def test_submit_stream_matches_process(torch_cuda):
+@pytest.mark.parametrize("split", [None, 0, 7])
+def test_submit_stream_matches_process(torch_cuda, split):
     """holo_submit / holo_flush (software pipeline over stacks) must deliver, bit for bit, the images of
     serial holo_process calls on the same stacks, in order, also when mixed with holo_process."""
     torch = torch_cuda
     cfg = G.small_config(n=128, T=16)
     stacks = [_to_dev(torch, G.stack_np(cfg, 20 + i)) for i in range(5)]
     h = _holo(128, 128, 16, 2, 16)
+    if split is not None:
+        h.tune(9, split)          # 0: projection in stream order; k > 0: on the side stream on k SMs
     ref = []
     for d in stacks:
         M = torch.empty((128, 128), dtype=torch.float32, device="cuda")
