@@ -450,12 +450,17 @@ static int launch_cov_real(holo_ctx* c, const float2* H, float2* C, cudaStream_t
     { const int rc = holo_make_tensor_map(&tmH, H, c->npix, T, COV_P); if (rc) return rc; }
     {
         HoloProf prof(c, HOLO_K_COV_PARTIAL, st);
-        k_cov_partial_real<<<dim3(gx, gy), COV_NW * 32, smem, st>>>(tmH, c->cov_partials, c->npix, T8, nstages, nslots, ngroups, ahead, plan);
+        k_cov_partial_real<<<dim3(gx, gy), COV_NW * 32, smem, st>>>(tmH, holo_cov_partials(c, c->cov_sel), c->npix, T8, nstages, nslots, ngroups, ahead, plan);
     }
     HOLO_CUDA_OK(cudaGetLastError());
-    const int nn = T * T;
+    c->cov_nparts = gx * ngroups;
+    return C ? holo_launch_cov_reduce(c, c->cov_sel, c->cov_nparts, C, st) : HOLO_OK;
+}
+
+int holo_launch_cov_reduce(holo_ctx* c, int sel, int nparts, float2* C, cudaStream_t st) {
+    const int T = c->T, T8 = (T + 7) / 8 * 8, n = T * T;
     HoloProf prof(c, HOLO_K_COV_REDUCE, st);
-    k_cov_reduce<<<(nn * 32 + 255) / 256, 256, 0, st>>>(c->cov_partials, gx * ngroups, T, T8, C);
+    k_cov_reduce<<<(n * 32 + 255) / 256, 256, 0, st>>>(holo_cov_partials(c, sel), nparts, T, T8, C);
     HOLO_CUDA_OK(cudaGetLastError());
     return HOLO_OK;
 }
@@ -488,7 +493,7 @@ int holo_launch_covariance(holo_ctx* c, const float2* H, float2* C, cudaStream_t
     { const int rc = holo_make_tensor_map(&tmH, H, c->npix, T, COV_P); if (rc) return rc; }
     {
         HoloProf prof(c, HOLO_K_COV_PARTIAL, st);
-        k_cov_partial<<<dim3(gx, plan.ngroups), COV_NW * 32, smem, st>>>(tmH, c->cov_partials, c->npix, T, T8, nstages, plan);
+        k_cov_partial<<<dim3(gx, plan.ngroups), COV_NW * 32, smem, st>>>(tmH, holo_cov_partials(c, c->cov_sel), c->npix, T, T8, nstages, plan);
     }
     HOLO_CUDA_OK(cudaGetLastError());
     const int n = T * T;

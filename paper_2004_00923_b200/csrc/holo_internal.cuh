@@ -55,7 +55,8 @@ struct holo_ctx {
     float2* scratch;        // FFT row->column intermediate, fft_group frames
     int scratch_frames;
     float2* H;              // [T][ny][nx]
-    float2* cov_partials;   // [cov_parts][T][T]
+    float2* cov_partials;   // [2 halves][cov_parts][T8][T8]; cov_sel picks the half (holo_submit: one per slot)
+    int cov_sel, cov_nparts; // half used by / partials written by the last covariance launch
     int cov_parts_cap;
     float2* C;
     float* evals;
@@ -114,7 +115,13 @@ struct HoloProf {
 // stage launchers (each only enqueues on `st`)
 int holo_launch_sum(holo_ctx* c, const uint16_t* frames, cudaStream_t st);
 int holo_launch_fresnel(holo_ctx* c, const uint16_t* frames, float2* H, cudaStream_t st, bool with_sum = true);
+// C == nullptr: partials only; holo_launch_cov_reduce then finishes (possibly on another stream, ordered after)
 int holo_launch_covariance(holo_ctx* c, const float2* H, float2* C, cudaStream_t st, bool real_only = false);
+int holo_launch_cov_reduce(holo_ctx* c, int sel, int nparts, float2* C, cudaStream_t st);
+static inline float2* holo_cov_partials(holo_ctx* c, int sel) {
+    const int T8 = (c->T + 7) / 8 * 8;
+    return c->cov_partials + (size_t)sel * c->cov_parts_cap * T8 * T8;
+}
 int holo_launch_eig(holo_ctx* c, const float2* C, float* evals, float2* V, cudaStream_t st);
 // mode 0: direct over columns [k_lo,k_hi] of V; mode 1: complement (total - columns outside)
 int holo_launch_project(holo_ctx* c, const float2* H, const float2* V, int k_lo, int k_hi,
