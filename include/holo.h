@@ -86,7 +86,8 @@ int holo_process(holo_ctx* ctx, const uint16_t* frames_dev, float* image_dev, ho
  * given to submit(i-1), then the covariance of stack i, and forks the single-CTA eigensolver of stack i
  * to a side stream owned by the handle, where it runs under the Fresnel kernels of stack i+1.
  * By default (T <= 32) the projection of stack i follows its eigensolver on the side stream and runs on about a
- * quarter of the SMs, next to the (ALU-bound) covariance of stack i+1 on the others.
+ * quarter of the SMs, next to the (ALU-bound) covariance of stack i+1 on the others (that covariance then sums over
+ * fewer CTAs: images equal those of holo_process up to FP32 summation order, and are bit-reproducible).
  * Contract: the image passed to submit(i) is complete, in `stream` order, after holo_flush, or after the
  * holo_submit after next (i+2); frames_dev may be reused as soon as `stream` has passed the submit.  The handle
  * allocates a second hologram stack (8*T*nx*ny bytes) at the first call.  holo_process / holo_flush

@@ -296,8 +296,10 @@ def test_process_determinism_and_host_entry(torch_cuda):
 
 @pytest.mark.parametrize("split", [None, 0, 7])
 def test_submit_stream_matches_process(torch_cuda, split):
-    """holo_submit / holo_flush (software pipeline over stacks) must deliver, bit for bit, the images of
-    serial holo_process calls on the same stacks, in order, also when mixed with holo_process."""
+    """holo_submit / holo_flush (software pipeline over stacks) must deliver the images of serial holo_process calls on
+    the same stacks, in order, also when mixed with holo_process: bit for bit with the projection in stream order
+    (split 0); with the SM split the covariance partials are partitioned over fewer CTAs, so the images agree to
+    FP32 summation order only -- and must still be bit-reproducible from run to run."""
     torch = torch_cuda
     cfg = G.small_config(n=128, T=16)
     stacks = [_to_dev(torch, G.stack_np(cfg, 20 + i)) for i in range(5)]
@@ -316,8 +318,20 @@ def test_submit_stream_matches_process(torch_cuda, split):
         h.submit(d, M, st)
     h.flush(st)
     st.synchronize()
+    def same(a, b):
+        if split == 0:
+            return torch.equal(a, b)
+        return rel_l2(a.cpu().numpy(), b.cpu().numpy()) <= 2e-5
+
     for a, b in zip(out, ref):
-        assert torch.equal(a, b)
+        assert same(a, b)
+    out2 = [torch.zeros_like(o) for o in out]
+    for d, M in zip(stacks, out2):
+        h.submit(d, M, st)
+    h.flush(st)
+    st.synchronize()
+    for a, b in zip(out, out2):
+        assert torch.equal(a, b)                  # deterministic
     # an owed image is delivered by a following holo_process; a new submit sequence starts clean
     A = torch.zeros_like(ref[0]); B = torch.zeros_like(ref[0]); C2 = torch.zeros_like(ref[0])
     h.submit(stacks[3], A, st)
@@ -325,7 +339,7 @@ def test_submit_stream_matches_process(torch_cuda, split):
     h.submit(stacks[4], C2, st)
     h.flush(st)
     st.synchronize()
-    assert torch.equal(A, ref[3]) and torch.equal(B, ref[1]) and torch.equal(C2, ref[4])
+    assert same(A, ref[3]) and torch.equal(B, ref[1]) and same(C2, ref[4])
     rc, status = h.status(st)
     assert rc == 0
     # host streaming entry: same images, delivered to pinned host buffers by holo_flush_host
@@ -335,7 +349,7 @@ def test_submit_stream_matches_process(torch_cuda, split):
         h.submit_host(f, o, st)
     h.flush_host(st)
     for o, b in zip(oh, ref):
-        assert torch.equal(o, b.cpu())
+        assert same(o, b.cpu())
     h.close()
 
 
