@@ -169,9 +169,20 @@ def run_ours(args, cfg):
 
     streaming = args.api == "submit"
 
+    pushing = args.api == "push"
+    n_push = (n_stacks * T - T) // cfg.stride          # pushes that fit in the resident stream after the first window
+
     def step(i):
         # one stack through the whole path; the streaming form delivers image i during step i+1 (or the flush)
-        if streaming:
+        if pushing:
+            # sliding window: only `stride` new frames per step; the stream is cycled, so once per cycle the
+            # sequence restarts with a whole window (a re-reference, counted as a step)
+            k = i % (n_push + 1)
+            if k == 0:
+                h.push(frames.data_ptr(), T, images[i % 4], st)
+            else:
+                h.push(frames.data_ptr() + (T + (k - 1) * cfg.stride) * n * n * 2, cfg.stride, images[i % 4], st)
+        elif streaming:
             h.submit(frames.data_ptr() + (i % n_win) * wbytes, images[i % 4], st)
         else:
             h.process(frames.data_ptr() + (i % n_win) * wbytes, images[i % 4], st)
@@ -332,7 +343,8 @@ def run_ours(args, cfg):
                        "l2_policy": "inputs larger than L2 (stream cycled, no flush needed)",
                        "parallelism": f"replicas x{world} (independent stacks, no collective)", "fft_group": G_fft,
                        "api": "holo_submit/holo_flush (stream of stacks, eigensolver of stack i under the Fresnel stage of stack i+1)"
-                              if streaming else "holo_process (one stack per call, strictly serial)"},
+                              if streaming else ("holo_push (sliding window, stride %d: only the new frames are transformed)" % cfg.stride) if pushing
+                              else "holo_process (one stack per call, strictly serial)"},
             "frames_per_s": value * cfg.stride, "clocks": clocks, "e2e": e2e,
             "gpu_launches": steps * h.launches_per_process(), "launches_per_step": h.launches_per_process(),
             "roofline": roof, "roofline_end_to_end": {"bound": "hbm", "achieved": round(e2e_gbps, 1), "peak": hbm_peak, "unit": "GB/s",
@@ -358,7 +370,7 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=24)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
-    ap.add_argument("--api", default="submit", choices=["submit", "process"],
+    ap.add_argument("--api", default="submit", choices=["submit", "process", "push"],
                     help="submit: streaming form (default); process: one serial holo_process per stack")
     ap.add_argument("--tune", action="append", default=[], help="experiment knob key=value (holo_tune), repeatable")
     args = ap.parse_args()

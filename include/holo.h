@@ -95,6 +95,16 @@ int holo_process(holo_ctx* ctx, const uint16_t* frames_dev, float* image_dev, ho
 int holo_submit(holo_ctx* ctx, const uint16_t* frames_dev, float* image_dev, holo_stream stream);
 int holo_flush(holo_ctx* ctx, holo_stream stream);
 
+/* Sliding window (BASELINE.json configs[3]: stride 8 over the stream): the handle keeps the
+ * holograms of the T most recent frames; holo_push transforms only the n_new newest frames (1 <= n_new <= T;
+ * the first call of a sequence must bring a whole window, n_new = T, and fixes the reference image the holograms
+ * are taken against) and renders the PCA image of the window that ends with them.  The result equals
+ * holo_process on those T frames up to FP32 rounding (the window mean is removed after the transform, which is
+ * exact by linearity; the covariance is centred in FP64).  Needs the deflation form of the projection (rejected
+ * components at most half of the kept ones).  Strictly stream ordered; holo_process / holo_submit on the same
+ * handle end the sequence.  Re-reference now and then (a push with n_new = T) if the mean brightness drifts. */
+int holo_push(holo_ctx* ctx, const uint16_t* new_frames_dev, int n_new, float* image_dev, holo_stream stream);
+
 /* Streaming form with HOST buffers: holo_submit_host copies stack i host -> device on a copy stream owned
  * by the handle (double-buffered staging, so the copy runs under the kernels of stack i-1), enqueues
  * holo_submit on `stream`, and enqueues the device -> host copy of the image of stack i-1.  It returns when

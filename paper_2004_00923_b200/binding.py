@@ -9,7 +9,7 @@ HOLO_OK, HOLO_ERR_ARG, HOLO_ERR_ALLOC, HOLO_ERR_CUDA, HOLO_ERR_STATE, HOLO_ERR_N
 HOLO_WS_SUM, HOLO_WS_H, HOLO_WS_C, HOLO_WS_EVALS, HOLO_WS_V, HOLO_WS_STATUS, HOLO_WS_QX, HOLO_WS_QY = range(8)
 
 EXPORTED_SYMBOLS = [
-    "holo_create", "holo_destroy", "holo_process", "holo_submit", "holo_flush", "holo_submit_host", "holo_flush_host", "holo_process_host", "holo_fresnel", "holo_covariance",
+    "holo_create", "holo_destroy", "holo_process", "holo_submit", "holo_flush", "holo_submit_host", "holo_flush_host", "holo_push", "holo_process_host", "holo_fresnel", "holo_covariance",
     "holo_eig", "holo_project", "holo_fourier_demod", "holo_set_range", "holo_set_assume_unitary",
     "holo_workspace", "holo_workspace_copy", "holo_status", "holo_launches_per_process", "holo_tune", "holo_last_error", "holo_version",
 ]
@@ -44,6 +44,7 @@ def load_library():
     L.holo_process_host.argtypes = [vp, vp, vp, vp]
     L.holo_submit.argtypes = [vp, vp, vp, vp]
     L.holo_flush.argtypes = [vp, vp]
+    L.holo_push.argtypes = [vp, vp, ip, vp, vp]
     L.holo_submit_host.argtypes = [vp, vp, vp, vp]
     L.holo_flush_host.argtypes = [vp, vp]
     L.holo_fresnel.argtypes = [vp, vp, vp, vp]
@@ -112,6 +113,9 @@ class Holo:
 
     def flush(self, stream=None):
         self._chk(self._L.holo_flush(self._h, _stream_ptr(stream)))
+
+    def push(self, new_frames_dev, n_new, image_dev, stream=None):
+        self._chk(self._L.holo_push(self._h, self._p(new_frames_dev), n_new, self._p(image_dev), _stream_ptr(stream)))
 
     def submit_host(self, frames_host, image_host, stream=None):
         self._chk(self._L.holo_submit_host(self._h, self._p(frames_host), self._p(image_host), _stream_ptr(stream)))

@@ -338,7 +338,9 @@ k_cov_partial_real(const __grid_constant__ CUtensorMap tmH, float2* __restrict__
 // fixed-order FP64 reduction over the partials: one warp per lower-triangle entry, lane l sums parts
 // l, l+32, ... in order, then a fixed shuffle tree (deterministic).  Writes the full Hermitian C (both
 // triangles), diagonal imaginary parts forced to 0.
-__global__ void __launch_bounds__(256) k_cov_reduce(const float2* __restrict__ partials, int nparts, int T, int T8, float2* __restrict__ C) {
+// Cd != nullptr: the FP64 sums are also kept ([T][T] double2, both triangles) for the centring step of holo_push
+__global__ void __launch_bounds__(256) k_cov_reduce(const float2* __restrict__ partials, int nparts, int T, int T8, float2* __restrict__ C,
+                                                    double2* __restrict__ Cd) {
     const int w = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
     if (w >= T * T) return;
     const int t = w / T, s = w - t * T;
@@ -362,6 +364,35 @@ __global__ void __launch_bounds__(256) k_cov_reduce(const float2* __restrict__ p
             C[t * T + s] = make_float2((float)re, (float)im);
             C[s * T + t] = make_float2((float)re, (float)-im);
         }
+        if (Cd) { Cd[t * T + s] = make_double2(re, s == t ? 0.0 : im); Cd[s * T + t] = make_double2(re, s == t ? 0.0 : -im); }
+    }
+}
+
+// Sliding-window form (holo_push): the ring holds G_t = F[q (I_t - m0)] for a FIXED reference image m0, and the
+// holograms of the current window are H_t = G_t - mean_t G.  Their covariance is C = J Gamma J with Gamma = G^H G and
+// J = I - 11^T/T:  C_ts = Gamma_ts - rho_t/T - conj(rho_s)/T + tau/T^2  (rho = row sums, tau = total), done in
+// FP64 on the unrounded sums of the reduction.  One CTA.
+__global__ void __launch_bounds__(256) k_center_gram(const double2* __restrict__ Gd, int T, float2* __restrict__ C) {
+    __shared__ double2 rho[HOLO_MAX_T];
+    __shared__ double2 tau;
+    for (int t = threadIdx.x; t < T; t += blockDim.x) {
+        double2 r = make_double2(0.0, 0.0);
+        for (int s = 0; s < T; ++s) { r.x += Gd[t * T + s].x; r.y += Gd[t * T + s].y; }
+        rho[t] = r;
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double2 a = make_double2(0.0, 0.0);
+        for (int t = 0; t < T; ++t) { a.x += rho[t].x; a.y += rho[t].y; }
+        tau = a;
+    }
+    __syncthreads();
+    const double iT = 1.0 / (double)T;
+    for (int i = threadIdx.x; i < T * T; i += blockDim.x) {
+        const int t = i / T, s = i - t * T;
+        const double re = Gd[i].x - (rho[t].x + rho[s].x) * iT + tau.x * iT * iT;
+        const double im = Gd[i].y - (rho[t].y - rho[s].y) * iT;           // tau is real for a Hermitian Gamma
+        C[i] = make_float2((float)re, t == s ? 0.f : (float)im);
     }
 }
 
@@ -460,8 +491,12 @@ static int launch_cov_real(holo_ctx* c, const float2* H, float2* C, cudaStream_t
 int holo_launch_cov_reduce(holo_ctx* c, int sel, int nparts, float2* C, cudaStream_t st) {
     const int T = c->T, T8 = (T + 7) / 8 * 8, n = T * T;
     HoloProf prof(c, HOLO_K_COV_REDUCE, st);
-    k_cov_reduce<<<(n * 32 + 255) / 256, 256, 0, st>>>(holo_cov_partials(c, sel), nparts, T, T8, C);
+    k_cov_reduce<<<(n * 32 + 255) / 256, 256, 0, st>>>(holo_cov_partials(c, sel), nparts, T, T8, C, c->center_gram ? c->Cd : nullptr);
     HOLO_CUDA_OK(cudaGetLastError());
+    if (c->center_gram) {                                  // holo_push: C <- J Gamma J
+        k_center_gram<<<1, 256, 0, st>>>(c->Cd, T, C);
+        HOLO_CUDA_OK(cudaGetLastError());
+    }
     return HOLO_OK;
 }
 
@@ -496,9 +531,6 @@ int holo_launch_covariance(holo_ctx* c, const float2* H, float2* C, cudaStream_t
         k_cov_partial<<<dim3(gx, plan.ngroups), COV_NW * 32, smem, st>>>(tmH, holo_cov_partials(c, c->cov_sel), c->npix, T, T8, nstages, plan);
     }
     HOLO_CUDA_OK(cudaGetLastError());
-    const int n = T * T;
-    HoloProf prof(c, HOLO_K_COV_REDUCE, st);
-    k_cov_reduce<<<(n * 32 + 255) / 256, 256, 0, st>>>(c->cov_partials, gx, T, T8, C);
-    HOLO_CUDA_OK(cudaGetLastError());
-    return HOLO_OK;
+    c->cov_nparts = gx;
+    return C ? holo_launch_cov_reduce(c, c->cov_sel, c->cov_nparts, C, st) : HOLO_OK;
 }

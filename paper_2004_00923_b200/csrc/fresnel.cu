@@ -546,9 +546,12 @@ int holo_launch_sum(holo_ctx* c, const uint16_t* frames, cudaStream_t st) {
     return HOLO_OK;
 }
 
-// with_sum = false: the caller has already run holo_launch_sum for these frames (ordered before `st`)
-int holo_launch_fresnel(holo_ctx* c, const uint16_t* frames, float2* H, cudaStream_t st, bool with_sum) {
+// with_sum = false: c->sum already holds the reference sum image S (d = (T I - S)/T); nproc = number of frames to
+// transform (frames[0..nproc) -> H[0..nproc)), default all T
+int holo_launch_fresnel(holo_ctx* c, const uint16_t* frames, float2* H, cudaStream_t st, bool with_sum, int nproc) {
+    if (nproc < 0) nproc = c->T;
     if (with_sum) { const int rc = holo_launch_sum(c, frames, st); if (rc) return rc; }
+    else if (use_fused(c)) HOLO_CUDA_OK(cudaMemsetAsync(c->counters, 0, (2 * c->T + 1) * sizeof(unsigned int), st));
     if (use_fused(c)) {
         FresnelArgs p{};
         const int Bq = c->nx == 1024 ? FUSED_B1024 : c->nx == 2048 ? FUSED_B2048 : fft_batch(c->nx);
@@ -557,7 +560,7 @@ int holo_launch_fresnel(holo_ctx* c, const uint16_t* frames, float2* H, cudaStre
         a.tw1 = c->px.tw1; a.tw2 = c->px.tw2; a.ld = c->nx; a.nseq = c->ny; a.T = c->T; a.invT = 1.0f / (float)c->T;
         FftArgs& b = p.cols;
         b.in = c->scratch; b.out = H; b.tw1 = c->py.tw1; b.tw2 = c->py.tw2; b.ld = c->nx; b.nseq = c->nx; b.T = c->T; b.invT = a.invT;
-        p.counters = c->counters; p.npix = c->npix; p.T = c->T; p.R = c->scratch_frames;
+        p.counters = c->counters; p.npix = c->npix; p.T = nproc; p.R = c->scratch_frames;
         p.L = c->tune[HOLO_TUNE_FFT_LAG] > 0 ? c->tune[HOLO_TUNE_FFT_LAG] : p.R / 2;
         if (p.L > p.R - 1) p.L = p.R - 1;
         if (p.L > p.T) p.L = p.T;
@@ -568,8 +571,8 @@ int holo_launch_fresnel(holo_ctx* c, const uint16_t* frames, float2* H, cudaStre
     }
     // A1 + A2, frame groups so that the row->column intermediate stays in L2
     const int G = c->scratch_frames;
-    for (int f0 = 0; f0 < c->T; f0 += G) {
-        const int nf = (c->T - f0 < G) ? c->T - f0 : G;
+    for (int f0 = 0; f0 < nproc; f0 += G) {
+        const int nf = (nproc - f0 < G) ? nproc - f0 : G;
         FftArgs a{};
         a.frames = frames + (long long)f0 * c->npix;
         a.sum = c->sum; a.qx = c->qxs; a.qy = c->qy;

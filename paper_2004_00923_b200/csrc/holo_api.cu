@@ -49,6 +49,7 @@ static void free_ctx(holo_ctx* c) {
         delete[] c->prof_ev;
         delete[] c->prof_cls;
     }
+    cudaFree(c->Cd);
     cudaFree(c->H1); cudaFree(c->C1); cudaFree(c->evals1); cudaFree(c->V1); cudaFree(c->status1);
     if (c->side) {
         cudaStreamDestroy(c->side);
@@ -195,6 +196,7 @@ extern "C" int holo_process(holo_ctx* c, const uint16_t* frames_dev, float* imag
     if ((rc = join_side(c, st, -1))) return rc;
     if ((rc = project_pending(c, st))) return rc;          // a holo_submit still owes its image: deliver it first
     c->nsubmit = 0;                                        // the next holo_submit starts again with slot 0
+    c->push_ready = 0;                                     // ... and a holo_push sequence has to start over
     if ((rc = holo_launch_fresnel(c, frames_dev, c->H, st))) return rc;
     if ((rc = holo_launch_covariance(c, c->H, c->C, st, /*real_only=*/true))) return rc;
     if ((rc = holo_launch_eig(c, c->C, c->evals, c->V, st))) return rc;
@@ -251,6 +253,7 @@ extern "C" int holo_submit(holo_ctx* c, const uint16_t* frames_dev, float* image
     cudaStream_t st = (cudaStream_t)stream;
     int rc;
     if ((rc = submit_init(c))) return rc;
+    c->push_ready = 0;
     const int s = (int)(c->nsubmit & 1);
     float2* H = s ? c->H1 : c->H;
     float2* C = s ? c->C1 : c->C;
@@ -293,6 +296,48 @@ extern "C" int holo_flush(holo_ctx* c, holo_stream stream) {
     const int rc = join_side(c, (cudaStream_t)stream, -1);
     if (rc) return rc;
     return project_pending(c, (cudaStream_t)stream);
+}
+
+// ---- sliding window (BASELINE.json configs[3]) ------------------------------------
+// The handle's hologram stack is used as a ring of the T most recent frames.  The holograms are taken against a
+// FIXED reference image m0 (the temporal mean of the first window; its sum image S0 stays in ctx->sum), G_t =
+// F[q (I_t - m0)], so a frame is transformed ONCE and stays valid while the window slides; the window's own mean
+// is removed afterwards, exactly (linearity): H_t = G_t - mean_t G.  Covariance: C = J (G^H G) J, centred in FP64
+// (k_center_gram); projection: the deflation kernel subtracts the per-pixel mean first.  Row / column order of C
+// follows the ring slots, which permutes C, V symmetrically and leaves eigenvalues and M unchanged.
+extern "C" int holo_push(holo_ctx* c, const uint16_t* new_frames_dev, int n_new, float* image_dev, holo_stream stream) {
+    CHECK_CTX(c); CHECK_PTR(new_frames_dev, "new_frames_dev"); CHECK_PTR(image_dev, "image_dev");
+    if (((uintptr_t)new_frames_dev & 15) || ((uintptr_t)image_dev & 7)) { holo_set_error("new_frames_dev must be 16-byte and image_dev 8-byte aligned"); return HOLO_ERR_ARG; }
+    const int T = c->T;
+    if (n_new < 1 || n_new > T) { holo_set_error("need 1 <= n_new <= T (got %d)", n_new); return HOLO_ERR_ARG; }
+    if (!c->push_ready && n_new != T) { holo_set_error("the first holo_push of a sequence must bring a whole window (n_new = T)"); return HOLO_ERR_STATE; }
+    cudaStream_t st = (cudaStream_t)stream;
+    int rc;
+    if ((rc = join_side(c, st, -1))) return rc;
+    if ((rc = project_pending(c, st))) return rc;
+    if (!c->Cd) HOLO_CUDA_OK(cudaMalloc(&c->Cd, (size_t)T * T * sizeof(double2)));
+    if (n_new == T) {
+        // (re)start: reference = mean of this window; transform all T frames
+        if ((rc = holo_launch_fresnel(c, new_frames_dev, c->H, st))) return rc;
+        c->push_ready = 1; c->push_head = 0;
+    } else {
+        // overwrite the n_new oldest slots (two pieces when the range wraps around the ring)
+        int done = 0;
+        while (done < n_new) {
+            const int slot = (c->push_head + done) % T;
+            const int n = (n_new - done < T - slot) ? n_new - done : T - slot;
+            if ((rc = holo_launch_fresnel(c, new_frames_dev + (size_t)done * c->npix, c->H + (size_t)slot * c->npix, st,
+                                          /*with_sum=*/false, n))) return rc;
+            done += n;
+        }
+        c->push_head = (c->push_head + n_new) % T;
+    }
+    c->center_gram = 1;
+    rc = holo_launch_covariance(c, c->H, c->C, st, /*real_only=*/true);
+    c->center_gram = 0;
+    if (rc) return rc;
+    if ((rc = holo_launch_eig(c, c->C, c->evals, c->V, st))) return rc;
+    return holo_launch_project(c, c->H, c->V, c->k_lo, c->k_hi, /*allow_complement=*/1, image_dev, st, /*center=*/1);
 }
 
 // ---- streaming host entry: H2D of stack i (copy stream) runs under the kernels of stack i-1 ----------

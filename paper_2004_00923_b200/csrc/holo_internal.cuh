@@ -76,6 +76,10 @@ struct holo_ctx {
     int pend_slot;
     long long nsubmit;
     cudaEvent_t ev_proj[2]; int proj_recorded[2];
+    // sliding-window form (holo_push)
+    double2* Cd;            // [T][T] unrounded Gram sums (allocated at the first push)
+    int center_gram;        // 1 while a push is being enqueued: the reduction also centres (C = J Gamma J)
+    int push_ready, push_head;   // ring = H: slot push_head is the oldest frame
     int cov_grid_cap, proj_grid_cap;   // CTA caps used by the SM-split mode of holo_submit (0 = none)
     // host staging for holo_process_host
     uint16_t* frames_stage;
@@ -114,7 +118,7 @@ struct HoloProf {
 
 // stage launchers (each only enqueues on `st`)
 int holo_launch_sum(holo_ctx* c, const uint16_t* frames, cudaStream_t st);
-int holo_launch_fresnel(holo_ctx* c, const uint16_t* frames, float2* H, cudaStream_t st, bool with_sum = true);
+int holo_launch_fresnel(holo_ctx* c, const uint16_t* frames, float2* H, cudaStream_t st, bool with_sum = true, int nproc = -1);
 // C == nullptr: partials only; holo_launch_cov_reduce then finishes (possibly on another stream, ordered after)
 int holo_launch_covariance(holo_ctx* c, const float2* H, float2* C, cudaStream_t st, bool real_only = false);
 int holo_launch_cov_reduce(holo_ctx* c, int sel, int nparts, float2* C, cudaStream_t st);
@@ -125,7 +129,7 @@ static inline float2* holo_cov_partials(holo_ctx* c, int sel) {
 int holo_launch_eig(holo_ctx* c, const float2* C, float* evals, float2* V, cudaStream_t st);
 // mode 0: direct over columns [k_lo,k_hi] of V; mode 1: complement (total - columns outside)
 int holo_launch_project(holo_ctx* c, const float2* H, const float2* V, int k_lo, int k_hi,
-                        int allow_complement, float* image, cudaStream_t st);
+                        int allow_complement, float* image, cudaStream_t st, int center = 0);
 int holo_fresnel_launch_count(holo_ctx* c);
 int holo_fft_plan_init(FftPlan* p, int N);
 void holo_fft_plan_free(FftPlan* p);

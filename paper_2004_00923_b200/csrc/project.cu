@@ -18,6 +18,7 @@ struct ProjArgs {
     int r0_lo, r0_hi;      // first 0-based inclusive column range (empty if lo > hi)
     int r1_lo, r1_hi;      // second range
     int complement;        // 1: M = total - sum
+    int center;            // 1: subtract the per-pixel mean over t first (sliding-window form: H_t = G_t - mean_t G)
 };
 
 template <int NC, int PIX>      // PIX = pixels per thread (2: float4 loads; 1 for very wide component sets)
@@ -107,6 +108,18 @@ __global__ void __launch_bounds__(256) k_project_deflate(const ProjArgs a, int n
         } else {
 #pragma unroll
             for (int x = 0; x < PIX; ++x) h[t][x] = make_float2(0.f, 0.f);
+        }
+    }
+    if (a.center) {
+#pragma unroll
+        for (int x = 0; x < PIX; ++x) {
+            float2 m = make_float2(0.f, 0.f);
+#pragma unroll
+            for (int t = 0; t < TMAX; ++t) { m.x += h[t][x].x; m.y += h[t][x].y; }
+            const float inv = 1.f / (float)a.T;
+            m.x *= inv; m.y *= inv;
+#pragma unroll
+            for (int t = 0; t < TMAX; ++t) if (t < a.T) { h[t][x].x -= m.x; h[t][x].y -= m.y; }
         }
     }
 #pragma unroll 1
@@ -204,6 +217,15 @@ k_project_deflate_tma(const __grid_constant__ CUtensorMap tmH, const ProjArgs a,
         __syncwarp();
         if (lane == 0) mbar_arrive(empty + s);           // the stage is in registers: hand it back at once
         if (warp == 0) issue();
+        if (a.center) {                                   // rows t >= T are zero (TMA fill): they do not enter the mean
+            float2 m = make_float2(0.f, 0.f);
+#pragma unroll
+            for (int t = 0; t < TMAX; ++t) { m.x += h[t].x; m.y += h[t].y; }
+            const float inv = 1.f / (float)a.T;
+            m.x *= inv; m.y *= inv;
+#pragma unroll
+            for (int t = 0; t < TMAX; ++t) if (t < a.T) { h[t].x -= m.x; h[t].y -= m.y; }
+        }
 #pragma unroll 1
         for (int c = 0; c < nc; ++c) {
             const float2* v = Vd + c * TMAX;
@@ -275,11 +297,11 @@ template <int NC> static int launch_proj_t(holo_ctx* c, const ProjArgs& a, cudaS
 }
 
 int holo_launch_project(holo_ctx* c, const float2* H, const float2* V, int k_lo, int k_hi,
-                        int allow_complement, float* image, cudaStream_t st) {
+                        int allow_complement, float* image, cudaStream_t st, int center) {
     const int T = c->T;
     const int nS = k_hi - k_lo + 1;
     ProjArgs a{};
-    a.H = H; a.V = V; a.M = image; a.npix = c->npix; a.T = T;
+    a.H = H; a.V = V; a.M = image; a.npix = c->npix; a.T = T; a.center = center;
     int nc;
     if (allow_complement && 2 * (T - nS) <= nS) {          // deflating costs 2 passes per rejected component
         a.complement = 1;
@@ -292,6 +314,7 @@ int holo_launch_project(holo_ctx* c, const float2* H, const float2* V, int k_lo,
         a.r1_lo = 0; a.r1_hi = -1;
         nc = nS;
     }
+    if (center && !a.complement) { holo_set_error("the centred projection needs the deflation form (rejected set at most half of the kept set)"); return HOLO_ERR_STATE; }
     if (a.complement) {
         if (T <= 8) return launch_deflate<8>(c, a, nc, st);
         if (T <= 16) return launch_deflate<16>(c, a, nc, st);

@@ -377,6 +377,41 @@ def test_process_real_covariance_identity(torch_cuda):
     h.close()
 
 
+@pytest.mark.parametrize("n,T,steps", [(128, 16, [4, 4, 4, 4, 4]), (64, 32, [8, 8, 5, 11, 8, 32, 8]), (64, 12, [3, 3, 3, 7])])
+def test_push_sliding_window_matches_oracle(torch_cuda, n, T, steps):
+    """holo_push: only the newest frames are transformed, against a fixed reference image; the
+    window mean is removed afterwards.  Every window's image must match the oracle's holo_process of that window
+    (north-star tolerance 1e-4 on M; here also the 2e-5 bug bound), including ring wrap-around (strides that do
+    not divide T) and a re-reference in mid-sequence (n_new = T)."""
+    torch = torch_cuda
+    total = T + sum(steps)
+    cfg = G.small_config(n=n, T=T, n_frames=total + T)
+    scene = G.make_scene(cfg, 77)
+    stream = G.frames_np(scene, 0, total)
+    dev = _to_dev(torch, stream)
+    h = _holo(n, n, T, 2, T)
+    M = torch.empty((n, n), dtype=torch.float32, device="cuda")
+    fbytes = n * n * 2
+    h.push(dev.data_ptr(), T, M)                                   # first window
+    end = T
+    wins = [(end, M.cpu().numpy().copy())]
+    for k in steps:
+        h.push(dev.data_ptr() + end * fbytes, k, M)
+        end += k
+        wins.append((end, M.cpu().numpy().copy()))
+    rc, status = h.status()
+    assert rc == 0
+    for end, Mg in wins:
+        fr = stream[end - T:end]
+        ev, gaps = eig_gaps(fr)
+        if gaps[0] < 0.02:                                         # k_lo = 2: the image is only defined with a gap there (R10)
+            continue
+        Mo = oracle.process(fr, LAM, PITCH, Z, 2, T)["M"]
+        err = rel_l2(Mg, Mo)
+        assert err <= TOL_M and err <= 2e-5, (end, err)
+    h.close()
+
+
 def test_bad_arguments(torch_cuda):
     from paper_2004_00923_b200 import Holo, HoloError
     for args in [(100, 64, 8, LAM, PITCH, Z, 2, 8), (64, 8, 8, LAM, PITCH, Z, 2, 8), (64, 64, 1, LAM, PITCH, Z, 1, 1),
