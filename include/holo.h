@@ -101,8 +101,12 @@ int holo_flush(holo_ctx* ctx, holo_stream stream);
  * are taken against) and renders the PCA image of the window that ends with them.  The result equals
  * holo_process on those T frames up to FP32 rounding (the window mean is removed after the transform, which is
  * exact by linearity; the covariance is centred in FP64).  Needs the deflation form of the projection (rejected
- * components at most half of the kept ones).  Strictly stream ordered; holo_process / holo_submit on the same
- * handle end the sequence.  Re-reference now and then (a push with n_new = T) if the mean brightness drifts. */
+ * components at most half of the kept ones).  holo_process / holo_submit on the same handle end the sequence.
+ * Re-reference now and then (a push with n_new = T) if the mean brightness drifts.
+ * Completion: with T in {16, 32, 64} and n_new a multiple of 8 (at most T/2) the call is pipelined like
+ * holo_submit (ring of T + T/2 hologram slots, eigensolver and projection on the side stream): the image is
+ * complete, in `stream` order, after holo_flush or after the push after next.  Otherwise (and with tune key 10 = 0)
+ * the call is strictly stream ordered.  Always safe: holo_flush before reading an image. */
 int holo_push(holo_ctx* ctx, const uint16_t* new_frames_dev, int n_new, float* image_dev, holo_stream stream);
 
 /* Streaming form with HOST buffers: holo_submit_host copies stack i host -> device on a copy stream owned
@@ -172,7 +176,8 @@ int holo_launches_per_process(holo_ctx* ctx);
  *   brackets (holo_profile_read), 6 lag in frames between row and column pass in the fused kernel (0 = ring/2),
  *   7 TMA-fed projection (default 1), 8 real-part covariance in holo_process / holo_submit (default 1; the
  *   covariance of holograms of real frames is real in exact arithmetic, R21), 9 SMs given to the
- *   side-stream projection in holo_submit (0 = projection in stream order after the next Fresnel stage). */
+ *   side-stream projection in holo_submit (0 = projection in stream order after the next Fresnel stage),
+ *   10 pipelined ring form of holo_push (default 1). */
 int holo_tune(holo_ctx* ctx, int key, int value);
 
 const char* holo_last_error(void);   /* thread-local, static storage */

@@ -230,7 +230,7 @@ struct RealPlan { int njobs[2]; RealJob job[2][COV_NW]; };
 // ------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(COV_NW * 32, 1)
 k_cov_partial_real(const __grid_constant__ CUtensorMap tmH, float2* __restrict__ partials, long long npix, int T8,
-                   int nstages, int nslots, int ngroups, int ahead, const RealPlan plan) {
+                   int nstages, int nslots, int ngroups, int ahead, const RealPlan plan, int rb0, int nrb) {
     extern __shared__ __align__(128) unsigned char smraw[];
     uint64_t* full = reinterpret_cast<uint64_t*>(smraw);
     uint64_t* empty = full + COV_MAX_STAGES;
@@ -253,7 +253,9 @@ k_cov_partial_real(const __grid_constant__ CUtensorMap tmH, float2* __restrict__
         mbar_wait(empty + ps, pph ^ 1u);
         if (lane == 0) mbar_arrive_expect_tx(full + ps, (uint32_t)stage_elems * (uint32_t)sizeof(float2));
         __syncwarp();
-        if (lane < nslots) tma_2d_g2s(ring + (size_t)ps * stage_elems + lane * 8 * COV_P, &tmH, (int)(pchunk * (2 * COV_P)), 8 * lane, full + ps);
+        // nrb != 0: the T rows are a window of a ring of nrb 8-row blocks that starts at block rb0 (holo_push)
+        if (lane < nslots) tma_2d_g2s(ring + (size_t)ps * stage_elems + lane * 8 * COV_P, &tmH, (int)(pchunk * (2 * COV_P)),
+                                      8 * (nrb ? (rb0 + lane) % nrb : lane), full + ps);
         pchunk += gridDim.x;
         if (++ps == nstages) { ps = 0; pph ^= 1u; }
     };
@@ -478,10 +480,10 @@ static int launch_cov_real(holo_ctx* c, const float2* H, float2* C, cudaStream_t
     if (gx * ngroups > c->cov_parts_cap) gx = c->cov_parts_cap / ngroups;
     if ((long long)gx > nchunks) gx = (int)nchunks;
     alignas(64) CUtensorMap tmH;
-    { const int rc = holo_make_tensor_map(&tmH, H, c->npix, T, COV_P); if (rc) return rc; }
+    { const int rc = holo_make_tensor_map(&tmH, H, c->npix, c->ring_nrb ? 8 * c->ring_nrb : T, COV_P); if (rc) return rc; }
     {
         HoloProf prof(c, HOLO_K_COV_PARTIAL, st);
-        k_cov_partial_real<<<dim3(gx, gy), COV_NW * 32, smem, st>>>(tmH, holo_cov_partials(c, c->cov_sel), c->npix, T8, nstages, nslots, ngroups, ahead, plan);
+        k_cov_partial_real<<<dim3(gx, gy), COV_NW * 32, smem, st>>>(tmH, holo_cov_partials(c, c->cov_sel), c->npix, T8, nstages, nslots, ngroups, ahead, plan, c->ring_rb0, c->ring_nrb);
     }
     HOLO_CUDA_OK(cudaGetLastError());
     c->cov_nparts = gx * ngroups;

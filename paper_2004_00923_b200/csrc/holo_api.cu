@@ -49,7 +49,7 @@ static void free_ctx(holo_ctx* c) {
         delete[] c->prof_ev;
         delete[] c->prof_cls;
     }
-    cudaFree(c->Cd);
+    cudaFree(c->Cd); cudaFree(c->ring);
     cudaFree(c->H1); cudaFree(c->C1); cudaFree(c->evals1); cudaFree(c->V1); cudaFree(c->status1);
     if (c->side) {
         cudaStreamDestroy(c->side);
@@ -99,6 +99,7 @@ static int create_impl(holo_ctx* c) {
     c->tune[HOLO_TUNE_FFT_PERSISTENT] = 1;
     c->tune[HOLO_TUNE_PROJ_TMA] = 1;
     c->tune[HOLO_TUNE_COV_REAL] = 1;
+    c->tune[HOLO_TUNE_PUSH_PIPE] = 1;
     // 40 of 148 SMs: measured optimum at 1024^2 x 32 (354 -> 320 us per stack); at T = 64 the projection is too slow
     // per SM (64 holograms in registers) and the split loses (3.87 -> 4.30 ms), so it is off there
     c->tune[HOLO_TUNE_SPLIT_SMS] = T <= 32 ? (c->num_sms * 27 + 50) / 100 : 0;
@@ -305,6 +306,23 @@ extern "C" int holo_flush(holo_ctx* c, holo_stream stream) {
 // is removed afterwards, exactly (linearity): H_t = G_t - mean_t G.  Covariance: C = J (G^H G) J, centred in FP64
 // (k_center_gram); projection: the deflation kernel subtracts the per-pixel mean first.  Row / column order of C
 // follows the ring slots, which permutes C, V symmetrically and leaves eigenvalues and M unchanged.
+static bool push_ring_possible(const holo_ctx* c) {
+    return c->tune[HOLO_TUNE_PUSH_PIPE] && (c->T == 16 || c->T == 32 || c->T == 64) && c->tune[HOLO_TUNE_COV_REAL] && c->tune[HOLO_TUNE_PROJ_TMA];
+}
+
+// window of the ring -> ctx->H (contiguous), when a push cannot use the ring (n_new not a multiple of 8, or too large)
+static int push_ring_to_flat(holo_ctx* c, cudaStream_t st) {
+    int rc;
+    if ((rc = join_side(c, st, -1))) return rc;
+    const int T = c->T, Rn = c->ring_slots;
+    const int first = (Rn - c->ring_a < T) ? Rn - c->ring_a : T;
+    HOLO_CUDA_OK(cudaMemcpyAsync(c->H, c->ring + (size_t)c->ring_a * c->npix, (size_t)first * c->npix * sizeof(float2), cudaMemcpyDeviceToDevice, st));
+    if (first < T)
+        HOLO_CUDA_OK(cudaMemcpyAsync(c->H + (size_t)first * c->npix, c->ring, (size_t)(T - first) * c->npix * sizeof(float2), cudaMemcpyDeviceToDevice, st));
+    c->push_ready = 1; c->push_head = 0;
+    return HOLO_OK;
+}
+
 extern "C" int holo_push(holo_ctx* c, const uint16_t* new_frames_dev, int n_new, float* image_dev, holo_stream stream) {
     CHECK_CTX(c); CHECK_PTR(new_frames_dev, "new_frames_dev"); CHECK_PTR(image_dev, "image_dev");
     if (((uintptr_t)new_frames_dev & 15) || ((uintptr_t)image_dev & 7)) { holo_set_error("new_frames_dev must be 16-byte and image_dev 8-byte aligned"); return HOLO_ERR_ARG; }
@@ -313,31 +331,78 @@ extern "C" int holo_push(holo_ctx* c, const uint16_t* new_frames_dev, int n_new,
     if (!c->push_ready && n_new != T) { holo_set_error("the first holo_push of a sequence must bring a whole window (n_new = T)"); return HOLO_ERR_STATE; }
     cudaStream_t st = (cudaStream_t)stream;
     int rc;
-    if ((rc = join_side(c, st, -1))) return rc;
-    if ((rc = project_pending(c, st))) return rc;
     if (!c->Cd) HOLO_CUDA_OK(cudaMalloc(&c->Cd, (size_t)T * T * sizeof(double2)));
+    const int extra = (T / 2 + 7) / 8 * 8 > 8 ? (T / 2 + 7) / 8 * 8 : 8;
     if (n_new == T) {
         // (re)start: reference = mean of this window; transform all T frames
-        if ((rc = holo_launch_fresnel(c, new_frames_dev, c->H, st))) return rc;
-        c->push_ready = 1; c->push_head = 0;
+        if ((rc = join_side(c, st, -1))) return rc;
+        if ((rc = project_pending(c, st))) return rc;
+        if (push_ring_possible(c)) {
+            if ((rc = submit_init(c))) return rc;                          // side stream, events, second C / V slot
+            if (!c->ring) { c->ring_slots = T + extra; HOLO_CUDA_OK(cudaMalloc(&c->ring, (size_t)c->ring_slots * c->npix * sizeof(float2))); }
+            if ((rc = holo_launch_fresnel(c, new_frames_dev, c->ring, st))) return rc;
+            c->push_ready = 2; c->ring_a = 0;
+        } else {
+            if ((rc = holo_launch_fresnel(c, new_frames_dev, c->H, st))) return rc;
+            c->push_ready = 1; c->push_head = 0;
+        }
     } else {
+        if (c->push_ready == 2 && (n_new % 8 != 0 || n_new > extra)) { if ((rc = push_ring_to_flat(c, st))) return rc; }
         // overwrite the n_new oldest slots (two pieces when the range wraps around the ring)
+        const int Rn = c->push_ready == 2 ? c->ring_slots : T;
+        float2* base = c->push_ready == 2 ? c->ring : c->H;
+        const int start = c->push_ready == 2 ? (c->ring_a + T) % Rn : c->push_head;
+        if (c->push_ready == 2) { if ((rc = join_side(c, st, (int)(c->npush & 1)))) return rc; }   // readers of these slots: the push before last
         int done = 0;
         while (done < n_new) {
-            const int slot = (c->push_head + done) % T;
-            const int n = (n_new - done < T - slot) ? n_new - done : T - slot;
-            if ((rc = holo_launch_fresnel(c, new_frames_dev + (size_t)done * c->npix, c->H + (size_t)slot * c->npix, st,
+            const int slot = (start + done) % Rn;
+            const int n = (n_new - done < Rn - slot) ? n_new - done : Rn - slot;
+            if ((rc = holo_launch_fresnel(c, new_frames_dev + (size_t)done * c->npix, base + (size_t)slot * c->npix, st,
                                           /*with_sum=*/false, n))) return rc;
             done += n;
         }
-        c->push_head = (c->push_head + n_new) % T;
+        if (c->push_ready == 2) c->ring_a = (c->ring_a + n_new) % Rn;
+        else c->push_head = (c->push_head + n_new) % T;
     }
+    if (c->push_ready == 1) {
+        // serial form: everything in stream order on ctx->H
+        c->center_gram = 1;
+        rc = holo_launch_covariance(c, c->H, c->C, st, /*real_only=*/true);
+        c->center_gram = 0;
+        if (rc) return rc;
+        if ((rc = holo_launch_eig(c, c->C, c->evals, c->V, st))) return rc;
+        return holo_launch_project(c, c->H, c->V, c->k_lo, c->k_hi, /*allow_complement=*/1, image_dev, st, /*center=*/1);
+    }
+    // pipelined form (same structure as holo_submit): eigensolver + projection on the side stream; the image is
+    // complete after holo_flush or after the push after next
+    const int s = (int)(c->npush & 1);
+    // no SM split here: with only n_new transforms per window the side chain (eigensolver + projection) is the longer
+    // one, and the projection is fastest on all SMs (measured at 1024^2 x 32, stride 8: 204 us vs 220 us with the split)
+    const int split = 0;
+    float2* C = s ? c->C1 : c->C;
+    c->ring_rb0 = c->ring_a / 8; c->ring_nrb = c->ring_slots / 8;
     c->center_gram = 1;
-    rc = holo_launch_covariance(c, c->H, c->C, st, /*real_only=*/true);
-    c->center_gram = 0;
+    c->cov_grid_cap = split > 0 ? c->num_sms - split : 0;
+    rc = holo_launch_covariance(c, c->ring, C, st, /*real_only=*/true);
+    c->center_gram = 0; c->cov_grid_cap = 0;
+    if (!rc) rc = cudaEventRecord(c->ev_cov[s], st) == cudaSuccess && cudaStreamWaitEvent(c->side, c->ev_cov[s], 0) == cudaSuccess ? HOLO_OK : HOLO_ERR_CUDA;
+    if (!rc) {
+        int32_t* status_main = c->status;
+        if (s) c->status = c->status1;
+        rc = holo_launch_eig(c, C, s ? c->evals1 : c->evals, s ? c->V1 : c->V, c->side);
+        c->status = status_main;
+    }
+    if (!rc) {
+        c->proj_grid_cap = split > 0 ? split : 0;
+        rc = holo_launch_project(c, c->ring, s ? c->V1 : c->V, c->k_lo, c->k_hi, /*allow_complement=*/1, image_dev, c->side, /*center=*/1);
+        c->proj_grid_cap = 0;
+    }
+    c->ring_rb0 = 0; c->ring_nrb = 0;
     if (rc) return rc;
-    if ((rc = holo_launch_eig(c, c->C, c->evals, c->V, st))) return rc;
-    return holo_launch_project(c, c->H, c->V, c->k_lo, c->k_hi, /*allow_complement=*/1, image_dev, st, /*center=*/1);
+    HOLO_CUDA_OK(cudaEventRecord(c->ev_proj[s], c->side));
+    c->proj_recorded[s] = 1;
+    c->npush++;
+    return HOLO_OK;
 }
 
 // ---- streaming host entry: H2D of stack i (copy stream) runs under the kernels of stack i-1 ----------

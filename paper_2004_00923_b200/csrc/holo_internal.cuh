@@ -21,6 +21,7 @@ enum {
     HOLO_TUNE_COV_REAL = 8,        // 1 = holo_process / holo_submit compute Re C only (C is real there, R21); default 1
     HOLO_TUNE_SPLIT_SMS = 9,       // holo_submit: k > 0 = projection on the side stream on k SMs, concurrent with the
                                    // next covariance on the other SMs (memory-bound next to ALU-bound); 0 = in stream order
+    HOLO_TUNE_PUSH_PIPE = 10,      // holo_push: 1 = pipelined ring form when T in {16,32,64} and n_new is a multiple of 8 (default)
     HOLO_TUNE_FFT_LAG = 6,         // frames between the row pass and the column pass in the fused kernel (0 = auto)         // 1 = bracket every kernel launch with events (holo_profile_read)
 };
 
@@ -80,6 +81,10 @@ struct holo_ctx {
     double2* Cd;            // [T][T] unrounded Gram sums (allocated at the first push)
     int center_gram;        // 1 while a push is being enqueued: the reduction also centres (C = J Gamma J)
     int push_ready, push_head;   // ring = H: slot push_head is the oldest frame
+    // pipelined push: a ring of ring_slots > T hologram slots; the current window starts at slot ring_a.  While
+    // ring_nrb != 0 the covariance / projection launchers read the window through the ring (8-row blocks modulo).
+    float2* ring; int ring_slots, ring_a; long long npush;
+    int ring_rb0, ring_nrb;
     int cov_grid_cap, proj_grid_cap;   // CTA caps used by the SM-split mode of holo_submit (0 = none)
     // host staging for holo_process_host
     uint16_t* frames_stage;

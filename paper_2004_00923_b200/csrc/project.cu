@@ -167,7 +167,7 @@ __global__ void __launch_bounds__(256) k_project_deflate(const ProjArgs a, int n
 #define PROJ_MAX_STAGES 8
 template <int TMAX, int PROJ_P>
 __global__ void __launch_bounds__(PROJ_P, 1)
-k_project_deflate_tma(const __grid_constant__ CUtensorMap tmH, const ProjArgs a, int nc, int nstages) {
+k_project_deflate_tma(const __grid_constant__ CUtensorMap tmH, const ProjArgs a, int nc, int nstages, int rb0, int nrb) {
     extern __shared__ __align__(128) unsigned char smraw[];
     uint64_t* full = reinterpret_cast<uint64_t*>(smraw);
     uint64_t* empty = full + PROJ_MAX_STAGES;
@@ -200,7 +200,7 @@ k_project_deflate_tma(const __grid_constant__ CUtensorMap tmH, const ProjArgs a,
         if (lane < (TMAX / 8) * (PROJ_P / 128)) {
             const int rb = lane % (TMAX / 8), pan = lane / (TMAX / 8);
             tma_2d_g2s(ring + (size_t)ps * stage_elems + pan * (TMAX * 128) + rb * 8 * 128, &tmH,
-                       (int)(pchunk * (2 * PROJ_P) + pan * 256), 8 * rb, full + ps);
+                       (int)(pchunk * (2 * PROJ_P) + pan * 256), 8 * (nrb ? (rb0 + rb) % nrb : rb), full + ps);   // nrb != 0: ring window
         }
         pchunk += gridDim.x;
         if (++ps == nstages) { ps = 0; pph ^= 1u; }
@@ -257,6 +257,9 @@ template <int TMAX> static int launch_deflate(holo_ctx* c, const ProjArgs& a, in
     const size_t stage_bytes = (size_t)TMAX * PROJ_P * sizeof(float2);
     int nstages = (int)((200 * 1024 - vbytes) / stage_bytes);
     if (nstages > PROJ_MAX_STAGES) nstages = PROJ_MAX_STAGES;
+    if (c->ring_nrb && !(c->tune[HOLO_TUNE_PROJ_TMA] && nstages >= 2 && a.npix % PROJ_P == 0 && a.T == TMAX)) {
+        holo_set_error("ring projection needs the TMA kernel and T in {8,16,32,64}"); return HOLO_ERR_STATE;
+    }
     if (c->tune[HOLO_TUNE_PROJ_TMA] && nstages >= 2 && a.npix % PROJ_P == 0) {
         const size_t smem = 128 + vbytes + (size_t)nstages * stage_bytes;
         static bool attr = false;
@@ -265,12 +268,12 @@ template <int TMAX> static int launch_deflate(holo_ctx* c, const ProjArgs& a, in
             attr = true;
         }
         alignas(64) CUtensorMap tmH;
-        { const int rc = holo_make_tensor_map(&tmH, a.H, a.npix, a.T, 128); if (rc) return rc; }
+        { const int rc = holo_make_tensor_map(&tmH, a.H, a.npix, c->ring_nrb ? 8 * c->ring_nrb : a.T, 128); if (rc) return rc; }
         const long long nchunks = a.npix / PROJ_P;
         const int cap = c->proj_grid_cap > 0 ? c->proj_grid_cap : c->num_sms;
         const int grid = (int)(nchunks < cap ? nchunks : cap);
         HoloProf prof(c, HOLO_K_PROJECT, st);
-        k_project_deflate_tma<TMAX, PROJ_P><<<grid, PROJ_P, smem, st>>>(tmH, a, nc, nstages);
+        k_project_deflate_tma<TMAX, PROJ_P><<<grid, PROJ_P, smem, st>>>(tmH, a, nc, nstages, c->ring_rb0, c->ring_nrb);
         HOLO_CUDA_OK(cudaGetLastError());
         return HOLO_OK;
     }

@@ -377,12 +377,14 @@ def test_process_real_covariance_identity(torch_cuda):
     h.close()
 
 
-@pytest.mark.parametrize("n,T,steps", [(128, 16, [4, 4, 4, 4, 4]), (64, 32, [8, 8, 5, 11, 8, 32, 8]), (64, 12, [3, 3, 3, 7])])
-def test_push_sliding_window_matches_oracle(torch_cuda, n, T, steps):
+@pytest.mark.parametrize("n,T,steps,flush_each", [(128, 16, [4, 4, 4, 4, 4], True), (64, 32, [8, 8, 5, 11, 8, 32, 8], True),
+                                                 (64, 12, [3, 3, 3, 7], True), (128, 32, [8] * 7, False), (64, 16, [8, 8, 8], False)])
+def test_push_sliding_window_matches_oracle(torch_cuda, n, T, steps, flush_each):
     """holo_push: only the newest frames are transformed, against a fixed reference image; the
     window mean is removed afterwards.  Every window's image must match the oracle's holo_process of that window
     (north-star tolerance 1e-4 on M; here also the 2e-5 bug bound), including ring wrap-around (strides that do
-    not divide T) and a re-reference in mid-sequence (n_new = T)."""
+    not divide T), a re-reference in mid-sequence (n_new = T), the pipelined ring form (T in {16,32,64}, n_new a
+    multiple of 8: images complete after holo_flush) and the migration from the ring to the flat form."""
     torch = torch_cuda
     total = T + sum(steps)
     cfg = G.small_config(n=n, T=T, n_frames=total + T)
@@ -390,15 +392,23 @@ def test_push_sliding_window_matches_oracle(torch_cuda, n, T, steps):
     stream = G.frames_np(scene, 0, total)
     dev = _to_dev(torch, stream)
     h = _holo(n, n, T, 2, T)
-    M = torch.empty((n, n), dtype=torch.float32, device="cuda")
     fbytes = n * n * 2
-    h.push(dev.data_ptr(), T, M)                                   # first window
+    outs = [torch.zeros((n, n), dtype=torch.float32, device="cuda") for _ in range(len(steps) + 1)]
+    ends = []
+    h.push(dev.data_ptr(), T, outs[0])                             # first window
     end = T
-    wins = [(end, M.cpu().numpy().copy())]
-    for k in steps:
-        h.push(dev.data_ptr() + end * fbytes, k, M)
+    ends.append(end)
+    if flush_each:
+        h.flush()
+    for i, k in enumerate(steps):
+        h.push(dev.data_ptr() + end * fbytes, k, outs[i + 1])
         end += k
-        wins.append((end, M.cpu().numpy().copy()))
+        ends.append(end)
+        if flush_each:
+            h.flush()
+    h.flush()
+    torch.cuda.synchronize()
+    wins = [(e, o.cpu().numpy()) for e, o in zip(ends, outs)]
     rc, status = h.status()
     assert rc == 0
     for end, Mg in wins:
