@@ -533,8 +533,18 @@ extern "C" int holo_workspace_copy(holo_ctx* c, int which, void* dst_dev, unsign
 extern "C" int holo_status(holo_ctx* c, int32_t status_host[4], holo_stream stream) {
     CHECK_CTX(c); CHECK_PTR(status_host, "status_host");
     cudaStream_t st = (cudaStream_t)stream;
+    // the eigensolvers of holo_submit / holo_push run on the side stream: join it first (the caller should have called
+    // holo_flush; this only makes the read safe), then read the word of the last solve of each workspace slot
+    HOLO_CUDA_OK(cudaStreamSynchronize(st));
+    if (c->side) HOLO_CUDA_OK(cudaStreamSynchronize(c->side));
     HOLO_CUDA_OK(cudaMemcpyAsync(status_host, c->status, 4 * sizeof(int32_t), cudaMemcpyDeviceToHost, st));
     HOLO_CUDA_OK(cudaStreamSynchronize(st));
+    if (c->status1 && !status_host[0]) {
+        int32_t other[4];
+        HOLO_CUDA_OK(cudaMemcpyAsync(other, c->status1, 4 * sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+        HOLO_CUDA_OK(cudaStreamSynchronize(st));
+        if (other[0]) memcpy(status_host, other, sizeof(other));      // report the slot that failed
+    }
     if (status_host[0]) { holo_set_error("Jacobi eigensolver hit the sweep cap (%d sweeps)", status_host[1]); return HOLO_ERR_NOCONV; }
     return HOLO_OK;
 }
