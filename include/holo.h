@@ -177,7 +177,7 @@ int holo_launches_per_process(holo_ctx* ctx);
  *   7 TMA-fed projection (default 1), 8 real-part covariance in holo_process / holo_submit (default 1; the
  *   covariance of holograms of real frames is real in exact arithmetic, R21), 9 SMs given to the
  *   side-stream projection in holo_submit (0 = projection in stream order after the next Fresnel stage),
- *   10 pipelined ring form of holo_push (default 1). */
+ *   10 pipelined ring form of holo_push (default 1), 11 incremental Gram update in that form (default 1). */
 int holo_tune(holo_ctx* ctx, int key, int value);
 
 const char* holo_last_error(void);   /* thread-local, static storage */

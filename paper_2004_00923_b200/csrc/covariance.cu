@@ -374,27 +374,56 @@ __global__ void __launch_bounds__(256) k_cov_reduce(const float2* __restrict__ p
 // holograms of the current window are H_t = G_t - mean_t G.  Their covariance is C = J Gamma J with Gamma = G^H G and
 // J = I - 11^T/T:  C_ts = Gamma_ts - rho_t/T - conj(rho_s)/T + tau/T^2  (rho = row sums, tau = total), done in
 // FP64 on the unrounded sums of the reduction.  One CTA.
-__global__ void __launch_bounds__(256) k_center_gram(const double2* __restrict__ Gd, int T, float2* __restrict__ C) {
+// Gs != nullptr: slot-indexed FP64 store of the (real) Gram of the hologram ring, Gs[slot_t * Rn + slot_s]; the window
+// is slots a0 .. a0+T-1 (mod Rn).  scatter = 1: Gd (a full recomputation) is also copied into Gs; scatter = 0: Gd is not
+// used, the window is gathered from Gs (incremental update: only the new rows / columns were recomputed).
+__global__ void __launch_bounds__(256) k_center_gram(const double2* __restrict__ Gd, int T, float2* __restrict__ C,
+                                                     double* __restrict__ Gs, int Rn, int a0, int scatter) {
     __shared__ double2 rho[HOLO_MAX_T];
     __shared__ double2 tau;
+    const bool gather = Gs && !scatter;
+    auto slot = [&](int t) { return (a0 + t) % Rn; };
+    auto get = [&](int t, int s) { return gather ? make_double2(Gs[slot(t) * Rn + slot(s)], 0.0) : Gd[t * T + s]; };
+    if (Gs && scatter)
+        for (int i = threadIdx.x; i < T * T; i += blockDim.x) { const int t = i / T, s = i - t * T; Gs[slot(t) * Rn + slot(s)] = Gd[i].x; }
     for (int t = threadIdx.x; t < T; t += blockDim.x) {
         double2 r = make_double2(0.0, 0.0);
-        for (int s = 0; s < T; ++s) { r.x += Gd[t * T + s].x; r.y += Gd[t * T + s].y; }
+        for (int s = 0; s < T; ++s) { const double2 g = get(t, s); r.x += g.x; r.y += g.y; }
         rho[t] = r;
     }
     __syncthreads();
     if (threadIdx.x == 0) {
-        double2 a = make_double2(0.0, 0.0);
-        for (int t = 0; t < T; ++t) { a.x += rho[t].x; a.y += rho[t].y; }
-        tau = a;
+        double2 acc = make_double2(0.0, 0.0);
+        for (int t = 0; t < T; ++t) { acc.x += rho[t].x; acc.y += rho[t].y; }
+        tau = acc;
     }
     __syncthreads();
     const double iT = 1.0 / (double)T;
     for (int i = threadIdx.x; i < T * T; i += blockDim.x) {
         const int t = i / T, s = i - t * T;
-        const double re = Gd[i].x - (rho[t].x + rho[s].x) * iT + tau.x * iT * iT;
-        const double im = Gd[i].y - (rho[t].y - rho[s].y) * iT;           // tau is real for a Hermitian Gamma
+        const double2 g = get(t, s);
+        const double re = g.x - (rho[t].x + rho[s].x) * iT + tau.x * iT * iT;
+        const double im = g.y - (rho[t].y - rho[s].y) * iT;               // tau is real for a Hermitian Gamma
         C[i] = make_float2((float)re, t == s ? 0.f : (float)im);
+    }
+}
+
+// incremental update: FP64 sums of the partial entries (row r, new column cn) -> Gs, both orientations.
+// grid = (T rows, newb blocks), 8 warps: warp j of the CTA takes column j of the block, lanes split the parts.
+__global__ void __launch_bounds__(256) k_cov_reduce_new(const float2* __restrict__ partials, int nparts, int T, int T8, int newb,
+                                                        double* __restrict__ Gs, int Rn, int a0) {
+    const int lane = threadIdx.x & 31, j = threadIdx.x >> 5;
+    const int r = blockIdx.x, cn = T8 - 8 * newb + 8 * blockIdx.y + j;
+    if (cn >= T) return;
+    const float2* p = partials + r * T8 + cn;
+    double re = 0.0;
+    for (int k = lane; k < nparts; k += 32) re += (double)p[(size_t)k * T8 * T8].x;
+#pragma unroll
+    for (int o = 16; o >= 1; o >>= 1) re += __shfl_xor_sync(0xffffffffu, re, o);
+    if (lane == 0) {
+        const int sr = (a0 + r) % Rn, sc = (a0 + cn) % Rn;
+        Gs[sr * Rn + sc] = re;
+        Gs[sc * Rn + sr] = re;
     }
 }
 
@@ -456,12 +485,18 @@ static int launch_cov_real(holo_ctx* c, const float2* H, float2* C, cudaStream_t
     memset(&plan, 0, sizeof(plan));
     RealJob all[16];
     int n = 0;
-    for (int a = 1; a < nb16; ++a)
-        for (int b = 0; b < a; ++b) { all[n++] = RealJob{0, a, 2 * b}; all[n++] = RealJob{0, a, 2 * b + 1}; }
-    for (int a = 0; a < nb16; ++a) all[n++] = RealJob{1, a, 0};
+    const int newb = c->cov_new_blocks;                    // holo_push: only the products with the newest 8-row blocks
+    if (newb > 0) {
+        for (int b = T8 / 8 - newb; b < T8 / 8; ++b)
+            for (int a = 0; a < nb16; ++a) all[n++] = RealJob{0, a, b};     // all rows x new block (upper-triangle entries too)
+    } else {
+        for (int a = 1; a < nb16; ++a)
+            for (int b = 0; b < a; ++b) { all[n++] = RealJob{0, a, 2 * b}; all[n++] = RealJob{0, a, 2 * b + 1}; }
+        for (int a = 0; a < nb16; ++a) all[n++] = RealJob{1, a, 0};
+    }
     const int gy = n > COV_NW ? 2 : 1;
     for (int k = 0; k < n; ++k) { const int g = gy == 2 ? (k & 1) : 0; plan.job[g][plan.njobs[g]++] = all[k]; }
-    const int ngroups = n == 4 ? 2 : n == 1 ? 4 : 1;       // spare warps take alternate chunks
+    const int ngroups = n == 4 ? 2 : n == 2 ? 4 : n == 1 ? 4 : 1;       // spare warps take alternate chunks
     const int nslots = nb16 * 2;
     const size_t stage_bytes = (size_t)nslots * 8 * COV_P * sizeof(float2);
     int nstages = (int)(COV_SMEM_BUDGET / stage_bytes);
@@ -487,6 +522,16 @@ static int launch_cov_real(holo_ctx* c, const float2* H, float2* C, cudaStream_t
     }
     HOLO_CUDA_OK(cudaGetLastError());
     c->cov_nparts = gx * ngroups;
+    if (newb > 0) {
+        // new rows / columns -> slot-indexed FP64 store, then gather + centre the window
+        const int Rn = 8 * c->ring_nrb, a0 = 8 * c->ring_rb0;
+        HoloProf prof(c, HOLO_K_COV_REDUCE, st);
+        k_cov_reduce_new<<<dim3(T, newb), 256, 0, st>>>(holo_cov_partials(c, c->cov_sel), c->cov_nparts, T, T8, newb, c->Gs, Rn, a0);
+        HOLO_CUDA_OK(cudaGetLastError());
+        k_center_gram<<<1, 256, 0, st>>>(nullptr, T, C, c->Gs, Rn, a0, 0);
+        HOLO_CUDA_OK(cudaGetLastError());
+        return HOLO_OK;
+    }
     return C ? holo_launch_cov_reduce(c, c->cov_sel, c->cov_nparts, C, st) : HOLO_OK;
 }
 
@@ -496,7 +541,7 @@ int holo_launch_cov_reduce(holo_ctx* c, int sel, int nparts, float2* C, cudaStre
     k_cov_reduce<<<(n * 32 + 255) / 256, 256, 0, st>>>(holo_cov_partials(c, sel), nparts, T, T8, C, c->center_gram ? c->Cd : nullptr);
     HOLO_CUDA_OK(cudaGetLastError());
     if (c->center_gram) {                                  // holo_push: C <- J Gamma J
-        k_center_gram<<<1, 256, 0, st>>>(c->Cd, T, C);
+        k_center_gram<<<1, 256, 0, st>>>(c->Cd, T, C, c->ring_nrb ? c->Gs : nullptr, 8 * c->ring_nrb, 8 * c->ring_rb0, 1);
         HOLO_CUDA_OK(cudaGetLastError());
     }
     return HOLO_OK;

@@ -49,7 +49,7 @@ static void free_ctx(holo_ctx* c) {
         delete[] c->prof_ev;
         delete[] c->prof_cls;
     }
-    cudaFree(c->Cd); cudaFree(c->ring);
+    cudaFree(c->Cd); cudaFree(c->ring); cudaFree(c->Gs);
     cudaFree(c->H1); cudaFree(c->C1); cudaFree(c->evals1); cudaFree(c->V1); cudaFree(c->status1);
     if (c->side) {
         cudaStreamDestroy(c->side);
@@ -100,6 +100,7 @@ static int create_impl(holo_ctx* c) {
     c->tune[HOLO_TUNE_PROJ_TMA] = 1;
     c->tune[HOLO_TUNE_COV_REAL] = 1;
     c->tune[HOLO_TUNE_PUSH_PIPE] = 1;
+    c->tune[HOLO_TUNE_PUSH_INCR] = 1;
     // 40 of 148 SMs: measured optimum at 1024^2 x 32 (354 -> 320 us per stack); at T = 64 the projection is too slow
     // per SM (64 holograms in registers) and the split loses (3.87 -> 4.30 ms), so it is off there
     c->tune[HOLO_TUNE_SPLIT_SMS] = T <= 32 ? (c->num_sms * 27 + 50) / 100 : 0;
@@ -339,7 +340,11 @@ extern "C" int holo_push(holo_ctx* c, const uint16_t* new_frames_dev, int n_new,
         if ((rc = project_pending(c, st))) return rc;
         if (push_ring_possible(c)) {
             if ((rc = submit_init(c))) return rc;                          // side stream, events, second C / V slot
-            if (!c->ring) { c->ring_slots = T + extra; HOLO_CUDA_OK(cudaMalloc(&c->ring, (size_t)c->ring_slots * c->npix * sizeof(float2))); }
+            if (!c->ring) {
+                c->ring_slots = T + extra;
+                HOLO_CUDA_OK(cudaMalloc(&c->ring, (size_t)c->ring_slots * c->npix * sizeof(float2)));
+                HOLO_CUDA_OK(cudaMalloc(&c->Gs, (size_t)c->ring_slots * c->ring_slots * sizeof(double)));
+            }
             if ((rc = holo_launch_fresnel(c, new_frames_dev, c->ring, st))) return rc;
             c->push_ready = 2; c->ring_a = 0;
         } else {
@@ -383,8 +388,12 @@ extern "C" int holo_push(holo_ctx* c, const uint16_t* new_frames_dev, int n_new,
     c->ring_rb0 = c->ring_a / 8; c->ring_nrb = c->ring_slots / 8;
     c->center_gram = 1;
     c->cov_grid_cap = split > 0 ? c->num_sms - split : 0;
+    // incremental Gram: only the products with the new frames (kept in a slot-indexed FP64 store), when the job
+    // count fits one CTA shape; a restart recomputes everything
+    const int njobs_new = (T / 16) * (n_new / 8);
+    c->cov_new_blocks = (n_new < T && c->tune[HOLO_TUNE_PUSH_INCR] && (njobs_new == 1 || njobs_new == 2 || njobs_new == 4 || njobs_new == 8)) ? n_new / 8 : 0;
     rc = holo_launch_covariance(c, c->ring, C, st, /*real_only=*/true);
-    c->center_gram = 0; c->cov_grid_cap = 0;
+    c->center_gram = 0; c->cov_grid_cap = 0; c->cov_new_blocks = 0;
     if (!rc) rc = cudaEventRecord(c->ev_cov[s], st) == cudaSuccess && cudaStreamWaitEvent(c->side, c->ev_cov[s], 0) == cudaSuccess ? HOLO_OK : HOLO_ERR_CUDA;
     if (!rc) {
         int32_t* status_main = c->status;

@@ -22,6 +22,7 @@ enum {
     HOLO_TUNE_SPLIT_SMS = 9,       // holo_submit: k > 0 = projection on the side stream on k SMs, concurrent with the
                                    // next covariance on the other SMs (memory-bound next to ALU-bound); 0 = in stream order
     HOLO_TUNE_PUSH_PIPE = 10,      // holo_push: 1 = pipelined ring form when T in {16,32,64} and n_new is a multiple of 8 (default)
+    HOLO_TUNE_PUSH_INCR = 11,      // holo_push (ring form): 1 = recompute only the Gram rows / columns of the new frames (default)
     HOLO_TUNE_FFT_LAG = 6,         // frames between the row pass and the column pass in the fused kernel (0 = auto)         // 1 = bracket every kernel launch with events (holo_profile_read)
 };
 
@@ -85,6 +86,8 @@ struct holo_ctx {
     // ring_nrb != 0 the covariance / projection launchers read the window through the ring (8-row blocks modulo).
     float2* ring; int ring_slots, ring_a; long long npush;
     int ring_rb0, ring_nrb;
+    double* Gs;             // [ring_slots][ring_slots] slot-indexed FP64 Gram of the ring (incremental update)
+    int cov_new_blocks;     // > 0: the next covariance launch recomputes only the products with the newest 8-frame blocks
     int cov_grid_cap, proj_grid_cap;   // CTA caps used by the SM-split mode of holo_submit (0 = none)
     // host staging for holo_process_host
     uint16_t* frames_stage;

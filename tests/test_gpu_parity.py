@@ -378,7 +378,8 @@ def test_process_real_covariance_identity(torch_cuda):
 
 
 @pytest.mark.parametrize("n,T,steps,flush_each", [(128, 16, [4, 4, 4, 4, 4], True), (64, 32, [8, 8, 5, 11, 8, 32, 8], True),
-                                                 (64, 12, [3, 3, 3, 7], True), (128, 32, [8] * 7, False), (64, 16, [8, 8, 8], False)])
+                                                 (64, 12, [3, 3, 3, 7], True), (128, 32, [8] * 7, False), (64, 16, [8, 8, 8], False),
+                                                 (64, 32, [8] * 14, False), (64, 32, [16, 16, 8, 16, 16], False), (32, 64, [8, 16, 32, 8], False)])
 def test_push_sliding_window_matches_oracle(torch_cuda, n, T, steps, flush_each):
     """holo_push: only the newest frames are transformed, against a fixed reference image; the
     window mean is removed afterwards.  Every window's image must match the oracle's holo_process of that window
