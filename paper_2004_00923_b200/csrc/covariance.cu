@@ -386,10 +386,13 @@ __global__ void __launch_bounds__(256) k_center_gram(const double2* __restrict__
     auto get = [&](int t, int s) { return gather ? make_double2(Gs[slot(t) * Rn + slot(s)], 0.0) : Gd[t * T + s]; };
     if (Gs && scatter)
         for (int i = threadIdx.x; i < T * T; i += blockDim.x) { const int t = i / T, s = i - t * T; Gs[slot(t) * Rn + slot(s)] = Gd[i].x; }
-    for (int t = threadIdx.x; t < T; t += blockDim.x) {
+    if (Gs && scatter) __syncthreads();
+    for (int t = threadIdx.x >> 5; t < T; t += blockDim.x >> 5) {         // one warp per row, fixed summation order
         double2 r = make_double2(0.0, 0.0);
-        for (int s = 0; s < T; ++s) { const double2 g = get(t, s); r.x += g.x; r.y += g.y; }
-        rho[t] = r;
+        for (int s = threadIdx.x & 31; s < T; s += 32) { const double2 g = get(t, s); r.x += g.x; r.y += g.y; }
+#pragma unroll
+        for (int o = 16; o >= 1; o >>= 1) { r.x += __shfl_xor_sync(0xffffffffu, r.x, o); r.y += __shfl_xor_sync(0xffffffffu, r.y, o); }
+        if ((threadIdx.x & 31) == 0) rho[t] = r;
     }
     __syncthreads();
     if (threadIdx.x == 0) {
