@@ -1,17 +1,19 @@
 #!/usr/bin/env python
 """bench.py -- PCA images/s (input frames/s) at 1024^2 x 32 uint16 (BASELINE.json metric), one JSON line.
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 3]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 3] [--api submit|process|push]
+                  [--mode 1|2]
 
-A "step" is one pass of the whole hot path (A0..A6, holo_process) over one stack of T frames.
-The stream (BASELINE.json configs[2]: 64 stacks = 2048 frames = 4 GiB of uint16) is resident in HBM
-before the timed region and is cycled through, so the inputs are far larger than L2 (126 MB).
-N > 1 (torchrun): one process per GPU, each with its own stream, no data-path collective (weak
-scaling); timing is bracketed by a barrier and reported as the max over ranks.
+A "step" is one pass of the whole hot path (A0..A6) over one stack of T frames (`--api push`: one window of the
+sliding-window form, `stride` new frames).  The stream is resident in HBM before the timed region and is cycled
+through; it is sized to at least 3x the 126 MB L2, so no step finds its inputs in L2 (`config.l2_policy` states
+the sizes).  N > 1 (torchrun): one process per GPU, each with its own stream of stacks, no data-path collective
+(weak scaling); timing is bracketed by a barrier and reported as the max over ranks.
 `--impl reference` times the CPU oracle (oracle/) on host cores on a bounded sample.
 """
 import argparse
 import json
+import math
 import os
 import subprocess
 import sys
@@ -21,8 +23,14 @@ import time
 ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
-METRIC = "PCA images/s at 1024x1024x32 uint16 (input frames/s = 32x)"
 PAPER_IMAGES_PER_S = 20.0        # "up to 20" PCA images/s, Titan RTX
+L2_BYTES = 126e6                 # B200_PROFILING.md
+FP32_PEAK_MEASURED_TFLOPS = 72.0 # profiles/r01_ubench_peaks.txt (register-only FFMA, csrc/ubench_peaks.cu); nominal 74.4
+FP32_LANES_PER_SM = 128
+
+
+def metric_name(cfg):
+    return f"PCA images/s at {cfg.n}x{cfg.n}x{cfg.T} uint16 (input frames/s = {cfg.stride}x)"
 
 
 def _peaks():
@@ -31,6 +39,47 @@ def _peaks():
         d = json.load(open(p))
         return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json)", d
     return 6650.0, "fallback (B200_PROFILING.md)", {}
+
+
+# ------------------------------------------------------------------------------------------------------------
+# rank / shard logic of the GPU arm (no GPU needed: tests/test_host_logic.py runs it under gloo, world_size 2)
+# ------------------------------------------------------------------------------------------------------------
+def rank_env():
+    return (int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1")), int(os.environ.get("LOCAL_RANK", "0")))
+
+
+def shard_plan(cfg, rank, world, stacks=None, min_resident_bytes=3 * L2_BYTES):
+    """What one rank holds and cycles through.  Stacks are independent units: every rank generates its OWN stream
+    (seed 1000 + rank) of the same shape -- weak scaling, no data-path collective.  The resident stream is at least
+    `min_resident_bytes` long (>= 3x L2), extended beyond the config's stream length with the same generator if needed."""
+    T, n = cfg.T, cfg.n
+    fbytes = T * n * n * 2
+    n_stacks = stacks or max(cfg.n_frames // T, int(math.ceil(min_resident_bytes / fbytes)))
+    n_frames = n_stacks * T
+    n_win = (n_frames - T) // cfg.stride + 1           # windows a step can start at (stride < T: overlapping)
+    n_push = (n_frames - T) // cfg.stride              # pushes that fit after the first window
+    return {"seed": 1000 + rank, "n_stacks": n_stacks, "n_frames": n_frames, "n_win": n_win, "n_push": n_push,
+            "stack_bytes": fbytes, "resident_bytes": n_stacks * fbytes, "window_stride_bytes": cfg.stride * n * n * 2}
+
+
+def reduce_max_ms(ms, dist=None, device=None):
+    """Max over ranks of a device-timed duration (every rank must call)."""
+    if dist is None:
+        return float(ms)
+    import torch
+    t = torch.tensor([ms], dtype=torch.float64, device=device or "cpu")
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def aggregate_value(world, steps, ms_max):
+    """Whole-job throughput: every rank did `steps` units in (at most) ms_max."""
+    return world * steps / (ms_max * 1e-3)
+
+
+def l2_policy(plan):
+    return (f"inputs larger than L2: {plan['resident_bytes'] / 1e6:.0f} MB resident stream cycled through "
+            f"({plan['resident_bytes'] / L2_BYTES:.1f}x the 126 MB L2), no flush needed")
 
 
 class ClockSampler:
@@ -79,18 +128,20 @@ class ClockSampler:
                 "power_w_max": max(power) if power else None, "reasons": sorted(reasons)}
 
 
-def stage_bytes(cfg):
-    """Algorithmic (compulsory) bytes per stack and stage, SURVEY.md 8(d) / DESIGN.md."""
+def stage_bytes(cfg, mode=1):
+    """Algorithmic (compulsory) bytes per stack and stage, SURVEY.md 8(d) / DESIGN.md.  mode 2 (Gram from the raw
+    frames, SURVEY.md 8(f)-2 stage 1) has no covariance read of the hologram stack: 20 T N_p + 12 N_p."""
     npix, T = cfg.n * cfg.n, cfg.T
-    return {"sum": 2 * T * npix + 4 * npix, "fft": 2 * T * npix + 4 * npix + 8 * T * npix,
-            "cov": 8 * T * npix, "eig": 16 * T * T, "proj": 8 * T * npix + 4 * npix,
-            "total": 28 * T * npix + 12 * npix}
+    d = {"sum": 2 * T * npix + 4 * npix, "fft": 2 * T * npix + 4 * npix + 8 * T * npix,
+         "cov": 8 * T * npix if mode == 1 else 0, "eig": 16 * T * T, "proj": 8 * T * npix + 4 * npix}
+    d["total"] = d["sum"] + d["fft"] + d["cov"] + d["proj"]
+    return d
 
 
 def run_reference(args, cfg):
-    """CPU oracle arm: each step = the oracle on a bounded sample (a centred crop of n_s x n_s pixels of
-    one stack, all T frames), scaled to full-frame images/s by the pixel ratio."""
-    rank = int(os.environ.get("RANK", "0"))
+    """CPU oracle arm: each step = the oracle on a bounded sample (a crop of n_s x n_s pixels of one stack, all T
+    frames), scaled to full-frame images/s by the pixel ratio."""
+    rank, world, _ = rank_env()
     if rank != 0:
         return
     import numpy as np
@@ -100,7 +151,6 @@ def run_reference(args, cfg):
     budget_s = 150.0
     scene = G.make_scene(cfg, 0)
     frames = G.frames_np(scene, 0, cfg.T)
-    # calibrate on a 128^2 crop, then pick the largest power-of-two crop that fits the budget
     c0 = frames[:, :128, :128].copy()
     t = time.time(); oracle.process(c0, cfg.lam, cfg.pitch, cfg.z, cfg.k_lo, cfg.k_hi); t128 = time.time() - t
     n_s = cfg.n
@@ -118,9 +168,11 @@ def run_reference(args, cfg):
     sample = f"{n_s}x{n_s}x{cfg.T} crop of one {cfg.name} stack per step ({frac:.4g} of a full stack), scaled by pixel ratio"
     cores = oracle.num_threads()
     print(json.dumps({
-        "impl": "reference", "metric": METRIC, "value": value, "unit": "images/s", "n_gpus": args.gpus,
+        "impl": "reference", "metric": metric_name(cfg), "value": value, "unit": "images/s", "n_gpus": args.gpus,
         "steps": steps, "warmup": warmup, "ms_per_step": dt / steps * 1e3, "higher_is_better": True,
-        "scaling": "weak", "vs_baseline": value / PAPER_IMAGES_PER_S, "dtype": "f64", "data": "synthetic",
+        "scaling": "weak", "vs_baseline": value / PAPER_IMAGES_PER_S if cfg.name.startswith("cfg3") else None,
+        "vs_baseline_note": "paper's figure on another machine (Titan RTX): context, not the target",
+        "dtype": "f64", "data": "synthetic",
         "config": {"workload": cfg.name, "nx": cfg.n, "ny": cfg.n, "T": cfg.T, "k_lo": cfg.k_lo, "k_hi": cfg.k_hi},
         "cpu_baseline": {"value": value, "unit": "images/s", "cores": cores, "kind": "oracle", "sample": sample},
         "e2e": {"value": value, "unit": "images/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
@@ -129,18 +181,117 @@ def run_reference(args, cfg):
 
 
 KCLASS = ["sum", "fft_rows", "fft_cols", "cov_partial", "cov_reduce", "eig", "project"]
-FP32_LANES_PER_SM = 128          # B200 SM: 4 SMSP x 32 FP32 lanes (blackwell guide / B300_MICROARCH.md)
+
+
+def kernel_name(cls, fused_fft, cov_real, mode):
+    return {"sum": "k_frame_sum" if mode == 1 else "k_sum_gram", "fft_rows": "k_fresnel" if fused_fft else "k_fft<rows>",
+            "fft_cols": "k_fft<cols>", "cov_partial": "k_cov_partial_real" if cov_real else "k_cov_partial",
+            "cov_reduce": "k_cov_reduce", "eig": "k_eig", "project": "k_project_deflate_tma / k_project"}[cls]
+
+
+def _traffic_table():
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch from the round's `ncu --set full` capture
+    (profiles/r02_traffic.csv: workload,kernel class,bytes; see profiles/r02.md for the command)."""
+    tab = {}
+    p = os.path.join(ROOT, "profiles", "r02_traffic.csv")
+    if os.path.exists(p):
+        for ln in open(p).read().splitlines()[1:]:
+            f = ln.split(",")
+            if len(f) == 3:
+                tab[(f[0], f[1])] = int(f[2])
+    return tab
+
+
+class Runner:
+    """One handle + one resident stream of one config; times K steps of one API on a stream."""
+
+    def __init__(self, cfg, plan, dev, tune=(), mode=1):
+        import torch
+        from gen import holo_gen as G
+        from paper_2004_00923_b200 import Holo
+        self.torch, self.cfg, self.plan, self.dev = torch, cfg, plan, dev
+        self.frames = G.stream_torch(cfg, plan["seed"], dev, n_frames=plan["n_frames"])
+        torch.cuda.synchronize()
+        self.h = Holo(cfg.n, cfg.n, cfg.T, cfg.lam, cfg.pitch, cfg.z, cfg.k_lo, cfg.k_hi)
+        for kv in tune:
+            k, v = kv.split("=")
+            self.h.tune(int(k), int(v))
+        if mode == 2:
+            self.h.set_mode(2)
+        self.images = torch.empty((4, cfg.n, cfg.n), dtype=torch.float32, device=dev)
+        self.st = torch.cuda.Stream(device=dev)
+
+    def step(self, api, i):
+        cfg, p, h, fr = self.cfg, self.plan, self.h, self.frames
+        if api == "push":
+            # sliding window: `stride` new frames per step; once per cycle of the resident stream the sequence
+            # restarts with a whole window (a re-reference, counted as a step)
+            k = i % (p["n_push"] + 1)
+            if k == 0:
+                h.push(fr.data_ptr(), cfg.T, self.images[i % 4], self.st)
+            else:
+                h.push(fr.data_ptr() + (cfg.T + (k - 1) * cfg.stride) * cfg.n * cfg.n * 2, cfg.stride, self.images[i % 4], self.st)
+        elif api == "submit":
+            h.submit(fr.data_ptr() + (i % p["n_win"]) * p["window_stride_bytes"], self.images[i % 4], self.st)
+        else:
+            h.process(fr.data_ptr() + (i % p["n_win"]) * p["window_stride_bytes"], self.images[i % 4], self.st)
+
+    def timed(self, api, steps, warmup, barrier, sampler=None):
+        torch = self.torch
+        for i in range(warmup):
+            self.step(api, i)
+        self.h.flush(self.st)
+        barrier()
+        t0 = time.time()
+        if sampler:
+            sampler.start()
+            time.sleep(0.12)
+            t0 = time.time()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(self.st)
+        for i in range(steps):
+            self.step(api, i)
+        self.h.flush(self.st)                  # the last image is part of the timed region
+        e1.record(self.st)
+        barrier()
+        clocks = sampler.stop(t0, time.time()) if sampler else None
+        return e0.elapsed_time(e1), clocks
+
+    def image_of_first_stack(self, api):
+        """The image of the first resident stack/window through the SAME entry point that was timed."""
+        torch, cfg = self.torch, self.cfg
+        M = torch.zeros((cfg.n, cfg.n), dtype=torch.float32, device=self.dev)
+        if api == "push":
+            self.h.push(self.frames.data_ptr(), cfg.T, M, self.st)
+        elif api == "submit":
+            self.h.submit(self.frames.data_ptr(), M, self.st)
+        else:
+            self.h.process(self.frames.data_ptr(), M, self.st)
+        self.h.flush(self.st)
+        self.st.synchronize()
+        return M
+
+    def oracle_check(self, api):
+        import numpy as np
+        import oracle
+        torch, cfg = self.torch, self.cfg
+        fr = self.frames[:cfg.T].cpu().view(torch.int16).numpy().view(np.uint16)
+        t0 = time.time()
+        out = oracle.process(fr, cfg.lam, cfg.pitch, cfg.z, cfg.k_lo, cfg.k_hi)
+        dt = time.time() - t0
+        Mg = self.image_of_first_stack(api).cpu().numpy()
+        err = float(np.linalg.norm(Mg - out["M"]) / np.linalg.norm(out["M"]))
+        return dt, err
+
+    def close(self):
+        self.h.close()
 
 
 def run_ours(args, cfg):
-    import numpy as np
     import torch
     from gen import holo_gen as G
-    from paper_2004_00923_b200 import Holo
 
-    rank = int(os.environ.get("RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    rank, world, local_rank = rank_env()
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device -- the product path has no CPU fallback")
     torch.cuda.set_device(local_rank)
@@ -149,43 +300,6 @@ def run_ours(args, cfg):
     if world > 1:
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=dev)
-    steps = args.steps or 2048
-    warmup = args.warmup if args.warmup is not None else 64
-    warmup = max(warmup, 3)
-    T, n = cfg.T, cfg.n
-    n_stacks = min(args.stacks or (cfg.n_frames // T), cfg.n_frames // T)
-    frames = G.stream_torch(cfg, 1000 + rank, dev, n_frames=n_stacks * T)
-    torch.cuda.synchronize()
-    h = Holo(n, n, T, cfg.lam, cfg.pitch, cfg.z, cfg.k_lo, cfg.k_hi)
-    for kv in args.tune:
-        k, v = kv.split("=")
-        h.tune(int(k), int(v))
-    images = torch.empty((4, n, n), dtype=torch.float32, device=dev)
-    st = torch.cuda.Stream(device=dev)
-    fbytes = T * n * n * 2
-    # stacks may overlap (config 4: stride 8 over the stream): step i starts at frame (i mod n_win) * stride
-    n_win = (n_stacks * T - T) // cfg.stride + 1
-    wbytes = cfg.stride * n * n * 2
-
-    streaming = args.api == "submit"
-
-    pushing = args.api == "push"
-    n_push = (n_stacks * T - T) // cfg.stride          # pushes that fit in the resident stream after the first window
-
-    def step(i):
-        # one stack through the whole path; the streaming form delivers image i during step i+1 (or the flush)
-        if pushing:
-            # sliding window: only `stride` new frames per step; the stream is cycled, so once per cycle the
-            # sequence restarts with a whole window (a re-reference, counted as a step)
-            k = i % (n_push + 1)
-            if k == 0:
-                h.push(frames.data_ptr(), T, images[i % 4], st)
-            else:
-                h.push(frames.data_ptr() + (T + (k - 1) * cfg.stride) * n * n * 2, cfg.stride, images[i % 4], st)
-        elif streaming:
-            h.submit(frames.data_ptr() + (i % n_win) * wbytes, images[i % 4], st)
-        else:
-            h.process(frames.data_ptr() + (i % n_win) * wbytes, images[i % 4], st)
 
     def barrier():
         torch.cuda.synchronize()
@@ -193,170 +307,219 @@ def run_ours(args, cfg):
             dist.barrier()
         torch.cuda.synchronize()
 
-    for i in range(warmup):
-        step(i)
-    h.flush(st)
-    barrier()
+    steps = args.steps or 2048
+    warmup = max(args.warmup if args.warmup is not None else 64, 3)
+    api, mode = args.api, args.mode
+    plan = shard_plan(cfg, rank, world, args.stacks)
+    T, n = cfg.T, cfg.n
+    R = Runner(cfg, plan, dev, args.tune, mode)
+    h = R.h
     sampler = ClockSampler(local_rank if "CUDA_VISIBLE_DEVICES" not in os.environ else
                            int(os.environ["CUDA_VISIBLE_DEVICES"].split(",")[local_rank]))
-    sampler.start()
-    time.sleep(0.12)
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    t_wall0 = time.time()
-    e0.record(st)
-    for i in range(steps):
-        step(i)
-    h.flush(st)                      # the last image is part of the timed region
-    e1.record(st)
-    barrier()
-    t_wall1 = time.time()
-    clocks = sampler.stop(t_wall0, t_wall1)
-    ms = e0.elapsed_time(e1)
-    if dist is not None:
-        t = torch.tensor([ms], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
-    rc, status = h.status(st)
-    value = world * steps / (ms * 1e-3)
+    ms, clocks = R.timed(api, steps, warmup, barrier, sampler)
+    ms = reduce_max_ms(ms, dist, dev)
+    rc, status = h.status(R.st)
+    value = aggregate_value(world, steps, ms)
 
-    # ---- per-kernel-class device times (library's own event brackets; second, instrumented pass)
+    # ---- per-kernel-class device times (library's own event brackets; second, instrumented pass).  The brackets
+    # are only meaningful without kernel concurrency: the instrumented pass uses the serial entry point (same
+    # kernels; in the streaming forms the projection and the eigensolver overlap other kernels on purpose)
     prof_steps = min(steps, 64)
     h.tune(5, 1)
-    # the brackets are only meaningful without kernel concurrency: the instrumented pass uses the serial entry point
-    # (same kernels; in the streaming form the projection and the eigensolver overlap other kernels on purpose)
     for i in range(prof_steps):
-        h.process(frames.data_ptr() + (i % n_win) * wbytes, images[i % 4], st)
+        R.step("process", i)
     prof = h.profile_read()
     h.tune(5, 0)
-    sb = stage_bytes(cfg)
+    sb = stage_bytes(cfg, mode)
     npix = n * n
     G_fft = h.fft_group()
     hbm_peak, peak_src, peaks = _peaks()
-    sm_clock = (clocks.get("sm_mhz") or peaks.get("sm_max_mhz") or 1965.0) * 1e6
     num_sms = torch.cuda.get_device_properties(dev).multi_processor_count
-    fp32_peak_tflops = num_sms * FP32_LANES_PER_SM * 2 * (peaks.get("sm_max_mhz", 1965.0) * 1e6) / 1e12
+    fp32_peak_tflops = FP32_PEAK_MEASURED_TFLOPS * num_sms / 148.0
     fused_fft = prof[2][1] == 0          # no separate column-pass launches: one persistent kernel does A1+A2 of all T frames
+    cov_real = "8=0" not in args.tune
     per_launch_bytes = {"sum": sb["sum"], "fft_rows": sb["fft"] if fused_fft else 2 * G_fft * npix + 4 * npix * G_fft / T,
-                        "fft_cols": 8 * G_fft * npix,
-                        "cov_partial": sb["cov"], "cov_reduce": 0, "eig": sb["eig"], "project": sb["proj"]}
+                        "fft_cols": 8 * G_fft * npix, "cov_partial": 8 * T * npix, "cov_reduce": 0, "eig": sb["eig"], "project": sb["proj"]}
     stages = {}
     tot_ms = sum(p[0] for p in prof) or 1.0
     for name, (ms_k, cnt) in zip(KCLASS, prof):
         if cnt == 0:
             continue
         us = ms_k / cnt * 1e3
-        stages[name] = {"us_per_launch": round(us, 2), "launches_per_step": cnt / prof_steps, "share": round(ms_k / tot_ms, 4),
+        stages[name] = {"kernel": kernel_name(name, fused_fft, cov_real, mode), "us_per_launch": round(us, 2),
+                        "launches_per_step": cnt / prof_steps, "share": round(ms_k / tot_ms, 4),
                         "GBps": round(per_launch_bytes[name] / (us * 1e-6) / 1e9, 1)}
-    # holo_process / holo_submit compute Re C only (C is real there, R21): half the complex Gram
-    cov_real = "8=0" not in args.tune
     cov_flops = (2 if cov_real else 4) * T * (T + 1) * npix
     if "cov_partial" in stages:
         stages["cov_partial"]["form"] = "real part (2T(T+1) flop/pixel)" if cov_real else "complex Hermitian half (4T(T+1) flop/pixel)"
         stages["cov_partial"]["TFLOPs_fp32"] = round(cov_flops / (stages["cov_partial"]["us_per_launch"] * 1e-6) / 1e12, 2)
-    import math
     fft_flops = 10.0 * T * npix * math.log2(n)          # 5 N log2 N per 1-D transform, rows + columns
     if "fft_rows" in stages and fused_fft:
         stages["fft_rows"]["TFLOPs_fp32"] = round(fft_flops / (stages["fft_rows"]["us_per_launch"] * 1e-6) / 1e12, 2)
     dom = max(stages, key=lambda k: stages[k]["share"])
-    traffic = None
-    tpath = os.path.join(ROOT, "profiles", "r01c_traffic.csv")     # dram__bytes_read.sum + dram__bytes_write.sum, one ncu --set full capture
-    if os.path.exists(tpath) and cfg.name.startswith("cfg3"):
-        for ln in open(tpath).read().splitlines()[1:]:
-            k, v = ln.split(",")
-            if k == dom:
-                traffic = int(v)
-    if dom == "cov_partial" and cov_flops / sb["cov"] > fp32_peak_tflops * 1e12 / (hbm_peak * 1e9):
-        roof = {"kernel": dom, "bound": "alu", "achieved": stages[dom]["TFLOPs_fp32"], "peak": round(fp32_peak_tflops, 1),
+    traffic = _traffic_table().get((cfg.name, dom))
+    if dom == "cov_partial" and cov_flops / (8 * T * npix) > fp32_peak_tflops * 1e12 / (hbm_peak * 1e9):
+        roof = {"kernel": stages[dom]["kernel"], "bound": "alu", "achieved": stages[dom]["TFLOPs_fp32"], "peak": round(fp32_peak_tflops, 1),
                 "unit": "TFLOP/s", "frac": round(stages[dom]["TFLOPs_fp32"] / fp32_peak_tflops, 4), "traffic": traffic,
-                "peak_source": f"{num_sms} SMs x {FP32_LANES_PER_SM} FP32 lanes x 2 x max SM clock (DESIGN.md)",
+                "peak_source": "measured register-only FFMA rate (profiles/r01_ubench_peaks.txt; nominal 148 SMs x 128 lanes x 2 x 1.965 GHz = 74.4)",
                 "hbm_frac": round(stages[dom]["GBps"] / hbm_peak, 4)}
     else:
-        roof = {"kernel": dom, "bound": "hbm", "achieved": stages[dom]["GBps"], "peak": hbm_peak, "unit": "GB/s",
-                "frac": round(stages[dom]["GBps"] / hbm_peak, 4), "traffic": traffic, "peak_source": peak_src}
+        roof = {"kernel": stages[dom]["kernel"], "bound": "hbm", "achieved": stages[dom]["GBps"], "peak": hbm_peak, "unit": "GB/s",
+                "frac": round(stages[dom]["GBps"] / hbm_peak, 4), "traffic": traffic, "peak_source": peak_src,
+                "us_per_launch": stages[dom]["us_per_launch"], "algorithmic_bytes_per_launch": per_launch_bytes[dom]}
         if dom == "fft_rows" and "TFLOPs_fp32" in stages[dom]:
-            # the Fresnel stage is balanced between HBM and the FP32 pipe: report the ALU view as well
             roof["alu_achieved_TFLOPs"] = stages[dom]["TFLOPs_fp32"]
             roof["alu_frac"] = round(stages[dom]["TFLOPs_fp32"] / fp32_peak_tflops, 4)
     e2e_gbps = sb["total"] * (steps / (ms * 1e-3)) / 1e9
 
     # ---- end to end through the host entry point (pinned host buffers, H2D + D2H inside the timed region)
     e2e = None
+    streaming = api != "process"
     if not args.no_e2e:
         n_host = 2
         host_frames = torch.empty((n_host, T, n, n), dtype=torch.int16).pin_memory()
-        host_frames.copy_(frames[:n_host * T].view(torch.int16).reshape(n_host, T, n, n).cpu())
+        host_frames.copy_(R.frames[:n_host * T].view(torch.int16).reshape(n_host, T, n, n).cpu())
         host_img = torch.empty((2, n, n), dtype=torch.float32).pin_memory()
         k2 = max(3, min(args.e2e_steps, steps))
 
         def e2e_step(i):
             if streaming:
-                h.submit_host(host_frames[i % n_host], host_img[i % 2], st)
+                h.submit_host(host_frames[i % n_host], host_img[i % 2], R.st)
             else:
-                h.process_host(host_frames[i % n_host], host_img[i % 2], st)
+                h.process_host(host_frames[i % n_host], host_img[i % 2], R.st)
 
         for i in range(3):
             e2e_step(i)
         if streaming:
-            h.flush_host(st)
+            h.flush_host(R.st)
         barrier()
         a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        a0.record(st)
+        a0.record(R.st)
         for i in range(k2):
             e2e_step(i)
         if streaming:
-            h.flush_host(st)                 # the last image reaches the host inside the timed region
-        a1.record(st)
+            h.flush_host(R.st)                 # the last image reaches the host inside the timed region
+        a1.record(R.st)
         barrier()
-        ms2 = a0.elapsed_time(a1)
-        if dist is not None:
-            t = torch.tensor([ms2], dtype=torch.float64, device=dev)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            ms2 = float(t.item())
-        e2e = {"value": world * k2 / (ms2 * 1e-3), "unit": "images/s", "h2d_bytes_per_step": fbytes,
+        ms2 = reduce_max_ms(a0.elapsed_time(a1), dist, dev)
+        e2e = {"value": aggregate_value(world, k2, ms2), "unit": "images/s", "h2d_bytes_per_step": plan["stack_bytes"],
                "d2h_bytes_per_step": n * n * 4, "steps": k2, "ms_per_step": ms2 / k2,
                "api": ("holo_submit_host/holo_flush_host (pinned host frames -> host images; the H2D copy of stack i runs under "
                        "the kernels of stack i-1)") if streaming else "holo_process_host (pinned host frames -> host image, synchronous)"}
 
-    # ---- CPU oracle on the box's host cores (rank 0, N = 1 only): a reported baseline, not the target
+    # ---- CPU oracle on the box's host cores (rank 0, N = 1 only): a reported baseline, not the target.  The GPU image
+    # it is compared with comes from the entry point that was timed.
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu:
         import oracle
-        fr = frames[:T].cpu().view(torch.int16).numpy().view(np.uint16)
-        t0 = time.time()
-        out = oracle.process(fr, cfg.lam, cfg.pitch, cfg.z, cfg.k_lo, cfg.k_hi)
-        dt = time.time() - t0
-        Mg = torch.empty((n, n), dtype=torch.float32, device=dev)
-        h.process(frames.data_ptr(), Mg, st)
-        st.synchronize()
-        err = float(np.linalg.norm(Mg.cpu().numpy() - out["M"]) / np.linalg.norm(out["M"]))
+        dt, err = R.oracle_check(api)
         cpu = {"value": 1.0 / dt, "unit": "images/s", "cores": oracle.num_threads(), "kind": "oracle",
-               "sample": f"1 full stack of {cfg.name} (the first of the GPU stream), {dt:.2f} s", "rel_l2_M_vs_gpu": err}
+               "sample": f"1 full stack of {cfg.name} (the first of the GPU stream), {dt:.2f} s", "rel_l2_M_vs_gpu": err,
+               "gpu_api_compared": api}
+
+    # ---- the other BASELINE.json configs and the paper's own filter window, short runs (rank 0, N = 1 only)
+    side = None
+    if rank == 0 and world == 1 and args.side and cfg.name.startswith("cfg3") and api == "submit":
+        side = {}
+        # the paper's window: ascending n1 = 1 .. n2 = 20 of 32 = descending k in [13, 32]: direct projection
+        h.set_range(13, 32)
+        ms_w, _ = R.timed("submit", 64, 8, barrier)
+        h.set_range(cfg.k_lo, cfg.k_hi)
+        side["cfg3_paper_window_k13_32"] = {"ms_per_step": ms_w / 64, "images_per_s": 64 / (ms_w * 1e-3),
+                                            "note": "same stream, component window of PAPER.md:86 (direct projection kernel)"}
+    lib_ctx = None
+    if rank == 0 and world == 1 and args.side and cfg.name.startswith("cfg3"):
+        lib_ctx = library_context(torch, R, barrier)
+    status_cycles = h.workspace_tensor(5).cpu().tolist()[4:7]
+    launches = h.launches_per_process()
+    R.close()
+    del R
+    torch.cuda.empty_cache()
+    if side is not None:
+        # (config, api, steps, resident stacks): streams of >= 3x L2, kept short so that the default run ends in minutes
+        for cn, sapi, ssteps, sstacks in ((2, "submit", 256, 24), (4, "push", 256, 16), (5, "submit", 24, 3)):
+            c2 = G.CONFIGS[cn]
+            p2 = shard_plan(c2, rank, world, stacks=sstacks)
+            R2 = Runner(c2, p2, dev)
+            ms_s, _ = R2.timed(sapi, ssteps, 6, barrier)
+            sb2 = stage_bytes(c2)
+            ent = {"api": sapi, "ms_per_step": ms_s / ssteps, "images_per_s": ssteps / (ms_s * 1e-3), "resident_bytes": p2["resident_bytes"]}
+            if sapi != "push":
+                ent["roofline_end_to_end_frac"] = round(sb2["total"] * (ssteps / (ms_s * 1e-3)) / 1e9 / hbm_peak, 4)
+                ent["bytes_per_step"] = sb2["total"]
+            else:
+                ent["new_frames_per_s"] = c2.stride * ssteps / (ms_s * 1e-3)
+            if not args.no_cpu:
+                dt2, err2 = R2.oracle_check(sapi)
+                ent["oracle_rel_l2_M_first_stack"] = err2
+                ent["oracle_s_per_stack"] = round(dt2, 2)
+            side[c2.name] = ent
+            R2.close()
+            del R2
+            torch.cuda.empty_cache()
 
     if rank == 0:
         line = {
-            "metric": METRIC, "value": value, "unit": "images/s", "n_gpus": world, "steps": steps, "warmup": warmup,
+            "metric": metric_name(cfg), "value": value, "unit": "images/s", "n_gpus": world, "steps": steps, "warmup": warmup,
             "ms_per_step": ms / steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": value / PAPER_IMAGES_PER_S if cfg.name.startswith("cfg3") else None,
+            "vs_baseline_note": "paper's 'up to 20 images/s' on a Titan RTX (PAPER.md:13,96): another machine, context only",
             "dtype": "f32", "data": "synthetic",
-            "config": {"workload": cfg.name, "nx": n, "ny": n, "T": T, "k_lo": cfg.k_lo, "k_hi": cfg.k_hi,
-                       "stacks_resident": n_stacks, "windows": n_win, "stride_frames": cfg.stride, "resident_input_bytes": n_stacks * fbytes,
-                       "l2_policy": "inputs larger than L2 (stream cycled, no flush needed)",
+            "config": {"workload": cfg.name, "nx": n, "ny": n, "T": T, "k_lo": cfg.k_lo, "k_hi": cfg.k_hi, "mode": mode,
+                       "stacks_resident": plan["n_stacks"], "windows": plan["n_win"], "stride_frames": cfg.stride,
+                       "resident_input_bytes": plan["resident_bytes"], "l2_policy": l2_policy(plan),
                        "parallelism": f"replicas x{world} (independent stacks, no collective)", "fft_group": G_fft,
-                       "api": "holo_submit/holo_flush (stream of stacks, eigensolver of stack i under the Fresnel stage of stack i+1)"
-                              if streaming else ("holo_push (sliding window, stride %d: only the new frames are transformed)" % cfg.stride) if pushing
-                              else "holo_process (one stack per call, strictly serial)"},
+                       "api": {"submit": "holo_submit/holo_flush (stream of stacks, software-pipelined)",
+                               "push": "holo_push (sliding window, stride %d: only the new frames are transformed)" % cfg.stride,
+                               "process": "holo_process (one stack per call, strictly serial)"}[api]},
             "frames_per_s": value * cfg.stride, "clocks": clocks, "e2e": e2e,
-            "gpu_launches": steps * h.launches_per_process(), "launches_per_step": h.launches_per_process(),
+            "gpu_launches": steps * launches, "launches_per_step": launches,
             "roofline": roof, "roofline_end_to_end": {"bound": "hbm", "achieved": round(e2e_gbps, 1), "peak": hbm_peak, "unit": "GB/s",
                                                       "frac": round(e2e_gbps / hbm_peak, 4), "bytes_per_step": sb["total"], "peak_source": peak_src},
-            "stages": stages, "stages_note": "per-kernel device time from an instrumented pass of serial holo_process calls (each kernel alone on the GPU)", "cpu_baseline": cpu, "eig_status": status,
-            "eig_cycles": h.workspace_tensor(5).cpu().tolist()[4:7],
+            "stages": stages, "stages_note": "per-kernel device time from an instrumented pass of serial holo_process calls (each kernel alone on the GPU)",
+            "cpu_baseline": cpu, "eig_status": status, "eig_cycles": status_cycles, "configs": side, "library_context": lib_ctx,
             "paper_context": {"images_per_s": PAPER_IMAGES_PER_S, "input_frames_per_s": 500, "hardware": "NVIDIA Titan RTX (PAPER.md:96)"},
         }
         print(json.dumps(line))
-    h.close()
     if dist is not None:
         dist.destroy_process_group()
+
+
+def library_context(torch, R, barrier):
+    """Context only, never on the library path: the paper's own decomposition (cuFFT + cublasCgemm +
+    cusolverDnCheevd) written with torch library calls on the same B200 and the same resident stacks."""
+    cfg = R.cfg
+    T, n = cfg.T, cfg.n
+    try:
+        qx = R.h.workspace_tensor(6)
+        qy = R.h.workspace_tensor(7)
+        q = (qy[:, None] * qx[None, :]).contiguous()
+
+        def one(i):
+            fr = R.frames[(i % R.plan["n_stacks"]) * T:(i % R.plan["n_stacks"] + 1) * T].view(torch.int16).to(torch.float32)
+            d = fr - fr.mean(0, keepdim=True)
+            H = torch.fft.fft2(d * q)
+            Hm = H.reshape(T, -1)
+            C = Hm.conj() @ Hm.T
+            ev, V = torch.linalg.eigh(C)
+            P = (Hm.T @ V[:, :T - cfg.k_lo + 1])                  # ascending order: drop the k_lo-1 largest
+            return (P.real ** 2 + P.imag ** 2).sum(1).reshape(n, n)
+
+        for i in range(3):
+            one(i)
+        barrier()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        k = 16
+        e0.record()
+        for i in range(k):
+            one(i)
+        e1.record()
+        barrier()
+        ms = e0.elapsed_time(e1)
+        return {"images_per_s": k / (ms * 1e-3), "ms_per_step": ms / k,
+                "what": "torch.fft.fft2 + complex matmul + torch.linalg.eigh + matmul on the same GPU (the paper's library decomposition); context, not a target"}
+    except Exception as e:                                       # a missing library must not break the bench line
+        return {"unavailable": str(e)[:200]}
 
 
 def main():
@@ -366,12 +529,14 @@ def main():
     ap.add_argument("--warmup", type=int, default=None)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=3)
-    ap.add_argument("--stacks", type=int, default=None, help="resident stacks (default: the whole stream)")
+    ap.add_argument("--mode", type=int, default=1, choices=[1, 2], help="1: prescribed stage decomposition; 2: Gram from the raw frames (SURVEY.md 8(f)-2)")
+    ap.add_argument("--stacks", type=int, default=None, help="resident stacks (default: >= 3x L2)")
     ap.add_argument("--e2e-steps", type=int, default=24)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--no-side", dest="side", action="store_false", help="skip the short runs of the other configs")
     ap.add_argument("--api", default="submit", choices=["submit", "process", "push"],
-                    help="submit: streaming form (default); process: one serial holo_process per stack")
+                    help="submit: streaming form (default); process: one serial holo_process per stack; push: sliding window")
     ap.add_argument("--tune", action="append", default=[], help="experiment knob key=value (holo_tune), repeatable")
     args = ap.parse_args()
     from gen import holo_gen as G

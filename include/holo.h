@@ -23,12 +23,29 @@
  *     evals float [T], DESCENDING, k = 1 is the largest (R1: the paper sorts ascending and keeps
  *     n1..n2; (n1,n2) <-> (k_lo,k_hi) = (T+1-n2, T+1-n1));  image float [ny][nx] in FFT-bin order.
  *   - `stream` is a cudaStream_t cast to void* (NULL = legacy default stream).  Every call only
- *     ENQUEUES work on that stream: no allocation, no host synchronisation, no host<->device copy
- *     (except the *_host entry point, which says so).  Calls are CUDA-graph capturable.
- *   - Return value: HOLO_OK or a negative error code; nothing is launched on HOLO_ERR_ARG.
+ *     ENQUEUES work: no host synchronisation and no host<->device copy except in the *_host entry
+ *     points, holo_status, holo_profile_read and holo_tune(key 0), which say so.
+ *     Allocation: holo_create allocates the workspace of holo_process and of the per-stage calls.
+ *     The following calls allocate more at their FIRST use on a handle (cudaMalloc, which may
+ *     synchronise the device) and never afterwards: holo_submit (second hologram stack, second
+ *     C / V / evals / status slot, a side stream and six events), holo_push (FP64 Gram store, and in
+ *     its pipelined form a ring of T + max(8, T/2) hologram slots plus the side stream and events),
+ *     holo_submit_host / holo_process_host (device staging buffers, a copy stream), holo_tune key 5
+ *     (events).  Warm a handle up with one call of the form you use before timing or capturing.
+ *   - CUDA graphs: holo_process and the per-stage calls (holo_fresnel, holo_covariance, holo_eig,
+ *     holo_project, holo_fourier_demod, holo_normalize) enqueue on the caller's stream only and
+ *     can be captured (tests/test_gpu_parity.py captures and replays holo_process).  holo_submit /
+ *     holo_push fork work to the handle's side stream and join it only in a LATER call
+ *     (holo_flush, the submit after next): capture a whole submit...flush sequence, not one call.
+ *   - Device: a handle belongs to the device that was current at holo_create; every call checks
+ *     that this device is current and returns HOLO_ERR_STATE otherwise (kernel attributes,
+ *     streams and events are per device).
+ *   - Return value: HOLO_OK or a negative error code; nothing is launched on an error return.
  *     holo_last_error() gives a thread-local message.  Asynchronous CUDA faults surface at the
- *     next call or at destroy.  Jacobi non-convergence is recorded in a device status word
- *     readable with holo_status(); results are never silently NaN.
+ *     next call or at destroy.  Jacobi non-convergence (sweep cap hit) is recorded in the device
+ *     status word readable with holo_status() AND in a host-visible flag: the first compute
+ *     call issued after that solve has finished returns HOLO_ERR_NOCONV without launching
+ *     anything and clears the flag (holo_status clears it too).  Results are never silently NaN.
  *   - Arguments: nx, ny powers of two in [16, 4096]; 2 <= T <= 64; lambda, pitch, z finite > 0;
  *     1 <= k_lo <= k_hi <= T (1-based, inclusive, descending eigenvalue order).
  *   - One in-flight call per handle per stream order: calls on one handle must be issued on the
@@ -146,7 +163,9 @@ int holo_project(holo_ctx* ctx, const void* H_dev, const void* V_dev, float* ima
  * w_mn = exp(-2 i pi (m-1)(n-1)/T)/sqrt(T), n1..n2 1-based inclusive (paper: 8..24 of 32). */
 int holo_fourier_demod(holo_ctx* ctx, const void* H_dev, int n1, int n2, float* image_dev, holo_stream stream);
 
-/* Change the component window (1-based inclusive, descending order).  Takes effect at the next call. */
+/* Change the component window (1-based inclusive, descending order).  Takes effect at the next call; an image still
+ * owed by an earlier holo_submit keeps the window of its own submit call.  While a holo_push sequence is open the
+ * new window must keep the deflation form available (HOLO_ERR_STATE otherwise). */
 int holo_set_range(holo_ctx* ctx, int k_lo, int k_hi);
 
 /* Allow holo_process/holo_project to use the exact identity sum_{k in S}|P_k|^2 =
@@ -162,7 +181,9 @@ const void* holo_workspace(holo_ctx* ctx, int which);
  * into dst_dev (caller-owned device memory). */
 int holo_workspace_copy(holo_ctx* ctx, int which, void* dst_dev, unsigned long long nbytes, holo_stream stream);
 
-/* Copies the 4-int status word of the last holo_eig/holo_process to the host (synchronises `stream`).
+/* Copies the first 4 ints of the 8-int status word (HOLO_WS_STATUS: no-convergence flag, sweeps used, rotations
+ * in the last sweep, 0) of the last eigensolve to the host.  Synchronises `stream` and the handle's side stream.
+ * After holo_submit / holo_push sequences both workspace slots are inspected and a failing one is reported.
  * Returns HOLO_ERR_NOCONV if the Jacobi sweep cap was hit, else HOLO_OK. */
 int holo_status(holo_ctx* ctx, int32_t status_host[4], holo_stream stream);
 
@@ -179,6 +200,15 @@ int holo_launches_per_process(holo_ctx* ctx);
  *   side-stream projection in holo_submit (0 = projection in stream order after the next Fresnel stage),
  *   10 pipelined ring form of holo_push (default 1), 11 incremental Gram update in that form (default 1). */
 int holo_tune(holo_ctx* ctx, int key, int value);
+
+/* Measurement hooks used by bench.py (not needed for normal use).
+ * holo_profile_read: while holo_tune(ctx, 5, 1) is on, every kernel launch is bracketed by a pair of CUDA events;
+ * this call synchronises the device and returns, per kernel class (0 temporal sum, 1 Fresnel / row pass, 2 column
+ * pass of the unfused form, 3 covariance partials, 4 covariance reduction, 5 eigensolver, 6 projection), the summed
+ * device time in ms_out[7] and the launch count in count_out[7] since the last read.
+ * holo_fft_group: frames in the row->column ring of the Fresnel stage (tune key 0). */
+int holo_profile_read(holo_ctx* ctx, double* ms_out, int* count_out);
+int holo_fft_group(holo_ctx* ctx);
 
 const char* holo_last_error(void);   /* thread-local, static storage */
 int holo_version(void);              /* major*10000 + minor*100 + patch */

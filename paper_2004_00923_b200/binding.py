@@ -11,7 +11,8 @@ HOLO_WS_SUM, HOLO_WS_H, HOLO_WS_C, HOLO_WS_EVALS, HOLO_WS_V, HOLO_WS_STATUS, HOL
 EXPORTED_SYMBOLS = [
     "holo_create", "holo_destroy", "holo_process", "holo_submit", "holo_flush", "holo_submit_host", "holo_flush_host", "holo_push", "holo_process_host", "holo_fresnel", "holo_covariance",
     "holo_eig", "holo_project", "holo_fourier_demod", "holo_set_range", "holo_set_assume_unitary",
-    "holo_workspace", "holo_workspace_copy", "holo_status", "holo_launches_per_process", "holo_tune", "holo_last_error", "holo_version",
+    "holo_workspace", "holo_workspace_copy", "holo_status", "holo_launches_per_process", "holo_tune", "holo_profile_read", "holo_fft_group",
+    "holo_last_error", "holo_version",
 ]
 
 

@@ -38,7 +38,8 @@ def build(force=False, verbose=False):
     if failed:
         raise RuntimeError("nvcc failed")
     if procs or not os.path.exists(LIB):
-        subprocess.check_call([NVCC, "-shared", "-o", LIB] + objs + ["-cudart", "static"])
+        subprocess.check_call([NVCC, "-gencode", "arch=compute_100a,code=sm_100a", "-Wno-deprecated-gpu-targets",
+                               "-shared", "-o", LIB] + objs + ["-cudart", "static"])
     ub_src, ub_bin = os.path.join(CSRC, "ubench_peaks.cu"), os.path.join(HERE, "ubench_peaks")
     if force or not os.path.exists(ub_bin) or os.path.getmtime(ub_bin) < os.path.getmtime(ub_src):
         subprocess.check_call([NVCC, "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-Wno-deprecated-gpu-targets",

@@ -47,31 +47,13 @@ __device__ __forceinline__ float warp_sum(float x) {
     return x;
 }
 
-#ifndef COV_SCALAR
-#define COV_SCALAR 1
-#endif
-#if COV_SCALAR
+// An accumulator is the pair (re, im).  (The packed fma.rn.f32x2 form of these updates was measured 16 % slower here:
+// the operand-pair moves land on the FMA pipe.)
 typedef float2 pair_t;
 __device__ __forceinline__ pair_t pack2(float lo, float hi) { return make_float2(lo, hi); }
 __device__ __forceinline__ void unpack2(pair_t v, float& lo, float& hi) { lo = v.x; hi = v.y; }
 __device__ __forceinline__ void ffma2(pair_t& acc, pair_t a, pair_t b) { acc.x = fmaf(a.x, b.x, acc.x); acc.y = fmaf(a.y, b.y, acc.y); }
 __device__ __forceinline__ pair_t pzero() { return make_float2(0.f, 0.f); }
-#else
-typedef unsigned long long pair_t;
-__device__ __forceinline__ pair_t pzero() { return 0ull; }
-__device__ __forceinline__ unsigned long long pack2(float lo, float hi) {
-    unsigned long long r;
-    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
-    return r;
-}
-__device__ __forceinline__ void unpack2(unsigned long long v, float& lo, float& hi) {
-    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
-}
-// acc = a * b + acc on both FP32 halves (IEEE round-to-nearest each)
-__device__ __forceinline__ void ffma2(unsigned long long& acc, unsigned long long a, unsigned long long b) {
-    asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(acc) : "l"(a), "l"(b));
-}
-#endif
 
 // partials layout: [part][T8][T8] float2 (T8 = T rounded up to 8), only entries s <= t are written
 __global__ void __launch_bounds__(COV_NW * 32, 1)
@@ -111,8 +93,7 @@ k_cov_partial(const __grid_constant__ CUtensorMap tmH, float2* __restrict__ part
     // ---------------------------------------------------- consumer warps
     // One pixel per lane per trip: 16 LDS.64 + 256 FFMA, a 4.5 KB loop body.  An accumulator is the pair
     // (re, im);  acc += conj(a) b  =  (ax,ax)*(bx,by) + (ay,-ay)*(by,bx)  (pair_t / ffma2 below).
-    // Measured alternatives (profiles/r01c.md): two pixels per trip with LDS.128 (same speed, twice the code),
-    // the packed fma.rn.f32x2 form (COV_SCALAR 0: 16 % slower -- the operand-pair moves land on the FMA pipe).
+    // Measured alternative (profiles/r01c.md): two pixels per trip with LDS.128 (same speed, twice the code).
     const CovJob job = g.job[warp];      // make_plan orders the jobs so that one SM sub-partition (warp & 3) runs one kind
     if (job.kind == 0) return;
     float2* out = partials + (size_t)blockIdx.x * T8 * T8;
@@ -507,11 +488,7 @@ static int launch_cov_real(holo_ctx* c, const float2* H, float2* C, cudaStream_t
     nstages -= nstages % ngroups;                          // a stage always serves the same warp group
     const int ahead = nstages > 3 ? nstages - 2 : nstages - 1;
     const size_t smem = 128 + (size_t)nstages * stage_bytes;
-    static bool attr = false;
-    if (!attr) {
-        HOLO_CUDA_OK(cudaFuncSetAttribute(k_cov_partial_real, cudaFuncAttributeMaxDynamicSharedMemorySize, COV_SMEM_BUDGET + 128));
-        attr = true;
-    }
+    { const int rc = holo_ensure_smem_attr((const void*)k_cov_partial_real, c->device, COV_SMEM_BUDGET + 128); if (rc) return rc; }
     const long long nchunks = c->npix / COV_P;
     int gx = (c->cov_grid_cap > 0 ? c->cov_grid_cap : c->tune[HOLO_TUNE_COV_GRIDX]) / gy;   // all CTAs co-resident: one per SM
     if (gx < 1) gx = 1;
@@ -521,7 +498,7 @@ static int launch_cov_real(holo_ctx* c, const float2* H, float2* C, cudaStream_t
     { const int rc = holo_make_tensor_map(&tmH, H, c->npix, c->ring_nrb ? 8 * c->ring_nrb : T, COV_P); if (rc) return rc; }
     {
         HoloProf prof(c, HOLO_K_COV_PARTIAL, st);
-        k_cov_partial_real<<<dim3(gx, gy), COV_NW * 32, smem, st>>>(tmH, holo_cov_partials(c, c->cov_sel), c->npix, T8, nstages, nslots, ngroups, ahead, plan, c->ring_rb0, c->ring_nrb);
+        k_cov_partial_real<<<dim3(gx, gy), COV_NW * 32, smem, st>>>(tmH, c->cov_partials, c->npix, T8, nstages, nslots, ngroups, ahead, plan, c->ring_rb0, c->ring_nrb);
     }
     HOLO_CUDA_OK(cudaGetLastError());
     c->cov_nparts = gx * ngroups;
@@ -529,19 +506,19 @@ static int launch_cov_real(holo_ctx* c, const float2* H, float2* C, cudaStream_t
         // new rows / columns -> slot-indexed FP64 store, then gather + centre the window
         const int Rn = 8 * c->ring_nrb, a0 = 8 * c->ring_rb0;
         HoloProf prof(c, HOLO_K_COV_REDUCE, st);
-        k_cov_reduce_new<<<dim3(T, newb), 256, 0, st>>>(holo_cov_partials(c, c->cov_sel), c->cov_nparts, T, T8, newb, c->Gs, Rn, a0);
+        k_cov_reduce_new<<<dim3(T, newb), 256, 0, st>>>(c->cov_partials, c->cov_nparts, T, T8, newb, c->Gs, Rn, a0);
         HOLO_CUDA_OK(cudaGetLastError());
         k_center_gram<<<1, 256, 0, st>>>(nullptr, T, C, c->Gs, Rn, a0, 0);
         HOLO_CUDA_OK(cudaGetLastError());
         return HOLO_OK;
     }
-    return C ? holo_launch_cov_reduce(c, c->cov_sel, c->cov_nparts, C, st) : HOLO_OK;
+    return C ? holo_launch_cov_reduce(c, c->cov_nparts, C, st) : HOLO_OK;
 }
 
-int holo_launch_cov_reduce(holo_ctx* c, int sel, int nparts, float2* C, cudaStream_t st) {
+int holo_launch_cov_reduce(holo_ctx* c, int nparts, float2* C, cudaStream_t st) {
     const int T = c->T, T8 = (T + 7) / 8 * 8, n = T * T;
     HoloProf prof(c, HOLO_K_COV_REDUCE, st);
-    k_cov_reduce<<<(n * 32 + 255) / 256, 256, 0, st>>>(holo_cov_partials(c, sel), nparts, T, T8, C, c->center_gram ? c->Cd : nullptr);
+    k_cov_reduce<<<(n * 32 + 255) / 256, 256, 0, st>>>(c->cov_partials, nparts, T, T8, C, c->center_gram ? c->Cd : nullptr);
     HOLO_CUDA_OK(cudaGetLastError());
     if (c->center_gram) {                                  // holo_push: C <- J Gamma J
         k_center_gram<<<1, 256, 0, st>>>(c->Cd, T, C, c->ring_nrb ? c->Gs : nullptr, 8 * c->ring_nrb, 8 * c->ring_rb0, 1);
@@ -564,11 +541,7 @@ int holo_launch_covariance(holo_ctx* c, const float2* H, float2* C, cudaStream_t
     if (nstages > COV_MAX_STAGES) nstages = COV_MAX_STAGES;
     if (nstages < 3) { holo_set_error("covariance stage ring does not fit"); return HOLO_ERR_STATE; }
     const size_t smem = 128 + (size_t)nstages * stage_bytes;
-    static bool attr = false;
-    if (!attr) {
-        HOLO_CUDA_OK(cudaFuncSetAttribute(k_cov_partial, cudaFuncAttributeMaxDynamicSharedMemorySize, COV_SMEM_BUDGET + 128));
-        attr = true;
-    }
+    { const int rc = holo_ensure_smem_attr((const void*)k_cov_partial, c->device, COV_SMEM_BUDGET + 128); if (rc) return rc; }
     const long long nchunks = c->npix / COV_P;
     int gx = c->tune[HOLO_TUNE_COV_GRIDX] / plan.ngroups;          // all CTAs co-resident: one per SM
     if (gx < 1) gx = 1;
@@ -578,9 +551,9 @@ int holo_launch_covariance(holo_ctx* c, const float2* H, float2* C, cudaStream_t
     { const int rc = holo_make_tensor_map(&tmH, H, c->npix, T, COV_P); if (rc) return rc; }
     {
         HoloProf prof(c, HOLO_K_COV_PARTIAL, st);
-        k_cov_partial<<<dim3(gx, plan.ngroups), COV_NW * 32, smem, st>>>(tmH, holo_cov_partials(c, c->cov_sel), c->npix, T, T8, nstages, plan);
+        k_cov_partial<<<dim3(gx, plan.ngroups), COV_NW * 32, smem, st>>>(tmH, c->cov_partials, c->npix, T, T8, nstages, plan);
     }
     HOLO_CUDA_OK(cudaGetLastError());
     c->cov_nparts = gx;
-    return C ? holo_launch_cov_reduce(c, c->cov_sel, c->cov_nparts, C, st) : HOLO_OK;
+    return C ? holo_launch_cov_reduce(c, c->cov_nparts, C, st) : HOLO_OK;
 }

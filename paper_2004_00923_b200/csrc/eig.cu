@@ -62,7 +62,7 @@ __host__ __device__ constexpr int rr_next(int pos, int Tp) {
 template <int TP>
 __global__ void __launch_bounds__((TP / 2) * (TP / 2) < 32 ? 32 : (TP / 2) * (TP / 2), 1)
 k_eig(const float2* __restrict__ C, int T, float* __restrict__ evals, float2* __restrict__ Vout,
-      int32_t* __restrict__ status, int max_sweeps) {
+      int32_t* __restrict__ status, int max_sweeps, int32_t* __restrict__ noconv) {
     extern __shared__ __align__(16) unsigned char raw[];
     constexpr int Tp = TP, LD = TP + 2, half = TP / 2, m = TP - 1;   // LD even: rows 16-byte aligned for LDS.128
     float2* A0 = reinterpret_cast<float2*>(raw);
@@ -253,6 +253,8 @@ k_eig(const float2* __restrict__ C, int T, float* __restrict__ evals, float2* __
         status[5] = (int)(clk2 - clk1);          // cycles: Jacobi sweeps
         status[6] = (int)(clock64() - clk2);     // cycles: Rayleigh refinement, sort, phase fix
         status[7] = 0;
+        // sticky host-visible flag (mapped pinned word): the next API call on the handle returns HOLO_ERR_NOCONV
+        if (!converged && noconv) { *(volatile int32_t*)noconv = 1; __threadfence_system(); }
     }
 }
 
@@ -263,14 +265,10 @@ static int launch_eig_t(holo_ctx* c, const float2* C, float* evals, float2* V, c
     // A0, A1, V0, V1 [TP][LD] + Cs [TP][TP] float2, red[32] float, lam[TP] double
     constexpr size_t smem = (size_t)4 * TP * LD * sizeof(float2) + (size_t)TP * TP * sizeof(float2) + 32 * sizeof(float)
                           + TP * sizeof(double);
-    static bool attr = false;
-    if (!attr) {
-        HOLO_CUDA_OK(cudaFuncSetAttribute(k_eig<TP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        attr = true;
-    }
+    { const int rc = holo_ensure_smem_attr((const void*)k_eig<TP>, c->device, smem); if (rc) return rc; }
     constexpr int threads = (TP / 2) * (TP / 2) < 32 ? 32 : (TP / 2) * (TP / 2);
     HoloProf prof(c, HOLO_K_EIG, st);
-    k_eig<TP><<<1, threads, smem, st>>>(C, T, evals, V, c->status, c->tune[HOLO_TUNE_EIG_MAX_SWEEPS]);
+    k_eig<TP><<<1, threads, smem, st>>>(C, T, evals, V, c->status, c->tune[HOLO_TUNE_EIG_MAX_SWEEPS], c->noconv_dev);
     HOLO_CUDA_OK(cudaGetLastError());
     return HOLO_OK;
 }

@@ -155,7 +155,6 @@ struct FftArgs {
     int tiles_per_frame;      // nseq / B
     int ntiles;               // nf * tiles_per_frame
     int T;
-    float invT;
 };
 
 // one tile = B sequences of one frame; in_foff / out_foff = element offset of the frame in a.in(frames) / a.out
@@ -443,18 +442,12 @@ void holo_fft_plan_free(FftPlan* p) {
 }
 
 template <int N, int E, int R1, int R2, int B, bool COL, bool PRO>
-static int launch_fft_t(const FftArgs& a, int num_sms, cudaStream_t st) {
+static int launch_fft_t(const FftArgs& a, int num_sms, int device, cudaStream_t st) {
     constexpr int threads = (N / E) * B;
     constexpr size_t smem = (R1 > 1) ? sizeof(float2) * (size_t)(N + N / E) * B : 0;
     auto kern = k_fft<N, E, R1, R2, B, COL, PRO>;
-    static int blocks_per_sm = 0;      // per instantiation
-    if (blocks_per_sm == 0) {
-        if (smem > 48 * 1024) HOLO_CUDA_OK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        int occ = 0;
-        HOLO_CUDA_OK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, threads, smem));
-        if (occ < 1) { holo_set_error("fft kernel N=%d does not fit on an SM", N); return HOLO_ERR_CUDA; }
-        blocks_per_sm = occ;
-    }
+    int blocks_per_sm = 0;
+    { const int rc = holo_cached_occupancy((const void*)kern, device, threads, smem, &blocks_per_sm); if (rc) return rc; }
     int grid = a.ntiles < num_sms * blocks_per_sm ? a.ntiles : num_sms * blocks_per_sm;
     kern<<<grid, threads, smem, st>>>(a);
     HOLO_CUDA_OK(cudaGetLastError());
@@ -463,17 +456,17 @@ static int launch_fft_t(const FftArgs& a, int num_sms, cudaStream_t st) {
 
 // B (sequences per CTA) per length: rows aim at 256 threads; columns at >= 64-byte segments
 template <bool COL, bool PRO>
-static int launch_fft(int N, const FftArgs& a, int num_sms, cudaStream_t st) {
+static int launch_fft(int N, const FftArgs& a, int num_sms, int device, cudaStream_t st) {
     switch (N) {
-        case 16:   return launch_fft_t<16, 16, 1, 1, 16, COL, PRO>(a, num_sms, st);
-        case 32:   return launch_fft_t<32, 32, 1, 1, 16, COL, PRO>(a, num_sms, st);
-        case 64:   return launch_fft_t<64, 16, 4, 1, 16, COL, PRO>(a, num_sms, st);
-        case 128:  return launch_fft_t<128, 16, 8, 1, 16, COL, PRO>(a, num_sms, st);
-        case 256:  return launch_fft_t<256, 16, 16, 1, 16, COL, PRO>(a, num_sms, st);
-        case 512:  return launch_fft_t<512, 32, 16, 1, 16, COL, PRO>(a, num_sms, st);
-        case 1024: return launch_fft_t<1024, 32, 32, 1, 8, COL, PRO>(a, num_sms, st);
-        case 2048: return launch_fft_t<2048, 32, 32, 2, 4, COL, PRO>(a, num_sms, st);
-        case 4096: return launch_fft_t<4096, 16, 16, 16, 4, COL, PRO>(a, num_sms, st);
+        case 16:   return launch_fft_t<16, 16, 1, 1, 16, COL, PRO>(a, num_sms, device, st);
+        case 32:   return launch_fft_t<32, 32, 1, 1, 16, COL, PRO>(a, num_sms, device, st);
+        case 64:   return launch_fft_t<64, 16, 4, 1, 16, COL, PRO>(a, num_sms, device, st);
+        case 128:  return launch_fft_t<128, 16, 8, 1, 16, COL, PRO>(a, num_sms, device, st);
+        case 256:  return launch_fft_t<256, 16, 16, 1, 16, COL, PRO>(a, num_sms, device, st);
+        case 512:  return launch_fft_t<512, 32, 16, 1, 16, COL, PRO>(a, num_sms, device, st);
+        case 1024: return launch_fft_t<1024, 32, 32, 1, 8, COL, PRO>(a, num_sms, device, st);
+        case 2048: return launch_fft_t<2048, 32, 32, 2, 4, COL, PRO>(a, num_sms, device, st);
+        case 4096: return launch_fft_t<4096, 16, 16, 16, 4, COL, PRO>(a, num_sms, device, st);
     }
     holo_set_error("unsupported FFT length %d", N);
     return HOLO_ERR_ARG;
@@ -487,18 +480,12 @@ static int launch_fft(int N, const FftArgs& a, int num_sms, cudaStream_t st) {
 static int fft_batch(int N) { return N <= 512 ? 16 : N == 1024 ? 8 : 4; }
 
 template <int N, int E, int R1, int R2, int B>
-static int launch_fresnel_t(const FresnelArgs& p, int num_sms, cudaStream_t st) {
+static int launch_fresnel_t(const FresnelArgs& p, int num_sms, int device, cudaStream_t st) {
     constexpr int threads = (N / E) * B;
     constexpr size_t smem = (R1 > 1) ? sizeof(float2) * (size_t)(N + N / E) * B : 0;
     auto kern = k_fresnel<N, E, R1, R2, B>;
-    static int blocks_per_sm = 0;
-    if (blocks_per_sm == 0) {
-        if (smem > 48 * 1024) HOLO_CUDA_OK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        int occ = 0;
-        HOLO_CUDA_OK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, threads, smem));
-        if (occ < 1) { holo_set_error("fused fresnel kernel N=%d does not fit on an SM", N); return HOLO_ERR_CUDA; }
-        blocks_per_sm = occ;
-    }
+    int blocks_per_sm = 0;
+    { const int rc = holo_cached_occupancy((const void*)kern, device, threads, smem, &blocks_per_sm); if (rc) return rc; }
     const long long total = (long long)p.T * (p.RT + p.CT);
     long long grid = (long long)num_sms * blocks_per_sm;      // one wave of persistent CTAs
     if (grid > total) grid = total;
@@ -507,17 +494,17 @@ static int launch_fresnel_t(const FresnelArgs& p, int num_sms, cudaStream_t st) 
     return HOLO_OK;
 }
 
-static int launch_fresnel_fused(int N, const FresnelArgs& p, int num_sms, cudaStream_t st) {
+static int launch_fresnel_fused(int N, const FresnelArgs& p, int num_sms, int device, cudaStream_t st) {
     switch (N) {
-        case 16:   return launch_fresnel_t<16, 16, 1, 1, 16>(p, num_sms, st);
-        case 32:   return launch_fresnel_t<32, 32, 1, 1, 16>(p, num_sms, st);
-        case 64:   return launch_fresnel_t<64, 16, 4, 1, 16>(p, num_sms, st);
-        case 128:  return launch_fresnel_t<128, 16, 8, 1, 16>(p, num_sms, st);
-        case 256:  return launch_fresnel_t<256, 16, 16, 1, 16>(p, num_sms, st);
-        case 512:  return launch_fresnel_t<512, 32, 16, 1, 16>(p, num_sms, st);
-        case 1024: return launch_fresnel_t<1024, 32, 32, 1, FUSED_B1024>(p, num_sms, st);
-        case 2048: return launch_fresnel_t<2048, 32, 32, 2, FUSED_B2048>(p, num_sms, st);
-        case 4096: return launch_fresnel_t<4096, 16, 16, 16, 4>(p, num_sms, st);
+        case 16:   return launch_fresnel_t<16, 16, 1, 1, 16>(p, num_sms, device, st);
+        case 32:   return launch_fresnel_t<32, 32, 1, 1, 16>(p, num_sms, device, st);
+        case 64:   return launch_fresnel_t<64, 16, 4, 1, 16>(p, num_sms, device, st);
+        case 128:  return launch_fresnel_t<128, 16, 8, 1, 16>(p, num_sms, device, st);
+        case 256:  return launch_fresnel_t<256, 16, 16, 1, 16>(p, num_sms, device, st);
+        case 512:  return launch_fresnel_t<512, 32, 16, 1, 16>(p, num_sms, device, st);
+        case 1024: return launch_fresnel_t<1024, 32, 32, 1, FUSED_B1024>(p, num_sms, device, st);
+        case 2048: return launch_fresnel_t<2048, 32, 32, 2, FUSED_B2048>(p, num_sms, device, st);
+        case 4096: return launch_fresnel_t<4096, 16, 16, 16, 4>(p, num_sms, device, st);
     }
     holo_set_error("unsupported FFT length %d", N);
     return HOLO_ERR_ARG;
@@ -557,9 +544,9 @@ int holo_launch_fresnel(holo_ctx* c, const uint16_t* frames, float2* H, cudaStre
         const int Bq = c->nx == 1024 ? FUSED_B1024 : c->nx == 2048 ? FUSED_B2048 : fft_batch(c->nx);
         FftArgs& a = p.rows;
         a.frames = frames; a.sum = c->sum; a.qx = c->qxs; a.qy = c->qy; a.in = nullptr; a.out = c->scratch;
-        a.tw1 = c->px.tw1; a.tw2 = c->px.tw2; a.ld = c->nx; a.nseq = c->ny; a.T = c->T; a.invT = 1.0f / (float)c->T;
+        a.tw1 = c->px.tw1; a.tw2 = c->px.tw2; a.ld = c->nx; a.nseq = c->ny; a.T = c->T;
         FftArgs& b = p.cols;
-        b.in = c->scratch; b.out = H; b.tw1 = c->py.tw1; b.tw2 = c->py.tw2; b.ld = c->nx; b.nseq = c->nx; b.T = c->T; b.invT = a.invT;
+        b.in = c->scratch; b.out = H; b.tw1 = c->py.tw1; b.tw2 = c->py.tw2; b.ld = c->nx; b.nseq = c->nx; b.T = c->T;
         p.counters = c->counters; p.npix = c->npix; p.T = nproc; p.R = c->scratch_frames;
         p.L = c->tune[HOLO_TUNE_FFT_LAG] > 0 ? c->tune[HOLO_TUNE_FFT_LAG] : p.R / 2;
         if (p.L > p.R - 1) p.L = p.R - 1;
@@ -567,7 +554,7 @@ int holo_launch_fresnel(holo_ctx* c, const uint16_t* frames, float2* H, cudaStre
         if (p.L < 1) p.L = 1;
         p.RT = c->ny / Bq; p.CT = c->nx / Bq;
         HoloProf prof(c, HOLO_K_FFT_ROWS, st);
-        return launch_fresnel_fused(c->nx, p, c->num_sms, st);
+        return launch_fresnel_fused(c->nx, p, c->num_sms, c->device, st);
     }
     // A1 + A2, frame groups so that the row->column intermediate stays in L2
     const int G = c->scratch_frames;
@@ -582,9 +569,9 @@ int holo_launch_fresnel(holo_ctx* c, const uint16_t* frames, float2* H, cudaStre
         a.ld = c->nx; a.nseq = c->ny;
         a.tiles_per_frame = c->ny / fft_batch(c->nx);
         a.ntiles = nf * a.tiles_per_frame;
-        a.T = c->T; a.invT = 1.0f / (float)c->T;
+        a.T = c->T;
         int rc;
-        { HoloProf prof(c, HOLO_K_FFT_ROWS, st); rc = launch_fft<false, true>(c->nx, a, c->num_sms, st); }
+        { HoloProf prof(c, HOLO_K_FFT_ROWS, st); rc = launch_fft<false, true>(c->nx, a, c->num_sms, c->device, st); }
         if (rc) return rc;
         FftArgs b{};
         b.in = c->scratch; b.out = H + (long long)f0 * c->npix;
@@ -593,8 +580,8 @@ int holo_launch_fresnel(holo_ctx* c, const uint16_t* frames, float2* H, cudaStre
         b.ld = c->nx; b.nseq = c->nx;
         b.tiles_per_frame = c->nx / fft_batch(c->ny);
         b.ntiles = nf * b.tiles_per_frame;
-        b.T = c->T; b.invT = a.invT;
-        { HoloProf prof(c, HOLO_K_FFT_COLS, st); rc = launch_fft<true, false>(c->ny, b, c->num_sms, st); }
+        b.T = c->T;
+        { HoloProf prof(c, HOLO_K_FFT_COLS, st); rc = launch_fft<true, false>(c->ny, b, c->num_sms, c->device, st); }
         if (rc) return rc;
     }
     return HOLO_OK;

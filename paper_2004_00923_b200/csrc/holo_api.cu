@@ -4,6 +4,7 @@
 #include <math.h>
 #include <stdarg.h>
 #include <string.h>
+#include <mutex>
 #include <new>
 #include <vector>
 
@@ -20,6 +21,39 @@ extern "C" const char* holo_last_error(void) { return g_err; }
 extern "C" int holo_version(void) { return 100; }   // 0.1.0
 
 static bool is_pow2(int n) { return n > 0 && (n & (n - 1)) == 0; }
+
+// ---- per-(function, device) caches: the opt-in to > 48 KB dynamic shared memory and the occupancy of a kernel are
+// properties of the pair, not of the process (a second handle on another GPU must set them again)
+namespace {
+struct FuncDevEntry { const void* func; int device; size_t smem; int threads; int occ; };
+std::mutex g_fd_mutex;
+std::vector<FuncDevEntry> g_fd_attr, g_fd_occ;
+}
+
+int holo_ensure_smem_attr(const void* func, int device, size_t bytes) {
+    std::lock_guard<std::mutex> lock(g_fd_mutex);
+    for (const FuncDevEntry& e : g_fd_attr)
+        if (e.func == func && e.device == device && e.smem >= bytes) return HOLO_OK;
+    if (bytes > 48 * 1024) HOLO_CUDA_OK(cudaFuncSetAttribute(func, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
+    g_fd_attr.push_back(FuncDevEntry{func, device, bytes, 0, 0});
+    return HOLO_OK;
+}
+
+int holo_cached_occupancy(const void* func, int device, int threads, size_t smem, int* blocks_per_sm) {
+    {
+        std::lock_guard<std::mutex> lock(g_fd_mutex);
+        for (const FuncDevEntry& e : g_fd_occ)
+            if (e.func == func && e.device == device && e.smem == smem && e.threads == threads) { *blocks_per_sm = e.occ; return HOLO_OK; }
+    }
+    { const int rc = holo_ensure_smem_attr(func, device, smem); if (rc) return rc; }
+    int occ = 0;
+    HOLO_CUDA_OK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, func, threads, smem));
+    if (occ < 1) { holo_set_error("kernel does not fit on an SM (%d threads, %zu bytes of shared memory)", threads, smem); return HOLO_ERR_CUDA; }
+    std::lock_guard<std::mutex> lock(g_fd_mutex);
+    g_fd_occ.push_back(FuncDevEntry{func, device, smem, threads, occ});
+    *blocks_per_sm = occ;
+    return HOLO_OK;
+}
 
 static int build_chirp(float2** dst, int n, double lambda_m, double pitch_m, double z_m, double scale) {
     // q_x[i] = exp(+i pi x_i^2/(lambda z)), x_i = (i - n/2) pitch; evaluated in double with the phase
@@ -42,7 +76,8 @@ static void free_ctx(holo_ctx* c) {
     cudaFree(c->qx); cudaFree(c->qy); cudaFree(c->qxs); cudaFree(c->Wdft);
     holo_fft_plan_free(&c->px); holo_fft_plan_free(&c->py);
     cudaFree(c->sum); cudaFree(c->scratch); cudaFree(c->H); cudaFree(c->cov_partials);
-    cudaFree(c->C); cudaFree(c->evals); cudaFree(c->V); cudaFree(c->Vsel); cudaFree(c->status);
+    cudaFree(c->C); cudaFree(c->evals); cudaFree(c->V); cudaFree(c->status);
+    if (c->noconv_host) cudaFreeHost(c->noconv_host);
     cudaFree(c->counters);
     if (c->prof_ev) {
         for (int i = 0; i < 2 * HOLO_PROF_CAP; ++i) cudaEventDestroy(c->prof_ev[i]);
@@ -109,18 +144,20 @@ static int create_impl(holo_ctx* c) {
     c->cov_parts_cap = 4 * c->num_sms;
     const int T8 = (T + 7) / 8 * 8;
     HOLO_CUDA_OK(cudaMalloc(&c->sum, np * sizeof(uint32_t)));
-    HOLO_CUDA_OK(cudaMalloc(&c->scratch, (size_t)T * np * 0 + (size_t)c->scratch_frames * np * sizeof(float2)));
+    HOLO_CUDA_OK(cudaMalloc(&c->scratch, (size_t)c->scratch_frames * np * sizeof(float2)));
     HOLO_CUDA_OK(cudaMalloc(&c->H, (size_t)T * np * sizeof(float2)));
-    HOLO_CUDA_OK(cudaMalloc(&c->cov_partials, (size_t)2 * c->cov_parts_cap * T8 * T8 * sizeof(float2)));
+    HOLO_CUDA_OK(cudaMalloc(&c->cov_partials, (size_t)c->cov_parts_cap * T8 * T8 * sizeof(float2)));
     HOLO_CUDA_OK(cudaMalloc(&c->C, (size_t)T * T * sizeof(float2)));
     HOLO_CUDA_OK(cudaMalloc(&c->evals, T * sizeof(float)));
     HOLO_CUDA_OK(cudaMalloc(&c->V, (size_t)T * T * sizeof(float2)));
-    HOLO_CUDA_OK(cudaMalloc(&c->Vsel, (size_t)T * HOLO_MAX_T * sizeof(float2)));
     HOLO_CUDA_OK(cudaMalloc(&c->status, 8 * sizeof(int32_t)));
     HOLO_CUDA_OK(cudaMalloc(&c->counters, 1024 * sizeof(unsigned int)));
     HOLO_CUDA_OK(cudaMemset(c->status, 0, 8 * sizeof(int32_t)));
     HOLO_CUDA_OK(cudaMemset(c->counters, 0, 1024 * sizeof(unsigned int)));
-    HOLO_CUDA_OK(cudaMemset(c->cov_partials, 0, (size_t)2 * c->cov_parts_cap * T8 * T8 * sizeof(float2)));
+    HOLO_CUDA_OK(cudaMemset(c->cov_partials, 0, (size_t)c->cov_parts_cap * T8 * T8 * sizeof(float2)));
+    HOLO_CUDA_OK(cudaHostAlloc(&c->noconv_host, sizeof(int32_t), cudaHostAllocMapped));
+    *c->noconv_host = 0;
+    HOLO_CUDA_OK(cudaHostGetDevicePointer((void**)&c->noconv_dev, c->noconv_host, 0));
     HOLO_CUDA_OK(cudaDeviceSynchronize());
     return HOLO_OK;
 }
@@ -153,7 +190,25 @@ extern "C" void holo_destroy(holo_ctx* c) {
     free_ctx(c);
 }
 
-#define CHECK_CTX(c) do { if (!(c)) { holo_set_error("NULL handle"); return HOLO_ERR_ARG; } } while (0)
+// Every entry point: the handle's device must be current (its streams, events and per-device kernel attributes belong
+// to it), and a Jacobi solve of an EARLIER call that hit the sweep cap is reported once, before anything is enqueued
+// (the eigensolver sets a mapped host word; no synchronisation here -- SURVEY.md 8(b)).
+static int enter(holo_ctx* c, bool report_noconv = true) {
+    if (!c) { holo_set_error("NULL handle"); return HOLO_ERR_ARG; }
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev != c->device) {
+        holo_set_error("the handle was created on device %d but device %d is current", c->device, dev);
+        return HOLO_ERR_STATE;
+    }
+    if (report_noconv && c->noconv_host && *(volatile int32_t*)c->noconv_host) {
+        *(volatile int32_t*)c->noconv_host = 0;
+        holo_set_error("the Jacobi eigensolver of an earlier call hit the sweep cap (see holo_status)");
+        return HOLO_ERR_NOCONV;
+    }
+    return HOLO_OK;
+}
+#define CHECK_CTX(c) do { const int _rc = enter(c); if (_rc) return _rc; } while (0)
+#define CHECK_CTX_QUIET(c) do { const int _rc = enter(c, false); if (_rc) return _rc; } while (0)
 #define CHECK_PTR(p, name) do { if (!(p)) { holo_set_error("NULL pointer: %s", name); return HOLO_ERR_ARG; } } while (0)
 
 extern "C" int holo_fresnel(holo_ctx* c, const uint16_t* frames_dev, void* H_dev, holo_stream stream) {
@@ -209,10 +264,10 @@ extern "C" int holo_process(holo_ctx* c, const uint16_t* frames_dev, float* imag
 // submit(i) enqueues on `stream`:  A0+A1+A2 of stack i  ->  [join eig(i-1)] A5+A6 of stack i-1  ->  A3 of
 // stack i  ->  fork: A4 of stack i on the handle's side stream.  The single-CTA eigensolver of stack i thus
 // runs under the Fresnel kernels of stack i+1 instead of idling 147 SMs; everything else keeps stream order.
-static int submit_init(holo_ctx* c) {
-    if (c->side) return HOLO_OK;
+static int submit_init(holo_ctx* c, bool second_stack = true) {
     const size_t T = (size_t)c->T;
-    HOLO_CUDA_OK(cudaMalloc(&c->H1, T * c->npix * sizeof(float2)));
+    if (second_stack && !c->H1) HOLO_CUDA_OK(cudaMalloc(&c->H1, T * c->npix * sizeof(float2)));
+    if (c->side) return HOLO_OK;
     HOLO_CUDA_OK(cudaMalloc(&c->C1, T * T * sizeof(float2)));
     HOLO_CUDA_OK(cudaMalloc(&c->evals1, T * sizeof(float)));
     HOLO_CUDA_OK(cudaMalloc(&c->V1, T * T * sizeof(float2)));
@@ -243,8 +298,8 @@ static int project_pending(holo_ctx* c, cudaStream_t st) {
     if (!c->pend_image) return HOLO_OK;
     const int s = c->pend_slot;
     HOLO_CUDA_OK(cudaStreamWaitEvent(st, c->ev_eig[s], 0));
-    const int rc = holo_launch_project(c, s ? c->H1 : c->H, s ? c->V1 : c->V, c->k_lo, c->k_hi,
-                                       c->tune[HOLO_TUNE_PROJ_COMPLEMENT], c->pend_image, st);
+    const int rc = holo_launch_project(c, s ? c->H1 : c->H, s ? c->V1 : c->V, c->pend_k_lo, c->pend_k_hi,
+                                       c->pend_complement, c->pend_image, st);      // the window of ITS submit call
     c->pend_image = nullptr;
     return rc;
 }
@@ -290,6 +345,7 @@ extern "C" int holo_submit(holo_ctx* c, const uint16_t* frames_dev, float* image
         return HOLO_OK;
     }
     c->pend_image = image_dev; c->pend_slot = s; c->nsubmit++;
+    c->pend_k_lo = c->k_lo; c->pend_k_hi = c->k_hi; c->pend_complement = c->tune[HOLO_TUNE_PROJ_COMPLEMENT];
     return HOLO_OK;
 }
 
@@ -330,6 +386,11 @@ extern "C" int holo_push(holo_ctx* c, const uint16_t* new_frames_dev, int n_new,
     const int T = c->T;
     if (n_new < 1 || n_new > T) { holo_set_error("need 1 <= n_new <= T (got %d)", n_new); return HOLO_ERR_ARG; }
     if (!c->push_ready && n_new != T) { holo_set_error("the first holo_push of a sequence must bring a whole window (n_new = T)"); return HOLO_ERR_STATE; }
+    {   // the centred projection exists only in the deflation form (rejected set at most half of the kept set)
+        const int nS = c->k_hi - c->k_lo + 1;
+        if (2 * (T - nS) > nS) { holo_set_error("holo_push needs a component window whose complement is at most half of it (got [%d, %d] of %d)", c->k_lo, c->k_hi, T); return HOLO_ERR_STATE; }
+        if (c->push_ready == 2 && !push_ring_possible(c)) { holo_set_error("tune keys 7, 8, 10 must not change in the middle of a pipelined holo_push sequence (restart with n_new = T)"); return HOLO_ERR_STATE; }
+    }
     cudaStream_t st = (cudaStream_t)stream;
     int rc;
     if (!c->Cd) HOLO_CUDA_OK(cudaMalloc(&c->Cd, (size_t)T * T * sizeof(double2)));
@@ -339,7 +400,7 @@ extern "C" int holo_push(holo_ctx* c, const uint16_t* new_frames_dev, int n_new,
         if ((rc = join_side(c, st, -1))) return rc;
         if ((rc = project_pending(c, st))) return rc;
         if (push_ring_possible(c)) {
-            if ((rc = submit_init(c))) return rc;                          // side stream, events, second C / V slot
+            if ((rc = submit_init(c, /*second_stack=*/false))) return rc;   // side stream, events, second C / V slot (no second H)
             if (!c->ring) {
                 c->ring_slots = T + extra;
                 HOLO_CUDA_OK(cudaMalloc(&c->ring, (size_t)c->ring_slots * c->npix * sizeof(float2)));
@@ -506,12 +567,16 @@ extern "C" int holo_process_host(holo_ctx* c, const uint16_t* frames_host, float
 extern "C" int holo_set_range(holo_ctx* c, int k_lo, int k_hi) {
     CHECK_CTX(c);
     if (k_lo < 1 || k_hi > c->T || k_lo > k_hi) { holo_set_error("need 1 <= k_lo <= k_hi <= T (got %d, %d)", k_lo, k_hi); return HOLO_ERR_ARG; }
+    if (c->push_ready && 2 * (c->T - (k_hi - k_lo + 1)) > (k_hi - k_lo + 1)) {
+        holo_set_error("a holo_push sequence is open: its window's complement must stay at most half of the window");
+        return HOLO_ERR_STATE;
+    }
     c->k_lo = k_lo; c->k_hi = k_hi;
     return HOLO_OK;
 }
 
 extern "C" int holo_set_assume_unitary(holo_ctx* c, int on) {
-    CHECK_CTX(c);
+    CHECK_CTX_QUIET(c);
     c->assume_unitary = on ? 1 : 0;
     return HOLO_OK;
 }
@@ -532,15 +597,18 @@ extern "C" const void* holo_workspace(holo_ctx* c, int which) {
 }
 
 extern "C" int holo_workspace_copy(holo_ctx* c, int which, void* dst_dev, unsigned long long nbytes, holo_stream stream) {
-    CHECK_CTX(c); CHECK_PTR(dst_dev, "dst_dev");
+    CHECK_CTX_QUIET(c); CHECK_PTR(dst_dev, "dst_dev");
     const void* src = holo_workspace(c, which);
     if (!src) { holo_set_error("bad workspace id %d", which); return HOLO_ERR_ARG; }
+    const size_t T = (size_t)c->T, np = (size_t)c->npix;
+    const size_t cap[8] = {np * 4, T * np * 8, T * T * 8, T * 4, T * T * 8, 8 * 4, (size_t)c->nx * 8, (size_t)c->ny * 8};
+    if (nbytes > cap[which]) { holo_set_error("workspace array %d holds %zu bytes (asked for %llu)", which, cap[which], nbytes); return HOLO_ERR_ARG; }
     HOLO_CUDA_OK(cudaMemcpyAsync(dst_dev, src, (size_t)nbytes, cudaMemcpyDeviceToDevice, (cudaStream_t)stream));
     return HOLO_OK;
 }
 
 extern "C" int holo_status(holo_ctx* c, int32_t status_host[4], holo_stream stream) {
-    CHECK_CTX(c); CHECK_PTR(status_host, "status_host");
+    CHECK_CTX_QUIET(c); CHECK_PTR(status_host, "status_host");
     cudaStream_t st = (cudaStream_t)stream;
     // the eigensolvers of holo_submit / holo_push run on the side stream: join it first (the caller should have called
     // holo_flush; this only makes the read safe), then read the word of the last solve of each workspace slot
@@ -554,18 +622,19 @@ extern "C" int holo_status(holo_ctx* c, int32_t status_host[4], holo_stream stre
         HOLO_CUDA_OK(cudaStreamSynchronize(st));
         if (other[0]) memcpy(status_host, other, sizeof(other));      // report the slot that failed
     }
+    *(volatile int32_t*)c->noconv_host = 0;                // reported here: the next call is not refused for it
     if (status_host[0]) { holo_set_error("Jacobi eigensolver hit the sweep cap (%d sweeps)", status_host[1]); return HOLO_ERR_NOCONV; }
     return HOLO_OK;
 }
 
 extern "C" int holo_launches_per_process(holo_ctx* c) {
-    CHECK_CTX(c);
+    CHECK_CTX_QUIET(c);
     return holo_fresnel_launch_count(c) + 2 /*cov partial + reduce*/ + 1 /*eig*/ + 1 /*project*/;
 }
 
-// not in holo.h: experiment knob used by bench.py sweeps (see holo_internal.cuh HOLO_TUNE_*)
+// experiment knobs (see holo_internal.cuh HOLO_TUNE_* and include/holo.h)
 extern "C" int holo_tune(holo_ctx* c, int key, int value) {
-    CHECK_CTX(c);
+    CHECK_CTX_QUIET(c);
     if (key < 0 || key >= HOLO_NUM_TUNE) { holo_set_error("bad tuning key"); return HOLO_ERR_ARG; }
     if (key == HOLO_TUNE_FFT_GROUP) {
         if (value < 1 || value > c->T) { holo_set_error("fft group out of range"); return HOLO_ERR_ARG; }
@@ -588,10 +657,10 @@ extern "C" int holo_tune(holo_ctx* c, int key, int value) {
     return HOLO_OK;
 }
 
-// not in the stable ABI: per-kernel-class device time accumulated since the last read, while
-// holo_tune(ctx, 5, 1) is on.  ms_out[HOLO_K_COUNT], count_out[HOLO_K_COUNT]; synchronises the device.
+// per-kernel-class device time accumulated since the last read, while holo_tune(ctx, 5, 1) is on.
+// ms_out[HOLO_K_COUNT], count_out[HOLO_K_COUNT]; synchronises the device.
 extern "C" int holo_profile_read(holo_ctx* c, double* ms_out, int* count_out) {
-    CHECK_CTX(c); CHECK_PTR(ms_out, "ms_out"); CHECK_PTR(count_out, "count_out");
+    CHECK_CTX_QUIET(c); CHECK_PTR(ms_out, "ms_out"); CHECK_PTR(count_out, "count_out");
     for (int k = 0; k < HOLO_K_COUNT; ++k) { ms_out[k] = 0.0; count_out[k] = 0; }
     if (!c->prof_ev) return HOLO_OK;
     HOLO_CUDA_OK(cudaDeviceSynchronize());

@@ -16,14 +16,14 @@ enum {
     HOLO_TUNE_PROJ_COMPLEMENT = 2, // 1 = allow complement form in holo_process (default 1)
     HOLO_TUNE_FFT_PERSISTENT = 3,  // 1 = single persistent fresnel kernel (default set at create)
     HOLO_TUNE_EIG_MAX_SWEEPS = 4,
-    HOLO_TUNE_PROFILE = 5,
+    HOLO_TUNE_PROFILE = 5,         // 1 = bracket every kernel launch with events (holo_profile_read)
     HOLO_TUNE_PROJ_TMA = 7,        // 1 = deflation projection fed by a TMA ring (default), 0 = register-streaming kernel
     HOLO_TUNE_COV_REAL = 8,        // 1 = holo_process / holo_submit compute Re C only (C is real there, R21); default 1
     HOLO_TUNE_SPLIT_SMS = 9,       // holo_submit: k > 0 = projection on the side stream on k SMs, concurrent with the
                                    // next covariance on the other SMs (memory-bound next to ALU-bound); 0 = in stream order
     HOLO_TUNE_PUSH_PIPE = 10,      // holo_push: 1 = pipelined ring form when T in {16,32,64} and n_new is a multiple of 8 (default)
     HOLO_TUNE_PUSH_INCR = 11,      // holo_push (ring form): 1 = recompute only the Gram rows / columns of the new frames (default)
-    HOLO_TUNE_FFT_LAG = 6,         // frames between the row pass and the column pass in the fused kernel (0 = auto)         // 1 = bracket every kernel launch with events (holo_profile_read)
+    HOLO_TUNE_FFT_LAG = 6,         // frames between the row pass and the column pass in the fused kernel (0 = auto)
 };
 
 // kernel classes for the profile hook
@@ -57,14 +57,15 @@ struct holo_ctx {
     float2* scratch;        // FFT row->column intermediate, fft_group frames
     int scratch_frames;
     float2* H;              // [T][ny][nx]
-    float2* cov_partials;   // [2 halves][cov_parts][T8][T8]; cov_sel picks the half (holo_submit: one per slot)
-    int cov_sel, cov_nparts; // half used by / partials written by the last covariance launch
+    float2* cov_partials;   // [cov_parts_cap][T8][T8]
+    int cov_nparts;         // partials written by the last covariance launch
     int cov_parts_cap;
     float2* C;
     float* evals;
     float2* V;
-    float2* Vsel;           // [T][HOLO_MAX_T] selected/zero-padded projection coefficients
-    int32_t* status;        // [4]
+    int32_t* status;        // [8], see HOLO_WS_STATUS
+    int32_t* noconv_host;   // pinned, mapped host word: set by the eigensolver when it hits the sweep cap (device alias below)
+    int32_t* noconv_dev;
     unsigned int* counters; // persistent-kernel tickets / dependency counters
     // profile hook
     cudaEvent_t* prof_ev;   // [2*HOLO_PROF_CAP]
@@ -75,7 +76,7 @@ struct holo_ctx {
     cudaStream_t side;
     cudaEvent_t ev_cov[2], ev_eig[2];
     float* pend_image;      // image of the stack whose projection is still owed (nullptr: none)
-    int pend_slot;
+    int pend_slot, pend_k_lo, pend_k_hi, pend_complement;   // its workspace slot and the component window at submit time
     long long nsubmit;
     cudaEvent_t ev_proj[2]; int proj_recorded[2];
     // sliding-window form (holo_push)
@@ -129,11 +130,10 @@ int holo_launch_sum(holo_ctx* c, const uint16_t* frames, cudaStream_t st);
 int holo_launch_fresnel(holo_ctx* c, const uint16_t* frames, float2* H, cudaStream_t st, bool with_sum = true, int nproc = -1);
 // C == nullptr: partials only; holo_launch_cov_reduce then finishes (possibly on another stream, ordered after)
 int holo_launch_covariance(holo_ctx* c, const float2* H, float2* C, cudaStream_t st, bool real_only = false);
-int holo_launch_cov_reduce(holo_ctx* c, int sel, int nparts, float2* C, cudaStream_t st);
-static inline float2* holo_cov_partials(holo_ctx* c, int sel) {
-    const int T8 = (c->T + 7) / 8 * 8;
-    return c->cov_partials + (size_t)sel * c->cov_parts_cap * T8 * T8;
-}
+int holo_launch_cov_reduce(holo_ctx* c, int nparts, float2* C, cudaStream_t st);
+// cudaFuncSetAttribute / occupancy are properties of a (function, device) pair: cached per pair, thread-safe
+int holo_ensure_smem_attr(const void* func, int device, size_t bytes);
+int holo_cached_occupancy(const void* func, int device, int threads, size_t smem, int* blocks_per_sm);
 int holo_launch_eig(holo_ctx* c, const float2* C, float* evals, float2* V, cudaStream_t st);
 // mode 0: direct over columns [k_lo,k_hi] of V; mode 1: complement (total - columns outside)
 int holo_launch_project(holo_ctx* c, const float2* H, const float2* V, int k_lo, int k_hi,

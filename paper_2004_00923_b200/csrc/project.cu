@@ -17,7 +17,7 @@ struct ProjArgs {
     int T;
     int r0_lo, r0_hi;      // first 0-based inclusive column range (empty if lo > hi)
     int r1_lo, r1_hi;      // second range
-    int complement;        // 1: M = total - sum
+    int complement;        // 1: deflation form (the ranges are the REJECTED components); always taken by the k_project_deflate* kernels
     int center;            // 1: subtract the per-pixel mean over t first (sliding-window form: H_t = G_t - mean_t G)
 };
 
@@ -42,9 +42,6 @@ __global__ void __launch_bounds__(256) k_project(const ProjArgs a) {
     for (int x = 0; x < PIX; ++x)
 #pragma unroll
         for (int c = 0; c < NC; ++c) acc[x][c] = make_float2(0.f, 0.f);
-    float tot[PIX];
-#pragma unroll
-    for (int x = 0; x < PIX; ++x) tot[x] = 0.f;
 #pragma unroll 4
     for (int t = 0; t < a.T; ++t) {
         float2 h[PIX];
@@ -54,8 +51,6 @@ __global__ void __launch_bounds__(256) k_project(const ProjArgs a) {
         } else {
             h[0] = __ldg(a.H + item + (long long)t * fstride);
         }
-#pragma unroll
-        for (int x = 0; x < PIX; ++x) tot[x] = fmaf(h[x].x, h[x].x, fmaf(h[x].y, h[x].y, tot[x]));
 #pragma unroll
         for (int c = 0; c < NC; ++c) {
             const float2 v = Vs[t * NC + c];
@@ -72,7 +67,6 @@ __global__ void __launch_bounds__(256) k_project(const ProjArgs a) {
         s[x] = 0.f;
 #pragma unroll
         for (int c = 0; c < NC; ++c) s[x] = fmaf(acc[x][c].x, acc[x][c].x, fmaf(acc[x][c].y, acc[x][c].y, s[x]));
-        if (a.complement) s[x] = tot[x] - s[x];
     }
     if constexpr (PIX == 2) reinterpret_cast<float2*>(a.M)[item] = make_float2(s[0], s[1]);
     else a.M[item] = s[0];
@@ -262,11 +256,7 @@ template <int TMAX> static int launch_deflate(holo_ctx* c, const ProjArgs& a, in
     }
     if (c->tune[HOLO_TUNE_PROJ_TMA] && nstages >= 2 && a.npix % PROJ_P == 0) {
         const size_t smem = 128 + vbytes + (size_t)nstages * stage_bytes;
-        static bool attr = false;
-        if (!attr) {
-            HOLO_CUDA_OK(cudaFuncSetAttribute(k_project_deflate_tma<TMAX, PROJ_P>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024 + 128));
-            attr = true;
-        }
+        { const int rc = holo_ensure_smem_attr((const void*)k_project_deflate_tma<TMAX, PROJ_P>, c->device, 200 * 1024 + 128); if (rc) return rc; }
         alignas(64) CUtensorMap tmH;
         { const int rc = holo_make_tensor_map(&tmH, a.H, a.npix, c->ring_nrb ? 8 * c->ring_nrb : a.T, 128); if (rc) return rc; }
         const long long nchunks = a.npix / PROJ_P;

@@ -1,7 +1,12 @@
+// ubench_peaks.cu -- measured denominators that MEASURED_PEAKS.json does not hold: the FP32 FFMA /
+// packed FFMA2 issue rate, HBM read / copy / memset bandwidth, and the L2 hit bandwidth (a buffer that fits the 126 MB
+// L2 read / written repeatedly) which bounds the row->column ring of the Fresnel stage.  Standalone binary; its output
+// is kept under profiles/.   nvcc -gencode arch=compute_100a,code=sm_100a -O3 -o ubench_peaks ubench_peaks.cu
 #include <cstdio>
 #include <cuda_runtime.h>
 #include <cstdint>
 #define CK(x) do{cudaError_t e=(x); if(e!=cudaSuccess){printf("ERR %s line %d\n",cudaGetErrorString(e),__LINE__); return 1;}}while(0)
+#define LAUNCH_OK() CK(cudaGetLastError())     /* a launch that failed must not be timed as a success */
 template<int NACC>
 __global__ void k_ffma(float* out, float a, float b, int iters){
   float acc[NACC];
@@ -74,16 +79,17 @@ int main(){
   int iters=20000;
   for(int thr: {256,512,1024}) for(int bps: {1,2,4}){
     if(thr*bps>2048) continue;
-    k_ffma<16><<<sms*bps,thr>>>(out,1.0001f,0.5f,100); cudaDeviceSynchronize();
-    cudaEventRecord(e0); k_ffma<16><<<sms*bps,thr>>>(out,1.0001f,0.5f,iters); cudaEventRecord(e1); CK(cudaEventSynchronize(e1)); cudaEventElapsedTime(&ms,e0,e1);
+    k_ffma<16><<<sms*bps,thr>>>(out,1.0001f,0.5f,100); LAUNCH_OK(); cudaDeviceSynchronize();
+    cudaEventRecord(e0); k_ffma<16><<<sms*bps,thr>>>(out,1.0001f,0.5f,iters); LAUNCH_OK(); cudaEventRecord(e1); CK(cudaEventSynchronize(e1)); cudaEventElapsedTime(&ms,e0,e1);
     printf("FFMA  thr=%4d bps=%d: %.2f TFLOPS\n",thr,bps, 2.0*16*iters*(double)sms*bps*thr/ms/1e9);
-    k_ffma2<16><<<sms*bps,thr>>>(out,1.0001f,0.5f,100); cudaDeviceSynchronize();
-    cudaEventRecord(e0); k_ffma2<16><<<sms*bps,thr>>>(out,1.0001f,0.5f,iters); cudaEventRecord(e1); CK(cudaEventSynchronize(e1)); cudaEventElapsedTime(&ms,e0,e1);
+    if(thr>512) continue;      // k_ffma2<16> holds 34 register pairs: more than 64 registers per thread, no 1024-thread launch
+    k_ffma2<16><<<sms*bps,thr>>>(out,1.0001f,0.5f,100); LAUNCH_OK(); cudaDeviceSynchronize();
+    cudaEventRecord(e0); k_ffma2<16><<<sms*bps,thr>>>(out,1.0001f,0.5f,iters); LAUNCH_OK(); cudaEventRecord(e1); CK(cudaEventSynchronize(e1)); cudaEventElapsedTime(&ms,e0,e1);
     printf("FFMA2 thr=%4d bps=%d: %.2f TFLOPS\n",thr,bps, 4.0*16*iters*(double)sms*bps*thr/ms/1e9);
   }
   for(int thr: {128,256,320}){
-    k_ffma_outer<<<sms,thr>>>(out,in,100); cudaDeviceSynchronize();
-    cudaEventRecord(e0); k_ffma_outer<<<sms,thr>>>(out,in,iters); cudaEventRecord(e1); CK(cudaEventSynchronize(e1)); cudaEventElapsedTime(&ms,e0,e1);
+    k_ffma_outer<<<sms,thr>>>(out,in,100); LAUNCH_OK(); cudaDeviceSynchronize();
+    cudaEventRecord(e0); k_ffma_outer<<<sms,thr>>>(out,in,iters); LAUNCH_OK(); cudaEventRecord(e1); CK(cudaEventSynchronize(e1)); cudaEventElapsedTime(&ms,e0,e1);
     printf("FFMA outer8x8 thr=%d: %.2f TFLOPS\n",thr, 2.0*64*iters*(double)sms*thr/ms/1e9);
   }
   size_t bytes=(size_t)4<<30; uint4 *a,*b; CK(cudaMalloc(&a,bytes)); CK(cudaMalloc(&b,bytes)); CK(cudaMemset(a,1,bytes)); CK(cudaMemset(b,0,bytes));
@@ -95,6 +101,16 @@ int main(){
     printf("copy  4GiB: %.1f GB/s (r+w)\n", 2.0*bytes/ms/1e6);
     cudaEventRecord(e0); cudaMemsetAsync(b,0,bytes); cudaEventRecord(e1); CK(cudaEventSynchronize(e1)); cudaEventElapsedTime(&ms,e0,e1);
     printf("memset 4GiB: %.1f GB/s\n", bytes/ms/1e6);
+  }
+  // ---- L2 hit bandwidth: a 32 MiB / 64 MiB buffer (fits the 126 MB L2) streamed repeatedly
+  for(size_t mb: {32, 64}){
+    size_t nb=mb<<20, m=nb/16; int reps=40;
+    k_read<<<sms*8,512>>>(a,m,b); LAUNCH_OK(); cudaDeviceSynchronize();
+    cudaEventRecord(e0); for(int r=0;r<reps;r++) k_read<<<sms*8,512>>>(a,m,b); LAUNCH_OK(); cudaEventRecord(e1); CK(cudaEventSynchronize(e1)); cudaEventElapsedTime(&ms,e0,e1);
+    printf("L2 read  %zu MiB x%d: %.1f GB/s\n", mb, reps, (double)nb*reps/ms/1e6);
+    k_copy<<<sms*8,512>>>(a,a+m,m); LAUNCH_OK(); cudaDeviceSynchronize();
+    cudaEventRecord(e0); for(int r=0;r<reps;r++) k_copy<<<sms*8,512>>>(a,a+m,m); LAUNCH_OK(); cudaEventRecord(e1); CK(cudaEventSynchronize(e1)); cudaEventElapsedTime(&ms,e0,e1);
+    printf("L2 copy  %zu MiB -> %zu MiB x%d: %.1f GB/s (r+w)\n", mb, mb, reps, 2.0*nb*reps/ms/1e6);
   }
   return 0;
 }
