@@ -135,9 +135,12 @@ def stream_torch(cfg: Config, seed: int, device, n_frames=None, chunk=32):
     """uint16 torch tensor (n_frames, n, n) on `device` -- same formulas, torch RNG for the shot
     noise (scene parameters still come from numpy's default_rng(seed)).  Bench harness only."""
     import torch
+    import dataclasses
+    n_frames = n_frames or cfg.n_frames
+    if n_frames > cfg.n_frames:                          # a longer stream of the same recipe (the phase walk continues)
+        cfg = dataclasses.replace(cfg, n_frames=n_frames)
     scene = make_scene(cfg, seed)
     n = cfg.n
-    n_frames = n_frames or cfg.n_frames
     g = torch.Generator(device=device)
     g.manual_seed(seed)
     O = torch.from_numpy(scene.O).to(device=device, dtype=torch.complex64)

@@ -6,5 +6,6 @@ There is NO CPU fallback: importing `binding` without the built library, or crea
 without a CUDA device, raises.
 """
 from .binding import (Holo, load_library, library_path, HoloError,  # noqa: F401
+                      HOLO_OK, HOLO_ERR_ARG, HOLO_ERR_ALLOC, HOLO_ERR_CUDA, HOLO_ERR_STATE, HOLO_ERR_NOCONV,
                       HOLO_WS_SUM, HOLO_WS_H, HOLO_WS_C, HOLO_WS_EVALS, HOLO_WS_V, HOLO_WS_STATUS,
                       HOLO_WS_QX, HOLO_WS_QY, EXPORTED_SYMBOLS)

@@ -72,6 +72,29 @@ __global__ void k_copy(const uint4* __restrict__ in, uint4* __restrict__ out, si
   size_t i=(size_t)blockIdx.x*blockDim.x+threadIdx.x; size_t stride=(size_t)gridDim.x*blockDim.x;
   for(; i<n; i+=stride) out[i]=in[i];
 }
+// the same buffer streamed `reps` times inside ONE launch (no launch gaps): L2 hit bandwidth when it fits L2
+__global__ void k_read_loop(const uint4* __restrict__ in, size_t n, int reps, uint4* out){
+  size_t stride=(size_t)gridDim.x*blockDim.x;
+  uint4 s=make_uint4(0,0,0,0);
+  for(int r=0;r<reps;r++){
+    size_t i=(size_t)blockIdx.x*blockDim.x+threadIdx.x;
+    for(; i+3*stride<n; i+=4*stride){
+      uint4 a,b,c,d;
+      asm volatile("ld.global.cg.v4.u32 {%0,%1,%2,%3}, [%4];":"=r"(a.x),"=r"(a.y),"=r"(a.z),"=r"(a.w):"l"(in+i));
+      asm volatile("ld.global.cg.v4.u32 {%0,%1,%2,%3}, [%4];":"=r"(b.x),"=r"(b.y),"=r"(b.z),"=r"(b.w):"l"(in+i+stride));
+      asm volatile("ld.global.cg.v4.u32 {%0,%1,%2,%3}, [%4];":"=r"(c.x),"=r"(c.y),"=r"(c.z),"=r"(c.w):"l"(in+i+2*stride));
+      asm volatile("ld.global.cg.v4.u32 {%0,%1,%2,%3}, [%4];":"=r"(d.x),"=r"(d.y),"=r"(d.z),"=r"(d.w):"l"(in+i+3*stride));
+      s.x^=a.x^b.x^c.x^d.x; s.y^=a.y^b.y^c.y^d.y; s.z^=a.z^b.z^c.z^d.z; s.w^=a.w^b.w^c.w^d.w;}
+  }
+  if(s.x==0x12345678u) out[0]=s;
+}
+__global__ void k_copy_loop(const uint4* __restrict__ in, uint4* __restrict__ out, size_t n, int reps){
+  size_t stride=(size_t)gridDim.x*blockDim.x;
+  for(int r=0;r<reps;r++)
+    for(size_t i=(size_t)blockIdx.x*blockDim.x+threadIdx.x; i<n; i+=stride){
+      uint4 a; asm volatile("ld.global.cg.v4.u32 {%0,%1,%2,%3}, [%4];":"=r"(a.x),"=r"(a.y),"=r"(a.z),"=r"(a.w):"l"(in+i));
+      a.x+=r; out[i]=a; }
+}
 int main(){
   int sms; cudaDeviceGetAttribute(&sms,cudaDevAttrMultiProcessorCount,0);
   float* out; CK(cudaMalloc(&out, 148*8*1024*4)); float* in; CK(cudaMalloc(&in,4096*4)); CK(cudaMemset(in,0,4096*4));
@@ -111,6 +134,15 @@ int main(){
     k_copy<<<sms*8,512>>>(a,a+m,m); LAUNCH_OK(); cudaDeviceSynchronize();
     cudaEventRecord(e0); for(int r=0;r<reps;r++) k_copy<<<sms*8,512>>>(a,a+m,m); LAUNCH_OK(); cudaEventRecord(e1); CK(cudaEventSynchronize(e1)); cudaEventElapsedTime(&ms,e0,e1);
     printf("L2 copy  %zu MiB -> %zu MiB x%d: %.1f GB/s (r+w)\n", mb, mb, reps, 2.0*nb*reps/ms/1e6);
+  }
+  for(size_t mb: {16, 32, 48}){
+    size_t nb=mb<<20, m=nb/16; int reps=100;
+    k_read_loop<<<sms*4,512>>>(a,m,2,b); LAUNCH_OK(); cudaDeviceSynchronize();
+    cudaEventRecord(e0); k_read_loop<<<sms*4,512>>>(a,m,reps,b); LAUNCH_OK(); cudaEventRecord(e1); CK(cudaEventSynchronize(e1)); cudaEventElapsedTime(&ms,e0,e1);
+    printf("L2 read loop  %zu MiB x%d in one launch: %.1f GB/s\n", mb, reps, (double)nb*reps/ms/1e6);
+    k_copy_loop<<<sms*4,512>>>(a,a+m,m,2); LAUNCH_OK(); cudaDeviceSynchronize();
+    cudaEventRecord(e0); k_copy_loop<<<sms*4,512>>>(a,a+m,m,reps); LAUNCH_OK(); cudaEventRecord(e1); CK(cudaEventSynchronize(e1)); cudaEventElapsedTime(&ms,e0,e1);
+    printf("L2 copy loop  %zu MiB -> %zu MiB x%d in one launch: %.1f GB/s (r+w)\n", mb, mb, reps, 2.0*nb*reps/ms/1e6);
   }
   return 0;
 }
