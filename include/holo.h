@@ -147,6 +147,21 @@ int holo_fresnel(holo_ctx* ctx, const uint16_t* frames_dev, void* H_dev, holo_st
  * count and reduction order; bit-identical across runs).  (Eq. 4) */
 int holo_covariance(holo_ctx* ctx, const void* H_dev, void* C_dev, holo_stream stream);
 
+/* A3 from the RAW frames (reading c-12 of Eq. 4): for holograms H_t = FFT2[q d_t] of real
+ * mean-subtracted frames (q unimodular, the transform unitary up to nx ny)  C = H^H H = nx ny D^T D  exactly, so the
+ * covariance needs neither the holograms nor floating point: the Gram of the uint16 frames is formed in exact integer
+ * arithmetic on the tensor cores (tcgen05.mma kind::i8 on the byte planes, s32 accumulators, int64 / __int128
+ * assembly), centred with the integer frame sum, and rounded once to float.  frames_dev (uint16 [T][ny][nx]) ->
+ * C_dev (float2 [T][T], real symmetric, Im = 0).  Also leaves S = sum_t I_t in the workspace (HOLO_WS_SUM). */
+int holo_raw_covariance(holo_ctx* ctx, const uint16_t* frames_dev, void* C_dev, holo_stream stream);
+
+/* Mode of holo_process / holo_submit.  1 (default): the stage decomposition as the paper writes it (Fresnel stage, then
+ * the covariance of the hologram stack).  2: holo_raw_covariance + eigensolver FIRST, then the Fresnel stage and the
+ * projection with V already known -- the hologram stack is read once instead of twice (20 T N_p + 12 N_p compulsory
+ * bytes instead of 28 T N_p + 12 N_p), and in holo_submit the image is complete in stream order when the call's work
+ * is done.  Same results up to FP32 rounding of C.  holo_push always works as in mode 1. */
+int holo_set_mode(holo_ctx* ctx, int mode);
+
 /* A4: any Hermitian C_dev (only its lower triangle t >= s and real diagonal are read) ->
  * evals_dev (float [T], descending), V_dev (float2 [T][T], unitary, column k-1 = eigenvector k,
  * phase fixed so that each column's largest-magnitude entry is real positive).  Single-CTA

@@ -10,7 +10,7 @@ HOLO_WS_SUM, HOLO_WS_H, HOLO_WS_C, HOLO_WS_EVALS, HOLO_WS_V, HOLO_WS_STATUS, HOL
 
 EXPORTED_SYMBOLS = [
     "holo_create", "holo_destroy", "holo_process", "holo_submit", "holo_flush", "holo_submit_host", "holo_flush_host", "holo_push", "holo_process_host", "holo_fresnel", "holo_covariance",
-    "holo_eig", "holo_project", "holo_fourier_demod", "holo_set_range", "holo_set_assume_unitary",
+    "holo_raw_covariance", "holo_set_mode", "holo_eig", "holo_project", "holo_fourier_demod", "holo_set_range", "holo_set_assume_unitary",
     "holo_workspace", "holo_workspace_copy", "holo_status", "holo_launches_per_process", "holo_tune", "holo_profile_read", "holo_fft_group",
     "holo_last_error", "holo_version",
 ]
@@ -50,6 +50,8 @@ def load_library():
     L.holo_flush_host.argtypes = [vp, vp]
     L.holo_fresnel.argtypes = [vp, vp, vp, vp]
     L.holo_covariance.argtypes = [vp, vp, vp, vp]
+    L.holo_raw_covariance.argtypes = [vp, vp, vp, vp]
+    L.holo_set_mode.argtypes = [vp, ip]
     L.holo_eig.argtypes = [vp, vp, vp, vp, vp]
     L.holo_project.argtypes = [vp, vp, vp, vp, vp]
     L.holo_fourier_demod.argtypes = [vp, vp, ip, ip, vp, vp]
@@ -132,6 +134,12 @@ class Holo:
 
     def covariance(self, H_dev, C_dev, stream=None):
         self._chk(self._L.holo_covariance(self._h, self._p(H_dev), self._p(C_dev), _stream_ptr(stream)))
+
+    def raw_covariance(self, frames_dev, C_dev, stream=None):
+        self._chk(self._L.holo_raw_covariance(self._h, self._p(frames_dev), self._p(C_dev), _stream_ptr(stream)))
+
+    def set_mode(self, mode):
+        self._chk(self._L.holo_set_mode(self._h, mode))
 
     def eig(self, C_dev, evals_dev, V_dev, stream=None):
         self._chk(self._L.holo_eig(self._h, self._p(C_dev), self._p(evals_dev), self._p(V_dev), _stream_ptr(stream)))

@@ -5,7 +5,7 @@ import sys
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
-SOURCES = ["holo_api.cu", "fresnel.cu", "covariance.cu", "eig.cu", "project.cu"]
+SOURCES = ["holo_api.cu", "fresnel.cu", "fresnel2.cu", "rawgram.cu", "covariance.cu", "eig.cu", "project.cu"]
 LIB = os.path.join(HERE, "libholo_b200.so")
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
@@ -15,7 +15,8 @@ FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std
 def _stale(obj, src):
     if not os.path.exists(obj):
         return True
-    deps = [src, os.path.join(CSRC, "holo_internal.cuh"), os.path.join(CSRC, "tma.cuh"), os.path.join(HERE, "..", "include", "holo.h")]
+    deps = [src, os.path.join(CSRC, "holo_internal.cuh"), os.path.join(CSRC, "tma.cuh"), os.path.join(CSRC, "fft_reg.cuh"),
+            os.path.join(HERE, "..", "include", "holo.h")]
     return os.path.getmtime(obj) < max(os.path.getmtime(d) for d in deps)
 
 

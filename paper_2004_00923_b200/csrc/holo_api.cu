@@ -78,7 +78,7 @@ static void free_ctx(holo_ctx* c) {
     cudaFree(c->sum); cudaFree(c->scratch); cudaFree(c->H); cudaFree(c->cov_partials);
     cudaFree(c->C); cudaFree(c->evals); cudaFree(c->V); cudaFree(c->status);
     if (c->noconv_host) cudaFreeHost(c->noconv_host);
-    cudaFree(c->counters);
+    cudaFree(c->counters); cudaFree(c->gram_X);
     if (c->prof_ev) {
         for (int i = 0; i < 2 * HOLO_PROF_CAP; ++i) cudaEventDestroy(c->prof_ev[i]);
         delete[] c->prof_ev;
@@ -131,7 +131,7 @@ static int create_impl(holo_ctx* c) {
     c->tune[HOLO_TUNE_FFT_GROUP] = (int)grp;
     c->tune[HOLO_TUNE_COV_GRIDX] = c->num_sms;
     c->tune[HOLO_TUNE_PROJ_COMPLEMENT] = 1;
-    c->tune[HOLO_TUNE_FFT_PERSISTENT] = 1;
+    c->tune[HOLO_TUNE_FFT_PERSISTENT] = 1;      // 2 = k_fresnel2 (packed two-sequence FFT, TMA-staged column tiles): correct, measured slower
     c->tune[HOLO_TUNE_PROJ_TMA] = 1;
     c->tune[HOLO_TUNE_COV_REAL] = 1;
     c->tune[HOLO_TUNE_PUSH_PIPE] = 1;
@@ -152,6 +152,8 @@ static int create_impl(holo_ctx* c) {
     HOLO_CUDA_OK(cudaMalloc(&c->V, (size_t)T * T * sizeof(float2)));
     HOLO_CUDA_OK(cudaMalloc(&c->status, 8 * sizeof(int32_t)));
     HOLO_CUDA_OK(cudaMalloc(&c->counters, 1024 * sizeof(unsigned int)));
+    HOLO_CUDA_OK(cudaMalloc(&c->gram_X, 128 * 128 * sizeof(unsigned long long)));
+    c->mode = 1;
     HOLO_CUDA_OK(cudaMemset(c->status, 0, 8 * sizeof(int32_t)));
     HOLO_CUDA_OK(cudaMemset(c->counters, 0, 1024 * sizeof(unsigned int)));
     HOLO_CUDA_OK(cudaMemset(c->cov_partials, 0, (size_t)c->cov_parts_cap * T8 * T8 * sizeof(float2)));
@@ -254,10 +256,32 @@ extern "C" int holo_process(holo_ctx* c, const uint16_t* frames_dev, float* imag
     if ((rc = project_pending(c, st))) return rc;          // a holo_submit still owes its image: deliver it first
     c->nsubmit = 0;                                        // the next holo_submit starts again with slot 0
     c->push_ready = 0;                                     // ... and a holo_push sequence has to start over
+    if (c->mode == 2) {
+        // covariance from the raw frames (exact integer Gram on the tensor cores, fused with the temporal sum): C and V are
+        // known BEFORE the holograms exist, and the hologram stack is read once (projection) instead of twice
+        if ((rc = holo_launch_sum_gram(c, frames_dev, c->C, st))) return rc;
+        if ((rc = holo_launch_eig(c, c->C, c->evals, c->V, st))) return rc;
+        if ((rc = holo_launch_fresnel(c, frames_dev, c->H, st, /*with_sum=*/false, -1, /*counters_zeroed=*/true))) return rc;
+        return holo_launch_project(c, c->H, c->V, c->k_lo, c->k_hi, c->tune[HOLO_TUNE_PROJ_COMPLEMENT], image_dev, st);
+    }
     if ((rc = holo_launch_fresnel(c, frames_dev, c->H, st))) return rc;
     if ((rc = holo_launch_covariance(c, c->H, c->C, st, /*real_only=*/true))) return rc;
     if ((rc = holo_launch_eig(c, c->C, c->evals, c->V, st))) return rc;
     return holo_launch_project(c, c->H, c->V, c->k_lo, c->k_hi, c->tune[HOLO_TUNE_PROJ_COMPLEMENT], image_dev, st);
+}
+
+extern "C" int holo_raw_covariance(holo_ctx* c, const uint16_t* frames_dev, void* C_dev, holo_stream stream) {
+    CHECK_CTX(c); CHECK_PTR(frames_dev, "frames_dev"); CHECK_PTR(C_dev, "C_dev");
+    if ((uintptr_t)frames_dev & 15) { holo_set_error("frames_dev must be 16-byte aligned"); return HOLO_ERR_ARG; }
+    return holo_launch_sum_gram(c, frames_dev, (float2*)C_dev, (cudaStream_t)stream);
+}
+
+extern "C" int holo_set_mode(holo_ctx* c, int mode) {
+    CHECK_CTX_QUIET(c);
+    if (mode != 1 && mode != 2) { holo_set_error("mode must be 1 (covariance of the hologram stack) or 2 (of the raw frames)"); return HOLO_ERR_ARG; }
+    if (c->pend_image || c->proj_recorded[0] || c->proj_recorded[1]) { holo_set_error("holo_flush the open holo_submit sequence before changing the mode"); return HOLO_ERR_STATE; }
+    c->mode = mode;
+    return HOLO_OK;
 }
 
 // ---- streaming form: software pipeline over consecutive stacks -------------------------------------
@@ -309,6 +333,21 @@ extern "C" int holo_submit(holo_ctx* c, const uint16_t* frames_dev, float* image
     if (((uintptr_t)frames_dev & 15) || ((uintptr_t)image_dev & 7)) { holo_set_error("frames_dev must be 16-byte and image_dev 8-byte aligned"); return HOLO_ERR_ARG; }
     cudaStream_t st = (cudaStream_t)stream;
     int rc;
+    if (c->mode == 2) {
+        // mode 2: the eigensolver runs on the side stream UNDER the Fresnel stage of the same stack (C comes from the raw
+        // frames), so the projection follows in stream order and the image is complete when this call's work is done
+        if ((rc = submit_init(c, /*second_stack=*/false))) return rc;
+        c->push_ready = 0;
+        if ((rc = holo_launch_sum_gram(c, frames_dev, c->C, st))) return rc;
+        HOLO_CUDA_OK(cudaEventRecord(c->ev_cov[0], st));
+        HOLO_CUDA_OK(cudaStreamWaitEvent(c->side, c->ev_cov[0], 0));
+        if ((rc = holo_launch_eig(c, c->C, c->evals, c->V, c->side))) return rc;
+        HOLO_CUDA_OK(cudaEventRecord(c->ev_eig[0], c->side));
+        if ((rc = holo_launch_fresnel(c, frames_dev, c->H, st, /*with_sum=*/false, -1, /*counters_zeroed=*/true))) return rc;
+        HOLO_CUDA_OK(cudaStreamWaitEvent(st, c->ev_eig[0], 0));
+        c->nsubmit++;
+        return holo_launch_project(c, c->H, c->V, c->k_lo, c->k_hi, c->tune[HOLO_TUNE_PROJ_COMPLEMENT], image_dev, st);
+    }
     if ((rc = submit_init(c))) return rc;
     c->push_ready = 0;
     const int s = (int)(c->nsubmit & 1);
@@ -629,6 +668,7 @@ extern "C" int holo_status(holo_ctx* c, int32_t status_host[4], holo_stream stre
 
 extern "C" int holo_launches_per_process(holo_ctx* c) {
     CHECK_CTX_QUIET(c);
+    if (c->mode == 2) return 2 /*sum + Gram, finish*/ + (holo_fresnel_launch_count(c) - 1) + 1 /*eig*/ + 1 /*project*/;
     return holo_fresnel_launch_count(c) + 2 /*cov partial + reduce*/ + 1 /*eig*/ + 1 /*project*/;
 }
 
@@ -651,6 +691,14 @@ extern "C" int holo_tune(holo_ctx* c, int key, int value) {
         c->prof_cls = new int[HOLO_PROF_CAP];
         for (int i = 0; i < 2 * HOLO_PROF_CAP; ++i) HOLO_CUDA_OK(cudaEventCreate(&c->prof_ev[i]));
         c->prof_n = 0;
+    }
+    if (key == HOLO_TUNE_L2_PERSIST_MB && value > 0) {
+        int maxb = 0;
+        HOLO_CUDA_OK(cudaDeviceGetAttribute(&maxb, cudaDevAttrMaxPersistingL2CacheSize, c->device));
+        size_t want = (size_t)value << 20;
+        if (want > (size_t)maxb) want = (size_t)maxb;
+        HOLO_CUDA_OK(cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, want));
+        fprintf(stderr, "holo_tune: persisting L2 set to %zu bytes (device maximum %d)\n", want, maxb);
     }
     if (key == HOLO_TUNE_COV_GRIDX && (value < 1 || value > c->cov_parts_cap)) { holo_set_error("cov grid out of range"); return HOLO_ERR_ARG; }
     c->tune[key] = value;

@@ -14,7 +14,7 @@ enum {
     HOLO_TUNE_FFT_GROUP = 0,     // frames per row/column pass group (scratch = group * 8*nx*ny bytes)
     HOLO_TUNE_COV_GRIDX = 1,     // covariance CTAs along pixels
     HOLO_TUNE_PROJ_COMPLEMENT = 2, // 1 = allow complement form in holo_process (default 1)
-    HOLO_TUNE_FFT_PERSISTENT = 3,  // 1 = single persistent fresnel kernel (default set at create)
+    HOLO_TUNE_FFT_PERSISTENT = 3,  // 2 = k_fresnel2 where supported (default), 1 = k_fresnel (single persistent kernel), 0 = separate launches
     HOLO_TUNE_EIG_MAX_SWEEPS = 4,
     HOLO_TUNE_PROFILE = 5,         // 1 = bracket every kernel launch with events (holo_profile_read)
     HOLO_TUNE_PROJ_TMA = 7,        // 1 = deflation projection fed by a TMA ring (default), 0 = register-streaming kernel
@@ -23,6 +23,7 @@ enum {
                                    // next covariance on the other SMs (memory-bound next to ALU-bound); 0 = in stream order
     HOLO_TUNE_PUSH_PIPE = 10,      // holo_push: 1 = pipelined ring form when T in {16,32,64} and n_new is a multiple of 8 (default)
     HOLO_TUNE_PUSH_INCR = 11,      // holo_push (ring form): 1 = recompute only the Gram rows / columns of the new frames (default)
+    HOLO_TUNE_L2_PERSIST_MB = 12,  // experiment: cudaLimitPersistingL2CacheSize in MiB (0 = leave the device setting alone)
     HOLO_TUNE_FFT_LAG = 6,         // frames between the row pass and the column pass in the fused kernel (0 = auto)
 };
 
@@ -63,6 +64,8 @@ struct holo_ctx {
     float2* C;
     float* evals;
     float2* V;
+    unsigned long long* gram_X;   // [128][128] int64 byte-plane Gram of the raw frames (mode 2, rawgram.cu)
+    int mode;               // 1: covariance from the hologram stack (Eq. 4 as written); 2: from the raw frames
     int32_t* status;        // [8], see HOLO_WS_STATUS
     int32_t* noconv_host;   // pinned, mapped host word: set by the eigensolver when it hits the sweep cap (device alias below)
     int32_t* noconv_dev;
@@ -127,7 +130,8 @@ struct HoloProf {
 
 // stage launchers (each only enqueues on `st`)
 int holo_launch_sum(holo_ctx* c, const uint16_t* frames, cudaStream_t st);
-int holo_launch_fresnel(holo_ctx* c, const uint16_t* frames, float2* H, cudaStream_t st, bool with_sum = true, int nproc = -1);
+int holo_launch_fresnel(holo_ctx* c, const uint16_t* frames, float2* H, cudaStream_t st, bool with_sum = true, int nproc = -1,
+                        bool counters_zeroed = false);
 // C == nullptr: partials only; holo_launch_cov_reduce then finishes (possibly on another stream, ordered after)
 int holo_launch_covariance(holo_ctx* c, const float2* H, float2* C, cudaStream_t st, bool real_only = false);
 int holo_launch_cov_reduce(holo_ctx* c, int nparts, float2* C, cudaStream_t st);
@@ -139,5 +143,10 @@ int holo_launch_eig(holo_ctx* c, const float2* C, float* evals, float2* V, cudaS
 int holo_launch_project(holo_ctx* c, const float2* H, const float2* V, int k_lo, int k_hi,
                         int allow_complement, float* image, cudaStream_t st, int center = 0);
 int holo_fresnel_launch_count(holo_ctx* c);
+// mode 2: S = sum_t I_t and C = nx ny D^T D from the raw frames (tcgen05 int8 Gram, rawgram.cu)
+int holo_launch_sum_gram(holo_ctx* c, const uint16_t* frames, float2* C, cudaStream_t st);
+// round-2 Fresnel kernel (fresnel2.cu): packed two-sequence FFT, TMA-staged column tiles; 1024 x 1024 frames
+bool holo_fresnel2_supported(const holo_ctx* c);
+int holo_launch_fresnel2(holo_ctx* c, const uint16_t* frames, float2* H, cudaStream_t st, int nproc);
 int holo_fft_plan_init(FftPlan* p, int N);
 void holo_fft_plan_free(FftPlan* p);

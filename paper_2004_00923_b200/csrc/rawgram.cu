@@ -1,0 +1,221 @@
+// rawgram.cu -- mode 2 (SURVEY.md 8(f)-2 stage 1, reading c-12): the covariance of Eq. 4 from the RAW
+// frames.  H_t = F[q d_t] with q unimodular and F unitary up to nx ny, so
+//     C_ts = sum_p conj(H_t(p)) H_s(p) = nx ny sum_x d_t(x) d_s(x),      d_t = I_t - mean_t I,
+// an exact identity.  With the integer frame sum S = sum_t I_t:  T^2 sum_x d_t d_s = T^2 G_ts - T (r_t + r_s) + tau,
+// G_ts = sum_x I_t I_s (the Gram of the raw uint16 frames), r_t = sum_s G_ts, tau = sum_t r_t -- all integers.
+//
+// G is a dense contraction over 10^6 pixels and runs on the 5th-generation tensor cores, EXACTLY: every uint16 pixel is
+// split into its two bytes, X = [hi_0 .. hi_{T-1}; lo_0 .. lo_{T-1}] (2T rows of u8, K = pixels), and
+// X X^T (tcgen05.mma kind::i8, u8 x u8 -> s32 accumulators in TMEM) holds the four blocks HH, HL, LH, LL with
+// G = 65536 HH + 256 (HL + LH) + LL.  One pass over the frames (2 T N_p bytes, the same read the temporal sum A0 needs):
+// the kernel also writes S.  No rounding anywhere before the final conversion of C to float.
+//   k_sum_gram   : persistent CTAs of 128 threads; a thread owns 2 adjacent pixels, loads them of all T frames, adds
+//                  them up (S) and writes their bytes into the K-major SWIZZLE_128B operand tile ([128 rows x 128 B] per 128
+//                  pixels, two tiles per stage, two stages); one thread issues the MMAs (M = 128, N = 64 or 128,
+//                  K = 32 per instruction) and commits them to the stage's mbarrier; the s32 accumulators are drained
+//                  (tcgen05.ld) into the global int64 byte-plane Gram with integer atomics before they can overflow
+//                  (every 16384 pixels) and at the end.
+//   k_gram_finish: one CTA assembles G (int64), centres it in __int128 and writes C (float2, Im = 0).
+#include "holo_internal.cuh"
+#include "tma.cuh"
+
+namespace {
+
+constexpr int RG_THREADS = 128;
+constexpr int RG_PIX = 2 * RG_THREADS;             // pixels per stage (two K tiles of 128 pixels)
+constexpr int RG_TILE = 128 * 128;                 // bytes of one operand tile: 128 rows x 128 B
+constexpr int RG_STAGE = 2 * RG_TILE;
+constexpr int RG_SMEM = 1024 + 2 * RG_STAGE + 64;
+constexpr int RG_FLUSH_ITERS = 64;                 // 64 x 256 pixels x 255^2 < 2^31
+
+__device__ __forceinline__ uint64_t make_sdesc(uint32_t saddr) {
+    // K-major, SWIZZLE_128B canonical layout: 8-row atoms of 1024 B (SBO = 1024), LBO = 16 B, descriptor version 1 (sm_100)
+    return (uint64_t)((saddr & 0x3FFFFu) >> 4) | ((uint64_t)1 << 16) | ((uint64_t)(1024 >> 4) << 32) | ((uint64_t)1 << 46) | ((uint64_t)2 << 61);
+}
+__device__ __forceinline__ void umma_i8(uint32_t tmem_d, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t accumulate) {
+    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+                 "tcgen05.mma.cta_group::1.kind::i8 [%0], %1, %2, %3, p;\n\t}"
+                 ::"r"(tmem_d), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate) : "memory");
+}
+__device__ __forceinline__ void umma_commit(uint64_t* bar) {
+    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+// 32 lanes x 32 bit, 16 consecutive columns: thread t of warp w gets row 32 w + t
+__device__ __forceinline__ void tmem_ld16(uint32_t taddr, int32_t* v) {
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
+                 : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
+                   "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
+                 : "r"(taddr));
+    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+}
+
+// frames uint16 [T][npix]; sum uint32 [npix]; X int64 [2 TP][2 TP], zeroed by the caller: the byte-plane Gram, summed over
+// all CTAs with 64-bit integer atomics (exact and order independent, hence deterministic); lower triangle only
+template <int TP>
+__global__ void __launch_bounds__(RG_THREADS, 3)
+k_sum_gram(const uint16_t* __restrict__ frames, uint32_t* __restrict__ sum, unsigned long long* __restrict__ X,
+           long long npix, int T, unsigned int* __restrict__ counters) {
+    constexpr int Tp = TP;
+    extern __shared__ unsigned char smraw_[];
+    const uint32_t s0 = smem_u32(smraw_);
+    const uint32_t pad = (1024u - (s0 & 1023u)) & 1023u;
+    unsigned char* base = smraw_ + pad;                       // 1024-byte aligned operand stages
+    const uint32_t sbase = s0 + pad;
+    uint64_t* mma_done = reinterpret_cast<uint64_t*>(base + 2 * RG_STAGE);
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(mma_done + 2);
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int N = 2 * Tp;                                     // MMA N (64 or 128); M = 128 always
+
+    if (blockIdx.x == 0 && tid < 2 * T + 1) counters[tid] = 0u;   // ticket / completion counters of the Fresnel kernel (as k_frame_sum)
+    // rows that no frame writes (t >= T within a plane, and rows >= 2 Tp) must read as zero: clear both stages once
+    for (int i = tid; i < 2 * RG_STAGE / 16; i += RG_THREADS) reinterpret_cast<uint4*>(base)[i] = make_uint4(0, 0, 0, 0);
+    if (tid == 0) {
+        mbar_init(mma_done + 0, 1); mbar_init(mma_done + 1, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    if (warp == 0) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(tmem_slot)), "r"(N) : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    }
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+    const uint32_t tmem = *tmem_slot;
+    const uint32_t idesc = (2u << 4) | ((uint32_t)(N >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);   // s32 += u8 x u8, K-major A and B
+
+    // operand tile addressing: pixel k of a tile, row r: byte (r / 8) * 1024 + (r % 8) * 128 + (((k / 16) ^ (r % 8)) * 16) + k % 16
+    const int ktile = tid >> 6;                               // which of the stage's two tiles the thread's pixels fall in
+    const int kin = (2 * tid) & 127;                          // first of its two pixels inside the tile
+    const long long nblocks = (npix + RG_PIX - 1) / RG_PIX;
+    uint32_t ph[2] = {0u, 0u};
+    int it = 0, pending[2] = {0, 0}, since_flush = 0;
+
+    auto drain = [&]() {                                      // accumulators -> int64 partial (all MMAs have completed)
+        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+        const int row = 32 * warp + lane;                     // TMEM lane = row of D
+        for (int c0 = 0; c0 < N; c0 += 16) {
+            int32_t v[16];
+            tmem_ld16(tmem + ((uint32_t)(32 * warp) << 16) + (uint32_t)c0, v);
+            if (row < N) {
+#pragma unroll
+                for (int j = 0; j < 16; ++j)
+                    if (c0 + j <= row && v[j] != 0) atomicAdd(X + (size_t)row * N + c0 + j, (unsigned long long)(long long)v[j]);
+            }
+        }
+        asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    };
+
+    for (long long blk = blockIdx.x; blk < nblocks; blk += gridDim.x, ++it) {
+        const int s = it & 1;
+        const long long p0 = blk * RG_PIX + 2 * tid;           // the thread's two pixels
+        const bool inb = p0 + 1 < npix;                        // npix is a multiple of 256 for every supported frame size
+        // the loads of this block are issued first (T in flight per thread)
+        uint32_t w[TP];
+#pragma unroll
+        for (int t = 0; t < TP; ++t) w[t] = (inb && t < T) ? __ldg(reinterpret_cast<const uint32_t*>(frames + (size_t)t * npix + p0)) : 0u;
+        if (pending[s]) { mbar_wait(mma_done + s, ph[s]); ph[s] ^= 1u; pending[s] = 0; }   // the MMAs that read this stage
+        unsigned char* tile = base + (size_t)s * RG_STAGE + (size_t)ktile * RG_TILE;
+        uint32_t sa = 0u, sb = 0u;
+#pragma unroll
+        for (int t = 0; t < TP; ++t) {
+            if (t >= T) break;
+            const uint32_t x = w[t];
+            sa += x & 0xffffu; sb += x >> 16;
+            const unsigned short lo = (unsigned short)__byte_perm(x, 0u, 0x4420) ;   // bytes (lo of pixel 0, lo of pixel 1)
+            const unsigned short hi = (unsigned short)__byte_perm(x, 0u, 0x4431);    // bytes (hi of pixel 0, hi of pixel 1)
+            const int rh = t, rl = Tp + t;
+            *reinterpret_cast<unsigned short*>(tile + (rh >> 3) * 1024 + (rh & 7) * 128 + ((((kin >> 4) ^ (rh & 7)) << 4) | (kin & 15))) = hi;
+            *reinterpret_cast<unsigned short*>(tile + (rl >> 3) * 1024 + (rl & 7) * 128 + ((((kin >> 4) ^ (rl & 7)) << 4) | (kin & 15))) = lo;
+        }
+        if (inb) *reinterpret_cast<uint2*>(sum + p0) = make_uint2(sa, sb);
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");     // the tensor core reads the tile through the async proxy
+        asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+        __syncthreads();
+        if (tid == 0) {
+            asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+            const uint32_t sa0 = sbase + (uint32_t)s * RG_STAGE;
+#pragma unroll
+            for (int kt = 0; kt < 2; ++kt)
+#pragma unroll
+                for (int k = 0; k < 4; ++k) {                  // K = 32 pixels per instruction: 32 bytes further into the 128-byte rows
+                    const uint64_t d = make_sdesc(sa0 + (uint32_t)kt * RG_TILE + (uint32_t)k * 32u);
+                    umma_i8(tmem, d, d, idesc, (since_flush | kt | k) ? 1u : 0u);
+                }
+            umma_commit(mma_done + s);
+        }
+        pending[s] = 1;
+        if (++since_flush == RG_FLUSH_ITERS) {                 // before the s32 accumulators can overflow
+            for (int q = 0; q < 2; ++q) if (pending[q]) { mbar_wait(mma_done + q, ph[q]); ph[q] ^= 1u; pending[q] = 0; }
+            drain();
+            __syncthreads();
+            since_flush = 0;
+        }
+    }
+    for (int q = 0; q < 2; ++q) if (pending[q]) { mbar_wait(mma_done + q, ph[q]); ph[q] ^= 1u; pending[q] = 0; }
+    if (since_flush) drain();
+    __syncthreads();
+    if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "r"(N) : "memory");
+}
+
+// X (lower triangle of the byte-plane Gram) -> G (exact) -> C = (nx ny / T^2) (T^2 G - T (r_t + r_s) + tau): the full
+// symmetric matrix, Im = 0.  G < 2^57 and r < 2^63 fit int64 for every supported size; the combination needs __int128.
+__global__ void __launch_bounds__(256) k_gram_finish(const unsigned long long* __restrict__ X, int T, int Tp, double scale,
+                                                     float2* __restrict__ C) {
+    __shared__ long long G[HOLO_MAX_T * HOLO_MAX_T];
+    __shared__ long long r[HOLO_MAX_T];
+    const int N = 2 * Tp;
+    auto Xs = [&](int i, int j) -> long long { return (long long)(i >= j ? X[(size_t)i * N + j] : X[(size_t)j * N + i]); };
+    for (int e = threadIdx.x; e < T * T; e += blockDim.x) {
+        const int t = e / T, s = e - t * T;
+        G[e] = Xs(t, s) * 65536 + (Xs(t, Tp + s) + Xs(Tp + t, s)) * 256 + Xs(Tp + t, Tp + s);
+    }
+    __syncthreads();
+    if (threadIdx.x < T) {
+        long long acc = 0;
+        for (int s = 0; s < T; ++s) acc += G[threadIdx.x * T + s];
+        r[threadIdx.x] = acc;
+    }
+    __syncthreads();
+    __int128 tau = 0;
+    for (int t = 0; t < T; ++t) tau += r[t];
+    for (int e = threadIdx.x; e < T * T; e += blockDim.x) {
+        const int t = e / T, s = e - t * T;
+        const __int128 v = (__int128)(T * T) * G[e] - (__int128)T * ((__int128)r[t] + r[s]) + tau;     // = T^2 sum_x d_t d_s, exact
+        const bool neg = v < 0;
+        const unsigned __int128 a = neg ? (unsigned __int128)(-v) : (unsigned __int128)v;
+        double dv = (double)(unsigned long long)(a >> 64) * 18446744073709551616.0 + (double)(unsigned long long)a;
+        if (neg) dv = -dv;
+        C[e] = make_float2((float)(dv * scale), 0.f);
+    }
+}
+
+}  // namespace
+
+// S = sum_t I_t (ctx->sum) and C = H^H H of the holograms these frames WOULD give, without forming them
+int holo_launch_sum_gram(holo_ctx* c, const uint16_t* frames, float2* C, cudaStream_t st) {
+    const int T = c->T, Tp = T <= 32 ? 32 : 64, N = 2 * Tp;
+    if (c->npix % RG_PIX != 0) { holo_set_error("raw-frame Gram needs nx*ny to be a multiple of %d", RG_PIX); return HOLO_ERR_ARG; }
+    const long long nblocks = c->npix / RG_PIX;
+    int grid = 3 * c->num_sms;                               // three CTAs per SM (64 KB of operand stages each)
+    if ((long long)grid > nblocks) grid = (int)nblocks;
+    int rc;
+    HOLO_CUDA_OK(cudaMemsetAsync(c->gram_X, 0, (size_t)N * N * sizeof(unsigned long long), st));
+    {
+        HoloProf prof(c, HOLO_K_SUM, st);
+        if (Tp == 32) {
+            if ((rc = holo_ensure_smem_attr((const void*)k_sum_gram<32>, c->device, RG_SMEM))) return rc;
+            k_sum_gram<32><<<grid, RG_THREADS, RG_SMEM, st>>>(frames, c->sum, c->gram_X, c->npix, T, c->counters);
+        } else {
+            if ((rc = holo_ensure_smem_attr((const void*)k_sum_gram<64>, c->device, RG_SMEM))) return rc;
+            k_sum_gram<64><<<grid, RG_THREADS, RG_SMEM, st>>>(frames, c->sum, c->gram_X, c->npix, T, c->counters);
+        }
+    }
+    HOLO_CUDA_OK(cudaGetLastError());
+    {
+        HoloProf prof(c, HOLO_K_COV_REDUCE, st);
+        k_gram_finish<<<1, 256, 0, st>>>(c->gram_X, T, Tp, (double)c->npix / ((double)T * (double)T), C);
+    }
+    HOLO_CUDA_OK(cudaGetLastError());
+    return HOLO_OK;
+}

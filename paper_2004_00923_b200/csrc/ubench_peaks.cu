@@ -5,6 +5,7 @@
 #include <cstdio>
 #include <cuda_runtime.h>
 #include <cstdint>
+#include <cuda.h>
 #define CK(x) do{cudaError_t e=(x); if(e!=cudaSuccess){printf("ERR %s line %d\n",cudaGetErrorString(e),__LINE__); return 1;}}while(0)
 #define LAUNCH_OK() CK(cudaGetLastError())     /* a launch that failed must not be timed as a success */
 template<int NACC>
@@ -95,6 +96,36 @@ __global__ void k_copy_loop(const uint4* __restrict__ in, uint4* __restrict__ ou
       uint4 a; asm volatile("ld.global.cg.v4.u32 {%0,%1,%2,%3}, [%4];":"=r"(a.x),"=r"(a.y),"=r"(a.z),"=r"(a.w):"l"(in+i));
       a.x+=r; out[i]=a; }
 }
+// ---- TMA throughput versus box row width: every CTA streams [rows x rowbytes] boxes (16 KB each, 4 in flight) of an
+// L2-resident tensor into shared memory (and back out with TMA stores when `store` is set)
+__device__ __forceinline__ uint32_t s_u32(const void* p){ return (uint32_t)__cvta_generic_to_shared(p); }
+__global__ void k_tma_rows(const __grid_constant__ CUtensorMap tm, int box_rows, int cols_boxes, int rows_boxes, int iters, int store){
+  extern __shared__ __align__(1024) unsigned char sm[];
+  uint64_t* bar = reinterpret_cast<uint64_t*>(sm + 4*16384);
+  if(threadIdx.x==0){ for(int s=0;s<4;s++){ asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;"::"r"(s_u32(bar+s))); } asm volatile("fence.mbarrier_init.release.cluster;":::"memory"); }
+  __syncthreads();
+  if(threadIdx.x!=0) return;
+  const int nboxes = cols_boxes*rows_boxes;
+  uint32_t ph[4]={0,0,0,0};
+  int issued=0, done=0; const int total=iters;
+  int b = blockIdx.x*37 % nboxes;
+  auto issue=[&](int s){
+    const int cb=b%cols_boxes, rb=b/cols_boxes; b+=gridDim.x; if(b>=nboxes) b-=nboxes;
+    if(store){ asm volatile("cp.async.bulk.tensor.2d.global.shared::cta.bulk_group [%0, {%1, %2}], [%3];"::"l"(&tm),"r"(cb*(16384/box_rows/4)),"r"(rb*box_rows),"r"(s_u32(sm+s*16384)):"memory"); asm volatile("cp.async.bulk.commit_group;":::"memory"); }
+    else { asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;"::"r"(s_u32(bar+s)),"r"(16384):"memory");
+      asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"::"r"(s_u32(sm+s*16384)),"l"(&tm),"r"(cb*(16384/box_rows/4)),"r"(rb*box_rows),"r"(s_u32(bar+s)):"memory"); }
+  };
+  for(;issued<4 && issued<total;issued++) issue(issued);
+  while(done<total){
+    const int s=done&3;
+    if(store){ asm volatile("cp.async.bulk.wait_group.read 3;":::"memory"); }
+    else { uint32_t ok; do{ asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}":"=r"(ok):"r"(s_u32(bar+s)),"r"(ph[s]):"memory"); }while(!ok); ph[s]^=1; }
+    done++;
+    if(issued<total){ issue(s); issued++; }
+  }
+  if(store) asm volatile("cp.async.bulk.wait_group 0;":::"memory");
+}
+typedef CUresult (*EncFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 int main(){
   int sms; cudaDeviceGetAttribute(&sms,cudaDevAttrMultiProcessorCount,0);
   float* out; CK(cudaMalloc(&out, 148*8*1024*4)); float* in; CK(cudaMalloc(&in,4096*4)); CK(cudaMemset(in,0,4096*4));
@@ -143,6 +174,21 @@ int main(){
     k_copy_loop<<<sms*4,512>>>(a,a+m,m,2); LAUNCH_OK(); cudaDeviceSynchronize();
     cudaEventRecord(e0); k_copy_loop<<<sms*4,512>>>(a,a+m,m,reps); LAUNCH_OK(); cudaEventRecord(e1); CK(cudaEventSynchronize(e1)); cudaEventElapsedTime(&ms,e0,e1);
     printf("L2 copy loop  %zu MiB -> %zu MiB x%d in one launch: %.1f GB/s (r+w)\n", mb, mb, reps, 2.0*nb*reps/ms/1e6);
+  }
+  {
+    void* fn=nullptr; cudaDriverEntryPointQueryResult q; CK(cudaGetDriverEntryPoint("cuTensorMapEncodeTiled",&fn,cudaEnableDefault,&q)); EncFn enc=(EncFn)fn;
+    CK(cudaFuncSetAttribute(k_tma_rows, cudaFuncAttributeMaxDynamicSharedMemorySize, 4*16384+64));
+    const int W=2048;                          // floats per tensor row (8 KB), 6144 rows = 48 MiB: fits L2
+    const int ROWS=6144;
+    for(int store=0; store<2; store++) for(int rowbytes: {32,64,128,256,1024}){
+      const int box_rows=16384/rowbytes; if(box_rows>256) continue;
+      alignas(64) CUtensorMap tm; cuuint64_t gd[2]={(cuuint64_t)W,(cuuint64_t)ROWS}, gs[1]={(cuuint64_t)W*4}; cuuint32_t bx[2]={(cuuint32_t)(rowbytes/4),(cuuint32_t)box_rows}, es[2]={1,1};
+      if(enc(&tm,CU_TENSOR_MAP_DATA_TYPE_FLOAT32,2,a,gd,gs,bx,es,CU_TENSOR_MAP_INTERLEAVE_NONE,CU_TENSOR_MAP_SWIZZLE_NONE,CU_TENSOR_MAP_L2_PROMOTION_NONE,CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE)!=CUDA_SUCCESS){ printf("encode failed\n"); continue; }
+      const int iters=2000;
+      k_tma_rows<<<sms,32,4*16384+64>>>(tm,box_rows,W*4/rowbytes,ROWS/box_rows,200,store); LAUNCH_OK(); CK(cudaDeviceSynchronize());
+      cudaEventRecord(e0); k_tma_rows<<<sms,32,4*16384+64>>>(tm,box_rows,W*4/rowbytes,ROWS/box_rows,iters,store); LAUNCH_OK(); cudaEventRecord(e1); CK(cudaEventSynchronize(e1)); cudaEventElapsedTime(&ms,e0,e1);
+      printf("TMA %s box [%3d rows x %4d B] (16 KB, 4 in flight per SM, L2-resident 48 MiB): %.1f GB/s, %.0f ns per box per SM\n", store?"store":"load ", box_rows, rowbytes, 16384.0*iters*sms/ms/1e6, ms*1e6/iters);
+    }
   }
   return 0;
 }

@@ -101,6 +101,75 @@ def test_covariance_parity_isolated(torch_cuda, T, npix_side):
     h.close()
 
 
+# ------------------------------------------------------------------ A3 from the raw frames (mode 2, tcgen05 int8 Gram)
+@pytest.mark.parametrize("n,T,full", [(16, 2, False), (32, 5, True), (64, 16, False), (128, 32, True), (64, 33, False), (64, 64, True),
+                                      (256, 47, False), (512, 32, False)])
+def test_raw_covariance_is_the_exact_integer_gram(torch_cuda, n, T, full):
+    """holo_raw_covariance: C = nx ny D^T D from the uint16 frames in exact integer arithmetic.
+    Checked against Python-integer sums (to the last float bit, up to the one final rounding) and against the oracle's
+    definition C = H^H H of the holograms; the frame sum it leaves behind is bit-exact."""
+    torch = torch_cuda
+    from tests.util import integer_gram
+    from paper_2004_00923_b200 import HOLO_WS_SUM
+    rng = np.random.default_rng(n * 3 + T)
+    fr = _rand_frames(rng, T, n, n, 0, 65536 if full else 4096)
+    if full:
+        fr[0, :, : n // 2] = 65535                           # long runs of the largest byte products
+    h = _holo(n, n, T, 1, T)
+    Cd = torch.empty((T, T), dtype=torch.complex64, device="cuda")
+    h.raw_covariance(_to_dev(torch, fr), Cd)
+    Cg = Cd.cpu().numpy()
+    Gi, _ = integer_gram(fr)                                  # sum_p (T I_t - S)(T I_s - S), exact
+    ref = np.array([[float(int(Gi[t, s]) * (n * n)) / float(T * T) for s in range(T)] for t in range(T)])
+    assert np.all(Cg.imag == 0)
+    assert np.array_equal(Cg.real, Cg.real.T)
+    assert np.max(np.abs(Cg.real.astype(np.float64) - ref)) <= 1.2e-7 * np.max(np.abs(ref)), "more than one rounding away from the exact Gram"
+    Co = oracle.covariance(oracle.fresnel(fr, LAM, PITCH, Z))
+    assert rel_l2(Cg, Co) <= FP32_C
+    S = h.workspace_tensor(HOLO_WS_SUM).cpu().numpy()
+    assert np.array_equal(S.astype(np.int64), fr.astype(np.int64).sum(0))
+    Cd2 = torch.empty_like(Cd)
+    h.raw_covariance(_to_dev(torch, fr), Cd2)
+    assert torch.equal(Cd.view(torch.float32), Cd2.view(torch.float32))       # integer atomics: order independent
+    h.close()
+
+
+@pytest.mark.parametrize("cfgn", [1, 3])
+def test_process_mode2_matches_oracle(torch_cuda, cfgn):
+    """Mode 2 of holo_process / holo_submit (covariance from the raw frames first, Fresnel stage and projection with V
+    known): same images as the oracle's path at BASELINE.json configs[0] and [2]."""
+    torch = torch_cuda
+    cfg = G.CONFIGS[cfgn]
+    if cfgn == 1:
+        fr = G.stack_np(cfg, 1)
+        dev = _to_dev(torch, fr)
+    else:
+        dev = G.stream_torch(cfg, 0, "cuda", n_frames=cfg.T)
+        fr = dev.cpu().view(torch.int16).numpy().view(np.uint16)
+    ev, gaps = eig_gaps(fr)
+    assert gaps[cfg.k_lo - 2] >= 0.05
+    h = _holo(cfg.n, cfg.n, cfg.T, cfg.k_lo, cfg.k_hi)
+    h.set_mode(2)
+    assert h.launches_per_process() == 5
+    M = torch.empty((cfg.n, cfg.n), dtype=torch.float32, device="cuda")
+    h.process(dev, M)
+    rc, st = h.status()
+    assert rc == 0, st
+    res, out = _compare_full(torch, cfg, fr, h, M.cpu().numpy())
+    assert res["M"] <= FP32_M and res["ev"] <= FP32_EV and res["C"] <= FP32_C and res["H"] <= FP32_H, res
+    # the streaming form: images complete in stream order, equal to the serial ones bit for bit
+    st2 = torch.cuda.Stream()
+    outs = [torch.zeros_like(M) for _ in range(3)]
+    torch.cuda.synchronize()
+    for o in outs:
+        h.submit(dev, o, st2)
+    st2.synchronize()
+    for o in outs:
+        assert torch.equal(o, M)
+    h.flush(st2)
+    h.close()
+
+
 # ------------------------------------------------------------------ A4 holo_eig (isolated)
 def _check_eig(torch, T, C64, k_gap=None):
     h = _holo(16, 16, T, 1, T)
