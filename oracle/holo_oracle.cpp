@@ -281,6 +281,44 @@ extern "C" int oracle_process(const uint16_t* frames, int nx, int ny, int T,
     return sw;
 }
 
+// Eq. 3: Hf = U Delta I_f V^{t*}; with H = U Delta V^{t*} this is Hf = (H V) I_f V^{t*}, written out in
+// that order: P = H V (Eq. 6, all k), components outside [k_lo,k_hi] dropped, Hf_t(p) = sum_k P_k(p) conj(V_{t,k}).
+extern "C" int oracle_svd_filter(const double* H_, long long n_pix, int T, const double* V_, int k_lo, int k_hi, double* Hf_) {
+    if (!H_ || !V_ || !Hf_ || T < 1 || n_pix < 0 || k_lo < 1 || k_hi > T || k_lo > k_hi) return -1;
+    std::vector<double> P((size_t)2 * T * n_pix);
+    if (oracle_project(H_, n_pix, T, V_, P.data())) return -1;
+    const cd* Pc = reinterpret_cast<const cd*>(P.data());
+    const cd* V = reinterpret_cast<const cd*>(V_);
+    cd* Hf = reinterpret_cast<cd*>(Hf_);
+#pragma omp parallel for schedule(static)
+    for (int t = 0; t < T; ++t)
+        for (long long p = 0; p < n_pix; ++p) {
+            cd acc(0, 0);
+            for (int k = k_lo; k <= k_hi; ++k) acc += Pc[(long long)(k - 1) * n_pix + p] * std::conj(V[t * T + (k - 1)]);
+            Hf[(long long)t * n_pix + p] = acc;
+        }
+    return 0;
+}
+
+// division of an image by its spatial average.
+extern "C" int oracle_normalize(const double* M, long long n_pix, double* out) {
+    if (!M || !out || n_pix < 1) return -1;
+    long double acc = 0.0L;
+    for (long long p = 0; p < n_pix; ++p) acc += M[p];
+    const double mean = (double)(acc / (long double)n_pix);
+    for (long long p = 0; p < n_pix; ++p) out[p] = (mean != 0.0) ? M[p] / mean : M[p];
+    return 0;
+}
+
+// Quadrant swap (zero-frequency bin to the centre), written as the index map.
+extern "C" int oracle_fftshift(const double* in, int ny, int nx, double* out) {
+    if (!in || !out || nx < 1 || ny < 1) return -1;
+    for (int j = 0; j < ny; ++j)
+        for (int i = 0; i < nx; ++i)
+            out[(size_t)((j + ny / 2) % ny) * nx + (size_t)((i + nx / 2) % nx)] = in[(size_t)j * nx + i];
+    return 0;
+}
+
 extern "C" int oracle_num_threads(void) {
 #ifdef _OPENMP
     return omp_get_max_threads();

@@ -16,6 +16,9 @@
  *   Hc    = H V I_f                                         (Eq. 6)
  *   M     = sum_{k in [k_lo,k_hi]} |Hc_k|^2                 (Eq. 7)
  *   Ht    = H W I_f,  M0 = sum |Ht|^2                       (Eq. 8-9)
+ *   Hf    = U Delta I_f V^{t*} = H V I_f V^{t*}             (Eq. 3: SVD filter)
+ *   Mn    = M / <M>   (division by the spatial average)
+ *   shift = quadrant swap of an image in FFT-bin order      (display convention, R6)
  *
  * Pins (tests/test_oracle_*.py, all "-m not gpu"): brute-force DFT, Parseval, point-source
  * closed forms, exact integer Gram, 2x2 closed form, T=2 closed form, LAPACK eigh/svd on tiny
@@ -72,6 +75,17 @@ int oracle_dft_basis(int T, double* W);
 int oracle_process(const uint16_t* frames, int nx, int ny, int T,
                    double lambda_m, double pitch_m, double z_m, int k_lo, int k_hi,
                    double* M, double* H_out, double* C_out, double* evals_out, double* V_out);
+
+/* Eq. 3: Hf = H V I_f V^{t*}: project on all components, keep k_lo..k_hi (1-based inclusive,
+ * descending order), come back to the frame basis.  Hf complex [T][n_pix]. */
+int oracle_svd_filter(const double* H, long long n_pix, int T, const double* V, int k_lo, int k_hi, double* Hf);
+
+/* PAPER.md:86 ("image normalization by their respective average value"): out(p) = M(p) / ((1/n_pix) sum_p M(p)).
+ * A zero image is returned unchanged. */
+int oracle_normalize(const double* M, long long n_pix, double* out);
+
+/* Quadrant swap: out[(j + ny/2) mod ny][(i + nx/2) mod nx] = in[j][i]  (zero frequency to the centre). */
+int oracle_fftshift(const double* in, int ny, int nx, double* out);
 
 int oracle_num_threads(void);
 

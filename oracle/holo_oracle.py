@@ -38,6 +38,9 @@ def _lib():
         L.oracle_project.argtypes = [dp, C.c_longlong, ip, dp, dp]
         L.oracle_envelope.argtypes = [dp, C.c_longlong, ip, ip, ip, dp]
         L.oracle_dft_basis.argtypes = [ip, dp]
+        L.oracle_svd_filter.argtypes = [dp, C.c_longlong, ip, dp, ip, ip, dp]
+        L.oracle_normalize.argtypes = [dp, C.c_longlong, dp]
+        L.oracle_fftshift.argtypes = [dp, ip, ip, dp]
         L.oracle_process.argtypes = [u16p, ip, ip, ip, C.c_double, C.c_double, C.c_double, ip, ip, dp, dp, dp, dp, dp]
     return _LIB
 
@@ -136,6 +139,31 @@ def dft_basis(T):
     W = np.empty((T, T), np.complex128)
     _chk(_lib().oracle_dft_basis(T, _d(W)))
     return W
+
+
+def svd_filter(H, V, k_lo, k_hi):
+    """Eq. 3: Hf = H V I_f V^H, complex128 with H's shape."""
+    H = np.ascontiguousarray(H, dtype=np.complex128)
+    V = np.ascontiguousarray(V, dtype=np.complex128)
+    T = H.shape[0]
+    Hf = np.empty_like(H)
+    _chk(_lib().oracle_svd_filter(_d(H), H.size // T, T, _d(V), k_lo, k_hi, _d(Hf)))
+    return Hf
+
+
+def normalize(M):
+    """image divided by its spatial average."""
+    M = np.ascontiguousarray(M, dtype=np.float64)
+    out = np.empty_like(M)
+    _chk(_lib().oracle_normalize(_d(M), M.size, _d(out)))
+    return out
+
+
+def fftshift(M):
+    M = np.ascontiguousarray(M, dtype=np.float64)
+    out = np.empty_like(M)
+    _chk(_lib().oracle_fftshift(_d(M), M.shape[0], M.shape[1], _d(out)))
+    return out
 
 
 def process(frames, lam, pitch, z, k_lo, k_hi, want_H=False):

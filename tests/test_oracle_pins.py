@@ -292,3 +292,53 @@ def test_generator_refocuses_inside_vessel_mask():
     assert inside / outside > 1.5
     mirror = np.roll(scene.mask[::-1, ::-1], (1, 1), (0, 1))           # x -> -x mod n
     assert M[mirror].mean() / M[~mirror].mean() < 1.15
+
+
+# ---------------------------------------------------------------- Eq. 3 SVD filter, normalisation (:86), fftshift
+def test_svd_filter_matches_library_svd_eq3():
+    """Eq. 3 literally: H = U Delta V^H (LAPACK, on H as an n_pix x T matrix), Hf = U Delta I_f V^H."""
+    rs = np.random.default_rng(7)
+    T, n = 6, 40
+    H = rs.standard_normal((T, n)) + 1j * rs.standard_normal((T, n))
+    ev, V, _ = oracle.eig(oracle.covariance(H))
+    U, sv, Vh = np.linalg.svd(H.T, full_matrices=False)          # H.T: rows = pixels, columns = frames
+    for k_lo, k_hi in ((1, T), (2, T), (2, 4), (3, 3)):
+        keep = np.zeros(T)
+        keep[k_lo - 1:k_hi] = 1.0                                 # singular values come in descending order too
+        ref = ((U * (sv * keep)) @ Vh).T
+        assert rel_l2(oracle.svd_filter(H, V, k_lo, k_hi), ref) <= 1e-10, (k_lo, k_hi)
+
+
+def test_svd_filter_identities():
+    rs = np.random.default_rng(8)
+    T, n = 8, 64
+    H = rs.standard_normal((T, n)) + 1j * rs.standard_normal((T, n))
+    ev, V, _ = oracle.eig(oracle.covariance(H))
+    assert rel_l2(oracle.svd_filter(H, V, 1, T), H) <= 1e-12       # I_f = identity: nothing is removed
+    Hf = oracle.svd_filter(H, V, 3, 6)
+    M = oracle.envelope(oracle.project(H, V), 3, 6)
+    assert rel_l2((np.abs(Hf) ** 2).sum(axis=0), M) <= 1e-12       # frame-basis energy = component energy (V unitary)
+    # idempotent, and the two complementary filters add up to H
+    assert rel_l2(oracle.svd_filter(Hf, V, 3, 6), Hf) <= 1e-12
+    rest = oracle.svd_filter(H, V, 1, 2) + oracle.svd_filter(H, V, 7, 8)
+    assert rel_l2(Hf + rest, H) <= 1e-12
+
+
+def test_normalize_mean_is_one_and_zero_image():
+    rs = np.random.default_rng(9)
+    M = rs.random((12, 20)) * 5 + 0.1
+    out = oracle.normalize(M)
+    assert abs(out.mean() - 1.0) <= 1e-14
+    assert rel_l2(out * M.sum() / M.size, M) <= 1e-14              # a pure rescaling
+    assert abs(oracle.normalize(3.0 * M) - out).max() <= 1e-14      # scale invariant
+    assert not np.any(oracle.normalize(np.zeros((4, 4))))
+
+
+def test_fftshift_matches_numpy_and_centres_dc():
+    rs = np.random.default_rng(10)
+    for shape in ((8, 8), (4, 16), (16, 2)):
+        M = rs.random(shape)
+        assert np.array_equal(oracle.fftshift(M), np.fft.fftshift(M))
+    a = np.abs(oracle.fft2(np.ones((8, 16)) + 0j)) ** 2             # all energy in bin (0, 0)
+    s = oracle.fftshift(a)
+    assert s[4, 8] == a[0, 0] and s.sum() == a[0, 0]
