@@ -178,6 +178,22 @@ int holo_project(holo_ctx* ctx, const void* H_dev, const void* V_dev, float* ima
  * w_mn = exp(-2 i pi (m-1)(n-1)/T)/sqrt(T), n1..n2 1-based inclusive (paper: 8..24 of 32). */
 int holo_fourier_demod(holo_ctx* ctx, const void* H_dev, int n1, int n2, float* image_dev, holo_stream stream);
 
+/* SVD filter (Eq. 3): Hf = U Delta I_f V^{t*} = H V I_f V^{t*} with the handle's current (k_lo,k_hi):
+ * Hf_t(p) = sum_{k=k_lo}^{k_hi} P_k(p) conj(V_{t,k}), the hologram stack with the rejected components removed, back in the
+ * frame basis (the input of the paper's downstream short-time Fourier analysis).  H_dev, Hf_dev float2 [T][ny][nx]
+ * (Hf_dev == H_dev is allowed), V_dev float2 [T][T] as written by holo_eig (any matrix is accepted; the identity
+ * sum_t |Hf_t|^2 = image of holo_project holds for unitary V).  Evaluated as Hf = H F with the T x T matrix F = V I_f V^{t*}. */
+int holo_svd_filter(holo_ctx* ctx, const void* H_dev, const void* V_dev, void* Hf_dev, holo_stream stream);
+
+/* Image normalisation of PAPER.md:86 ("image normalization by their respective average value"): image <- image / mean(image),
+ * in place, image_dev float [ny][nx].  The mean is a fixed-order FP64 reduction (bit-reproducible); an all-zero image is
+ * left unchanged.  Two small kernels on `stream`. */
+int holo_normalize(holo_ctx* ctx, float* image_dev, holo_stream stream);
+
+/* Quadrant swap of an image in FFT-bin order: out[(j + ny/2) mod ny][(i + nx/2) mod nx] = in[j][i] (zero frequency to the
+ * centre; R6: every other call leaves images in raw FFT-bin order).  Out of place: in_dev != out_dev. */
+int holo_fftshift(holo_ctx* ctx, const float* in_dev, float* out_dev, holo_stream stream);
+
 /* Change the component window (1-based inclusive, descending order).  Takes effect at the next call; an image still
  * owed by an earlier holo_submit keeps the window of its own submit call.  While a holo_push sequence is open the
  * new window must keep the deflation form available (HOLO_ERR_STATE otherwise). */

@@ -10,7 +10,7 @@ HOLO_WS_SUM, HOLO_WS_H, HOLO_WS_C, HOLO_WS_EVALS, HOLO_WS_V, HOLO_WS_STATUS, HOL
 
 EXPORTED_SYMBOLS = [
     "holo_create", "holo_destroy", "holo_process", "holo_submit", "holo_flush", "holo_submit_host", "holo_flush_host", "holo_push", "holo_process_host", "holo_fresnel", "holo_covariance",
-    "holo_raw_covariance", "holo_set_mode", "holo_eig", "holo_project", "holo_fourier_demod", "holo_set_range", "holo_set_assume_unitary",
+    "holo_raw_covariance", "holo_set_mode", "holo_eig", "holo_project", "holo_fourier_demod", "holo_svd_filter", "holo_normalize", "holo_fftshift", "holo_set_range", "holo_set_assume_unitary",
     "holo_workspace", "holo_workspace_copy", "holo_status", "holo_launches_per_process", "holo_tune", "holo_profile_read", "holo_fft_group",
     "holo_last_error", "holo_version",
 ]
@@ -55,6 +55,9 @@ def load_library():
     L.holo_eig.argtypes = [vp, vp, vp, vp, vp]
     L.holo_project.argtypes = [vp, vp, vp, vp, vp]
     L.holo_fourier_demod.argtypes = [vp, vp, ip, ip, vp, vp]
+    L.holo_svd_filter.argtypes = [vp, vp, vp, vp, vp]
+    L.holo_normalize.argtypes = [vp, vp, vp]
+    L.holo_fftshift.argtypes = [vp, vp, vp, vp]
     L.holo_set_range.argtypes = [vp, ip, ip]
     L.holo_set_assume_unitary.argtypes = [vp, ip]
     L.holo_workspace.restype = vp
@@ -149,6 +152,15 @@ class Holo:
 
     def fourier_demod(self, H_dev, n1, n2, image_dev, stream=None):
         self._chk(self._L.holo_fourier_demod(self._h, self._p(H_dev), n1, n2, self._p(image_dev), _stream_ptr(stream)))
+
+    def svd_filter(self, H_dev, V_dev, Hf_dev, stream=None):
+        self._chk(self._L.holo_svd_filter(self._h, self._p(H_dev), self._p(V_dev), self._p(Hf_dev), _stream_ptr(stream)))
+
+    def normalize(self, image_dev, stream=None):
+        self._chk(self._L.holo_normalize(self._h, self._p(image_dev), _stream_ptr(stream)))
+
+    def fftshift(self, in_dev, out_dev, stream=None):
+        self._chk(self._L.holo_fftshift(self._h, self._p(in_dev), self._p(out_dev), _stream_ptr(stream)))
 
     def set_range(self, k_lo, k_hi):
         self._chk(self._L.holo_set_range(self._h, k_lo, k_hi))

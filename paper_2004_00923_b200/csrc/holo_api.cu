@@ -73,7 +73,7 @@ static int build_chirp(float2** dst, int n, double lambda_m, double pitch_m, dou
 
 static void free_ctx(holo_ctx* c) {
     if (!c) return;
-    cudaFree(c->qx); cudaFree(c->qy); cudaFree(c->qxs); cudaFree(c->Wdft);
+    cudaFree(c->qx); cudaFree(c->qy); cudaFree(c->qxs); cudaFree(c->Wdft); cudaFree(c->Fmat); cudaFree(c->norm_partials);
     holo_fft_plan_free(&c->px); holo_fft_plan_free(&c->py);
     cudaFree(c->sum); cudaFree(c->scratch); cudaFree(c->H); cudaFree(c->cov_partials);
     cudaFree(c->C); cudaFree(c->evals); cudaFree(c->V); cudaFree(c->status);
@@ -153,6 +153,8 @@ static int create_impl(holo_ctx* c) {
     HOLO_CUDA_OK(cudaMalloc(&c->status, 8 * sizeof(int32_t)));
     HOLO_CUDA_OK(cudaMalloc(&c->counters, 1024 * sizeof(unsigned int)));
     HOLO_CUDA_OK(cudaMalloc(&c->gram_X, 128 * 128 * sizeof(unsigned long long)));
+    HOLO_CUDA_OK(cudaMalloc(&c->Fmat, (size_t)T * T * sizeof(float2)));
+    HOLO_CUDA_OK(cudaMalloc(&c->norm_partials, HOLO_NORM_PARTS * sizeof(double)));
     c->mode = 1;
     HOLO_CUDA_OK(cudaMemset(c->status, 0, 8 * sizeof(int32_t)));
     HOLO_CUDA_OK(cudaMemset(c->counters, 0, 1024 * sizeof(unsigned int)));
@@ -242,6 +244,23 @@ extern "C" int holo_fourier_demod(holo_ctx* c, const void* H_dev, int n1, int n2
     if (n1 < 1 || n2 > c->T || n1 > n2) { holo_set_error("need 1 <= n1 <= n2 <= T"); return HOLO_ERR_ARG; }
     if (((uintptr_t)H_dev & 15) || ((uintptr_t)image_dev & 7)) { holo_set_error("H_dev must be 16-byte and image_dev 8-byte aligned"); return HOLO_ERR_ARG; }
     return holo_launch_project(c, (const float2*)H_dev, c->Wdft, n1, n2, /*W is unitary*/ 1, image_dev, (cudaStream_t)stream);
+}
+
+extern "C" int holo_svd_filter(holo_ctx* c, const void* H_dev, const void* V_dev, void* Hf_dev, holo_stream stream) {
+    CHECK_CTX(c); CHECK_PTR(H_dev, "H_dev"); CHECK_PTR(V_dev, "V_dev"); CHECK_PTR(Hf_dev, "Hf_dev");
+    if (((uintptr_t)H_dev & 7) || ((uintptr_t)Hf_dev & 7)) { holo_set_error("H_dev and Hf_dev must be 8-byte aligned"); return HOLO_ERR_ARG; }
+    return holo_launch_svd_filter(c, (const float2*)H_dev, (const float2*)V_dev, c->k_lo, c->k_hi, (float2*)Hf_dev, (cudaStream_t)stream);
+}
+
+extern "C" int holo_normalize(holo_ctx* c, float* image_dev, holo_stream stream) {
+    CHECK_CTX(c); CHECK_PTR(image_dev, "image_dev");
+    return holo_launch_normalize(c, image_dev, (cudaStream_t)stream);
+}
+
+extern "C" int holo_fftshift(holo_ctx* c, const float* in_dev, float* out_dev, holo_stream stream) {
+    CHECK_CTX(c); CHECK_PTR(in_dev, "in_dev"); CHECK_PTR(out_dev, "out_dev");
+    if (in_dev == out_dev) { holo_set_error("holo_fftshift works out of place: in_dev == out_dev"); return HOLO_ERR_ARG; }
+    return holo_launch_fftshift(c, in_dev, out_dev, (cudaStream_t)stream);
 }
 
 static int project_pending(holo_ctx* c, cudaStream_t st);

@@ -8,6 +8,7 @@
 
 #define HOLO_MAX_T 64
 #define HOLO_NUM_TUNE 16
+#define HOLO_NORM_PARTS 1024
 
 // tuning keys (holo_tune); not part of the stable ABI
 enum {
@@ -53,6 +54,8 @@ struct holo_ctx {
     float2* qxs;            // qx / T (the mean-subtraction scale folded into the row-pass prologue)
     FftPlan px, py;
     float2* Wdft;           // Eq. 8 DFT basis [T][T]
+    float2* Fmat;           // [T][T] filter matrix V I_f V^H of holo_svd_filter (Eq. 3)
+    double* norm_partials;  // [HOLO_NORM_PARTS] partial sums of holo_normalize
     // workspace
     uint32_t* sum;          // [ny][nx]
     float2* scratch;        // FFT row->column intermediate, fft_group frames
@@ -143,6 +146,10 @@ int holo_launch_eig(holo_ctx* c, const float2* C, float* evals, float2* V, cudaS
 int holo_launch_project(holo_ctx* c, const float2* H, const float2* V, int k_lo, int k_hi,
                         int allow_complement, float* image, cudaStream_t st, int center = 0);
 int holo_fresnel_launch_count(holo_ctx* c);
+// display.cu: PAPER.md:86 normalisation, quadrant swap, Eq. 3 SVD filter
+int holo_launch_normalize(holo_ctx* c, float* image, cudaStream_t st);
+int holo_launch_fftshift(holo_ctx* c, const float* in, float* out, cudaStream_t st);
+int holo_launch_svd_filter(holo_ctx* c, const float2* H, const float2* V, int k_lo, int k_hi, float2* Hf, cudaStream_t st);
 // mode 2: S = sum_t I_t and C = nx ny D^T D from the raw frames (tcgen05 int8 Gram, rawgram.cu)
 int holo_launch_sum_gram(holo_ctx* c, const uint16_t* frames, float2* C, cudaStream_t st);
 // round-2 Fresnel kernel (fresnel2.cu): packed two-sequence FFT, TMA-staged column tiles; 1024 x 1024 frames

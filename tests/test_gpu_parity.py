@@ -267,6 +267,58 @@ def test_fourier_demod_eq8(torch_cuda):
     h.close()
 
 
+# ------------------------------------------------------------------ Eq. 3 SVD filter, PAPER.md:86 normalisation, fftshift
+@pytest.mark.parametrize("T,n,k_lo,k_hi", [(32, 64, 2, 32), (32, 64, 13, 32), (16, 128, 1, 16), (7, 32, 3, 5), (64, 32, 3, 64)])
+def test_svd_filter_eq3(torch_cuda, T, n, k_lo, k_hi):
+    torch = torch_cuda
+    rng = np.random.default_rng(100 + T + k_lo)
+    H32 = (rng.standard_normal((T, n, n)) + 1j * rng.standard_normal((T, n, n))).astype(np.complex64)
+    H64 = H32.astype(np.complex128)
+    _, V, _ = oracle.eig(oracle.covariance(H64))
+    V32 = V.astype(np.complex64)
+    h = _holo(n, n, T, k_lo, k_hi)
+    Hd = _to_dev(torch, H32)
+    Hf = torch.empty_like(Hd)
+    h.svd_filter(Hd, _to_dev(torch, V32), Hf)
+    ref = oracle.svd_filter(H64, V32.astype(np.complex128), k_lo, k_hi)      # the same (rounded) V on both sides
+    err = rel_l2(Hf.cpu().numpy(), ref)
+    assert err <= TOL_STAGE and err <= FP32_H, err
+    # in place, and the frame-basis energy of Hf is the image of holo_project (R12 identity, unitary V)
+    h.svd_filter(Hd, _to_dev(torch, V32), Hd)
+    assert torch.equal(Hd.view(torch.float32), Hf.view(torch.float32))
+    M = torch.empty((n, n), dtype=torch.float32, device="cuda")
+    h.project(_to_dev(torch, H32), _to_dev(torch, V32), M)
+    E = (Hf.abs().double() ** 2).sum(dim=0)
+    assert rel_l2(E.cpu().numpy(), M.cpu().numpy()) <= 5e-5
+    h.close()
+
+
+@pytest.mark.parametrize("nx,ny", [(16, 16), (64, 256), (1024, 1024)])
+def test_normalize_and_fftshift(torch_cuda, nx, ny):
+    torch = torch_cuda
+    rng = np.random.default_rng(nx + ny)
+    M = (rng.random((ny, nx)) * 1e9 + 1e7).astype(np.float32)                # the magnitude of a real PCA image
+    h = _holo(nx, ny, 2, 1, 2)
+    Md = _to_dev(torch, M)
+    h.normalize(Md)
+    ref = oracle.normalize(M.astype(np.float64))
+    out = Md.cpu().numpy()
+    assert rel_l2(out, ref) <= 2e-7                                          # one rounding of the scale, one of the product
+    assert abs(out.astype(np.float64).mean() - 1.0) <= 1e-6
+    Md2 = _to_dev(torch, M)
+    h.normalize(Md2)
+    assert torch.equal(Md, Md2)                                              # fixed-order reduction: bit-reproducible
+    Z0 = torch.zeros((ny, nx), dtype=torch.float32, device="cuda")
+    h.normalize(Z0)
+    assert not bool(Z0.any())                                                # zero image: unchanged, no NaN
+    S = torch.empty_like(Md)
+    h.fftshift(Md, S)
+    assert np.array_equal(S.cpu().numpy(), oracle.fftshift(out.astype(np.float64)).astype(np.float32))   # pure permutation: bit-exact
+    with pytest.raises(Exception):
+        h.fftshift(Md, Md)
+    h.close()
+
+
 # ------------------------------------------------------------------ chained holo_process
 def _process_and_compare(torch, cfg, fr, k_lo, k_hi, complement=1):
     from paper_2004_00923_b200 import HOLO_WS_EVALS, HOLO_WS_V, HOLO_WS_C
