@@ -159,7 +159,19 @@ int holo_raw_covariance(holo_ctx* ctx, const uint16_t* frames_dev, void* C_dev, 
  * the covariance of the hologram stack).  2: holo_raw_covariance + eigensolver FIRST, then the Fresnel stage and the
  * projection with V already known -- the hologram stack is read once instead of twice (20 T N_p + 12 N_p compulsory
  * bytes instead of 28 T N_p + 12 N_p), and in holo_submit the image is complete in stream order when the call's work
- * is done.  Same results up to FP32 rounding of C.  holo_push always works as in mode 1. */
+ * is done.  Same results up to FP32 rounding of C.
+ * 3 (SURVEY.md 8(f)-2 stage 2): mode 2's covariance and eigenvectors, then the image WITHOUT a hologram stack.  With V real
+ * (the covariance of the raw frames is real symmetric) the deflation of DESIGN.md R12 commutes with the transform:
+ *     M = sum_{k in S} |P_k|^2 = sum_t | FFT2[ q (d_t - sum_{k not in S} e_k V_tk) ] |^2,     e_k = sum_t d_t V_tk,
+ * so the rejected components are removed from the RAW frames (one small pass writes the images e_k, at most 4 of them:
+ * k_lo - 1 + T - k_hi <= 4, else HOLO_ERR_STATE), the row pass writes its output once (8 T N_p bytes, the only large
+ * intermediate), and the column pass is reduced to sum_t |.|^2 in registers: no hologram stack is written, the projection
+ * kernel and its read of the stack disappear.  No cancellation (the subtraction happens before the transform, on integers
+ * of at most 2^22).  HOLO_WS_H is not filled in this mode.  holo_submit in mode 3 is pipelined by one stack (the covariance
+ * of stack i and its eigensolver on the side stream run with the image of stack i-1): the image of submit(i) is complete
+ * after the next holo_submit or holo_flush, and frames_dev of submit(i) is READ AGAIN by that next call -- keep it valid
+ * and unchanged until then (holo_submit_host does this for you).  First use allocates 13 N_p floats (may synchronise).
+ * holo_push always works as in mode 1. */
 int holo_set_mode(holo_ctx* ctx, int mode);
 
 /* A4: any Hermitian C_dev (only its lower triangle t >= s and real diagonal are read) ->

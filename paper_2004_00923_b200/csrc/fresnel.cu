@@ -7,6 +7,7 @@
 #include "fft_reg.cuh"
 #include <math.h>
 #include <vector>
+#include <type_traits>
 
 // ------------------------------------------------------------------------------------------------
 // A0: per-pixel temporal sum  S(p) = sum_t I_t(p)   (uint32: exact, T*65535 < 2^32)
@@ -53,6 +54,10 @@ struct FftArgs {
     int tiles_per_frame;      // nseq / B
     int ntiles;               // nf * tiles_per_frame
     int T;
+    // raw-domain deflation (mode 3, DEFL prologue): d'_t = (T I_t - S) - sum_k eT_k V_{t,k}
+    const float* defl_img;    // [ndefl][ny][nx]  eT_k = sum_t (T I_t - S) V_{t,k} of the rejected components
+    const float* defl_coef;   // [T][ndefl]       V_{t,k} (real: C is real symmetric there, R21)
+    int ndefl;
 };
 
 // one tile = B sequences of one frame; in_foff / out_foff = element offset of the frame in a.in(frames) / a.out
@@ -61,15 +66,19 @@ struct NoHook { __device__ __forceinline__ void operator()() const {} };
 // `mid` is called once by every thread in the middle of the tile (after the pass-0 butterflies; the fused
 // kernel does its scheduling work there, when the stores of the previous tile have long drained)
 // LDC: row pitch in elements known at compile time (0: use a.ld) -- turns every address into base + immediate
-template <int N, int E, int R1, int R2, int B, bool COL, bool PRO, int LDC = 0, class Mid = NoHook>
+// DEFL: the prologue also removes the rejected components in the raw domain (frame index `frame` selects the V row).
+// ENERGY: nothing is stored; |X|^2 of output slot s (the s-th value this thread would store, see tile_out_offset) is added
+// to acc[s] instead.
+template <int N, int E, int R1, int R2, int B, bool COL, bool PRO, int LDC = 0, class Mid = NoHook, bool DEFL = false, bool ENERGY = false>
 __device__ __forceinline__ void fft_tile(const FftArgs& a, long long in_foff, long long out_foff, int tile_in_frame, float2* sm,
-                                         Mid mid = Mid()) {
+                                         Mid mid = Mid(), int frame = 0, float* acc = nullptr) {
     constexpr int TPS = N / E;
     constexpr int PADN = N + N / E;
     constexpr bool MULTI = (R1 > 1);
     // a row whose N/E threads are exactly one warp is exchanged through that warp's private slice of the buffer:
     // warp-level synchronisation only (the eight warps of a row tile then run freely against each other)
     constexpr bool WARP_SEQ = !COL && (N / E == 32);
+    constexpr bool FREE_RUN = std::is_same<Mid, NoHook>::value;
     auto sync_tile = [&]() { if constexpr (WARP_SEQ) __syncwarp(); else __syncthreads(); };
     const int tid = threadIdx.x;
     const int j = COL ? tid / B : tid % TPS;
@@ -88,20 +97,50 @@ __device__ __forceinline__ void fft_tile(const FftArgs& a, long long in_foff, lo
         const uint64_t pol_in = (FUSED && COL) ? l2_evict_last() : l2_evict_first();
         const uint64_t pol_out = (FUSED && !COL) ? l2_evict_last() : l2_evict_first();
         auto store = [&](float2* q, float2 val) { if constexpr (FUSED) st_hint(q, val, pol_out); else *q = val; };
+        // output slot `slot` of this thread: element offset `off` (in units of estride) from op
+        auto emit = [&](int slot, float2* op_, int off, float2 val) {
+            if constexpr (ENERGY) acc[slot] = fmaf(val.x, val.x, fmaf(val.y, val.y, acc[slot]));
+            else store(op_ + off * estride, val);
+        };
         float2 v[E];
         // ---------------- pass 0: radix E, Ns = 1, inputs straight from global
         if constexpr (PRO) {
             const float2 qyv = __ldg(a.qy + s0);
             const uint16_t* fr = a.frames + ibase;
             const uint32_t* sp = a.sum + (long long)s0 * ld;
+            if constexpr (!DEFL) {
 #pragma unroll
-            for (int r = 0; r < E; ++r) {
-                const int i = j + r * TPS;
-                const int I = FUSED ? ldnc_u16_hint(fr + i, pol_in) : (int)__ldg(fr + i);
-                const int S = (int)__ldg(sp + i);
-                const float d = (float)(a.T * I - S);                  // exact integer; the 1/T lives in the qx table
-                const float2 q = cmul(__ldg(a.qx + i), qyv);
-                v[r] = make_float2(d * q.x, d * q.y);
+                for (int r = 0; r < E; ++r) {
+                    const int i = j + r * TPS;
+                    const int I = FUSED ? ldnc_u16_hint(fr + i, pol_in) : (int)__ldg(fr + i);
+                    const int S = (int)__ldg(sp + i);
+                    const float d = (float)(a.T * I - S);                  // exact integer; the 1/T lives in the qx table
+                    const float2 q = cmul(__ldg(a.qx + i), qyv);
+                    v[r] = make_float2(d * q.x, d * q.y);
+                }
+            } else {
+                // d' = (T I - S) - sum_k eT_k V_{t,k}: all loads of one component are issued together (E in flight per thread)
+#pragma unroll
+                for (int r = 0; r < E; ++r) {
+                    const int i = j + r * TPS;
+                    v[r].x = (float)(a.T * (int)__ldg(fr + i) - (int)__ldg(sp + i));
+                }
+                const float* ep = a.defl_img + (long long)s0 * ld + j;
+                for (int kk = 0; kk < a.ndefl; ++kk) {
+                    const float cf = -__ldg(a.defl_coef + frame * a.ndefl + kk);
+                    float e[E];
+#pragma unroll
+                    for (int r = 0; r < E; ++r) e[r] = __ldg(ep + r * TPS);
+#pragma unroll
+                    for (int r = 0; r < E; ++r) v[r].x = fmaf(e[r], cf, v[r].x);
+                    ep += (long long)a.nseq * ld;
+                }
+#pragma unroll
+                for (int r = 0; r < E; ++r) {
+                    const float2 q = cmul(__ldg(a.qx + j + r * TPS), qyv);
+                    const float d = v[r].x;
+                    v[r] = make_float2(d * q.x, d * q.y);
+                }
             }
         } else {
             const float2* ip = a.in + ibase;
@@ -113,7 +152,7 @@ __device__ __forceinline__ void fft_tile(const FftArgs& a, long long in_foff, lo
         if constexpr (!MULTI) {
             mid();
 #pragma unroll
-            for (int r = 0; r < E; ++r) store(op + r * estride, v[brev<E>(r)]);
+            for (int r = 0; r < E; ++r) emit(r, op, r, v[brev<E>(r)]);
         } else {
 #pragma unroll
             for (int r = 0; r < E; ++r) sm[sidx(j * E + r)] = v[brev<E>(r)];
@@ -138,7 +177,7 @@ __device__ __forceinline__ void fft_tile(const FftArgs& a, long long in_foff, lo
                 const int j0 = (b - k) * R1 + k;
                 if constexpr (R2 == 1) {
 #pragma unroll
-                    for (int r = 0; r < R1; ++r) store(op + (j0 + r * E) * estride, v[m * R1 + brev<R1>(r)]);
+                    for (int r = 0; r < R1; ++r) emit(m * R1 + r, op, j0 + r * E, v[m * R1 + brev<R1>(r)]);
                 } else {
 #pragma unroll
                     for (int r = 0; r < R1; ++r) sm[sidx(j0 + r * E)] = v[m * R1 + brev<R1>(r)];
@@ -162,21 +201,106 @@ __device__ __forceinline__ void fft_tile(const FftArgs& a, long long in_foff, lo
                     for (int r = 1; r < R2; ++r) v[m * R2 + r] = cmul(v[m * R2 + r], __ldg(a.tw2 + r * NS2 + b));
                     fft_reg<R2>(v + m * R2);
 #pragma unroll
-                    for (int r = 0; r < R2; ++r) store(op + (b + r * NS2) * estride, v[m * R2 + brev<R2>(r)]);
+                    for (int r = 0; r < R2; ++r) emit(m * R2 + r, op, b + r * NS2, v[m * R2 + brev<R2>(r)]);
                 }
             }
-            __syncthreads();        // smem is reused by the next tile
+            // smem is reused by the next tile.  Row tiles of one warp per row (private slices) outside the fused kernel need
+            // no CTA-wide barrier at all: the warps of a CTA then drift apart and overlap each other's load and store phases
+            if constexpr (WARP_SEQ && FREE_RUN) __syncwarp(); else __syncthreads();
         }
     }
 }
 
-template <int N, int E, int R1, int R2, int B, bool COL, bool PRO>
+template <int N, int E, int R1, int R2, int B, bool COL, bool PRO, bool DEFL = false>
 __global__ void __launch_bounds__((N / E) * B) k_fft(const FftArgs a) {
     extern __shared__ float2 sm[];
     for (int tile = blockIdx.x; tile < a.ntiles; tile += gridDim.x) {
         const int fl = tile / a.tiles_per_frame;
-        fft_tile<N, E, R1, R2, B, COL, PRO>(a, (long long)fl * a.in_fstride, (long long)fl * a.out_fstride,
-                                            tile - fl * a.tiles_per_frame, sm);
+        fft_tile<N, E, R1, R2, B, COL, PRO, 0, NoHook, DEFL>(a, (long long)fl * a.in_fstride, (long long)fl * a.out_fstride,
+                                                             tile - fl * a.tiles_per_frame, sm, NoHook(), fl);
+    }
+}
+
+// element offset (in units of the sequence stride) of output slot `slot` of the calling thread: mirrors the emission
+// order of fft_tile
+template <int N, int E, int R1, int R2, int B, bool COL>
+__device__ __forceinline__ int tile_out_offset(int slot) {
+    constexpr int TPS = N / E;
+    const int j = COL ? (int)threadIdx.x / B : (int)threadIdx.x % TPS;
+    if constexpr (R1 == 1) return slot;
+    else if constexpr (R2 == 1) {
+        const int m = slot / R1, r = slot % R1;
+        const int b = j + m * TPS, k = b % E;
+        return (b - k) * R1 + k + r * E;
+    } else {
+        const int m = slot / R2, r = slot % R2;
+        return j + m * TPS + r * (E * R1);
+    }
+}
+
+// Mode 3 (SURVEY.md 8(f)-2 stage 2), second pass: the column transform of frames [t0, t1) of one column tile, REDUCED to
+// its energy: out(p) = sum_{t in [t0,t1)} |H'_t(p)|^2 with H'_t the hologram of the deflated frame t (rejected components
+// already removed in the raw domain by the row pass), so that sum over all t is the image of Eq. 7 (R12
+// identity: sum_{k in S}|P_k|^2 = sum_t |H_t - sum_{k not in S} P_k conj(V_tk)|^2 for unitary V).  The hologram stack is
+// never written.  grid = (column tiles, frame splits); split s writes out + s * npix (a plain store: deterministic).
+template <int N, int E, int R1, int R2, int B>
+__global__ void __launch_bounds__((N / E) * B, 512 / ((N / E) * B) > 0 ? 512 / ((N / E) * B) : 1)
+k_col_energy(const FftArgs a, float* __restrict__ out, long long npix, int nframes, int nsplit) {
+    extern __shared__ float2 sm[];
+    const int tile = blockIdx.x, split = blockIdx.y;
+    const int per = (nframes + nsplit - 1) / nsplit;
+    const int t0 = split * per, t1 = t0 + per < nframes ? t0 + per : nframes;
+    float acc[E];
+#pragma unroll
+    for (int s = 0; s < E; ++s) acc[s] = 0.f;
+    for (int t = t0; t < t1; ++t)
+        fft_tile<N, E, R1, R2, B, true, false, 0, NoHook, false, true>(a, (long long)t * a.in_fstride, 0, tile, sm, NoHook(), 0, acc);
+    const int c = (int)threadIdx.x % B;
+    float* op = out + (long long)split * npix + (long long)tile * B + c;
+#pragma unroll
+    for (int s = 0; s < E; ++s) op[(long long)tile_out_offset<N, E, R1, R2, B, true>(s) * a.ld] = acc[s];
+}
+
+// out = sum of nsplit partial images (fixed order)
+__global__ void __launch_bounds__(256) k_sum_partial_images(const float* __restrict__ part, int nsplit, long long npix, float* __restrict__ out) {
+    const long long n4 = npix >> 2;                         // npix is a multiple of 256
+    const float4* p4 = reinterpret_cast<const float4*>(part);
+    for (long long p = (long long)blockIdx.x * 256 + threadIdx.x; p < n4; p += (long long)gridDim.x * 256) {
+        float4 s = __ldg(p4 + p);
+        for (int k = 1; k < nsplit; ++k) { const float4 w = __ldg(p4 + (long long)k * n4 + p); s.x += w.x; s.y += w.y; s.z += w.z; s.w += w.w; }
+        reinterpret_cast<float4*>(out)[p] = s;
+    }
+}
+
+// eT_k(x) = sum_t (T I_t(x) - S(x)) V_{t,k} for the rejected components k (column indices cols[kk] of V), and the
+// coefficient table coef[t][kk] = Re V_{t,cols[kk]}.  One thread per pixel pair.
+__global__ void __launch_bounds__(256) k_deflate_images(const uint16_t* __restrict__ frames, const uint32_t* __restrict__ sum,
+                                                        const float2* __restrict__ V, long long npix, int T, int ndefl,
+                                                        int c0_lo, int c0_n, int c1_lo, float* __restrict__ img, float* __restrict__ coef) {
+    __shared__ float Vs[HOLO_MAX_T * 4];
+    for (int i = threadIdx.x; i < T * ndefl; i += blockDim.x) {
+        const int t = i / ndefl, kk = i - t * ndefl;
+        const int col = kk < c0_n ? c0_lo + kk : c1_lo + (kk - c0_n);
+        const float v = V[t * T + col].x;
+        Vs[i] = v;
+        if (blockIdx.x == 0) coef[i] = v;
+    }
+    __syncthreads();
+    const long long npair = npix >> 1;
+    for (long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x; q < npair; q += (long long)gridDim.x * blockDim.x) {
+        const uint2 S = reinterpret_cast<const uint2*>(sum)[q];
+        float e0[4] = {0.f, 0.f, 0.f, 0.f}, e1[4] = {0.f, 0.f, 0.f, 0.f};
+#pragma unroll 8
+        for (int t = 0; t < T; ++t) {
+            const uint32_t w = __ldg(reinterpret_cast<const uint32_t*>(frames + (long long)t * npix) + q);
+            const float d0 = (float)(T * (int)(w & 0xffffu) - (int)S.x), d1 = (float)(T * (int)(w >> 16) - (int)S.y);
+#pragma unroll
+            for (int kk = 0; kk < 4; ++kk)
+                if (kk < ndefl) { const float v = Vs[t * ndefl + kk]; e0[kk] = fmaf(d0, v, e0[kk]); e1[kk] = fmaf(d1, v, e1[kk]); }
+        }
+#pragma unroll
+        for (int kk = 0; kk < 4; ++kk)
+            if (kk < ndefl) reinterpret_cast<float2*>(img + (long long)kk * npix)[q] = make_float2(e0[kk], e1[kk]);
     }
 }
 
@@ -330,11 +454,11 @@ void holo_fft_plan_free(FftPlan* p) {
     p->tw1 = p->tw2 = nullptr;
 }
 
-template <int N, int E, int R1, int R2, int B, bool COL, bool PRO>
+template <int N, int E, int R1, int R2, int B, bool COL, bool PRO, bool DEFL = false>
 static int launch_fft_t(const FftArgs& a, int num_sms, int device, cudaStream_t st) {
     constexpr int threads = (N / E) * B;
     constexpr size_t smem = (R1 > 1) ? sizeof(float2) * (size_t)(N + N / E) * B : 0;
-    auto kern = k_fft<N, E, R1, R2, B, COL, PRO>;
+    auto kern = k_fft<N, E, R1, R2, B, COL, PRO, DEFL>;
     int blocks_per_sm = 0;
     { const int rc = holo_cached_occupancy((const void*)kern, device, threads, smem, &blocks_per_sm); if (rc) return rc; }
     int grid = a.ntiles < num_sms * blocks_per_sm ? a.ntiles : num_sms * blocks_per_sm;
@@ -344,18 +468,44 @@ static int launch_fft_t(const FftArgs& a, int num_sms, int device, cudaStream_t 
 }
 
 // B (sequences per CTA) per length: rows aim at 256 threads; columns at >= 64-byte segments
-template <bool COL, bool PRO>
+template <bool COL, bool PRO, bool DEFL = false>
 static int launch_fft(int N, const FftArgs& a, int num_sms, int device, cudaStream_t st) {
     switch (N) {
-        case 16:   return launch_fft_t<16, 16, 1, 1, 16, COL, PRO>(a, num_sms, device, st);
-        case 32:   return launch_fft_t<32, 32, 1, 1, 16, COL, PRO>(a, num_sms, device, st);
-        case 64:   return launch_fft_t<64, 16, 4, 1, 16, COL, PRO>(a, num_sms, device, st);
-        case 128:  return launch_fft_t<128, 16, 8, 1, 16, COL, PRO>(a, num_sms, device, st);
-        case 256:  return launch_fft_t<256, 16, 16, 1, 16, COL, PRO>(a, num_sms, device, st);
-        case 512:  return launch_fft_t<512, 32, 16, 1, 16, COL, PRO>(a, num_sms, device, st);
-        case 1024: return launch_fft_t<1024, 32, 32, 1, 8, COL, PRO>(a, num_sms, device, st);
-        case 2048: return launch_fft_t<2048, 32, 32, 2, 4, COL, PRO>(a, num_sms, device, st);
-        case 4096: return launch_fft_t<4096, 16, 16, 16, 4, COL, PRO>(a, num_sms, device, st);
+        case 16:   return launch_fft_t<16, 16, 1, 1, 16, COL, PRO, DEFL>(a, num_sms, device, st);
+        case 32:   return launch_fft_t<32, 32, 1, 1, 16, COL, PRO, DEFL>(a, num_sms, device, st);
+        case 64:   return launch_fft_t<64, 16, 4, 1, 16, COL, PRO, DEFL>(a, num_sms, device, st);
+        case 128:  return launch_fft_t<128, 16, 8, 1, 16, COL, PRO, DEFL>(a, num_sms, device, st);
+        case 256:  return launch_fft_t<256, 16, 16, 1, 16, COL, PRO, DEFL>(a, num_sms, device, st);
+        case 512:  return launch_fft_t<512, 32, 16, 1, 16, COL, PRO, DEFL>(a, num_sms, device, st);
+        case 1024: return launch_fft_t<1024, 32, 32, 1, 8, COL, PRO, DEFL>(a, num_sms, device, st);
+        case 2048: return launch_fft_t<2048, 32, 32, 2, 4, COL, PRO, DEFL>(a, num_sms, device, st);
+        case 4096: return launch_fft_t<4096, 16, 16, 16, 4, COL, PRO, DEFL>(a, num_sms, device, st);
+    }
+    holo_set_error("unsupported FFT length %d", N);
+    return HOLO_ERR_ARG;
+}
+
+template <int N, int E, int R1, int R2, int B>
+static int launch_col_energy_t(const FftArgs& a, float* out, long long npix, int nframes, int nsplit, int device, cudaStream_t st) {
+    constexpr int threads = (N / E) * B;
+    constexpr size_t smem = (R1 > 1) ? sizeof(float2) * (size_t)(N + N / E) * B : 0;
+    auto kern = k_col_energy<N, E, R1, R2, B>;
+    { const int rc = holo_ensure_smem_attr((const void*)kern, device, smem); if (rc) return rc; }
+    kern<<<dim3((unsigned)a.tiles_per_frame, (unsigned)nsplit), threads, smem, st>>>(a, out, npix, nframes, nsplit);
+    HOLO_CUDA_OK(cudaGetLastError());
+    return HOLO_OK;
+}
+static int launch_col_energy(int N, const FftArgs& a, float* out, long long npix, int nframes, int nsplit, int device, cudaStream_t st) {
+    switch (N) {
+        case 16:   return launch_col_energy_t<16, 16, 1, 1, 16>(a, out, npix, nframes, nsplit, device, st);
+        case 32:   return launch_col_energy_t<32, 32, 1, 1, 16>(a, out, npix, nframes, nsplit, device, st);
+        case 64:   return launch_col_energy_t<64, 16, 4, 1, 16>(a, out, npix, nframes, nsplit, device, st);
+        case 128:  return launch_col_energy_t<128, 16, 8, 1, 16>(a, out, npix, nframes, nsplit, device, st);
+        case 256:  return launch_col_energy_t<256, 16, 16, 1, 16>(a, out, npix, nframes, nsplit, device, st);
+        case 512:  return launch_col_energy_t<512, 32, 16, 1, 16>(a, out, npix, nframes, nsplit, device, st);
+        case 1024: return launch_col_energy_t<1024, 32, 32, 1, 8>(a, out, npix, nframes, nsplit, device, st);
+        case 2048: return launch_col_energy_t<2048, 32, 32, 2, 4>(a, out, npix, nframes, nsplit, device, st);
+        case 4096: return launch_col_energy_t<4096, 16, 16, 16, 4>(a, out, npix, nframes, nsplit, device, st);
     }
     holo_set_error("unsupported FFT length %d", N);
     return HOLO_ERR_ARG;
@@ -475,6 +625,69 @@ int holo_launch_fresnel(holo_ctx* c, const uint16_t* frames, float2* H, cudaStre
         b.T = c->T;
         { HoloProf prof(c, HOLO_K_FFT_COLS, st); rc = launch_fft<true, false>(c->ny, b, c->num_sms, c->device, st); }
         if (rc) return rc;
+    }
+    return HOLO_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// Mode 3 (SURVEY.md 8(f)-2 stage 2): the image without the hologram stack.  Needs S = sum_t I_t in c->sum and the
+// eigenvectors V (real: the covariance of the raw frames is real symmetric, R21).
+//   1. k_deflate_images: eT_k = sum_t (T I_t - S) V_tk for the rejected components k (at most 4)
+//   2. row pass of all T frames with the deflation in the prologue -> G = row transform of q (d_t - sum_k e_k V_tk)
+//      (complex64 [T][ny][nx] in c->H: the only large intermediate, written and read once)
+//   3. k_col_energy: column transform reduced to sum_t |.|^2, frame splits -> k_sum_partial_images
+// ------------------------------------------------------------------------------------------------
+int holo_mode3_splits(const holo_ctx* c) {
+    const int ct = c->nx / fft_batch(c->ny);
+    int ns = (2 * c->num_sms) / (ct > 0 ? ct : 1);
+    if (ns < 1) ns = 1;
+    if (ns > c->T) ns = c->T;
+    if (ns > 8) ns = 8;
+    return ns;
+}
+
+int holo_launch_energy_image(holo_ctx* c, const uint16_t* frames, const float2* V, int k_lo, int k_hi, float* image, cudaStream_t st) {
+    const int T = c->T;
+    const int n0 = k_lo - 1, n1 = T - k_hi, ndefl = n0 + n1;
+    if (ndefl > 4) { holo_set_error("mode 3 removes at most 4 components in the raw domain (asked for %d)", ndefl); return HOLO_ERR_STATE; }
+    if (ndefl > 0) {
+        HoloProf prof(c, HOLO_K_SUM, st);
+        const long long npair = c->npix >> 1;
+        long long want = (npair + 255) / 256;
+        const int grid = (int)(want < (long long)c->num_sms * 8 ? want : (long long)c->num_sms * 8);
+        k_deflate_images<<<grid, 256, 0, st>>>(frames, c->sum, V, c->npix, T, ndefl, 0, n0, k_hi, c->defl_img, c->defl_coef);
+        HOLO_CUDA_OK(cudaGetLastError());
+    }
+    FftArgs a{};
+    a.frames = frames; a.sum = c->sum; a.qx = c->qxs; a.qy = c->qy; a.in = nullptr; a.out = c->H;
+    a.tw1 = c->px.tw1; a.tw2 = c->px.tw2;
+    a.in_fstride = c->npix; a.out_fstride = c->npix;
+    a.ld = c->nx; a.nseq = c->ny;
+    a.tiles_per_frame = c->ny / fft_batch(c->nx);
+    a.ntiles = T * a.tiles_per_frame;
+    a.T = T;
+    a.defl_img = c->defl_img; a.defl_coef = c->defl_coef; a.ndefl = ndefl;
+    int rc;
+    { HoloProf prof(c, HOLO_K_FFT_ROWS, st);
+      rc = ndefl ? launch_fft<false, true, true>(c->nx, a, c->num_sms, c->device, st) : launch_fft<false, true, false>(c->nx, a, c->num_sms, c->device, st); }
+    if (rc) return rc;
+    FftArgs b{};
+    b.in = c->H; b.out = nullptr;
+    b.tw1 = c->py.tw1; b.tw2 = c->py.tw2;
+    b.in_fstride = c->npix; b.out_fstride = 0;
+    b.ld = c->nx; b.nseq = c->nx;
+    b.tiles_per_frame = c->nx / fft_batch(c->ny);
+    b.ntiles = b.tiles_per_frame;
+    b.T = T;
+    const int ns = holo_mode3_splits(c);
+    { HoloProf prof(c, HOLO_K_FFT_COLS, st);
+      rc = launch_col_energy(c->ny, b, ns > 1 ? c->energy_parts : image, c->npix, T, ns, c->device, st); }
+    if (rc) return rc;
+    if (ns > 1) {
+        HoloProf prof(c, HOLO_K_PROJECT, st);
+        const long long want = ((c->npix >> 2) + 255) / 256;
+        k_sum_partial_images<<<(int)(want < 8ll * c->num_sms ? want : 8ll * c->num_sms), 256, 0, st>>>(c->energy_parts, ns, c->npix, image);
+        HOLO_CUDA_OK(cudaGetLastError());
     }
     return HOLO_OK;
 }

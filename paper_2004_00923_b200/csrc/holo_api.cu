@@ -78,7 +78,8 @@ static void free_ctx(holo_ctx* c) {
     cudaFree(c->sum); cudaFree(c->scratch); cudaFree(c->H); cudaFree(c->cov_partials);
     cudaFree(c->C); cudaFree(c->evals); cudaFree(c->V); cudaFree(c->status);
     if (c->noconv_host) cudaFreeHost(c->noconv_host);
-    cudaFree(c->counters); cudaFree(c->gram_X);
+    cudaFree(c->counters); cudaFree(c->gram_X); cudaFree(c->gram_Xp);
+    cudaFree(c->defl_img); cudaFree(c->defl_coef); cudaFree(c->energy_parts); cudaFree(c->sum1);
     if (c->prof_ev) {
         for (int i = 0; i < 2 * HOLO_PROF_CAP; ++i) cudaEventDestroy(c->prof_ev[i]);
         delete[] c->prof_ev;
@@ -153,6 +154,10 @@ static int create_impl(holo_ctx* c) {
     HOLO_CUDA_OK(cudaMalloc(&c->status, 8 * sizeof(int32_t)));
     HOLO_CUDA_OK(cudaMalloc(&c->counters, 1024 * sizeof(unsigned int)));
     HOLO_CUDA_OK(cudaMalloc(&c->gram_X, 128 * 128 * sizeof(unsigned long long)));
+    {
+        const size_t Ng = T <= 32 ? 64 : 128;
+        HOLO_CUDA_OK(cudaMalloc(&c->gram_Xp, Ng * (Ng + 1) / 2 * (size_t)(3 * c->num_sms) * sizeof(unsigned long long)));
+    }
     HOLO_CUDA_OK(cudaMalloc(&c->Fmat, (size_t)T * T * sizeof(float2)));
     HOLO_CUDA_OK(cudaMalloc(&c->norm_partials, HOLO_NORM_PARTS * sizeof(double)));
     c->mode = 1;
@@ -264,6 +269,7 @@ extern "C" int holo_fftshift(holo_ctx* c, const float* in_dev, float* out_dev, h
 }
 
 static int project_pending(holo_ctx* c, cudaStream_t st);
+static int energy_pending(holo_ctx* c, cudaStream_t st);
 static int join_side(holo_ctx* c, cudaStream_t st, int slot);
 
 extern "C" int holo_process(holo_ctx* c, const uint16_t* frames_dev, float* image_dev, holo_stream stream) {
@@ -273,8 +279,16 @@ extern "C" int holo_process(holo_ctx* c, const uint16_t* frames_dev, float* imag
     int rc;
     if ((rc = join_side(c, st, -1))) return rc;
     if ((rc = project_pending(c, st))) return rc;          // a holo_submit still owes its image: deliver it first
+    if ((rc = energy_pending(c, st))) return rc;
     c->nsubmit = 0;                                        // the next holo_submit starts again with slot 0
     c->push_ready = 0;                                     // ... and a holo_push sequence has to start over
+    if (c->mode == 3) {
+        // mode 2's covariance and eigenvectors, then the image straight from the raw frames: rejected components removed in
+        // the raw domain, row pass, column pass reduced to sum_t |.|^2 -- no hologram stack, no projection kernel
+        if ((rc = holo_launch_sum_gram(c, frames_dev, c->C, st))) return rc;
+        if ((rc = holo_launch_eig(c, c->C, c->evals, c->V, st))) return rc;
+        return holo_launch_energy_image(c, frames_dev, c->V, c->k_lo, c->k_hi, image_dev, st);
+    }
     if (c->mode == 2) {
         // covariance from the raw frames (exact integer Gram on the tensor cores, fused with the temporal sum): C and V are
         // known BEFORE the holograms exist, and the hologram stack is read once (projection) instead of twice
@@ -297,8 +311,16 @@ extern "C" int holo_raw_covariance(holo_ctx* c, const uint16_t* frames_dev, void
 
 extern "C" int holo_set_mode(holo_ctx* c, int mode) {
     CHECK_CTX_QUIET(c);
-    if (mode != 1 && mode != 2) { holo_set_error("mode must be 1 (covariance of the hologram stack) or 2 (of the raw frames)"); return HOLO_ERR_ARG; }
-    if (c->pend_image || c->proj_recorded[0] || c->proj_recorded[1]) { holo_set_error("holo_flush the open holo_submit sequence before changing the mode"); return HOLO_ERR_STATE; }
+    if (mode < 1 || mode > 3) { holo_set_error("mode must be 1 (covariance of the hologram stack), 2 (of the raw frames) or 3 (2 + image without the hologram stack)"); return HOLO_ERR_ARG; }
+    if (c->pend_image || c->pend3_image || c->proj_recorded[0] || c->proj_recorded[1]) { holo_set_error("holo_flush the open holo_submit sequence before changing the mode"); return HOLO_ERR_STATE; }
+    if (mode == 3) {
+        if ((c->k_lo - 1) + (c->T - c->k_hi) > 4) { holo_set_error("mode 3 removes at most 4 components (k_lo - 1 + T - k_hi <= 4)"); return HOLO_ERR_STATE; }
+        if (!c->defl_img) {                                  // first use: the mode's own workspace (allocation, may synchronise)
+            HOLO_CUDA_OK(cudaMalloc(&c->defl_img, (size_t)4 * c->npix * sizeof(float)));
+            HOLO_CUDA_OK(cudaMalloc(&c->defl_coef, (size_t)HOLO_MAX_T * 4 * sizeof(float)));
+            HOLO_CUDA_OK(cudaMalloc(&c->energy_parts, (size_t)8 * c->npix * sizeof(float)));
+        }
+    }
     c->mode = mode;
     return HOLO_OK;
 }
@@ -347,11 +369,52 @@ static int project_pending(holo_ctx* c, cudaStream_t st) {
     return rc;
 }
 
+// mode 3, streaming form: the stack whose image is still owed (its frames are read again by the energy pass)
+static int energy_pending(holo_ctx* c, cudaStream_t st) {
+    if (!c->pend3_image) return HOLO_OK;
+    const int s = c->pend3_slot;
+    HOLO_CUDA_OK(cudaStreamWaitEvent(st, c->ev_eig[s], 0));
+    uint32_t* sum_main = c->sum;
+    if (s) c->sum = c->sum1;
+    const int rc = holo_launch_energy_image(c, c->pend3_frames, s ? c->V1 : c->V, c->pend_k_lo, c->pend_k_hi, c->pend3_image, st);
+    c->sum = sum_main;
+    c->pend3_image = nullptr; c->pend3_frames = nullptr;
+    return rc;
+}
+
 extern "C" int holo_submit(holo_ctx* c, const uint16_t* frames_dev, float* image_dev, holo_stream stream) {
     CHECK_CTX(c); CHECK_PTR(frames_dev, "frames_dev"); CHECK_PTR(image_dev, "image_dev");
     if (((uintptr_t)frames_dev & 15) || ((uintptr_t)image_dev & 7)) { holo_set_error("frames_dev must be 16-byte and image_dev 8-byte aligned"); return HOLO_ERR_ARG; }
     cudaStream_t st = (cudaStream_t)stream;
     int rc;
+    if (c->mode == 3) {
+        // mode 3: everything of a stack needs its eigenvectors first (the rejected components are removed in the raw domain),
+        // so the pipeline is: covariance of stack i (tensor cores, from the raw frames) -> fork its eigensolver to the side
+        // stream -> image of stack i-1 (deflation images, row pass, column energy) with the eigensolver of stack i under it.
+        // frames_dev of stack i is read AGAIN by the next holo_submit / holo_flush: it must stay valid until then.
+        if ((rc = submit_init(c, /*second_stack=*/false))) return rc;
+        if (!c->sum1) HOLO_CUDA_OK(cudaMalloc(&c->sum1, (size_t)c->npix * sizeof(uint32_t)));
+        c->push_ready = 0;
+        const int s = (int)(c->nsubmit & 1);
+        uint32_t* sum_main = c->sum;
+        if (s) c->sum = c->sum1;
+        rc = holo_launch_sum_gram(c, frames_dev, s ? c->C1 : c->C, st);
+        c->sum = sum_main;
+        if (rc) return rc;
+        HOLO_CUDA_OK(cudaEventRecord(c->ev_cov[s], st));
+        HOLO_CUDA_OK(cudaStreamWaitEvent(c->side, c->ev_cov[s], 0));
+        int32_t* status_main = c->status;
+        if (s) c->status = c->status1;
+        rc = holo_launch_eig(c, s ? c->C1 : c->C, s ? c->evals1 : c->evals, s ? c->V1 : c->V, c->side);
+        c->status = status_main;
+        if (rc) return rc;
+        HOLO_CUDA_OK(cudaEventRecord(c->ev_eig[s], c->side));
+        if ((rc = energy_pending(c, st))) return rc;              // image of stack i-1
+        c->pend3_image = image_dev; c->pend3_frames = frames_dev; c->pend3_slot = s;
+        c->pend_k_lo = c->k_lo; c->pend_k_hi = c->k_hi;
+        c->nsubmit++;
+        return HOLO_OK;
+    }
     if (c->mode == 2) {
         // mode 2: the eigensolver runs on the side stream UNDER the Fresnel stage of the same stack (C comes from the raw
         // frames), so the projection follows in stream order and the image is complete when this call's work is done
@@ -409,8 +472,9 @@ extern "C" int holo_submit(holo_ctx* c, const uint16_t* frames_dev, float* image
 
 extern "C" int holo_flush(holo_ctx* c, holo_stream stream) {
     CHECK_CTX(c);
-    const int rc = join_side(c, (cudaStream_t)stream, -1);
+    int rc = join_side(c, (cudaStream_t)stream, -1);
     if (rc) return rc;
+    if ((rc = energy_pending(c, (cudaStream_t)stream))) return rc;
     return project_pending(c, (cudaStream_t)stream);
 }
 
@@ -565,7 +629,7 @@ extern "C" int holo_submit_host(holo_ctx* c, const uint16_t* frames_host, float*
     HOLO_CUDA_OK(cudaMemcpyAsync(c->fstage[s], frames_host, fbytes, cudaMemcpyHostToDevice, c->copy));
     HOLO_CUDA_OK(cudaEventRecord(c->ev_h2d[s], c->copy));
     HOLO_CUDA_OK(cudaStreamWaitEvent(st, c->ev_h2d[s], 0));
-    if (c->tune[HOLO_TUNE_SPLIT_SMS] > 0) {
+    if (c->mode == 1 && c->tune[HOLO_TUNE_SPLIT_SMS] > 0) {
         // SM-split mode: the projection of stack i-2 (same slot) is joined first and its image copied out BEFORE
         // anything of stack i is enqueued, so the copy is ordered before the projection of stack i reuses the slot
         if ((rc = join_side(c, st, s))) return rc;
@@ -580,7 +644,8 @@ extern "C" int holo_submit_host(holo_ctx* c, const uint16_t* frames_host, float*
         return HOLO_OK;
     }
     if ((rc = holo_submit(c, c->fstage[s], c->istage[s], stream))) return rc;   // enqueues the projection of stack i-1
-    HOLO_CUDA_OK(cudaEventRecord(c->ev_free[s], st));
+    // mode 3 reads the frames of stack i again in the next submit / flush: what is free now is the stage of stack i-1
+    HOLO_CUDA_OK(cudaEventRecord(c->ev_free[c->mode == 3 ? s ^ 1 : s], st));
     if ((rc = deliver_host(c, st))) return rc;
     c->pend_image_host = image_host; c->pend_islot = s; c->nsubmit_host++;
     HOLO_CUDA_OK(cudaEventSynchronize(c->ev_h2d[s]));        // frames_host may be reused on return
@@ -629,6 +694,7 @@ extern "C" int holo_set_range(holo_ctx* c, int k_lo, int k_hi) {
         holo_set_error("a holo_push sequence is open: its window's complement must stay at most half of the window");
         return HOLO_ERR_STATE;
     }
+    if (c->mode == 3 && (k_lo - 1) + (c->T - k_hi) > 4) { holo_set_error("mode 3 removes at most 4 components (k_lo - 1 + T - k_hi <= 4)"); return HOLO_ERR_STATE; }
     c->k_lo = k_lo; c->k_hi = k_hi;
     return HOLO_OK;
 }
@@ -687,6 +753,10 @@ extern "C" int holo_status(holo_ctx* c, int32_t status_host[4], holo_stream stre
 
 extern "C" int holo_launches_per_process(holo_ctx* c) {
     CHECK_CTX_QUIET(c);
+    if (c->mode == 3) {
+        const int ndefl = (c->k_lo - 1) + (c->T - c->k_hi);
+        return 2 /*sum + Gram, reduce + finish*/ + 1 /*eig*/ + (ndefl ? 1 : 0) + 2 /*row pass, column energy*/ + (holo_mode3_splits(c) > 1 ? 1 : 0);
+    }
     if (c->mode == 2) return 2 /*sum + Gram, finish*/ + (holo_fresnel_launch_count(c) - 1) + 1 /*eig*/ + 1 /*project*/;
     return holo_fresnel_launch_count(c) + 2 /*cov partial + reduce*/ + 1 /*eig*/ + 1 /*project*/;
 }

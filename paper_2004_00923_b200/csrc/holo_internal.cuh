@@ -67,7 +67,13 @@ struct holo_ctx {
     float2* C;
     float* evals;
     float2* V;
+    float* defl_img;        // mode 3: [4][ny][nx] raw-domain images of the rejected components (allocated at first use)
+    float* defl_coef;       // mode 3: [T][4] their eigenvector entries
+    float* energy_parts;    // mode 3: [splits][ny][nx] partial energy images
+    uint32_t* sum1;         // mode 3, streaming form: frame sum of the second slot
+    const uint16_t* pend3_frames; float* pend3_image; int pend3_slot;   // mode 3, streaming form: the stack whose image is owed
     unsigned long long* gram_X;   // [128][128] int64 byte-plane Gram of the raw frames (mode 2, rawgram.cu)
+    unsigned long long* gram_Xp;  // [N (N + 1) / 2][3 num_sms] per-CTA partials of it (N = 64 or 128)
     int mode;               // 1: covariance from the hologram stack (Eq. 4 as written); 2: from the raw frames
     int32_t* status;        // [8], see HOLO_WS_STATUS
     int32_t* noconv_host;   // pinned, mapped host word: set by the eigensolver when it hits the sweep cap (device alias below)
@@ -146,6 +152,9 @@ int holo_launch_eig(holo_ctx* c, const float2* C, float* evals, float2* V, cudaS
 int holo_launch_project(holo_ctx* c, const float2* H, const float2* V, int k_lo, int k_hi,
                         int allow_complement, float* image, cudaStream_t st, int center = 0);
 int holo_fresnel_launch_count(holo_ctx* c);
+// mode 3: image = sum_t |FFT2[q (d_t - sum_{k rejected} e_k V_tk)]|^2 without storing the hologram stack (c->sum and V must be ready)
+int holo_launch_energy_image(holo_ctx* c, const uint16_t* frames, const float2* V, int k_lo, int k_hi, float* image, cudaStream_t st);
+int holo_mode3_splits(const holo_ctx* c);
 // display.cu: PAPER.md:86 normalisation, quadrant swap, Eq. 3 SVD filter
 int holo_launch_normalize(holo_ctx* c, float* image, cudaStream_t st);
 int holo_launch_fftshift(holo_ctx* c, const float* in, float* out, cudaStream_t st);

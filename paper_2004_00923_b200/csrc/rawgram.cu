@@ -9,13 +9,15 @@
 // X X^T (tcgen05.mma kind::i8, u8 x u8 -> s32 accumulators in TMEM) holds the four blocks HH, HL, LH, LL with
 // G = 65536 HH + 256 (HL + LH) + LL.  One pass over the frames (2 T N_p bytes, the same read the temporal sum A0 needs):
 // the kernel also writes S.  No rounding anywhere before the final conversion of C to float.
-//   k_sum_gram   : persistent CTAs of 128 threads; a thread owns 2 adjacent pixels, loads them of all T frames, adds
+//   k_sum_gram   : persistent CTAs of 128 threads; a thread owns 2 adjacent pixels, loads them of all T frames (the loads of
+//                  the next block are issued before the current one is processed), adds
 //                  them up (S) and writes their bytes into the K-major SWIZZLE_128B operand tile ([128 rows x 128 B] per 128
 //                  pixels, two tiles per stage, two stages); one thread issues the MMAs (M = 128, N = 64 or 128,
 //                  K = 32 per instruction) and commits them to the stage's mbarrier; the s32 accumulators are drained
 //                  (tcgen05.ld) into the global int64 byte-plane Gram with integer atomics before they can overflow
 //                  (every 16384 pixels) and at the end.
-//   k_gram_finish: one CTA assembles G (int64), centres it in __int128 and writes C (float2, Im = 0).
+//   k_gram_reduce_finish: one warp per entry adds the per-CTA slots up; the last CTA assembles G (int64), centres it in
+//                  __int128 and writes C (float2, Im = 0).
 #include "holo_internal.cuh"
 #include "tma.cuh"
 
@@ -49,8 +51,8 @@ __device__ __forceinline__ void tmem_ld16(uint32_t taddr, int32_t* v) {
     asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
 }
 
-// frames uint16 [T][npix]; sum uint32 [npix]; X int64 [2 TP][2 TP], zeroed by the caller: the byte-plane Gram, summed over
-// all CTAs with 64-bit integer atomics (exact and order independent, hence deterministic); lower triangle only
+// frames uint16 [T][npix]; sum uint32 [npix]; X int64 [lower-triangle entries of the 2 TP x 2 TP byte-plane Gram][CTAs]: every
+// CTA writes its own slot (integer sums: exact and order independent, hence deterministic)
 template <int TP>
 __global__ void __launch_bounds__(RG_THREADS, 3)
 k_sum_gram(const uint16_t* __restrict__ frames, uint32_t* __restrict__ sum, unsigned long long* __restrict__ X,
@@ -91,29 +93,54 @@ k_sum_gram(const uint16_t* __restrict__ frames, uint32_t* __restrict__ sum, unsi
     uint32_t ph[2] = {0u, 0u};
     int it = 0, pending[2] = {0, 0}, since_flush = 0;
 
-    auto drain = [&]() {                                      // accumulators -> int64 partial (all MMAs have completed)
+    // accumulators -> this CTA's own slot of the partial store Xp[lower-triangle entry][CTA] (plain stores: the per-entry
+    // 64-bit atomics of 444 CTAs on 2080 addresses cost 40 % of the kernel); k_gram_reduce adds the slots up
+    bool first_drain = true;
+    auto drain = [&]() {                                      // (all MMAs have completed)
         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
         const int row = 32 * warp + lane;                     // TMEM lane = row of D
         for (int c0 = 0; c0 < N; c0 += 16) {
             int32_t v[16];
             tmem_ld16(tmem + ((uint32_t)(32 * warp) << 16) + (uint32_t)c0, v);
             if (row < N) {
+                long long* dst = reinterpret_cast<long long*>(X) + ((size_t)row * (row + 1) / 2 + c0) * gridDim.x + blockIdx.x;
 #pragma unroll
                 for (int j = 0; j < 16; ++j)
-                    if (c0 + j <= row && v[j] != 0) atomicAdd(X + (size_t)row * N + c0 + j, (unsigned long long)(long long)v[j]);
+                    if (c0 + j <= row) {
+                        long long* q = dst + (size_t)j * gridDim.x;
+                        *q = first_drain ? (long long)v[j] : *q + (long long)v[j];
+                    }
             }
         }
+        first_drain = false;
         asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     };
+    if ((long long)blockIdx.x >= nblocks) {                   // (cannot happen with grid <= nblocks; keeps the slot defined)
+        const int row = 32 * warp + lane;
+        if (row < N) for (int c = 0; c <= row; ++c) reinterpret_cast<long long*>(X)[((size_t)row * (row + 1) / 2 + c) * gridDim.x + blockIdx.x] = 0;
+    }
 
+    // software pipeline: the loads of block n + 1 are in flight (T per thread) while block n is split into byte planes
+    constexpr bool PF = TP <= 32;                              // (at TP = 64 the second register set would spill)
+    uint32_t w[TP], wn[PF ? TP : 1];
+    auto load_block = [&](long long blk, uint32_t* dst) {
+        const long long q0 = blk * RG_PIX + 2 * tid;
+        const bool ok = q0 + 1 < npix;                         // npix is a multiple of 256 for every supported frame size
+#pragma unroll
+        for (int t = 0; t < TP; ++t) dst[t] = (ok && t < T) ? __ldg(reinterpret_cast<const uint32_t*>(frames + (size_t)t * npix + q0)) : 0u;
+    };
+    if (PF && (long long)blockIdx.x < nblocks) load_block(blockIdx.x, wn);
     for (long long blk = blockIdx.x; blk < nblocks; blk += gridDim.x, ++it) {
         const int s = it & 1;
         const long long p0 = blk * RG_PIX + 2 * tid;           // the thread's two pixels
-        const bool inb = p0 + 1 < npix;                        // npix is a multiple of 256 for every supported frame size
-        // the loads of this block are issued first (T in flight per thread)
-        uint32_t w[TP];
+        const bool inb = p0 + 1 < npix;
+        if constexpr (PF) {
 #pragma unroll
-        for (int t = 0; t < TP; ++t) w[t] = (inb && t < T) ? __ldg(reinterpret_cast<const uint32_t*>(frames + (size_t)t * npix + p0)) : 0u;
+            for (int t = 0; t < TP; ++t) w[t] = wn[t];
+            if (blk + gridDim.x < nblocks) load_block(blk + gridDim.x, wn);
+        } else {
+            load_block(blk, w);
+        }
         if (pending[s]) { mbar_wait(mma_done + s, ph[s]); ph[s] ^= 1u; pending[s] = 0; }   // the MMAs that read this stage
         unsigned char* tile = base + (size_t)s * RG_STAGE + (size_t)ktile * RG_TILE;
         uint32_t sa = 0u, sb = 0u;
@@ -153,32 +180,77 @@ k_sum_gram(const uint16_t* __restrict__ frames, uint32_t* __restrict__ sum, unsi
         }
     }
     for (int q = 0; q < 2; ++q) if (pending[q]) { mbar_wait(mma_done + q, ph[q]); ph[q] ^= 1u; pending[q] = 0; }
-    if (since_flush) drain();
+    if (since_flush || first_drain) drain();
     __syncthreads();
     if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "r"(N) : "memory");
 }
 
-// X (lower triangle of the byte-plane Gram) -> G (exact) -> C = (nx ny / T^2) (T^2 G - T (r_t + r_s) + tau): the full
-// symmetric matrix, Im = 0.  G < 2^57 and r < 2^63 fit int64 for every supported size; the combination needs __int128.
-__global__ void __launch_bounds__(256) k_gram_finish(const unsigned long long* __restrict__ X, int T, int Tp, double scale,
-                                                     float2* __restrict__ C) {
+// Xp[entry][part] -> X[row][col] (lower triangle of the byte-plane Gram, int64): one warp per entry (integer sums: exact,
+// order independent).  The CTA that finishes last then assembles G = 65536 HH + 256 (HL + LH) + LL (int64), centres it in
+// __int128,  C = (nx ny / T^2) (T^2 G - T (r_t + r_s) + tau),  and writes the full symmetric matrix (Im = 0), rounded once.
+// G < 2^57 and r < 2^63 fit int64 for every supported size.
+__global__ void __launch_bounds__(256) k_gram_reduce_finish(const long long* __restrict__ Xp, int nparts, int N, unsigned long long* __restrict__ X,
+                                                            unsigned int* __restrict__ done, int T, int Tp, double scale, float2* __restrict__ C) {
     __shared__ long long G[HOLO_MAX_T * HOLO_MAX_T];
     __shared__ long long r[HOLO_MAX_T];
-    const int N = 2 * Tp;
-    auto Xs = [&](int i, int j) -> long long { return (long long)(i >= j ? X[(size_t)i * N + j] : X[(size_t)j * N + i]); };
-    for (int e = threadIdx.x; e < T * T; e += blockDim.x) {
-        const int t = e / T, s = e - t * T;
-        G[e] = Xs(t, s) * 65536 + (Xs(t, Tp + s) + Xs(Tp + t, s)) * 256 + Xs(Tp + t, Tp + s);
-    }
-    __syncthreads();
-    if (threadIdx.x < T) {
+    __shared__ long long tau_lo; __shared__ long long tau_hi;   // tau as a 128-bit value
+    __shared__ int s_last;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int entry = blockIdx.x * 8 + warp;
+    const int nent = N * (N + 1) / 2;
+    if (entry < nent) {
+        const long long* src = Xp + (size_t)entry * nparts;
         long long acc = 0;
-        for (int s = 0; s < T; ++s) acc += G[threadIdx.x * T + s];
-        r[threadIdx.x] = acc;
+        for (int i = lane; i < nparts; i += 32) acc += src[i];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+        if (lane == 0) {
+            int row = (int)((sqrtf(8.f * (float)entry + 1.f) - 1.f) * 0.5f);
+            while ((row + 1) * (row + 2) / 2 <= entry) ++row;
+            while (row * (row + 1) / 2 > entry) --row;
+            X[(size_t)row * N + (entry - row * (row + 1) / 2)] = (unsigned long long)acc;
+        }
+    }
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) s_last = atomicAdd(done, 1u) == gridDim.x - 1;
+    __syncthreads();
+    if (!s_last) return;
+    __threadfence();
+    if (threadIdx.x == 0) *done = 0u;                          // ready for the next launch
+    auto Xs = [&](int i, int j) -> long long { return (long long)__ldcg(i >= j ? X + (size_t)i * N + j : X + (size_t)j * N + i); };
+    for (int e0 = 0; e0 < T * T; e0 += 4 * 256) {
+        long long v[4][4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const int e = e0 + u * 256 + threadIdx.x;
+            if (e < T * T) {
+                const int t = e / T, s = e - t * T;
+                v[u][0] = Xs(t, s); v[u][1] = Xs(t, Tp + s); v[u][2] = Xs(Tp + t, s); v[u][3] = Xs(Tp + t, Tp + s);
+            }
+        }
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const int e = e0 + u * 256 + threadIdx.x;
+            if (e < T * T) G[e] = v[u][0] * 65536 + (v[u][1] + v[u][2]) * 256 + v[u][3];
+        }
     }
     __syncthreads();
-    __int128 tau = 0;
-    for (int t = 0; t < T; ++t) tau += r[t];
+    for (int t = warp; t < T; t += 8) {                        // row sums: one warp per row
+        long long acc = 0;
+        for (int s = lane; s < T; s += 32) acc += G[t * T + s];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+        if (lane == 0) r[t] = acc;
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        __int128 tau = 0;
+        for (int t = 0; t < T; ++t) tau += r[t];
+        tau_lo = (long long)(unsigned long long)tau; tau_hi = (long long)(tau >> 64);
+    }
+    __syncthreads();
+    const __int128 tau = ((__int128)tau_hi << 64) | (unsigned __int128)(unsigned long long)tau_lo;
     for (int e = threadIdx.x; e < T * T; e += blockDim.x) {
         const int t = e / T, s = e - t * T;
         const __int128 v = (__int128)(T * T) * G[e] - (__int128)T * ((__int128)r[t] + r[s]) + tau;     // = T^2 sum_x d_t d_s, exact
@@ -200,21 +272,22 @@ int holo_launch_sum_gram(holo_ctx* c, const uint16_t* frames, float2* C, cudaStr
     int grid = 3 * c->num_sms;                               // three CTAs per SM (64 KB of operand stages each)
     if ((long long)grid > nblocks) grid = (int)nblocks;
     int rc;
-    HOLO_CUDA_OK(cudaMemsetAsync(c->gram_X, 0, (size_t)N * N * sizeof(unsigned long long), st));
     {
         HoloProf prof(c, HOLO_K_SUM, st);
         if (Tp == 32) {
             if ((rc = holo_ensure_smem_attr((const void*)k_sum_gram<32>, c->device, RG_SMEM))) return rc;
-            k_sum_gram<32><<<grid, RG_THREADS, RG_SMEM, st>>>(frames, c->sum, c->gram_X, c->npix, T, c->counters);
+            k_sum_gram<32><<<grid, RG_THREADS, RG_SMEM, st>>>(frames, c->sum, c->gram_Xp, c->npix, T, c->counters);
         } else {
             if ((rc = holo_ensure_smem_attr((const void*)k_sum_gram<64>, c->device, RG_SMEM))) return rc;
-            k_sum_gram<64><<<grid, RG_THREADS, RG_SMEM, st>>>(frames, c->sum, c->gram_X, c->npix, T, c->counters);
+            k_sum_gram<64><<<grid, RG_THREADS, RG_SMEM, st>>>(frames, c->sum, c->gram_Xp, c->npix, T, c->counters);
         }
     }
     HOLO_CUDA_OK(cudaGetLastError());
     {
         HoloProf prof(c, HOLO_K_COV_REDUCE, st);
-        k_gram_finish<<<1, 256, 0, st>>>(c->gram_X, T, Tp, (double)c->npix / ((double)T * (double)T), C);
+        const int nent = N * (N + 1) / 2;
+        k_gram_reduce_finish<<<(nent + 7) / 8, 256, 0, st>>>(reinterpret_cast<const long long*>(c->gram_Xp), grid, N, c->gram_X, c->counters + 1000,
+                                                             T, Tp, (double)c->npix / ((double)T * (double)T), C);
     }
     HOLO_CUDA_OK(cudaGetLastError());
     return HOLO_OK;

@@ -170,6 +170,73 @@ def test_process_mode2_matches_oracle(torch_cuda, cfgn):
     h.close()
 
 
+# ------------------------------------------------------------------ mode 3: the image without the hologram stack
+@pytest.mark.parametrize("n,T,k_lo,k_hi", [(16, 2, 1, 2), (32, 5, 2, 5), (64, 16, 1, 16), (64, 16, 3, 15), (128, 32, 2, 32),
+                                            (256, 16, 2, 16), (64, 33, 2, 31), (128, 64, 3, 64), (512, 8, 2, 8)])
+def test_process_mode3_small_shapes(torch_cuda, n, T, k_lo, k_hi):
+    """Mode 3 (SURVEY.md 8(f)-2 stage 2): rejected components removed in the raw domain, row pass, column pass reduced to
+    sum_t |.|^2 -- against the oracle's definition (Eq. 6-7 on the hologram stack it never forms)."""
+    torch = torch_cuda
+    rng = np.random.default_rng(n + 31 * T + k_lo)
+    fr = _rand_frames(rng, T, n, n)
+    fr[: T // 2 + 1] += (rng.integers(0, 600, (n, n))).astype(np.uint16)      # a strong first component
+    h = _holo(n, n, T, k_lo, k_hi)
+    h.set_mode(3)
+    M = torch.empty((n, n), dtype=torch.float32, device="cuda")
+    h.process(_to_dev(torch, fr), M)
+    rc, st = h.status()
+    assert rc == 0, st
+    out = oracle.process(fr, LAM, PITCH, Z, k_lo, k_hi)
+    from paper_2004_00923_b200 import HOLO_WS_EVALS, HOLO_WS_V
+    ev = h.workspace_tensor(HOLO_WS_EVALS).cpu().numpy().astype(np.float64)
+    assert rel_l2(ev, out["evals"]) <= FP32_EV
+    Vg = h.workspace_tensor(HOLO_WS_V).cpu().numpy()
+    assert np.all(Vg.imag == 0), "C from the raw frames is real symmetric: V must be exactly real"
+    err = rel_l2(M.cpu().numpy(), out["M"])
+    assert err <= TOL_M and err <= FP32_M, err
+    M2 = torch.empty_like(M)
+    h.process(_to_dev(torch, fr), M2)
+    assert torch.equal(M, M2)                                                 # deterministic
+    h.close()
+
+
+@pytest.mark.parametrize("cfgn", [1, 2, 3])
+def test_process_mode3_matches_oracle_on_configs(torch_cuda, cfgn):
+    """BASELINE.json configs[0..2] at full size through mode 3 (holo_process and holo_submit)."""
+    torch = torch_cuda
+    cfg = G.CONFIGS[cfgn]
+    if cfgn == 1:
+        fr = G.stack_np(cfg, 1)
+        dev = _to_dev(torch, fr)
+    else:
+        dev = G.stream_torch(cfg, 0, "cuda", n_frames=cfg.T)
+        fr = dev.cpu().view(torch.int16).numpy().view(np.uint16)
+    ev, gaps = eig_gaps(fr)
+    assert gaps[cfg.k_lo - 2] >= 0.05
+    h = _holo(cfg.n, cfg.n, cfg.T, cfg.k_lo, cfg.k_hi)
+    h.set_mode(3)
+    M = torch.empty((cfg.n, cfg.n), dtype=torch.float32, device="cuda")
+    h.process(dev, M)
+    rc, st = h.status()
+    assert rc == 0, st
+    out = oracle.process(fr, cfg.lam, cfg.pitch, cfg.z, cfg.k_lo, cfg.k_hi)
+    err = rel_l2(M.cpu().numpy(), out["M"])
+    assert err <= TOL_M and err <= FP32_M, err
+    st2 = torch.cuda.Stream()
+    outs = [torch.zeros_like(M) for _ in range(3)]
+    torch.cuda.synchronize()
+    for o in outs:
+        h.submit(dev, o, st2)
+    h.flush(st2)
+    st2.synchronize()
+    for o in outs:
+        assert torch.equal(o, M)
+    # the paper's own window needs 12 rejected components: mode 3 refuses, nothing is launched
+    with pytest.raises(Exception):
+        h.set_range(13, cfg.T)
+    h.close()
+
+
 # ------------------------------------------------------------------ A4 holo_eig (isolated)
 def _check_eig(torch, T, C64, k_gap=None):
     h = _holo(16, 16, T, 1, T)
