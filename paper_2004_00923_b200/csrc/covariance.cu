@@ -531,6 +531,8 @@ int holo_launch_cov_reduce(holo_ctx* c, int nparts, float2* C, cudaStream_t st) 
 int holo_launch_covariance(holo_ctx* c, const float2* H, float2* C, cudaStream_t st, bool real_only) {
     const int T = c->T, T8 = (T + 7) / 8 * 8, nb = T8 / 8;
     if (nb < 1 || nb > 8) { holo_set_error("T out of range"); return HOLO_ERR_ARG; }
+    if (real_only && c->tune[HOLO_TUNE_COV_REAL] && c->tune[HOLO_TUNE_COV_TF32] && !c->center_gram && !c->cov_new_blocks && !c->ring_nrb)
+        return holo_launch_cov_tf32(c, H, C, st);
     if (real_only && c->tune[HOLO_TUNE_COV_REAL]) return launch_cov_real(c, H, C, st);
     CovPlan plan;
     make_plan(nb, &plan);

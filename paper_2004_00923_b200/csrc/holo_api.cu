@@ -141,6 +141,12 @@ static int create_impl(holo_ctx* c) {
     // per SM (64 holograms in registers) and the split loses (3.87 -> 4.30 ms), so it is off there
     c->tune[HOLO_TUNE_SPLIT_SMS] = T <= 32 ? (c->num_sms * 27 + 50) / 100 : 0;
     c->tune[HOLO_TUNE_EIG_MAX_SWEEPS] = 30;
+    // real covariance on the tensor cores (TF32, inputs rounded to nearest, accumulators added to FP64 every 4 stages = 512
+    // products): measured 584 vs 919 us at 2048^2 x 64 with 2e-6 on the eigenvalues; at T <= 32 the gain is 12 % (75 vs 85 us)
+    // and the FP32 kernel stays the default (profiles/r02_tf32_gram.md)
+    // (the rounding noise of single-pass TF32 averages out as 1 / sqrt(pixels): below 2^20 pixels the split form is used)
+    c->tune[HOLO_TUNE_COV_TF32] = (T > 32 && np % 256 == 0) ? (np >= (1ll << 20) ? 1 : 3) : 0;
+    c->tune[HOLO_TUNE_COV_TF32_DRAIN] = 4;
     c->scratch_frames = (int)grp;
     c->cov_parts_cap = 4 * c->num_sms;
     const int T8 = (T + 7) / 8 * 8;

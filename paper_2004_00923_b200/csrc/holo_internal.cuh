@@ -25,6 +25,9 @@ enum {
     HOLO_TUNE_PUSH_PIPE = 10,      // holo_push: 1 = pipelined ring form when T in {16,32,64} and n_new is a multiple of 8 (default)
     HOLO_TUNE_PUSH_INCR = 11,      // holo_push (ring form): 1 = recompute only the Gram rows / columns of the new frames (default)
     HOLO_TUNE_L2_PERSIST_MB = 12,  // experiment: cudaLimitPersistingL2CacheSize in MiB (0 = leave the device setting alone)
+    HOLO_TUNE_COV_TF32 = 13,       // real covariance of holo_process / holo_submit on the tensor cores: 0 = FP32 FFMA kernel,
+                                   // 1 = TF32 (inputs rounded to nearest), 3 = 3 x TF32 split; default 1 at T > 32, else 0
+    HOLO_TUNE_COV_TF32_DRAIN = 14, // stages accumulated in TMEM before the accumulators are added to FP64 (default 4)
     HOLO_TUNE_FFT_LAG = 6,         // frames between the row pass and the column pass in the fused kernel (0 = auto)
 };
 
@@ -144,6 +147,7 @@ int holo_launch_fresnel(holo_ctx* c, const uint16_t* frames, float2* H, cudaStre
 // C == nullptr: partials only; holo_launch_cov_reduce then finishes (possibly on another stream, ordered after)
 int holo_launch_covariance(holo_ctx* c, const float2* H, float2* C, cudaStream_t st, bool real_only = false);
 int holo_launch_cov_reduce(holo_ctx* c, int nparts, float2* C, cudaStream_t st);
+int holo_launch_cov_tf32(holo_ctx* c, const float2* H, float2* C, cudaStream_t st);   // covtf32.cu
 // cudaFuncSetAttribute / occupancy are properties of a (function, device) pair: cached per pair, thread-safe
 int holo_ensure_smem_attr(const void* func, int device, size_t bytes);
 int holo_cached_occupancy(const void* func, int device, int threads, size_t smem, int* blocks_per_sm);

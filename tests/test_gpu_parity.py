@@ -170,6 +170,43 @@ def test_process_mode2_matches_oracle(torch_cuda, cfgn):
     h.close()
 
 
+# ------------------------------------------------------------------ A3 on the tensor cores (TF32)
+@pytest.mark.parametrize("n,T,variant", [(64, 64, 1), (64, 64, 3), (64, 33, 1), (128, 47, 3), (64, 32, 1), (128, 16, 3), (32, 5, 3), (256, 64, 1), (512, 64, 1)])
+def test_process_covariance_tf32(torch_cuda, n, T, variant):
+    """The real covariance of holo_process through tcgen05.mma kind::tf32 (tune key 13; default at T > 32): C against the
+    exact integer Gram, eigenvalues and image against the oracle."""
+    torch = torch_cuda
+    from tests.util import integer_gram
+    from paper_2004_00923_b200 import HOLO_WS_C, HOLO_WS_EVALS
+    rng = np.random.default_rng(7 * n + T)
+    fr = _rand_frames(rng, T, n, n)
+    fr[: T // 2 + 1] += (rng.integers(0, 600, (n, n))).astype(np.uint16)
+    h = _holo(n, n, T, 2, T)
+    h.tune(13, variant)
+    M = torch.empty((n, n), dtype=torch.float32, device="cuda")
+    h.process(_to_dev(torch, fr), M)
+    rc, st = h.status()
+    assert rc == 0, st
+    Gi, _ = integer_gram(fr)
+    ref = np.array([[float(int(Gi[t, s]) * (n * n)) / float(T * T) for s in range(T)] for t in range(T)])
+    Cg = h.workspace_tensor(HOLO_WS_C).cpu().numpy()
+    assert np.all(Cg.imag == 0) and np.array_equal(Cg.real, Cg.real.T)
+    # 3 x TF32 keeps the FP32 bound at any size; single-pass TF32 carries a rounding noise of 2^-11 per operand that averages
+    # out over the 2 n^2 products of an entry (measured 2.7e-5 at 64^2, 7e-7 at 1024^2): bound 5e-3 / sqrt(2 n^2) + 3e-6
+    bound = FP32_C if variant == 3 else 5e-3 / np.sqrt(2.0 * n * n) + 3e-6
+    errC = rel_l2(Cg.real.astype(np.float64), ref)
+    assert errC <= TOL_STAGE and errC <= bound, errC
+    out = oracle.process(fr, LAM, PITCH, Z, 2, T)
+    ev = h.workspace_tensor(HOLO_WS_EVALS).cpu().numpy().astype(np.float64)
+    assert rel_l2(ev, out["evals"]) <= (FP32_EV if variant == 3 else min(TOL_EV, 2 * bound))
+    err = rel_l2(M.cpu().numpy(), out["M"])
+    assert err <= TOL_M and err <= (FP32_M if variant == 3 else max(FP32_M, 4 * bound)), err
+    M2 = torch.empty_like(M)
+    h.process(_to_dev(torch, fr), M2)
+    assert torch.equal(M, M2)
+    h.close()
+
+
 # ------------------------------------------------------------------ mode 3: the image without the hologram stack
 @pytest.mark.parametrize("n,T,k_lo,k_hi", [(16, 2, 1, 2), (32, 5, 2, 5), (64, 16, 1, 16), (64, 16, 3, 15), (128, 32, 2, 32),
                                             (256, 16, 2, 16), (64, 33, 2, 31), (128, 64, 3, 64), (512, 8, 2, 8)])
