@@ -258,6 +258,198 @@ k_eig(const float2* __restrict__ C, int T, float* __restrict__ evals, float2* __
     }
 }
 
+// ------------------------------------------------------------------------------------------------
+// Real symmetric form of the same solver.  Inside holo_process / holo_submit / holo_push the covariance is real
+// symmetric in exact arithmetic (R21: holograms of real frames; exactly so when it comes from the integer Gram
+// of the raw frames), and it is stored with Im = 0: rotations, updates and eigenvectors are then real, the step body is
+// 60 % of the complex one (it is bound by instruction issue: one thread per 2x2 block, two rotations per thread) and
+// the shared-memory footprint is halved.  Same ordering, thresholds, FP64 refinement, sorting and sign convention
+// (largest-magnitude entry positive), same status words.
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ bool jacobi_rot_real(float app, float aqq, float apq, float thr2, float& c, float& s) {
+    const float mag2 = apq * apq;
+    const bool rot = mag2 > thr2;
+    const float d = aqq - app;
+    const float x = fmaxf(fmaf(d, d, 4.f * mag2), 1e-36f);
+    const float root = x * rsqrt_fast(x);
+    const float u = copysignf(2.f, d) * rcp_fast(fabsf(d) + root);      // t / |apq|
+    const float cc = rsqrt_fast(fmaf(u * u, mag2, 1.f));
+    const float uc = rot ? u * cc : 0.f;
+    c = rot ? cc : 1.f;
+    s = apq * uc;
+    return rot;
+}
+
+template <int TP>
+__global__ void __launch_bounds__((TP / 2) * (TP / 2) < 32 ? 32 : (TP / 2) * (TP / 2), 1)
+k_eig_real(const float2* __restrict__ C, int T, float* __restrict__ evals, float2* __restrict__ Vout,
+           int32_t* __restrict__ status, int max_sweeps, int32_t* __restrict__ noconv) {
+    extern __shared__ __align__(16) unsigned char raw[];
+    constexpr int Tp = TP, LD = TP + 2, half = TP / 2, m = TP - 1;   // LD even: pairs 8-byte aligned
+    float* A0 = reinterpret_cast<float*>(raw);
+    float* A1 = A0 + Tp * LD;
+    float* V0 = A1 + Tp * LD;
+    float* V1 = V0 + Tp * LD;
+    float* Cs = V1 + Tp * LD;                                       // [T][T] full symmetric copy of the input
+    float* red = Cs + Tp * Tp;                                      // [32]
+    double* lam = reinterpret_cast<double*>(red + 32);              // [Tp]
+    double* dscr = lam + Tp;                                        // [T*T]
+
+    const int tid = threadIdx.x, nt = blockDim.x;
+    const long long clk0 = clock64();
+    float dmax = 0.f;
+    for (int i = tid; i < T * T; i += nt) {
+        const int r = i / T, c = i - r * T;
+        const float a = c <= r ? C[i].x : C[c * T + r].x;           // lower triangle
+        Cs[i] = a;
+        dmax = fmaxf(dmax, fabsf(a));
+    }
+#pragma unroll
+    for (int o = 16; o >= 1; o >>= 1) dmax = fmaxf(dmax, __shfl_xor_sync(0xffffffffu, dmax, o));
+    if ((tid & 31) == 0) red[tid >> 5] = dmax;
+    __syncthreads();
+    dmax = 0.f;
+    for (int w = 0; w < (nt >> 5); ++w) dmax = fmaxf(dmax, red[w]);
+    int ex = 0;
+    if (dmax > 0.f && dmax < 3.0e38f) frexpf(dmax, &ex);
+    const float scale = ldexpf(1.f, -ex);
+    float n2 = 0.f;
+    for (int i = tid; i < Tp * Tp; i += nt) {
+        const int r = i / Tp, c = i - r * Tp;
+        float a = 0.f;
+        if (r < T && c < T) a = Cs[r * T + c] * scale;
+        A0[r * LD + c] = a;
+        V0[r * LD + c] = r == c ? 1.f : 0.f;
+        n2 = fmaf(a, a, n2);
+    }
+    const float normF2 = block_sum(n2, red);
+    const float eps = 5.96e-8f;
+    const float thr2 = (0.25f * eps * eps / (float)(T * T)) * normF2;
+    const float tol2 = (float)(T * T) * eps * eps * normF2;
+
+    const int bi = tid / half, bj = tid % half;
+    const bool worker = tid < half * half;
+    const int r0 = 2 * bi, c0 = 2 * bj;
+    const int rd0 = rr_next(r0, Tp), rd1 = rr_next(r0 + 1, Tp), cd0 = rr_next(c0, Tp), cd1 = rr_next(c0 + 1, Tp);
+    const int oB0 = r0 * LD + c0, oB1 = oB0 + LD;
+    const int oDi = r0 * LD + r0, oDj = c0 * LD + c0;
+    const int w00 = rd0 * LD + cd0, w01 = rd0 * LD + cd1, w10 = rd1 * LD + cd0, w11 = rd1 * LD + cd1;
+    const int wv00 = r0 * LD + cd0, wv01 = r0 * LD + cd1, wv10 = wv00 + LD, wv11 = wv01 + LD;
+    float *Ac = A0, *An = A1, *Vc = V0, *Vn = V1;
+    int sweeps = 0, converged = 0, last_rot = 0;
+    const long long clk1 = clock64();
+    for (; sweeps < max_sweeps; ++sweeps) {
+        float o2 = 0.f;
+        for (int i = tid; i < Tp * Tp; i += nt) {
+            const int r = i / Tp, c = i - r * Tp;
+            if (r != c) { const float a = Ac[r * LD + c]; o2 = fmaf(a, a, o2); }
+        }
+        const float off2 = block_sum(o2, red);
+        if (off2 <= tol2) { converged = 1; break; }
+        int applied = 0;
+#pragma unroll 1
+        for (int step = 0; step < m; ++step) {
+            if (worker) {
+                const float2 di = *reinterpret_cast<const float2*>(Ac + oDi);       // [app, apq]
+                const float aqqi = Ac[oDi + LD + 1];
+                const float2 dj = *reinterpret_cast<const float2*>(Ac + oDj);
+                const float aqqj = Ac[oDj + LD + 1];
+                const float2 B0 = *reinterpret_cast<const float2*>(Ac + oB0);       // [b00, b01]
+                const float2 B1 = *reinterpret_cast<const float2*>(Ac + oB1);       // [b10, b11]
+                const float2 U0 = *reinterpret_cast<const float2*>(Vc + oB0);
+                const float2 U1 = *reinterpret_cast<const float2*>(Vc + oB1);
+                float ci, cj, si, sj;
+                const bool ri = jacobi_rot_real(di.x, aqqi, di.y, thr2, ci, si);
+                jacobi_rot_real(dj.x, aqqj, dj.y, thr2, cj, sj);
+                applied += (bi == bj) && ri;
+                // B' = J_i^T B J_j,  J = [[c, s], [-s, c]]
+                const float x00 = fmaf(cj, B0.x, -sj * B0.y), x01 = fmaf(cj, B0.y, sj * B0.x);
+                const float x10 = fmaf(cj, B1.x, -sj * B1.y), x11 = fmaf(cj, B1.y, sj * B1.x);
+                float y00 = fmaf(ci, x00, -si * x10), y10 = fmaf(ci, x10, si * x00);
+                float y01 = fmaf(ci, x01, -si * x11), y11 = fmaf(ci, x11, si * x01);
+                if (bi == bj && ri) { y01 = 0.f; y10 = 0.f; }                       // the pivot block: exactly diagonal afterwards
+                An[w00] = y00; An[w01] = y01; An[w10] = y10; An[w11] = y11;
+                Vn[wv00] = fmaf(cj, U0.x, -sj * U0.y); Vn[wv01] = fmaf(cj, U0.y, sj * U0.x);
+                Vn[wv10] = fmaf(cj, U1.x, -sj * U1.y); Vn[wv11] = fmaf(cj, U1.y, sj * U1.x);
+            }
+            __syncthreads();
+            float* tmp = Ac; Ac = An; An = tmp;
+            tmp = Vc; Vc = Vn; Vn = tmp;
+        }
+        last_rot = (int)(block_sum((float)applied, red) + 0.5f);
+        if (last_rot == 0) { converged = 1; ++sweeps; break; }
+    }
+    __syncthreads();
+    const long long clk2 = clock64();
+    const float* V = Vc;
+    {   // FP64 Rayleigh quotients against the original C
+        constexpr int RB = 4;
+        const int k = tid % T, g = tid / T, ng = nt / T > 0 ? nt / T : 1;
+        for (int tb = g * RB; tb < T && tid < ng * T; tb += ng * RB) {
+            double wr[RB];
+#pragma unroll
+            for (int j = 0; j < RB; ++j) wr[j] = 0.0;
+            for (int s = 0; s < T; ++s) {
+                const double vx = (double)V[s * LD + k];
+#pragma unroll
+                for (int j = 0; j < RB; ++j) wr[j] += (double)Cs[min(tb + j, T - 1) * T + s] * vx;
+            }
+#pragma unroll
+            for (int j = 0; j < RB; ++j) {
+                const int t = tb + j;
+                if (t < T) dscr[t * T + k] = (double)V[t * LD + k] * wr[j];
+            }
+        }
+    }
+    __syncthreads();
+    if (tid < T) {
+        double l = 0.0, nn = 0.0;
+        for (int t = 0; t < T; ++t) { l += dscr[t * T + tid]; const double v = (double)V[t * LD + tid]; nn += v * v; }
+        lam[tid] = nn > 0.0 ? l / nn : 0.0;
+    }
+    __syncthreads();
+    if (tid < T) {
+        const double l = lam[tid];
+        int r = 0;
+        for (int j = 0; j < T; ++j) { const double lj = lam[j]; r += (lj > l) || (lj == l && j < tid); }
+        float best = -1.f, bv = 1.f, nn = 0.f;
+        for (int t = 0; t < T; ++t) {
+            const float v = V[t * LD + tid];
+            const float a2 = v * v;
+            nn += a2;
+            if (a2 > best) { best = a2; bv = v; }
+        }
+        const float sgn = (best > 0.f) ? copysignf(1.f / sqrtf(nn), bv) : 1.f;      // normalise, largest-magnitude entry positive
+        for (int t = 0; t < T; ++t) Vout[t * T + r] = make_float2(V[t * LD + tid] * sgn, 0.f);
+        evals[r] = (float)l;
+    }
+    if (tid == 0) {
+        status[0] = converged ? 0 : 1;
+        status[1] = sweeps;
+        status[2] = last_rot;
+        status[3] = 0;
+        status[4] = (int)(clk1 - clk0);
+        status[5] = (int)(clk2 - clk1);
+        status[6] = (int)(clock64() - clk2);
+        status[7] = 0;
+        if (!converged && noconv) { *(volatile int32_t*)noconv = 1; __threadfence_system(); }
+    }
+}
+
+template <int TP>
+static int launch_eig_real_t(holo_ctx* c, const float2* C, float* evals, float2* V, cudaStream_t st) {
+    const int T = c->T;
+    constexpr int LD = TP + 2;
+    constexpr size_t smem = (size_t)4 * TP * LD * sizeof(float) + (size_t)TP * TP * sizeof(float) + 32 * sizeof(float)
+                          + TP * sizeof(double) + (size_t)TP * TP * sizeof(double);
+    { const int rc = holo_ensure_smem_attr((const void*)k_eig_real<TP>, c->device, smem); if (rc) return rc; }
+    constexpr int threads = (TP / 2) * (TP / 2) < 32 ? 32 : (TP / 2) * (TP / 2);
+    HoloProf prof(c, HOLO_K_EIG, st);
+    k_eig_real<TP><<<1, threads, smem, st>>>(C, T, evals, V, c->status, c->tune[HOLO_TUNE_EIG_MAX_SWEEPS], c->noconv_dev);
+    HOLO_CUDA_OK(cudaGetLastError());
+    return HOLO_OK;
+}
+
 template <int TP>
 static int launch_eig_t(holo_ctx* c, const float2* C, float* evals, float2* V, cudaStream_t st) {
     const int T = c->T;
@@ -273,8 +465,15 @@ static int launch_eig_t(holo_ctx* c, const float2* C, float* evals, float2* V, c
     return HOLO_OK;
 }
 
-int holo_launch_eig(holo_ctx* c, const float2* C, float* evals, float2* V, cudaStream_t st) {
+int holo_launch_eig(holo_ctx* c, const float2* C, float* evals, float2* V, cudaStream_t st, bool real_symmetric) {
     const int T = c->T;
+    if (real_symmetric) {
+        if (T <= 4) return launch_eig_real_t<4>(c, C, evals, V, st);
+        if (T <= 8) return launch_eig_real_t<8>(c, C, evals, V, st);
+        if (T <= 16) return launch_eig_real_t<16>(c, C, evals, V, st);
+        if (T <= 32) return launch_eig_real_t<32>(c, C, evals, V, st);
+        return launch_eig_real_t<64>(c, C, evals, V, st);
+    }
     if (T <= 4) return launch_eig_t<4>(c, C, evals, V, st);
     if (T <= 8) return launch_eig_t<8>(c, C, evals, V, st);
     if (T <= 16) return launch_eig_t<16>(c, C, evals, V, st);

@@ -292,20 +292,20 @@ extern "C" int holo_process(holo_ctx* c, const uint16_t* frames_dev, float* imag
         // mode 2's covariance and eigenvectors, then the image straight from the raw frames: rejected components removed in
         // the raw domain, row pass, column pass reduced to sum_t |.|^2 -- no hologram stack, no projection kernel
         if ((rc = holo_launch_sum_gram(c, frames_dev, c->C, st))) return rc;
-        if ((rc = holo_launch_eig(c, c->C, c->evals, c->V, st))) return rc;
+        if ((rc = holo_launch_eig(c, c->C, c->evals, c->V, st, true))) return rc;
         return holo_launch_energy_image(c, frames_dev, c->V, c->k_lo, c->k_hi, image_dev, st);
     }
     if (c->mode == 2) {
         // covariance from the raw frames (exact integer Gram on the tensor cores, fused with the temporal sum): C and V are
         // known BEFORE the holograms exist, and the hologram stack is read once (projection) instead of twice
         if ((rc = holo_launch_sum_gram(c, frames_dev, c->C, st))) return rc;
-        if ((rc = holo_launch_eig(c, c->C, c->evals, c->V, st))) return rc;
+        if ((rc = holo_launch_eig(c, c->C, c->evals, c->V, st, true))) return rc;
         if ((rc = holo_launch_fresnel(c, frames_dev, c->H, st, /*with_sum=*/false, -1, /*counters_zeroed=*/true))) return rc;
         return holo_launch_project(c, c->H, c->V, c->k_lo, c->k_hi, c->tune[HOLO_TUNE_PROJ_COMPLEMENT], image_dev, st);
     }
     if ((rc = holo_launch_fresnel(c, frames_dev, c->H, st))) return rc;
     if ((rc = holo_launch_covariance(c, c->H, c->C, st, /*real_only=*/true))) return rc;
-    if ((rc = holo_launch_eig(c, c->C, c->evals, c->V, st))) return rc;
+    if ((rc = holo_launch_eig(c, c->C, c->evals, c->V, st, c->tune[HOLO_TUNE_COV_REAL] != 0))) return rc;
     return holo_launch_project(c, c->H, c->V, c->k_lo, c->k_hi, c->tune[HOLO_TUNE_PROJ_COMPLEMENT], image_dev, st);
 }
 
@@ -411,7 +411,7 @@ extern "C" int holo_submit(holo_ctx* c, const uint16_t* frames_dev, float* image
         HOLO_CUDA_OK(cudaStreamWaitEvent(c->side, c->ev_cov[s], 0));
         int32_t* status_main = c->status;
         if (s) c->status = c->status1;
-        rc = holo_launch_eig(c, s ? c->C1 : c->C, s ? c->evals1 : c->evals, s ? c->V1 : c->V, c->side);
+        rc = holo_launch_eig(c, s ? c->C1 : c->C, s ? c->evals1 : c->evals, s ? c->V1 : c->V, c->side, true);
         c->status = status_main;
         if (rc) return rc;
         HOLO_CUDA_OK(cudaEventRecord(c->ev_eig[s], c->side));
@@ -429,7 +429,7 @@ extern "C" int holo_submit(holo_ctx* c, const uint16_t* frames_dev, float* image
         if ((rc = holo_launch_sum_gram(c, frames_dev, c->C, st))) return rc;
         HOLO_CUDA_OK(cudaEventRecord(c->ev_cov[0], st));
         HOLO_CUDA_OK(cudaStreamWaitEvent(c->side, c->ev_cov[0], 0));
-        if ((rc = holo_launch_eig(c, c->C, c->evals, c->V, c->side))) return rc;
+        if ((rc = holo_launch_eig(c, c->C, c->evals, c->V, c->side, true))) return rc;
         HOLO_CUDA_OK(cudaEventRecord(c->ev_eig[0], c->side));
         if ((rc = holo_launch_fresnel(c, frames_dev, c->H, st, /*with_sum=*/false, -1, /*counters_zeroed=*/true))) return rc;
         HOLO_CUDA_OK(cudaStreamWaitEvent(st, c->ev_eig[0], 0));
@@ -455,7 +455,7 @@ extern "C" int holo_submit(holo_ctx* c, const uint16_t* frames_dev, float* image
     HOLO_CUDA_OK(cudaStreamWaitEvent(c->side, c->ev_cov[s], 0));
     int32_t* status_main = c->status;
     if (s) c->status = c->status1;
-    rc = holo_launch_eig(c, C, s ? c->evals1 : c->evals, s ? c->V1 : c->V, c->side);
+    rc = holo_launch_eig(c, C, s ? c->evals1 : c->evals, s ? c->V1 : c->V, c->side, c->tune[HOLO_TUNE_COV_REAL] != 0);
     c->status = status_main;
     if (rc) return rc;
     HOLO_CUDA_OK(cudaEventRecord(c->ev_eig[s], c->side));
@@ -564,7 +564,7 @@ extern "C" int holo_push(holo_ctx* c, const uint16_t* new_frames_dev, int n_new,
         rc = holo_launch_covariance(c, c->H, c->C, st, /*real_only=*/true);
         c->center_gram = 0;
         if (rc) return rc;
-        if ((rc = holo_launch_eig(c, c->C, c->evals, c->V, st))) return rc;
+        if ((rc = holo_launch_eig(c, c->C, c->evals, c->V, st, c->tune[HOLO_TUNE_COV_REAL] != 0))) return rc;
         return holo_launch_project(c, c->H, c->V, c->k_lo, c->k_hi, /*allow_complement=*/1, image_dev, st, /*center=*/1);
     }
     // pipelined form (same structure as holo_submit): eigensolver + projection on the side stream; the image is
@@ -587,7 +587,7 @@ extern "C" int holo_push(holo_ctx* c, const uint16_t* new_frames_dev, int n_new,
     if (!rc) {
         int32_t* status_main = c->status;
         if (s) c->status = c->status1;
-        rc = holo_launch_eig(c, C, s ? c->evals1 : c->evals, s ? c->V1 : c->V, c->side);
+        rc = holo_launch_eig(c, C, s ? c->evals1 : c->evals, s ? c->V1 : c->V, c->side, c->tune[HOLO_TUNE_COV_REAL] != 0);
         c->status = status_main;
     }
     if (!rc) {

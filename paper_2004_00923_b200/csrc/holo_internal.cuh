@@ -151,7 +151,8 @@ int holo_launch_cov_tf32(holo_ctx* c, const float2* H, float2* C, cudaStream_t s
 // cudaFuncSetAttribute / occupancy are properties of a (function, device) pair: cached per pair, thread-safe
 int holo_ensure_smem_attr(const void* func, int device, size_t bytes);
 int holo_cached_occupancy(const void* func, int device, int threads, size_t smem, int* blocks_per_sm);
-int holo_launch_eig(holo_ctx* c, const float2* C, float* evals, float2* V, cudaStream_t st);
+// real_symmetric: the caller guarantees Im C = 0 (stored so): real rotations, real eigenvectors (Im V = 0 exactly)
+int holo_launch_eig(holo_ctx* c, const float2* C, float* evals, float2* V, cudaStream_t st, bool real_symmetric = false);
 // mode 0: direct over columns [k_lo,k_hi] of V; mode 1: complement (total - columns outside)
 int holo_launch_project(holo_ctx* c, const float2* H, const float2* V, int k_lo, int k_hi,
                         int allow_complement, float* image, cudaStream_t st, int center = 0);
