@@ -272,35 +272,56 @@ __global__ void __launch_bounds__(256) k_sum_partial_images(const float* __restr
     }
 }
 
-// eT_k(x) = sum_t (T I_t(x) - S(x)) V_{t,k} for the rejected components k (column indices cols[kk] of V), and the
-// coefficient table coef[t][kk] = Re V_{t,cols[kk]}.  One thread per pixel pair.
+// eT_k(x) = sum_t (T I_t(x) - S(x)) V_{t,k} for the rejected components k (column indices of V: c0_lo + kk for kk < c0_n,
+// then c1_lo + ...), and the coefficient table coef[t][kk] = Re V_{t,k}.  Eight pixels per thread (16-byte loads, eight
+// frames in flight), NDEFL accumulators per pixel.
+template <int NDEFL>
 __global__ void __launch_bounds__(256) k_deflate_images(const uint16_t* __restrict__ frames, const uint32_t* __restrict__ sum,
-                                                        const float2* __restrict__ V, long long npix, int T, int ndefl,
+                                                        const float2* __restrict__ V, long long npix, int T,
                                                         int c0_lo, int c0_n, int c1_lo, float* __restrict__ img, float* __restrict__ coef) {
-    __shared__ float Vs[HOLO_MAX_T * 4];
-    for (int i = threadIdx.x; i < T * ndefl; i += blockDim.x) {
-        const int t = i / ndefl, kk = i - t * ndefl;
+    __shared__ float Vs[HOLO_MAX_T * NDEFL];
+    for (int i = threadIdx.x; i < T * NDEFL; i += blockDim.x) {
+        const int t = i / NDEFL, kk = i - t * NDEFL;
         const int col = kk < c0_n ? c0_lo + kk : c1_lo + (kk - c0_n);
         const float v = V[t * T + col].x;
         Vs[i] = v;
         if (blockIdx.x == 0) coef[i] = v;
     }
     __syncthreads();
-    const long long npair = npix >> 1;
-    for (long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x; q < npair; q += (long long)gridDim.x * blockDim.x) {
-        const uint2 S = reinterpret_cast<const uint2*>(sum)[q];
-        float e0[4] = {0.f, 0.f, 0.f, 0.f}, e1[4] = {0.f, 0.f, 0.f, 0.f};
+    const long long nvec = npix >> 3;
+    const float Tf = (float)T;
+    for (long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x; q < nvec; q += (long long)gridDim.x * blockDim.x) {
+        const uint4 sa = __ldg(reinterpret_cast<const uint4*>(sum) + 2 * q), sb = __ldg(reinterpret_cast<const uint4*>(sum) + 2 * q + 1);
+        const float S[8] = {(float)sa.x, (float)sa.y, (float)sa.z, (float)sa.w, (float)sb.x, (float)sb.y, (float)sb.z, (float)sb.w};   // < 2^22: exact
+        float e[NDEFL][8];
+#pragma unroll
+        for (int kk = 0; kk < NDEFL; ++kk)
+#pragma unroll
+            for (int x = 0; x < 8; ++x) e[kk][x] = 0.f;
+        const uint4* src = reinterpret_cast<const uint4*>(frames) + q;
 #pragma unroll 8
         for (int t = 0; t < T; ++t) {
-            const uint32_t w = __ldg(reinterpret_cast<const uint32_t*>(frames + (long long)t * npix) + q);
-            const float d0 = (float)(T * (int)(w & 0xffffu) - (int)S.x), d1 = (float)(T * (int)(w >> 16) - (int)S.y);
+            const uint4 w = __ldg(src + (long long)t * nvec);
+            const uint32_t ws[4] = {w.x, w.y, w.z, w.w};
+            float d[8];
 #pragma unroll
-            for (int kk = 0; kk < 4; ++kk)
-                if (kk < ndefl) { const float v = Vs[t * ndefl + kk]; e0[kk] = fmaf(d0, v, e0[kk]); e1[kk] = fmaf(d1, v, e1[kk]); }
+            for (int x = 0; x < 4; ++x) {
+                d[2 * x] = fmaf(Tf, (float)(ws[x] & 0xffffu), -S[2 * x]);          // T I - S: integers below 2^23, exact in FP32
+                d[2 * x + 1] = fmaf(Tf, (float)(ws[x] >> 16), -S[2 * x + 1]);
+            }
+#pragma unroll
+            for (int kk = 0; kk < NDEFL; ++kk) {
+                const float v = Vs[t * NDEFL + kk];
+#pragma unroll
+                for (int x = 0; x < 8; ++x) e[kk][x] = fmaf(d[x], v, e[kk][x]);
+            }
         }
 #pragma unroll
-        for (int kk = 0; kk < 4; ++kk)
-            if (kk < ndefl) reinterpret_cast<float2*>(img + (long long)kk * npix)[q] = make_float2(e0[kk], e1[kk]);
+        for (int kk = 0; kk < NDEFL; ++kk) {
+            float4* dst = reinterpret_cast<float4*>(img + (long long)kk * npix) + 2 * q;
+            dst[0] = make_float4(e[kk][0], e[kk][1], e[kk][2], e[kk][3]);
+            dst[1] = make_float4(e[kk][4], e[kk][5], e[kk][6], e[kk][7]);
+        }
     }
 }
 
@@ -652,10 +673,15 @@ int holo_launch_energy_image(holo_ctx* c, const uint16_t* frames, const float2* 
     if (ndefl > 4) { holo_set_error("mode 3 removes at most 4 components in the raw domain (asked for %d)", ndefl); return HOLO_ERR_STATE; }
     if (ndefl > 0) {
         HoloProf prof(c, HOLO_K_SUM, st);
-        const long long npair = c->npix >> 1;
-        long long want = (npair + 255) / 256;
+        const long long nvec = c->npix >> 3;
+        long long want = (nvec + 255) / 256;
         const int grid = (int)(want < (long long)c->num_sms * 8 ? want : (long long)c->num_sms * 8);
-        k_deflate_images<<<grid, 256, 0, st>>>(frames, c->sum, V, c->npix, T, ndefl, 0, n0, k_hi, c->defl_img, c->defl_coef);
+        switch (ndefl) {
+            case 1: k_deflate_images<1><<<grid, 256, 0, st>>>(frames, c->sum, V, c->npix, T, 0, n0, k_hi, c->defl_img, c->defl_coef); break;
+            case 2: k_deflate_images<2><<<grid, 256, 0, st>>>(frames, c->sum, V, c->npix, T, 0, n0, k_hi, c->defl_img, c->defl_coef); break;
+            case 3: k_deflate_images<3><<<grid, 256, 0, st>>>(frames, c->sum, V, c->npix, T, 0, n0, k_hi, c->defl_img, c->defl_coef); break;
+            default: k_deflate_images<4><<<grid, 256, 0, st>>>(frames, c->sum, V, c->npix, T, 0, n0, k_hi, c->defl_img, c->defl_coef); break;
+        }
         HOLO_CUDA_OK(cudaGetLastError());
     }
     FftArgs a{};

@@ -404,11 +404,12 @@ extern "C" int holo_submit(holo_ctx* c, const uint16_t* frames_dev, float* image
         const int s = (int)(c->nsubmit & 1);
         uint32_t* sum_main = c->sum;
         if (s) c->sum = c->sum1;
-        rc = holo_launch_sum_gram(c, frames_dev, s ? c->C1 : c->C, st);
+        rc = holo_launch_sum_gram(c, frames_dev, s ? c->C1 : c->C, st, /*finish=*/false);
         c->sum = sum_main;
         if (rc) return rc;
         HOLO_CUDA_OK(cudaEventRecord(c->ev_cov[s], st));
         HOLO_CUDA_OK(cudaStreamWaitEvent(c->side, c->ev_cov[s], 0));
+        if ((rc = holo_launch_gram_finish(c, s ? c->C1 : c->C, c->side))) return rc;     // off the main stream's critical path
         int32_t* status_main = c->status;
         if (s) c->status = c->status1;
         rc = holo_launch_eig(c, s ? c->C1 : c->C, s ? c->evals1 : c->evals, s ? c->V1 : c->V, c->side, true);
@@ -426,9 +427,10 @@ extern "C" int holo_submit(holo_ctx* c, const uint16_t* frames_dev, float* image
         // frames), so the projection follows in stream order and the image is complete when this call's work is done
         if ((rc = submit_init(c, /*second_stack=*/false))) return rc;
         c->push_ready = 0;
-        if ((rc = holo_launch_sum_gram(c, frames_dev, c->C, st))) return rc;
+        if ((rc = holo_launch_sum_gram(c, frames_dev, c->C, st, /*finish=*/false))) return rc;
         HOLO_CUDA_OK(cudaEventRecord(c->ev_cov[0], st));
         HOLO_CUDA_OK(cudaStreamWaitEvent(c->side, c->ev_cov[0], 0));
+        if ((rc = holo_launch_gram_finish(c, c->C, c->side))) return rc;
         if ((rc = holo_launch_eig(c, c->C, c->evals, c->V, c->side, true))) return rc;
         HOLO_CUDA_OK(cudaEventRecord(c->ev_eig[0], c->side));
         if ((rc = holo_launch_fresnel(c, frames_dev, c->H, st, /*with_sum=*/false, -1, /*counters_zeroed=*/true))) return rc;

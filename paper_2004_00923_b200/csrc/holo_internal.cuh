@@ -76,6 +76,7 @@ struct holo_ctx {
     uint32_t* sum1;         // mode 3, streaming form: frame sum of the second slot
     const uint16_t* pend3_frames; float* pend3_image; int pend3_slot;   // mode 3, streaming form: the stack whose image is owed
     unsigned long long* gram_X;   // [128][128] int64 byte-plane Gram of the raw frames (mode 2, rawgram.cu)
+    int gram_nparts;              // CTAs of the last k_sum_gram launch
     unsigned long long* gram_Xp;  // [N (N + 1) / 2][3 num_sms] per-CTA partials of it (N = 64 or 128)
     int mode;               // 1: covariance from the hologram stack (Eq. 4 as written); 2: from the raw frames
     int32_t* status;        // [8], see HOLO_WS_STATUS
@@ -165,7 +166,8 @@ int holo_launch_normalize(holo_ctx* c, float* image, cudaStream_t st);
 int holo_launch_fftshift(holo_ctx* c, const float* in, float* out, cudaStream_t st);
 int holo_launch_svd_filter(holo_ctx* c, const float2* H, const float2* V, int k_lo, int k_hi, float2* Hf, cudaStream_t st);
 // mode 2: S = sum_t I_t and C = nx ny D^T D from the raw frames (tcgen05 int8 Gram, rawgram.cu)
-int holo_launch_sum_gram(holo_ctx* c, const uint16_t* frames, float2* C, cudaStream_t st);
+int holo_launch_sum_gram(holo_ctx* c, const uint16_t* frames, float2* C, cudaStream_t st, bool finish = true);
+int holo_launch_gram_finish(holo_ctx* c, float2* C, cudaStream_t st);
 // round-2 Fresnel kernel (fresnel2.cu): packed two-sequence FFT, TMA-staged column tiles; 1024 x 1024 frames
 bool holo_fresnel2_supported(const holo_ctx* c);
 int holo_launch_fresnel2(holo_ctx* c, const uint16_t* frames, float2* H, cudaStream_t st, int nproc);

@@ -122,7 +122,7 @@ k_sum_gram(const uint16_t* __restrict__ frames, uint32_t* __restrict__ sum, unsi
 
     // software pipeline: the loads of block n + 1 are in flight (T per thread) while block n is split into byte planes
     constexpr bool PF = TP <= 32;                              // (at TP = 64 the second register set would spill)
-    uint32_t w[TP], wn[PF ? TP : 1];
+    uint32_t w[TP], wn[PF ? TP : 1], wn2[PF ? TP : 1];
     auto load_block = [&](long long blk, uint32_t* dst) {
         const long long q0 = blk * RG_PIX + 2 * tid;
         const bool ok = q0 + 1 < npix;                         // npix is a multiple of 256 for every supported frame size
@@ -130,14 +130,15 @@ k_sum_gram(const uint16_t* __restrict__ frames, uint32_t* __restrict__ sum, unsi
         for (int t = 0; t < TP; ++t) dst[t] = (ok && t < T) ? __ldg(reinterpret_cast<const uint32_t*>(frames + (size_t)t * npix + q0)) : 0u;
     };
     if (PF && (long long)blockIdx.x < nblocks) load_block(blockIdx.x, wn);
+    if (PF && (long long)blockIdx.x + gridDim.x < nblocks) load_block((long long)blockIdx.x + gridDim.x, wn2);
     for (long long blk = blockIdx.x; blk < nblocks; blk += gridDim.x, ++it) {
         const int s = it & 1;
         const long long p0 = blk * RG_PIX + 2 * tid;           // the thread's two pixels
         const bool inb = p0 + 1 < npix;
         if constexpr (PF) {
 #pragma unroll
-            for (int t = 0; t < TP; ++t) w[t] = wn[t];
-            if (blk + gridDim.x < nblocks) load_block(blk + gridDim.x, wn);
+            for (int t = 0; t < TP; ++t) { w[t] = wn[t]; wn[t] = wn2[t]; }
+            if (blk + 2 * (long long)gridDim.x < nblocks) load_block(blk + 2 * (long long)gridDim.x, wn2);
         } else {
             load_block(blk, w);
         }
@@ -264,9 +265,12 @@ __global__ void __launch_bounds__(256) k_gram_reduce_finish(const long long* __r
 
 }  // namespace
 
-// S = sum_t I_t (ctx->sum) and C = H^H H of the holograms these frames WOULD give, without forming them
-int holo_launch_sum_gram(holo_ctx* c, const uint16_t* frames, float2* C, cudaStream_t st) {
-    const int T = c->T, Tp = T <= 32 ? 32 : 64, N = 2 * Tp;
+// S = sum_t I_t (ctx->sum) and C = H^H H of the holograms these frames WOULD give, without forming them.
+// finish = false: only the pass over the frames (S and the per-CTA partials of the byte-plane Gram); the caller then runs
+// holo_launch_gram_finish, possibly on another stream ordered after `st` (the streaming forms put it in front of the
+// eigensolver on the side stream, off the main stream's critical path)
+int holo_launch_sum_gram(holo_ctx* c, const uint16_t* frames, float2* C, cudaStream_t st, bool finish) {
+    const int T = c->T, Tp = T <= 32 ? 32 : 64;
     if (c->npix % RG_PIX != 0) { holo_set_error("raw-frame Gram needs nx*ny to be a multiple of %d", RG_PIX); return HOLO_ERR_ARG; }
     const long long nblocks = c->npix / RG_PIX;
     int grid = 3 * c->num_sms;                               // three CTAs per SM (64 KB of operand stages each)
@@ -283,12 +287,16 @@ int holo_launch_sum_gram(holo_ctx* c, const uint16_t* frames, float2* C, cudaStr
         }
     }
     HOLO_CUDA_OK(cudaGetLastError());
-    {
-        HoloProf prof(c, HOLO_K_COV_REDUCE, st);
-        const int nent = N * (N + 1) / 2;
-        k_gram_reduce_finish<<<(nent + 7) / 8, 256, 0, st>>>(reinterpret_cast<const long long*>(c->gram_Xp), grid, N, c->gram_X, c->counters + 1000,
-                                                             T, Tp, (double)c->npix / ((double)T * (double)T), C);
-    }
+    c->gram_nparts = grid;
+    return finish ? holo_launch_gram_finish(c, C, st) : HOLO_OK;
+}
+
+int holo_launch_gram_finish(holo_ctx* c, float2* C, cudaStream_t st) {
+    const int T = c->T, Tp = T <= 32 ? 32 : 64, N = 2 * Tp;
+    HoloProf prof(c, HOLO_K_COV_REDUCE, st);
+    const int nent = N * (N + 1) / 2;
+    k_gram_reduce_finish<<<(nent + 7) / 8, 256, 0, st>>>(reinterpret_cast<const long long*>(c->gram_Xp), c->gram_nparts, N, c->gram_X, c->counters + 1000,
+                                                         T, Tp, (double)c->npix / ((double)T * (double)T), C);
     HOLO_CUDA_OK(cudaGetLastError());
     return HOLO_OK;
 }
