@@ -27,7 +27,7 @@ constexpr int RG_THREADS = 128;
 constexpr int RG_PIX = 2 * RG_THREADS;             // pixels per stage (two K tiles of 128 pixels)
 constexpr int RG_TILE = 128 * 128;                 // bytes of one operand tile: 128 rows x 128 B
 constexpr int RG_STAGE = 2 * RG_TILE;
-constexpr int RG_SMEM = 1024 + 2 * RG_STAGE + 64;
+constexpr int RG_SMEM = 1024 + 2 * RG_STAGE + 64 + 2 * 64 * 16;
 constexpr int RG_FLUSH_ITERS = 64;                 // 64 x 256 pixels x 255^2 < 2^31
 
 __device__ __forceinline__ uint64_t make_sdesc(uint32_t saddr) {
@@ -52,12 +52,18 @@ __device__ __forceinline__ void tmem_ld16(uint32_t taddr, int32_t* v) {
 }
 
 // frames uint16 [T][npix]; sum uint32 [npix]; X int64 [lower-triangle entries of the 2 TP x 2 TP byte-plane Gram][CTAs]: every
-// CTA writes its own slot (integer sums: exact and order independent, hence deterministic)
-template <int TP>
+// CTA writes its own slot (integer sums: exact and order independent, hence deterministic).
+// Thread mapping of a 256-pixel stage: thread = (pixel quad q = tid % 64, frame parity h = tid / 64); it loads its four
+// pixels (8 bytes) of the frames t = 2 i + h, splits them into the two byte planes with two PRMTs and stores one 32-bit
+// word per plane row; the operand-tile addresses are four per-thread bases + immediates.  The two threads of a quad
+// combine their partial frame sums through shared memory (double-buffered by stage, ordered by the stage's barrier).
+// FULL: T == TP (no predicates on the loads).
+template <int TP, bool FULL>
 __global__ void __launch_bounds__(RG_THREADS, 3)
 k_sum_gram(const uint16_t* __restrict__ frames, uint32_t* __restrict__ sum, unsigned long long* __restrict__ X,
            long long npix, int T, unsigned int* __restrict__ counters) {
-    constexpr int Tp = TP;
+    constexpr int Tp = TP, NI = TP / 2;                       // NI frames per thread
+    constexpr bool PF = TP <= 32;                             // next block prefetched in registers (would spill at TP = 64)
     extern __shared__ unsigned char smraw_[];
     const uint32_t s0 = smem_u32(smraw_);
     const uint32_t pad = (1024u - (s0 & 1023u)) & 1023u;
@@ -65,6 +71,7 @@ k_sum_gram(const uint16_t* __restrict__ frames, uint32_t* __restrict__ sum, unsi
     const uint32_t sbase = s0 + pad;
     uint64_t* mma_done = reinterpret_cast<uint64_t*>(base + 2 * RG_STAGE);
     uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(mma_done + 2);
+    uint4* sscr = reinterpret_cast<uint4*>(base + 2 * RG_STAGE + 64);          // [2][64] partial frame sums of the h = 1 threads
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int N = 2 * Tp;                                     // MMA N (64 or 128); M = 128 always
 
@@ -87,14 +94,20 @@ k_sum_gram(const uint16_t* __restrict__ frames, uint32_t* __restrict__ sum, unsi
     const uint32_t idesc = (2u << 4) | ((uint32_t)(N >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);   // s32 += u8 x u8, K-major A and B
 
     // operand tile addressing: pixel k of a tile, row r: byte (r / 8) * 1024 + (r % 8) * 128 + (((k / 16) ^ (r % 8)) * 16) + k % 16
-    const int ktile = tid >> 6;                               // which of the stage's two tiles the thread's pixels fall in
-    const int kin = (2 * tid) & 127;                          // first of its two pixels inside the tile
-    const long long nblocks = (npix + RG_PIX - 1) / RG_PIX;
+    const int q = tid & 63, h = tid >> 6;
+    const int kin = (4 * q) & 127;                            // first of the thread's four pixels inside its tile
+    uint32_t rowoff[4];                                       // row t = 2 i + h: variant v = i % 4, + (i / 4) * 1024 (+ plane offset)
+#pragma unroll
+    for (int v = 0; v < 4; ++v) {
+        const int r7 = 2 * v + h;
+        rowoff[v] = (uint32_t)((q >> 5) * RG_TILE + r7 * 128 + ((((kin >> 4) ^ r7) << 4) | (kin & 15)));
+    }
+    const long long nblocks = (npix + RG_PIX - 1) / RG_PIX;   // npix is a multiple of 256 for every supported frame size
     uint32_t ph[2] = {0u, 0u};
-    int it = 0, pending[2] = {0, 0}, since_flush = 0;
+    int pending[2] = {0, 0}, since_flush = 0;
 
     // accumulators -> this CTA's own slot of the partial store Xp[lower-triangle entry][CTA] (plain stores: the per-entry
-    // 64-bit atomics of 444 CTAs on 2080 addresses cost 40 % of the kernel); k_gram_reduce adds the slots up
+    // 64-bit atomics of 444 CTAs on 2080 addresses cost 40 % of the kernel); k_gram_reduce_finish adds the slots up
     bool first_drain = true;
     auto drain = [&]() {                                      // (all MMAs have completed)
         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
@@ -107,59 +120,47 @@ k_sum_gram(const uint16_t* __restrict__ frames, uint32_t* __restrict__ sum, unsi
 #pragma unroll
                 for (int j = 0; j < 16; ++j)
                     if (c0 + j <= row) {
-                        long long* q = dst + (size_t)j * gridDim.x;
-                        *q = first_drain ? (long long)v[j] : *q + (long long)v[j];
+                        long long* qd = dst + (size_t)j * gridDim.x;
+                        *qd = first_drain ? (long long)v[j] : *qd + (long long)v[j];
                     }
             }
         }
         first_drain = false;
         asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     };
-    if ((long long)blockIdx.x >= nblocks) {                   // (cannot happen with grid <= nblocks; keeps the slot defined)
-        const int row = 32 * warp + lane;
-        if (row < N) for (int c = 0; c <= row; ++c) reinterpret_cast<long long*>(X)[((size_t)row * (row + 1) / 2 + c) * gridDim.x + blockIdx.x] = 0;
-    }
 
-    // software pipeline: the loads of block n + 1 are in flight (T per thread) while block n is split into byte planes
-    constexpr bool PF = TP <= 32;                              // (at TP = 64 the second register set would spill)
-    uint32_t w[TP], wn[PF ? TP : 1], wn2[PF ? TP : 1];
-    auto load_block = [&](long long blk, uint32_t* dst) {
-        const long long q0 = blk * RG_PIX + 2 * tid;
-        const bool ok = q0 + 1 < npix;                         // npix is a multiple of 256 for every supported frame size
+    const size_t fstep = (size_t)2 * (size_t)npix;            // elements between two frames of a thread
+    auto load_block = [&](long long blk, uint2* dst) {
+        const uint16_t* src = frames + (size_t)h * (size_t)npix + (size_t)blk * RG_PIX + 4 * q;
 #pragma unroll
-        for (int t = 0; t < TP; ++t) dst[t] = (ok && t < T) ? __ldg(reinterpret_cast<const uint32_t*>(frames + (size_t)t * npix + q0)) : 0u;
+        for (int i = 0; i < NI; ++i) {
+            if (FULL || 2 * i + h < T) dst[i] = __ldg(reinterpret_cast<const uint2*>(src));
+            else dst[i] = make_uint2(0u, 0u);
+            src += fstep;
+        }
     };
-    if (PF && (long long)blockIdx.x < nblocks) load_block(blockIdx.x, wn);
-    if (PF && (long long)blockIdx.x + gridDim.x < nblocks) load_block((long long)blockIdx.x + gridDim.x, wn2);
-    for (long long blk = blockIdx.x; blk < nblocks; blk += gridDim.x, ++it) {
-        const int s = it & 1;
-        const long long p0 = blk * RG_PIX + 2 * tid;           // the thread's two pixels
-        const bool inb = p0 + 1 < npix;
-        if constexpr (PF) {
-#pragma unroll
-            for (int t = 0; t < TP; ++t) { w[t] = wn[t]; wn[t] = wn2[t]; }
-            if (blk + 2 * (long long)gridDim.x < nblocks) load_block(blk + 2 * (long long)gridDim.x, wn2);
-        } else {
-            load_block(blk, w);
-        }
+    // one stage: byte planes of block `blk` (registers w) -> operand stage s, frame sums, MMAs
+    auto process = [&](const uint2* w, long long blk, int s) {
         if (pending[s]) { mbar_wait(mma_done + s, ph[s]); ph[s] ^= 1u; pending[s] = 0; }   // the MMAs that read this stage
-        unsigned char* tile = base + (size_t)s * RG_STAGE + (size_t)ktile * RG_TILE;
-        uint32_t sa = 0u, sb = 0u;
+        unsigned char* st = base + (size_t)s * RG_STAGE;
+        uint32_t a0 = 0u, a1 = 0u, a2 = 0u, a3 = 0u;
 #pragma unroll
-        for (int t = 0; t < TP; ++t) {
-            if (t >= T) break;
-            const uint32_t x = w[t];
-            sa += x & 0xffffu; sb += x >> 16;
-            const unsigned short lo = (unsigned short)__byte_perm(x, 0u, 0x4420) ;   // bytes (lo of pixel 0, lo of pixel 1)
-            const unsigned short hi = (unsigned short)__byte_perm(x, 0u, 0x4431);    // bytes (hi of pixel 0, hi of pixel 1)
-            const int rh = t, rl = Tp + t;
-            *reinterpret_cast<unsigned short*>(tile + (rh >> 3) * 1024 + (rh & 7) * 128 + ((((kin >> 4) ^ (rh & 7)) << 4) | (kin & 15))) = hi;
-            *reinterpret_cast<unsigned short*>(tile + (rl >> 3) * 1024 + (rl & 7) * 128 + ((((kin >> 4) ^ (rl & 7)) << 4) | (kin & 15))) = lo;
+        for (int i = 0; i < NI; ++i) {
+            const uint2 x = w[i];
+            a0 += x.x & 0xffffu; a1 += x.x >> 16; a2 += x.y & 0xffffu; a3 += x.y >> 16;
+            const uint32_t lo = __byte_perm(x.x, x.y, 0x6420), hi = __byte_perm(x.x, x.y, 0x7531);
+            unsigned char* p = st + rowoff[i & 3] + (i >> 2) * 1024;               // row 2 i + h of the hi plane
+            *reinterpret_cast<uint32_t*>(p) = hi;
+            *reinterpret_cast<uint32_t*>(p + (Tp >> 3) * 1024) = lo;             // row Tp + 2 i + h
         }
-        if (inb) *reinterpret_cast<uint2*>(sum + p0) = make_uint2(sa, sb);
+        if (h) sscr[s * 64 + q] = make_uint4(a0, a1, a2, a3);
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");     // the tensor core reads the tile through the async proxy
         asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
         __syncthreads();
+        if (!h) {
+            const uint4 o = sscr[s * 64 + q];
+            *reinterpret_cast<uint4*>(sum + blk * RG_PIX + 4 * q) = make_uint4(a0 + o.x, a1 + o.y, a2 + o.z, a3 + o.w);
+        }
         if (tid == 0) {
             asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
             const uint32_t sa0 = sbase + (uint32_t)s * RG_STAGE;
@@ -174,13 +175,30 @@ k_sum_gram(const uint16_t* __restrict__ frames, uint32_t* __restrict__ sum, unsi
         }
         pending[s] = 1;
         if (++since_flush == RG_FLUSH_ITERS) {                 // before the s32 accumulators can overflow
-            for (int q = 0; q < 2; ++q) if (pending[q]) { mbar_wait(mma_done + q, ph[q]); ph[q] ^= 1u; pending[q] = 0; }
+            for (int k = 0; k < 2; ++k) if (pending[k]) { mbar_wait(mma_done + k, ph[k]); ph[k] ^= 1u; pending[k] = 0; }
             drain();
             __syncthreads();
             since_flush = 0;
         }
+    };
+
+    // software pipeline, unrolled by two: block n + 1 is in flight (NI loads per thread) while block n is processed
+    uint2 wa[NI], wb[NI];
+    const long long g = gridDim.x;
+    long long blk = blockIdx.x;
+    if (blk < nblocks) load_block(blk, wa);
+    while (blk < nblocks) {
+        if (PF && blk + g < nblocks) load_block(blk + g, wb);
+        process(wa, blk, 0);
+        blk += g;
+        if (blk >= nblocks) break;
+        if (!PF) load_block(blk, wb);
+        if (PF && blk + g < nblocks) load_block(blk + g, wa);
+        process(wb, blk, 1);
+        blk += g;
+        if (!PF && blk < nblocks) load_block(blk, wa);
     }
-    for (int q = 0; q < 2; ++q) if (pending[q]) { mbar_wait(mma_done + q, ph[q]); ph[q] ^= 1u; pending[q] = 0; }
+    for (int k = 0; k < 2; ++k) if (pending[k]) { mbar_wait(mma_done + k, ph[k]); ph[k] ^= 1u; pending[k] = 0; }
     if (since_flush || first_drain) drain();
     __syncthreads();
     if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "r"(N) : "memory");
@@ -278,13 +296,14 @@ int holo_launch_sum_gram(holo_ctx* c, const uint16_t* frames, float2* C, cudaStr
     int rc;
     {
         HoloProf prof(c, HOLO_K_SUM, st);
-        if (Tp == 32) {
-            if ((rc = holo_ensure_smem_attr((const void*)k_sum_gram<32>, c->device, RG_SMEM))) return rc;
-            k_sum_gram<32><<<grid, RG_THREADS, RG_SMEM, st>>>(frames, c->sum, c->gram_Xp, c->npix, T, c->counters);
-        } else {
-            if ((rc = holo_ensure_smem_attr((const void*)k_sum_gram<64>, c->device, RG_SMEM))) return rc;
-            k_sum_gram<64><<<grid, RG_THREADS, RG_SMEM, st>>>(frames, c->sum, c->gram_Xp, c->npix, T, c->counters);
-        }
+        auto launch = [&](auto kern) -> int {
+            if ((rc = holo_ensure_smem_attr((const void*)kern, c->device, RG_SMEM))) return rc;
+            kern<<<grid, RG_THREADS, RG_SMEM, st>>>(frames, c->sum, c->gram_Xp, c->npix, T, c->counters);
+            return HOLO_OK;
+        };
+        if (Tp == 32) rc = T == 32 ? launch(k_sum_gram<32, true>) : launch(k_sum_gram<32, false>);
+        else          rc = T == 64 ? launch(k_sum_gram<64, true>) : launch(k_sum_gram<64, false>);
+        if (rc) return rc;
     }
     HOLO_CUDA_OK(cudaGetLastError());
     c->gram_nparts = grid;
