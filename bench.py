@@ -2,7 +2,7 @@
 """bench.py -- PCA images/s (input frames/s) at 1024^2 x 32 uint16 (BASELINE.json metric), one JSON line.
 
   python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 3] [--api submit|process|push]
-                  [--mode 1|2]
+                  [--mode 1|2|3]
 
 A "step" is one pass of the whole hot path (A0..A6) over one stack of T frames (`--api push`: one window of the
 sliding-window form, `stride` new frames).  The stream is resident in HBM before the timed region and is cycled
@@ -130,8 +130,17 @@ class ClockSampler:
 
 def stage_bytes(cfg, mode=1):
     """Algorithmic (compulsory) bytes per stack and stage, SURVEY.md 8(d) / DESIGN.md.  mode 2 (Gram from the raw
-    frames, SURVEY.md 8(f)-2 stage 1) has no covariance read of the hologram stack: 20 T N_p + 12 N_p."""
+    frames, SURVEY.md 8(f)-2 stage 1) has no covariance read of the hologram stack: 20 T N_p + 12 N_p.  mode 3 (stage 2:
+    no hologram stack) reads the frames three times (Gram + sum, deflation images, row pass), writes and reads the
+    row-pass output once and writes the image: 22 T N_p + (20 + 8 n_rej) N_p with n_rej rejected components."""
     npix, T = cfg.n * cfg.n, cfg.T
+    if mode == 3:
+        nrej = (cfg.k_lo - 1) + (T - cfg.k_hi)
+        d = {"sum": 2 * T * npix + 4 * npix, "defl": (2 * T * npix + 4 * npix + 4 * nrej * npix) if nrej else 0,
+             "rows": 2 * T * npix + 4 * npix + 4 * nrej * npix + 8 * T * npix, "cols": 8 * T * npix + 4 * npix, "eig": 16 * T * T}
+        d["total"] = d["sum"] + d["defl"] + d["rows"] + d["cols"]
+        d["fft"], d["proj"], d["cov"] = d["rows"], 0, 0
+        return d
     d = {"sum": 2 * T * npix + 4 * npix, "fft": 2 * T * npix + 4 * npix + 8 * T * npix,
          "cov": 8 * T * npix if mode == 1 else 0, "eig": 16 * T * T, "proj": 8 * T * npix + 4 * npix}
     d["total"] = d["sum"] + d["fft"] + d["cov"] + d["proj"]
@@ -183,10 +192,14 @@ def run_reference(args, cfg):
 KCLASS = ["sum", "fft_rows", "fft_cols", "cov_partial", "cov_reduce", "eig", "project"]
 
 
-def kernel_name(cls, fused_fft, cov_real, mode):
+def kernel_name(cls, fused_fft, cov_real, mode, T=32):
+    if mode == 3:
+        return {"sum": "k_sum_gram + k_deflate_images", "fft_rows": "k_fft<rows, deflating prologue>", "fft_cols": "k_col_energy",
+                "cov_reduce": "k_gram_reduce_finish", "eig": "k_eig_real", "project": "k_sum_partial_images"}[cls]
     return {"sum": "k_frame_sum" if mode == 1 else "k_sum_gram", "fft_rows": "k_fresnel" if fused_fft else "k_fft<rows>",
-            "fft_cols": "k_fft<cols>", "cov_partial": "k_cov_partial_real" if cov_real else "k_cov_partial",
-            "cov_reduce": "k_cov_reduce", "eig": "k_eig", "project": "k_project_deflate_tma / k_project"}[cls]
+            "fft_cols": "k_fft<cols>", "cov_partial": ("k_cov_tf32" if T > 32 else "k_cov_partial_real") if cov_real else "k_cov_partial",
+            "cov_reduce": "k_cov_reduce" if mode == 1 else "k_gram_reduce_finish", "eig": "k_eig_real" if cov_real else "k_eig",
+            "project": "k_project_deflate_tma / k_project"}[cls]
 
 
 def _traffic_table():
@@ -216,8 +229,8 @@ class Runner:
         for kv in tune:
             k, v = kv.split("=")
             self.h.tune(int(k), int(v))
-        if mode == 2:
-            self.h.set_mode(2)
+        if mode != 1:
+            self.h.set_mode(mode)
         self.images = torch.empty((4, cfg.n, cfg.n), dtype=torch.float32, device=dev)
         self.st = torch.cuda.Stream(device=dev)
 
@@ -336,17 +349,19 @@ def run_ours(args, cfg):
     hbm_peak, peak_src, peaks = _peaks()
     num_sms = torch.cuda.get_device_properties(dev).multi_processor_count
     fp32_peak_tflops = FP32_PEAK_MEASURED_TFLOPS * num_sms / 148.0
-    fused_fft = prof[2][1] == 0          # no separate column-pass launches: one persistent kernel does A1+A2 of all T frames
+    fused_fft = prof[2][1] == 0 and mode != 3   # no separate column-pass launches: one persistent kernel does A1+A2 of all T frames
     cov_real = "8=0" not in args.tune
     per_launch_bytes = {"sum": sb["sum"], "fft_rows": sb["fft"] if fused_fft else 2 * G_fft * npix + 4 * npix * G_fft / T,
                         "fft_cols": 8 * G_fft * npix, "cov_partial": 8 * T * npix, "cov_reduce": 0, "eig": sb["eig"], "project": sb["proj"]}
+    if mode == 3:       # "sum" brackets two launches (Gram + sum, deflation images): their mean; "project" is the partial-image sum
+        per_launch_bytes.update({"sum": (sb["sum"] + sb["defl"]) / 2, "fft_rows": sb["rows"], "fft_cols": sb["cols"], "project": 12 * npix})
     stages = {}
     tot_ms = sum(p[0] for p in prof) or 1.0
     for name, (ms_k, cnt) in zip(KCLASS, prof):
         if cnt == 0:
             continue
         us = ms_k / cnt * 1e3
-        stages[name] = {"kernel": kernel_name(name, fused_fft, cov_real, mode), "us_per_launch": round(us, 2),
+        stages[name] = {"kernel": kernel_name(name, fused_fft, cov_real, mode, T), "us_per_launch": round(us, 2),
                         "launches_per_step": cnt / prof_steps, "share": round(ms_k / tot_ms, 4),
                         "GBps": round(per_launch_bytes[name] / (us * 1e-6) / 1e9, 1)}
     cov_flops = (2 if cov_real else 4) * T * (T + 1) * npix
@@ -358,7 +373,7 @@ def run_ours(args, cfg):
         stages["fft_rows"]["TFLOPs_fp32"] = round(fft_flops / (stages["fft_rows"]["us_per_launch"] * 1e-6) / 1e12, 2)
     dom = max(stages, key=lambda k: stages[k]["share"])
     traffic = _traffic_table().get((cfg.name, dom))
-    if dom == "cov_partial" and cov_flops / (8 * T * npix) > fp32_peak_tflops * 1e12 / (hbm_peak * 1e9):
+    if dom == "cov_partial" and T <= 32 and cov_flops / (8 * T * npix) > fp32_peak_tflops * 1e12 / (hbm_peak * 1e9):
         roof = {"kernel": stages[dom]["kernel"], "bound": "alu", "achieved": stages[dom]["TFLOPs_fp32"], "peak": round(fp32_peak_tflops, 1),
                 "unit": "TFLOP/s", "frac": round(stages[dom]["TFLOPs_fp32"] / fp32_peak_tflops, 4), "traffic": traffic,
                 "peak_source": "measured register-only FFMA rate (profiles/r01_ubench_peaks.txt; nominal 148 SMs x 128 lanes x 2 x 1.965 GHz = 74.4)",
@@ -437,13 +452,14 @@ def run_ours(args, cfg):
     torch.cuda.empty_cache()
     if side is not None:
         # (config, api, steps, resident stacks): streams of >= 3x L2, kept short so that the default run ends in minutes
-        for cn, sapi, ssteps, sstacks in ((2, "submit", 256, 24), (4, "push", 256, 16), (5, "submit", 24, 3)):
+        for cn, sapi, ssteps, sstacks, smode in ((3, "submit", 512, 0, 3), (2, "submit", 256, 24, 1), (2, "submit", 256, 24, 3), (4, "push", 256, 16, 1),
+                                                 (5, "submit", 24, 3, 1), (5, "submit", 24, 3, 3)):
             c2 = G.CONFIGS[cn]
-            p2 = shard_plan(c2, rank, world, stacks=sstacks)
-            R2 = Runner(c2, p2, dev)
+            p2 = shard_plan(c2, rank, world, stacks=sstacks or None)
+            R2 = Runner(c2, p2, dev, mode=smode)
             ms_s, _ = R2.timed(sapi, ssteps, 6, barrier)
-            sb2 = stage_bytes(c2)
-            ent = {"api": sapi, "ms_per_step": ms_s / ssteps, "images_per_s": ssteps / (ms_s * 1e-3), "resident_bytes": p2["resident_bytes"]}
+            sb2 = stage_bytes(c2, smode)
+            ent = {"api": sapi, "mode": smode, "ms_per_step": ms_s / ssteps, "images_per_s": ssteps / (ms_s * 1e-3), "resident_bytes": p2["resident_bytes"]}
             if sapi != "push":
                 ent["roofline_end_to_end_frac"] = round(sb2["total"] * (ssteps / (ms_s * 1e-3)) / 1e9 / hbm_peak, 4)
                 ent["bytes_per_step"] = sb2["total"]
@@ -453,7 +469,7 @@ def run_ours(args, cfg):
                 dt2, err2 = R2.oracle_check(sapi)
                 ent["oracle_rel_l2_M_first_stack"] = err2
                 ent["oracle_s_per_stack"] = round(dt2, 2)
-            side[c2.name] = ent
+            side[c2.name + ("_mode3" if smode == 3 else "")] = ent
             R2.close()
             del R2
             torch.cuda.empty_cache()
@@ -529,7 +545,9 @@ def main():
     ap.add_argument("--warmup", type=int, default=None)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=3)
-    ap.add_argument("--mode", type=int, default=1, choices=[1, 2], help="1: prescribed stage decomposition; 2: Gram from the raw frames (SURVEY.md 8(f)-2)")
+    ap.add_argument("--mode", type=int, default=1, choices=[1, 2, 3],
+                    help="1: prescribed stage decomposition (default); 2: Gram from the raw frames (SURVEY.md 8(f)-2 stage 1); "
+                         "3: 2 + image without a hologram stack (stage 2)")
     ap.add_argument("--stacks", type=int, default=None, help="resident stacks (default: >= 3x L2)")
     ap.add_argument("--e2e-steps", type=int, default=24)
     ap.add_argument("--no-e2e", action="store_true")

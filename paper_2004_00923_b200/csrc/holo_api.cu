@@ -94,6 +94,7 @@ static void free_ctx(holo_ctx* c) {
     if (c->copy) {
         cudaStreamDestroy(c->copy);
         for (int i = 0; i < 2; ++i) { cudaFree(c->fstage[i]); cudaFree(c->istage[i]); cudaEventDestroy(c->ev_h2d[i]); cudaEventDestroy(c->ev_free[i]); }
+        if (c->fstage[2]) { cudaFree(c->fstage[2]); cudaEventDestroy(c->ev_h2d[2]); cudaEventDestroy(c->ev_free[2]); }
     }
     if (c->frames_stage) cudaFree(c->frames_stage);
     if (c->image_stage) cudaFree(c->image_stage);
@@ -631,8 +632,29 @@ extern "C" int holo_submit_host(holo_ctx* c, const uint16_t* frames_host, float*
     cudaStream_t st = (cudaStream_t)stream;
     int rc;
     if ((rc = host_init(c))) return rc;
-    const int s = (int)(c->nsubmit_host & 1);
     const size_t fbytes = (size_t)c->T * c->npix * sizeof(uint16_t);
+    if (c->mode == 3) {
+        // mode 3 reads the frames of stack i again in the NEXT submit (energy pass): three frame stages, so that the copy of
+        // stack i+1 still runs under the kernels enqueued by this call
+        if (!c->fstage[2]) {
+            HOLO_CUDA_OK(cudaMalloc(&c->fstage[2], fbytes));
+            HOLO_CUDA_OK(cudaEventCreateWithFlags(&c->ev_h2d[2], cudaEventDisableTiming));
+            HOLO_CUDA_OK(cudaEventCreateWithFlags(&c->ev_free[2], cudaEventDisableTiming));
+        }
+        const long long i = c->nsubmit_host;
+        const int s3 = (int)(i % 3), si = (int)(i & 1);
+        if (i >= 3) HOLO_CUDA_OK(cudaStreamWaitEvent(c->copy, c->ev_free[s3], 0));           // read last by the submit of stack i-2
+        HOLO_CUDA_OK(cudaMemcpyAsync(c->fstage[s3], frames_host, fbytes, cudaMemcpyHostToDevice, c->copy));
+        HOLO_CUDA_OK(cudaEventRecord(c->ev_h2d[s3], c->copy));
+        HOLO_CUDA_OK(cudaStreamWaitEvent(st, c->ev_h2d[s3], 0));
+        if ((rc = holo_submit(c, c->fstage[s3], c->istage[si], stream))) return rc;          // enqueues the image of stack i-1
+        if (i >= 1) HOLO_CUDA_OK(cudaEventRecord(c->ev_free[(int)((i - 1) % 3)], st));
+        if ((rc = deliver_host(c, st))) return rc;
+        c->pend_image_host = image_host; c->pend_islot = si; c->nsubmit_host++;
+        HOLO_CUDA_OK(cudaEventSynchronize(c->ev_h2d[s3]));       // frames_host may be reused on return
+        return HOLO_OK;
+    }
+    const int s = (int)(c->nsubmit_host & 1);
     if (c->nsubmit_host >= 2) HOLO_CUDA_OK(cudaStreamWaitEvent(c->copy, c->ev_free[s], 0));   // stage s was read by stack i-2
     HOLO_CUDA_OK(cudaMemcpyAsync(c->fstage[s], frames_host, fbytes, cudaMemcpyHostToDevice, c->copy));
     HOLO_CUDA_OK(cudaEventRecord(c->ev_h2d[s], c->copy));
@@ -652,8 +674,7 @@ extern "C" int holo_submit_host(holo_ctx* c, const uint16_t* frames_host, float*
         return HOLO_OK;
     }
     if ((rc = holo_submit(c, c->fstage[s], c->istage[s], stream))) return rc;   // enqueues the projection of stack i-1
-    // mode 3 reads the frames of stack i again in the next submit / flush: what is free now is the stage of stack i-1
-    HOLO_CUDA_OK(cudaEventRecord(c->ev_free[c->mode == 3 ? s ^ 1 : s], st));
+    HOLO_CUDA_OK(cudaEventRecord(c->ev_free[s], st));
     if ((rc = deliver_host(c, st))) return rc;
     c->pend_image_host = image_host; c->pend_islot = s; c->nsubmit_host++;
     HOLO_CUDA_OK(cudaEventSynchronize(c->ev_h2d[s]));        // frames_host may be reused on return

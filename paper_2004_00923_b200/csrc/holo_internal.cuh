@@ -110,9 +110,9 @@ struct holo_ctx {
     uint16_t* frames_stage;
     float* image_stage;
     // streaming host entry (holo_submit_host / holo_flush_host): double-buffered staging + copy stream
-    uint16_t* fstage[2]; float* istage[2];
+    uint16_t* fstage[3]; float* istage[2];      // (the third frame stage only in mode 3, whose frames are read again one call later)
     cudaStream_t copy;
-    cudaEvent_t ev_h2d[2], ev_free[2];
+    cudaEvent_t ev_h2d[3], ev_free[3];
     float* pend_image_host; int pend_islot;
     float* pend_host_slot[2];          // SM-split mode: host image owed per staging slot
     long long nsubmit_host;

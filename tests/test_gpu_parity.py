@@ -578,6 +578,48 @@ def test_submit_stream_matches_process(torch_cuda, split):
     h.close()
 
 
+@pytest.mark.parametrize("mode", [2, 3])
+def test_submit_stream_modes_2_3_match_process(torch_cuda, mode):
+    """holo_submit / holo_submit_host in modes 2 and 3 on a stream of DIFFERENT stacks: every image equals the serial
+    holo_process image of its stack bit for bit (mode 3 is pipelined by one stack and reads the frames of stack i again in
+    the next call; the host entry keeps three frame stages for that)."""
+    torch = torch_cuda
+    cfg = G.small_config(n=128, T=32)
+    stacks = [_to_dev(torch, G.stack_np(cfg, 40 + i)) for i in range(7)]
+    h = _holo(128, 128, 32, 2, 32)
+    h.set_mode(mode)
+    ref = []
+    for sfr in stacks:
+        M = torch.empty((128, 128), dtype=torch.float32, device="cuda")
+        h.process(sfr, M)
+        ref.append(M)
+    torch.cuda.synchronize()
+    st = torch.cuda.Stream()
+    outs = [torch.zeros((128, 128), dtype=torch.float32, device="cuda") for _ in stacks]
+    for sfr, o in zip(stacks, outs):
+        h.submit(sfr, o, st)
+    h.flush(st)
+    st.synchronize()
+    for o, r in zip(outs, ref):
+        assert torch.equal(o, r)
+    # a serial call in the middle of a sequence delivers the owed image first
+    A, B = torch.zeros_like(ref[0]), torch.zeros_like(ref[0])
+    h.submit(stacks[2], A, st)
+    h.process(stacks[5], B, st)
+    st.synchronize()
+    assert torch.equal(A, ref[2]) and torch.equal(B, ref[5])
+    fh = [torch.from_numpy(G.stack_np(cfg, 40 + i).view(np.int16)).pin_memory() for i in range(7)]
+    oh = [torch.zeros((128, 128), dtype=torch.float32).pin_memory() for _ in range(7)]
+    for f, o in zip(fh, oh):
+        h.submit_host(f, o, st)
+    h.flush_host(st)
+    for o, r in zip(oh, ref):
+        assert torch.equal(o, r.cpu())
+    rc, status = h.status(st)
+    assert rc == 0
+    h.close()
+
+
 def test_process_real_covariance_identity(torch_cuda):
     """DESIGN.md R21: holo_process accumulates Re C only (C is real for holograms of real frames).  Its C must have
     a zero imaginary part and agree with the complex Gram of holo_covariance on the same H; M must agree too."""
