@@ -58,6 +58,9 @@ struct FftArgs {
     const float* defl_img;    // [ndefl][ny][nx]  eT_k = sum_t (T I_t - S) V_{t,k} of the rejected components
     const float* defl_coef;   // [T][ndefl]       V_{t,k} (real: C is real symmetric there, R21)
     int ndefl;
+    unsigned int* ticket;     // != nullptr: row kernels of one warp per row draw single rows from this counter (zeroed by the
+                              // caller's earlier kernel) instead of a static partition: a CTA that shares its SM with the
+                              // eigensolver of the side stream then simply takes fewer rows
 };
 
 // one tile = B sequences of one frame; in_foff / out_foff = element offset of the frame in a.in(frames) / a.out
@@ -71,7 +74,7 @@ struct NoHook { __device__ __forceinline__ void operator()() const {} };
 // to acc[s] instead.
 template <int N, int E, int R1, int R2, int B, bool COL, bool PRO, int LDC = 0, class Mid = NoHook, bool DEFL = false, bool ENERGY = false>
 __device__ __forceinline__ void fft_tile(const FftArgs& a, long long in_foff, long long out_foff, int tile_in_frame, float2* sm,
-                                         Mid mid = Mid(), int frame = 0, float* acc = nullptr) {
+                                         Mid mid = Mid(), int frame = 0, float* acc = nullptr, int seq_override = -1) {
     constexpr int TPS = N / E;
     constexpr int PADN = N + N / E;
     constexpr bool MULTI = (R1 > 1);
@@ -88,7 +91,7 @@ __device__ __forceinline__ void fft_tile(const FftArgs& a, long long in_foff, lo
         return COL ? p * B + c : c * PADN + p;
     };
     {
-        const int s0 = tile_in_frame * B + c;                          // sequence index (row y or column x)
+        const int s0 = seq_override >= 0 ? seq_override : tile_in_frame * B + c;   // sequence index (row y or column x)
         const int ld = LDC ? LDC : a.ld;
         const long long ibase = in_foff + (COL ? (long long)s0 : (long long)s0 * ld);
         const long long obase = out_foff + (COL ? (long long)s0 : (long long)s0 * ld);
@@ -214,6 +217,21 @@ __device__ __forceinline__ void fft_tile(const FftArgs& a, long long in_foff, lo
 template <int N, int E, int R1, int R2, int B, bool COL, bool PRO, bool DEFL = false>
 __global__ void __launch_bounds__((N / E) * B) k_fft(const FftArgs a) {
     extern __shared__ float2 sm[];
+    if constexpr (!COL && N / E == 32) {
+        if (a.ticket) {                                      // one warp per row, rows drawn one by one (no CTA-wide step at all)
+            const unsigned int nrows = (unsigned int)a.ntiles * B;
+            for (;;) {
+                unsigned int r = 0u;
+                if ((threadIdx.x & 31) == 0) r = atomicAdd(a.ticket, 1u);
+                r = __shfl_sync(0xffffffffu, r, 0);
+                if (r >= nrows) break;
+                const int fl = (int)(r / (unsigned int)a.nseq), row = (int)(r - (unsigned int)fl * a.nseq);
+                fft_tile<N, E, R1, R2, B, COL, PRO, 0, NoHook, DEFL>(a, (long long)fl * a.in_fstride, (long long)fl * a.out_fstride,
+                                                                     0, sm, NoHook(), fl, nullptr, row);
+            }
+            return;
+        }
+    }
     for (int tile = blockIdx.x; tile < a.ntiles; tile += gridDim.x) {
         const int fl = tile / a.tiles_per_frame;
         fft_tile<N, E, R1, R2, B, COL, PRO, 0, NoHook, DEFL>(a, (long long)fl * a.in_fstride, (long long)fl * a.out_fstride,
@@ -693,6 +711,7 @@ int holo_launch_energy_image(holo_ctx* c, const uint16_t* frames, const float2* 
     a.ntiles = T * a.tiles_per_frame;
     a.T = T;
     a.defl_img = c->defl_img; a.defl_coef = c->defl_coef; a.ndefl = ndefl;
+    a.ticket = c->counters + 1001;                        // zeroed by k_sum_gram, which always precedes this call in stream order
     int rc;
     { HoloProf prof(c, HOLO_K_FFT_ROWS, st);
       rc = ndefl ? launch_fft<false, true, true>(c->nx, a, c->num_sms, c->device, st) : launch_fft<false, true, false>(c->nx, a, c->num_sms, c->device, st); }
