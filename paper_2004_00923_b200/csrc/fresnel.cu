@@ -713,6 +713,8 @@ int holo_launch_energy_image(holo_ctx* c, const uint16_t* frames, const float2* 
     a.defl_img = c->defl_img; a.defl_coef = c->defl_coef; a.ndefl = ndefl;
     a.ticket = c->counters + 1001;                        // zeroed by k_sum_gram, which always precedes this call in stream order
     int rc;
+    if (c->tune[HOLO_TUNE_ROWS2] && holo_rows2_supported(c)) rc = holo_launch_rows2(c, frames, c->H, ndefl, st);
+    else
     { HoloProf prof(c, HOLO_K_FFT_ROWS, st);
       rc = ndefl ? launch_fft<false, true, true>(c->nx, a, c->num_sms, c->device, st) : launch_fft<false, true, false>(c->nx, a, c->num_sms, c->device, st); }
     if (rc) return rc;

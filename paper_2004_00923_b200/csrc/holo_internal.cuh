@@ -27,7 +27,8 @@ enum {
     HOLO_TUNE_L2_PERSIST_MB = 12,  // experiment: cudaLimitPersistingL2CacheSize in MiB (0 = leave the device setting alone)
     HOLO_TUNE_COV_TF32 = 13,       // real covariance of holo_process / holo_submit on the tensor cores: 0 = FP32 FFMA kernel,
                                    // 1 = TF32 (inputs rounded to nearest), 3 = 3 x TF32 split; default 1 at T > 32, else 0
-    HOLO_TUNE_COV_TF32_DRAIN = 14, // stages accumulated in TMEM before the accumulators are added to FP64 (default 4)
+    HOLO_TUNE_COV_TF32_DRAIN = 14,
+    HOLO_TUNE_ROWS2 = 15,          // mode 3: packed two-frame row pass where supported (1024^2, even T) // stages accumulated in TMEM before the accumulators are added to FP64 (default 4)
     HOLO_TUNE_FFT_LAG = 6,         // frames between the row pass and the column pass in the fused kernel (0 = auto)
 };
 
@@ -171,5 +172,8 @@ int holo_launch_gram_finish(holo_ctx* c, float2* C, cudaStream_t st);
 // round-2 Fresnel kernel (fresnel2.cu): packed two-sequence FFT, TMA-staged column tiles; 1024 x 1024 frames
 bool holo_fresnel2_supported(const holo_ctx* c);
 int holo_launch_fresnel2(holo_ctx* c, const uint16_t* frames, float2* H, cudaStream_t st, int nproc);
+// packed two-frame row pass of mode 3 (fresnel2.cu): 1024 x 1024 frames, even T
+bool holo_rows2_supported(const holo_ctx* c);
+int holo_launch_rows2(holo_ctx* c, const uint16_t* frames, float2* out, int ndefl, cudaStream_t st);
 int holo_fft_plan_init(FftPlan* p, int N);
 void holo_fft_plan_free(FftPlan* p);

@@ -271,6 +271,13 @@ def test_process_mode3_matches_oracle_on_configs(torch_cuda, cfgn):
     # the paper's own window needs 12 rejected components: mode 3 refuses, nothing is launched
     with pytest.raises(Exception):
         h.set_range(13, cfg.T)
+    if cfg.n == 1024:
+        # the scalar row pass (one frame per warp) instead of the packed two-frame one: same image up to FP32 rounding
+        h.tune(15, 0)
+        Ms = torch.empty_like(M)
+        h.process(dev, Ms)
+        err = rel_l2(Ms.cpu().numpy(), out["M"])
+        assert err <= TOL_M and err <= FP32_M, err
     h.close()
 
 
