@@ -372,7 +372,7 @@ def run_ours(args, cfg):
     if "fft_rows" in stages and fused_fft:
         stages["fft_rows"]["TFLOPs_fp32"] = round(fft_flops / (stages["fft_rows"]["us_per_launch"] * 1e-6) / 1e12, 2)
     dom = max(stages, key=lambda k: stages[k]["share"])
-    traffic = _traffic_table().get((cfg.name, dom))
+    traffic = _traffic_table().get((cfg.name + ("_mode3" if mode == 3 else ""), dom))
     if dom == "cov_partial" and T <= 32 and cov_flops / (8 * T * npix) > fp32_peak_tflops * 1e12 / (hbm_peak * 1e9):
         roof = {"kernel": stages[dom]["kernel"], "bound": "alu", "achieved": stages[dom]["TFLOPs_fp32"], "peak": round(fp32_peak_tflops, 1),
                 "unit": "TFLOP/s", "frac": round(stages[dom]["TFLOPs_fp32"] / fp32_peak_tflops, 4), "traffic": traffic,
