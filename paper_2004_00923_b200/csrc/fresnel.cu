@@ -592,10 +592,8 @@ static bool use_fused(const holo_ctx* c) {
     return c->nx == c->ny && c->tune[HOLO_TUNE_FFT_PERSISTENT] && c->scratch_frames >= 2 && 2 * c->T + 1 <= 256;
 }
 
-static bool use_fused2(const holo_ctx* c) { return c->tune[HOLO_TUNE_FFT_PERSISTENT] == 2 && holo_fresnel2_supported(c); }
-
 int holo_fresnel_launch_count(holo_ctx* c) {
-    if (use_fused2(c) || use_fused(c)) return 2;
+    if (use_fused(c)) return 2;
     int g = c->scratch_frames;
     int groups = (c->T + g - 1) / g;
     return 1 + 2 * groups;
@@ -618,8 +616,7 @@ int holo_launch_sum(holo_ctx* c, const uint16_t* frames, cudaStream_t st) {
 int holo_launch_fresnel(holo_ctx* c, const uint16_t* frames, float2* H, cudaStream_t st, bool with_sum, int nproc, bool counters_zeroed) {
     if (nproc < 0) nproc = c->T;
     if (with_sum) { const int rc = holo_launch_sum(c, frames, st); if (rc) return rc; }
-    else if (!counters_zeroed && (use_fused2(c) || use_fused(c))) HOLO_CUDA_OK(cudaMemsetAsync(c->counters, 0, (2 * c->T + 1) * sizeof(unsigned int), st));
-    if (use_fused2(c)) return holo_launch_fresnel2(c, frames, H, st, nproc);
+    else if (!counters_zeroed && use_fused(c)) HOLO_CUDA_OK(cudaMemsetAsync(c->counters, 0, (2 * c->T + 1) * sizeof(unsigned int), st));
     if (use_fused(c)) {
         FresnelArgs p{};
         const int Bq = c->nx == 1024 ? FUSED_B1024 : c->nx == 2048 ? FUSED_B2048 : fft_batch(c->nx);

@@ -133,7 +133,7 @@ static int create_impl(holo_ctx* c) {
     c->tune[HOLO_TUNE_FFT_GROUP] = (int)grp;
     c->tune[HOLO_TUNE_COV_GRIDX] = c->num_sms;
     c->tune[HOLO_TUNE_PROJ_COMPLEMENT] = 1;
-    c->tune[HOLO_TUNE_FFT_PERSISTENT] = 1;      // 2 = k_fresnel2 (packed two-sequence FFT, TMA-staged column tiles): correct, measured slower
+    c->tune[HOLO_TUNE_FFT_PERSISTENT] = 1;
     c->tune[HOLO_TUNE_PROJ_TMA] = 1;
     c->tune[HOLO_TUNE_COV_REAL] = 1;
     c->tune[HOLO_TUNE_PUSH_PIPE] = 1;

@@ -15,7 +15,7 @@ enum {
     HOLO_TUNE_FFT_GROUP = 0,     // frames per row/column pass group (scratch = group * 8*nx*ny bytes)
     HOLO_TUNE_COV_GRIDX = 1,     // covariance CTAs along pixels
     HOLO_TUNE_PROJ_COMPLEMENT = 2, // 1 = allow complement form in holo_process (default 1)
-    HOLO_TUNE_FFT_PERSISTENT = 3,  // 2 = k_fresnel2 where supported (default), 1 = k_fresnel (single persistent kernel), 0 = separate launches
+    HOLO_TUNE_FFT_PERSISTENT = 3,  // 1 = k_fresnel (single persistent kernel, default), 0 = separate row / column launches
     HOLO_TUNE_EIG_MAX_SWEEPS = 4,
     HOLO_TUNE_PROFILE = 5,         // 1 = bracket every kernel launch with events (holo_profile_read)
     HOLO_TUNE_PROJ_TMA = 7,        // 1 = deflation projection fed by a TMA ring (default), 0 = register-streaming kernel
@@ -169,9 +169,6 @@ int holo_launch_svd_filter(holo_ctx* c, const float2* H, const float2* V, int k_
 // mode 2: S = sum_t I_t and C = nx ny D^T D from the raw frames (tcgen05 int8 Gram, rawgram.cu)
 int holo_launch_sum_gram(holo_ctx* c, const uint16_t* frames, float2* C, cudaStream_t st, bool finish = true);
 int holo_launch_gram_finish(holo_ctx* c, float2* C, cudaStream_t st);
-// round-2 Fresnel kernel (fresnel2.cu): packed two-sequence FFT, TMA-staged column tiles; 1024 x 1024 frames
-bool holo_fresnel2_supported(const holo_ctx* c);
-int holo_launch_fresnel2(holo_ctx* c, const uint16_t* frames, float2* H, cudaStream_t st, int nproc);
 // packed two-frame row pass of mode 3 (fresnel2.cu): 1024 x 1024 frames, even T
 bool holo_rows2_supported(const holo_ctx* c);
 int holo_launch_rows2(holo_ctx* c, const uint16_t* frames, float2* out, int ndefl, cudaStream_t st);
