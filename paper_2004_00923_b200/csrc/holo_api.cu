@@ -18,7 +18,7 @@ void holo_set_error(const char* fmt, ...) {
 }
 
 extern "C" const char* holo_last_error(void) { return g_err; }
-extern "C" int holo_version(void) { return 100; }   // 0.1.0
+extern "C" int holo_version(void) { return 200; }   // 0.2.0
 
 static bool is_pow2(int n) { return n > 0 && (n & (n - 1)) == 0; }
 
@@ -810,14 +810,6 @@ extern "C" int holo_tune(holo_ctx* c, int key, int value) {
         c->prof_cls = new int[HOLO_PROF_CAP];
         for (int i = 0; i < 2 * HOLO_PROF_CAP; ++i) HOLO_CUDA_OK(cudaEventCreate(&c->prof_ev[i]));
         c->prof_n = 0;
-    }
-    if (key == HOLO_TUNE_L2_PERSIST_MB && value > 0) {
-        int maxb = 0;
-        HOLO_CUDA_OK(cudaDeviceGetAttribute(&maxb, cudaDevAttrMaxPersistingL2CacheSize, c->device));
-        size_t want = (size_t)value << 20;
-        if (want > (size_t)maxb) want = (size_t)maxb;
-        HOLO_CUDA_OK(cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, want));
-        fprintf(stderr, "holo_tune: persisting L2 set to %zu bytes (device maximum %d)\n", want, maxb);
     }
     if (key == HOLO_TUNE_COV_GRIDX && (value < 1 || value > c->cov_parts_cap)) { holo_set_error("cov grid out of range"); return HOLO_ERR_ARG; }
     c->tune[key] = value;

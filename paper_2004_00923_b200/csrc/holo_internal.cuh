@@ -24,7 +24,6 @@ enum {
                                    // next covariance on the other SMs (memory-bound next to ALU-bound); 0 = in stream order
     HOLO_TUNE_PUSH_PIPE = 10,      // holo_push: 1 = pipelined ring form when T in {16,32,64} and n_new is a multiple of 8 (default)
     HOLO_TUNE_PUSH_INCR = 11,      // holo_push (ring form): 1 = recompute only the Gram rows / columns of the new frames (default)
-    HOLO_TUNE_L2_PERSIST_MB = 12,  // experiment: cudaLimitPersistingL2CacheSize in MiB (0 = leave the device setting alone)
     HOLO_TUNE_COV_TF32 = 13,       // real covariance of holo_process / holo_submit on the tensor cores: 0 = FP32 FFMA kernel,
                                    // 1 = TF32 (inputs rounded to nearest), 3 = 3 x TF32 split; default 1 at T > 32, else 0
     HOLO_TUNE_COV_TF32_DRAIN = 14,
