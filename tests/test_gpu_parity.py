@@ -237,6 +237,42 @@ def test_process_mode3_small_shapes(torch_cuda, n, T, k_lo, k_hi):
     h.close()
 
 
+@pytest.mark.parametrize("nx,ny,T,k_lo,k_hi", [(128, 64, 8, 2, 8), (64, 256, 12, 2, 11), (2048, 16, 4, 2, 4), (16, 1024, 6, 1, 5)])
+def test_process_mode3_nonsquare(torch_cuda, nx, ny, T, k_lo, k_hi):
+    """Mode 3 on non-square frames (the scalar row pass and the column-energy pass of every FFT length involved)."""
+    torch = torch_cuda
+    rng = np.random.default_rng(nx + 3 * ny + T)
+    fr = _rand_frames(rng, T, ny, nx)
+    fr[: T // 2 + 1] += (rng.integers(0, 600, (ny, nx))).astype(np.uint16)
+    h = _holo(nx, ny, T, k_lo, k_hi)
+    h.set_mode(3)
+    M = torch.empty((ny, nx), dtype=torch.float32, device="cuda")
+    h.process(_to_dev(torch, fr), M)
+    rc, st = h.status()
+    assert rc == 0, st
+    out = oracle.process(fr, LAM, PITCH, Z, k_lo, k_hi)
+    err = rel_l2(M.cpu().numpy(), out["M"])
+    assert err <= TOL_M and err <= FP32_M, err
+    h.close()
+
+
+def test_mode3_refuses_wide_rejection_sets(torch_cuda):
+    h = _holo(64, 64, 16, 8, 16)                      # 7 rejected components
+    with pytest.raises(Exception):
+        h.set_mode(3)
+    h.set_range(3, 15)                                # 2 + 1 rejected: fine
+    h.set_mode(3)
+    with pytest.raises(Exception):
+        h.set_range(6, 16)                            # 5 rejected: refused, the window stays
+    rng = np.random.default_rng(3)
+    fr = _rand_frames(rng, 16, 64, 64)
+    M = torch_cuda.empty((64, 64), dtype=torch_cuda.float32, device="cuda")
+    h.process(_to_dev(torch_cuda, fr), M)
+    out = oracle.process(fr, LAM, PITCH, Z, 3, 15)
+    assert rel_l2(M.cpu().numpy(), out["M"]) <= FP32_M
+    h.close()
+
+
 @pytest.mark.parametrize("cfgn", [1, 2, 3])
 def test_process_mode3_matches_oracle_on_configs(torch_cuda, cfgn):
     """BASELINE.json configs[0..2] at full size through mode 3 (holo_process and holo_submit)."""
