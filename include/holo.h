@@ -242,6 +242,7 @@ int holo_launches_per_process(holo_ctx* ctx);
  *   covariance of holograms of real frames is real in exact arithmetic, R21), 9 SMs given to the
  *   side-stream projection in holo_submit (0 = projection in stream order after the next Fresnel stage),
  *   10 pipelined ring form of holo_push (default 1), 11 incremental Gram update in that form (default 1),
+ *   12 direct projection of more than 4 components on the tensor cores (3 x TF32, T <= 32; default 1; 0 = FP32 kernel),
  *   13 real covariance of holo_process / holo_submit on the tensor cores (tcgen05.mma kind::tf32 on values
  *   rounded to nearest, FP64 partials): 0 = FP32 FFMA kernel (default at T <= 32), 1 = TF32 (default at T > 32), 3 = 3 x TF32,
  *   14 operand stages accumulated in TMEM between two FP64 drains of key 13 (default 4 = 512 products),

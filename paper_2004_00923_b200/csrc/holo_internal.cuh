@@ -27,6 +27,7 @@ enum {
     HOLO_TUNE_COV_TF32 = 13,       // real covariance of holo_process / holo_submit on the tensor cores: 0 = FP32 FFMA kernel,
                                    // 1 = TF32 (inputs rounded to nearest), 3 = 3 x TF32 split; default 1 at T > 32, else 0
     HOLO_TUNE_COV_TF32_DRAIN = 14,
+    HOLO_TUNE_PROJ_TC = 12,        // direct projection of more than 4 components on the tensor cores (T <= 32; default 1)
     HOLO_TUNE_ROWS2 = 15,          // mode 3: packed two-frame row pass where supported (1024^2, even T) // stages accumulated in TMEM before the accumulators are added to FP64 (default 4)
     HOLO_TUNE_FFT_LAG = 6,         // frames between the row pass and the column pass in the fused kernel (0 = auto)
 };
@@ -157,6 +158,9 @@ int holo_launch_eig(holo_ctx* c, const float2* C, float* evals, float2* V, cudaS
 // mode 0: direct over columns [k_lo,k_hi] of V; mode 1: complement (total - columns outside)
 int holo_launch_project(holo_ctx* c, const float2* H, const float2* V, int k_lo, int k_hi,
                         int allow_complement, float* image, cudaStream_t st, int center = 0);
+// project_tc.cu: direct projection of wide component windows on the tensor cores (3 x TF32), T <= 32
+bool holo_project_tc_supported(const holo_ctx* c, int nS);
+int holo_launch_project_tc(holo_ctx* c, const float2* H, const float2* V, int k_lo, int k_hi, float* image, cudaStream_t st);
 int holo_fresnel_launch_count(holo_ctx* c);
 // mode 3: image = sum_t |FFT2[q (d_t - sum_{k rejected} e_k V_tk)]|^2 without storing the hologram stack (c->sum and V must be ready)
 int holo_launch_energy_image(holo_ctx* c, const uint16_t* frames, const float2* V, int k_lo, int k_hi, float* image, cudaStream_t st);

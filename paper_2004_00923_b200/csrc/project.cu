@@ -314,6 +314,8 @@ int holo_launch_project(holo_ctx* c, const float2* H, const float2* V, int k_lo,
         if (T <= 32) return launch_deflate<32>(c, a, nc, st);
         return launch_deflate<64>(c, a, nc, st);
     }
+    if (nc > 4 && !c->ring_nrb && c->tune[HOLO_TUNE_PROJ_TC] && holo_project_tc_supported(c, nc))
+        return holo_launch_project_tc(c, H, V, k_lo, k_hi, image, st);
     if (nc <= 1) return launch_proj_t<1>(c, a, st);
     if (nc <= 2) return launch_proj_t<2>(c, a, st);
     if (nc <= 4) return launch_proj_t<4>(c, a, st);
