@@ -218,12 +218,12 @@ def _traffic_table():
 class Runner:
     """One handle + one resident stream of one config; times K steps of one API on a stream."""
 
-    def __init__(self, cfg, plan, dev, tune=(), mode=1):
+    def __init__(self, cfg, plan, dev, tune=(), mode=1, frames=None):
         import torch
         from gen import holo_gen as G
         from paper_2004_00923_b200 import Holo
         self.torch, self.cfg, self.plan, self.dev = torch, cfg, plan, dev
-        self.frames = G.stream_torch(cfg, plan["seed"], dev, n_frames=plan["n_frames"])
+        self.frames = frames if frames is not None else G.stream_torch(cfg, plan["seed"], dev, n_frames=plan["n_frames"])
         torch.cuda.synchronize()
         self.h = Holo(cfg.n, cfg.n, cfg.T, cfg.lam, cfg.pitch, cfg.z, cfg.k_lo, cfg.k_hi)
         for kv in tune:
@@ -442,6 +442,14 @@ def run_ours(args, cfg):
         h.set_range(cfg.k_lo, cfg.k_hi)
         side["cfg3_paper_window_k13_32"] = {"ms_per_step": ms_w / 64, "images_per_s": 64 / (ms_w * 1e-3),
                                             "note": "same stream, component window of PAPER.md:86 (direct projection kernel)"}
+        # the same window through mode 3 (eigen-basis form: 20 transforms of the kept components' raw-domain images)
+        R3 = Runner(cfg, plan, dev, args.tune, 3, frames=R.frames)
+        R3.h.set_range(13, 32)
+        ms_w3, _ = R3.timed("submit", 256, 8, barrier)
+        side["cfg3_paper_window_k13_32_mode3"] = {"ms_per_step": ms_w3 / 256, "images_per_s": 256 / (ms_w3 * 1e-3), "mode": 3,
+                                                  "note": "same stream and window, mode 3"}
+        R3.close()
+        del R3
     lib_ctx = None
     if rank == 0 and world == 1 and args.side and cfg.name.startswith("cfg3"):
         lib_ctx = library_context(torch, R, barrier)

@@ -163,10 +163,12 @@ int holo_raw_covariance(holo_ctx* ctx, const uint16_t* frames_dev, void* C_dev, 
  * 3 (SURVEY.md 8(f)-2 stage 2): mode 2's covariance and eigenvectors, then the image WITHOUT a hologram stack.  With V real
  * (the covariance of the raw frames is real symmetric) the deflation of DESIGN.md R12 commutes with the transform:
  *     M = sum_{k in S} |P_k|^2 = sum_t | FFT2[ q (d_t - sum_{k not in S} e_k V_tk) ] |^2,     e_k = sum_t d_t V_tk,
- * so the rejected components are removed from the RAW frames (one small pass writes the images e_k, at most 4 of them:
- * k_lo - 1 + T - k_hi <= 4, else HOLO_ERR_STATE), the row pass writes its output once (8 T N_p bytes, the only large
- * intermediate), and the column pass is reduced to sum_t |.|^2 in registers: no hologram stack is written, the projection
- * kernel and its read of the stack disappear.  No cancellation (the subtraction happens before the transform, on integers
+ * so the rejected components are removed from the RAW frames (one small pass writes the images e_k), the row pass writes
+ * its output once (8 T N_p bytes, the only large intermediate), and the column pass is reduced to sum_t |.|^2 in registers:
+ * no hologram stack is written, the projection kernel and its read of the stack disappear.  Windows that reject more than
+ * 4 components or keep at most 3/4 of them (the paper's own k in [13, 32]) take the eigen-basis form of the same identity,
+ * M = sum_{k in S} | FFT2[ q e_k ] |^2: the n_S images e_k of the KEPT components are transformed instead of the T frames
+ * (their workspace, 4 T N_p bytes, is allocated by holo_set_mode / holo_set_range when such a window is first seen).  No cancellation (the subtraction happens before the transform, on integers
  * of at most 2^22).  HOLO_WS_H is not filled in this mode.  holo_submit in mode 3 is pipelined by one stack (the covariance
  * of stack i and its eigensolver on the side stream run with the image of stack i-1): the image of submit(i) is complete
  * after the next holo_submit or holo_flush, and frames_dev of submit(i) is READ AGAIN by that next call -- keep it valid

@@ -58,6 +58,7 @@ struct FftArgs {
     const float* defl_img;    // [ndefl][ny][nx]  eT_k = sum_t (T I_t - S) V_{t,k} of the rejected components
     const float* defl_coef;   // [T][ndefl]       V_{t,k} (real: C is real symmetric there, R21)
     int ndefl;
+    const float* eimg;        // prologue mode 2: real input images [nframes][ny][nx] (in_fstride elements apart)
     unsigned int* ticket;     // != nullptr: row kernels of one warp per row draw single rows from this counter (zeroed by the
                               // caller's earlier kernel) instead of a static partition: a CTA that shares its SM with the
                               // eigensolver of the side stream then simply takes fewer rows
@@ -69,10 +70,11 @@ struct NoHook { __device__ __forceinline__ void operator()() const {} };
 // `mid` is called once by every thread in the middle of the tile (after the pass-0 butterflies; the fused
 // kernel does its scheduling work there, when the stores of the previous tile have long drained)
 // LDC: row pitch in elements known at compile time (0: use a.ld) -- turns every address into base + immediate
-// DEFL: the prologue also removes the rejected components in the raw domain (frame index `frame` selects the V row).
+// DEFL (prologue mode of PRO tiles): 0 = d = T I - S; 1 = the rejected components are also removed in the raw domain (frame
+// index `frame` selects the V row); 2 = the input is a real float image (a.eimg: eigen-images of mode 3), d = eimg.
 // ENERGY: nothing is stored; |X|^2 of output slot s (the s-th value this thread would store, see tile_out_offset) is added
 // to acc[s] instead.
-template <int N, int E, int R1, int R2, int B, bool COL, bool PRO, int LDC = 0, class Mid = NoHook, bool DEFL = false, bool ENERGY = false>
+template <int N, int E, int R1, int R2, int B, bool COL, bool PRO, int LDC = 0, class Mid = NoHook, int DEFL = 0, bool ENERGY = false>
 __device__ __forceinline__ void fft_tile(const FftArgs& a, long long in_foff, long long out_foff, int tile_in_frame, float2* sm,
                                          Mid mid = Mid(), int frame = 0, float* acc = nullptr, int seq_override = -1) {
     constexpr int TPS = N / E;
@@ -111,7 +113,17 @@ __device__ __forceinline__ void fft_tile(const FftArgs& a, long long in_foff, lo
             const float2 qyv = __ldg(a.qy + s0);
             const uint16_t* fr = a.frames + ibase;
             const uint32_t* sp = a.sum + (long long)s0 * ld;
-            if constexpr (!DEFL) {
+            if constexpr (DEFL == 2) {
+                const float* ep = a.eimg + in_foff + (long long)s0 * ld + j;
+                float e[E];
+#pragma unroll
+                for (int r = 0; r < E; ++r) e[r] = __ldg(ep + r * TPS);
+#pragma unroll
+                for (int r = 0; r < E; ++r) {
+                    const float2 q = cmul(__ldg(a.qx + j + r * TPS), qyv);
+                    v[r] = make_float2(e[r] * q.x, e[r] * q.y);
+                }
+            } else if constexpr (DEFL == 0) {
 #pragma unroll
                 for (int r = 0; r < E; ++r) {
                     const int i = j + r * TPS;
@@ -214,7 +226,7 @@ __device__ __forceinline__ void fft_tile(const FftArgs& a, long long in_foff, lo
     }
 }
 
-template <int N, int E, int R1, int R2, int B, bool COL, bool PRO, bool DEFL = false>
+template <int N, int E, int R1, int R2, int B, bool COL, bool PRO, int DEFL = 0>
 __global__ void __launch_bounds__((N / E) * B) k_fft(const FftArgs a) {
     extern __shared__ float2 sm[];
     if constexpr (!COL && N / E == 32) {
@@ -272,7 +284,7 @@ k_col_energy(const FftArgs a, float* __restrict__ out, long long npix, int nfram
 #pragma unroll
     for (int s = 0; s < E; ++s) acc[s] = 0.f;
     for (int t = t0; t < t1; ++t)
-        fft_tile<N, E, R1, R2, B, true, false, 0, NoHook, false, true>(a, (long long)t * a.in_fstride, 0, tile, sm, NoHook(), 0, acc);
+        fft_tile<N, E, R1, R2, B, true, false, 0, NoHook, 0, true>(a, (long long)t * a.in_fstride, 0, tile, sm, NoHook(), 0, acc);
     const int c = (int)threadIdx.x % B;
     float* op = out + (long long)split * npix + (long long)tile * B + c;
 #pragma unroll
@@ -287,6 +299,61 @@ __global__ void __launch_bounds__(256) k_sum_partial_images(const float* __restr
         float4 s = __ldg(p4 + p);
         for (int k = 1; k < nsplit; ++k) { const float4 w = __ldg(p4 + (long long)k * n4 + p); s.x += w.x; s.y += w.y; s.z += w.z; s.w += w.w; }
         reinterpret_cast<float4*>(out)[p] = s;
+    }
+}
+
+// Mode 3, eigen-basis form: E_k(x) = sum_t (T I_t(x) - S(x)) Re V_{t,k} for the KEPT components k = c_lo .. c_lo + nS - 1
+// (float [nS][npix]).  With V real and orthonormal, sum_{k in S} |F[q E_k]|^2 = sum_{k in S} |P_k|^2 T^2: the image of Eq. 7
+// from nS transforms instead of T, for any window.  PX pixels per thread: the frame values stay in registers, the
+// coefficients are broadcast from shared memory (one LDS per PX FMAs).
+template <int TMAX, int PX>
+__global__ void __launch_bounds__(128) k_eigen_images(const uint16_t* __restrict__ frames, const uint32_t* __restrict__ sum,
+                                                      const float2* __restrict__ V, long long npix, int T, int c_lo, int nS, float* __restrict__ img) {
+    extern __shared__ float Vs_e[];                        // [nS][TMAX], zero padded in t
+    for (int i = threadIdx.x; i < nS * TMAX; i += blockDim.x) {
+        const int k = i / TMAX, t = i - k * TMAX;
+        Vs_e[i] = t < T ? V[t * T + c_lo + k].x : 0.f;
+    }
+    __syncthreads();
+    const long long nvec = npix / PX;
+    const float Tf = (float)T;
+    for (long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x; q < nvec; q += (long long)gridDim.x * blockDim.x) {
+        float d[TMAX][PX];
+        float S[PX];
+#pragma unroll
+        for (int x = 0; x < PX; ++x) S[x] = (float)__ldg(sum + q * PX + x);
+#pragma unroll
+        for (int t = 0; t < TMAX; ++t) {
+            if (t < T) {
+                if constexpr (PX == 4) {
+                    const uint2 w = __ldg(reinterpret_cast<const uint2*>(frames + (long long)t * npix) + q);
+                    d[t][0] = fmaf(Tf, (float)(w.x & 0xffffu), -S[0]); d[t][1] = fmaf(Tf, (float)(w.x >> 16), -S[1]);
+                    d[t][2] = fmaf(Tf, (float)(w.y & 0xffffu), -S[2]); d[t][3] = fmaf(Tf, (float)(w.y >> 16), -S[3]);
+                } else {
+                    const uint32_t w = __ldg(reinterpret_cast<const uint32_t*>(frames + (long long)t * npix) + q);
+                    d[t][0] = fmaf(Tf, (float)(w & 0xffffu), -S[0]); d[t][1] = fmaf(Tf, (float)(w >> 16), -S[1]);
+                }
+            } else {
+#pragma unroll
+                for (int x = 0; x < PX; ++x) d[t][x] = 0.f;
+            }
+        }
+#pragma unroll 1
+        for (int k = 0; k < nS; ++k) {
+            const float* v = Vs_e + k * TMAX;
+            float acc[PX];
+#pragma unroll
+            for (int x = 0; x < PX; ++x) acc[x] = 0.f;
+#pragma unroll
+            for (int t = 0; t < TMAX; ++t) {
+                const float w = v[t];
+#pragma unroll
+                for (int x = 0; x < PX; ++x) acc[x] = fmaf(d[t][x], w, acc[x]);
+            }
+            float* dst = img + (long long)k * npix + q * PX;
+            if constexpr (PX == 4) *reinterpret_cast<float4*>(dst) = make_float4(acc[0], acc[1], acc[2], acc[3]);
+            else *reinterpret_cast<float2*>(dst) = make_float2(acc[0], acc[1]);
+        }
     }
 }
 
@@ -493,7 +560,7 @@ void holo_fft_plan_free(FftPlan* p) {
     p->tw1 = p->tw2 = nullptr;
 }
 
-template <int N, int E, int R1, int R2, int B, bool COL, bool PRO, bool DEFL = false>
+template <int N, int E, int R1, int R2, int B, bool COL, bool PRO, int DEFL = 0>
 static int launch_fft_t(const FftArgs& a, int num_sms, int device, cudaStream_t st) {
     constexpr int threads = (N / E) * B;
     constexpr size_t smem = (R1 > 1) ? sizeof(float2) * (size_t)(N + N / E) * B : 0;
@@ -507,7 +574,7 @@ static int launch_fft_t(const FftArgs& a, int num_sms, int device, cudaStream_t 
 }
 
 // B (sequences per CTA) per length: rows aim at 256 threads; columns at >= 64-byte segments
-template <bool COL, bool PRO, bool DEFL = false>
+template <bool COL, bool PRO, int DEFL = 0>
 static int launch_fft(int N, const FftArgs& a, int num_sms, int device, cudaStream_t st) {
     switch (N) {
         case 16:   return launch_fft_t<16, 16, 1, 1, 16, COL, PRO, DEFL>(a, num_sms, device, st);
@@ -673,20 +740,39 @@ int holo_launch_fresnel(holo_ctx* c, const uint16_t* frames, float2* H, cudaStre
 //      (complex64 [T][ny][nx] in c->H: the only large intermediate, written and read once)
 //   3. k_col_energy: column transform reduced to sum_t |.|^2, frame splits -> k_sum_partial_images
 // ------------------------------------------------------------------------------------------------
-int holo_mode3_splits(const holo_ctx* c) {
+int holo_mode3_splits(const holo_ctx* c, int nframes) {
     const int ct = c->nx / fft_batch(c->ny);
     int ns = (2 * c->num_sms) / (ct > 0 ? ct : 1);
     if (ns < 1) ns = 1;
-    if (ns > c->T) ns = c->T;
+    if (ns > nframes) ns = nframes;
     if (ns > 8) ns = 8;
     return ns;
 }
 
+// frame basis (T transforms, at most 4 components removed in the raw domain) or eigen basis (nS transforms of the kept
+// components' raw-domain images): the cheaper one that is possible
+bool holo_mode3_eigen_form(const holo_ctx* c, int k_lo, int k_hi) {
+    const int T = c->T, nS = k_hi - k_lo + 1, ndefl = T - nS;
+    return ndefl > 4 || 4 * nS <= 3 * T;
+}
+
 int holo_launch_energy_image(holo_ctx* c, const uint16_t* frames, const float2* V, int k_lo, int k_hi, float* image, cudaStream_t st) {
     const int T = c->T;
-    const int n0 = k_lo - 1, n1 = T - k_hi, ndefl = n0 + n1;
-    if (ndefl > 4) { holo_set_error("mode 3 removes at most 4 components in the raw domain (asked for %d)", ndefl); return HOLO_ERR_STATE; }
-    if (ndefl > 0) {
+    const int n0 = k_lo - 1, n1 = T - k_hi, ndefl = n0 + n1, nS = k_hi - k_lo + 1;
+    const bool eigen = holo_mode3_eigen_form(c, k_lo, k_hi);
+    if (eigen && !c->eig_img) { holo_set_error("internal: eigen-image workspace missing (holo_set_mode / holo_set_range allocate it)"); return HOLO_ERR_STATE; }
+    int rc = HOLO_OK;
+    const int nframes = eigen ? nS : T;
+    if (eigen) {
+        HoloProf prof(c, HOLO_K_SUM, st);
+        const int px = T <= 32 ? 4 : 2;
+        const long long nvec = c->npix / px;
+        long long want = (nvec + 127) / 128;
+        const int grid = (int)(want < (long long)c->num_sms * 8 ? want : (long long)c->num_sms * 8);
+        if (T <= 32) k_eigen_images<32, 4><<<grid, 128, (size_t)nS * 32 * sizeof(float), st>>>(frames, c->sum, V, c->npix, T, k_lo - 1, nS, c->eig_img);
+        else         k_eigen_images<64, 2><<<grid, 128, (size_t)nS * 64 * sizeof(float), st>>>(frames, c->sum, V, c->npix, T, k_lo - 1, nS, c->eig_img);
+        HOLO_CUDA_OK(cudaGetLastError());
+    } else if (ndefl > 0) {
         HoloProf prof(c, HOLO_K_SUM, st);
         const long long nvec = c->npix >> 3;
         long long want = (nvec + 255) / 256;
@@ -705,15 +791,16 @@ int holo_launch_energy_image(holo_ctx* c, const uint16_t* frames, const float2* 
     a.in_fstride = c->npix; a.out_fstride = c->npix;
     a.ld = c->nx; a.nseq = c->ny;
     a.tiles_per_frame = c->ny / fft_batch(c->nx);
-    a.ntiles = T * a.tiles_per_frame;
+    a.ntiles = nframes * a.tiles_per_frame;
     a.T = T;
     a.defl_img = c->defl_img; a.defl_coef = c->defl_coef; a.ndefl = ndefl;
+    a.eimg = c->eig_img;
     a.ticket = c->counters + 1001;                        // zeroed by k_sum_gram, which always precedes this call in stream order
-    int rc;
-    if (c->tune[HOLO_TUNE_ROWS2] && holo_rows2_supported(c)) rc = holo_launch_rows2(c, frames, c->H, ndefl, st);
+    if (eigen) { HoloProf prof(c, HOLO_K_FFT_ROWS, st); rc = launch_fft<false, true, 2>(c->nx, a, c->num_sms, c->device, st); }
+    else if (c->tune[HOLO_TUNE_ROWS2] && holo_rows2_supported(c)) rc = holo_launch_rows2(c, frames, c->H, ndefl, st);
     else
     { HoloProf prof(c, HOLO_K_FFT_ROWS, st);
-      rc = ndefl ? launch_fft<false, true, true>(c->nx, a, c->num_sms, c->device, st) : launch_fft<false, true, false>(c->nx, a, c->num_sms, c->device, st); }
+      rc = ndefl ? launch_fft<false, true, 1>(c->nx, a, c->num_sms, c->device, st) : launch_fft<false, true, 0>(c->nx, a, c->num_sms, c->device, st); }
     if (rc) return rc;
     FftArgs b{};
     b.in = c->H; b.out = nullptr;
@@ -723,9 +810,9 @@ int holo_launch_energy_image(holo_ctx* c, const uint16_t* frames, const float2* 
     b.tiles_per_frame = c->nx / fft_batch(c->ny);
     b.ntiles = b.tiles_per_frame;
     b.T = T;
-    const int ns = holo_mode3_splits(c);
+    const int ns = holo_mode3_splits(c, nframes);
     { HoloProf prof(c, HOLO_K_FFT_COLS, st);
-      rc = launch_col_energy(c->ny, b, ns > 1 ? c->energy_parts : image, c->npix, T, ns, c->device, st); }
+      rc = launch_col_energy(c->ny, b, ns > 1 ? c->energy_parts : image, c->npix, nframes, ns, c->device, st); }
     if (rc) return rc;
     if (ns > 1) {
         HoloProf prof(c, HOLO_K_PROJECT, st);

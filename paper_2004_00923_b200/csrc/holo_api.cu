@@ -79,7 +79,7 @@ static void free_ctx(holo_ctx* c) {
     cudaFree(c->C); cudaFree(c->evals); cudaFree(c->V); cudaFree(c->status);
     if (c->noconv_host) cudaFreeHost(c->noconv_host);
     cudaFree(c->counters); cudaFree(c->gram_X); cudaFree(c->gram_Xp);
-    cudaFree(c->defl_img); cudaFree(c->defl_coef); cudaFree(c->energy_parts); cudaFree(c->sum1);
+    cudaFree(c->defl_img); cudaFree(c->defl_coef); cudaFree(c->energy_parts); cudaFree(c->sum1); cudaFree(c->eig_img);
     if (c->prof_ev) {
         for (int i = 0; i < 2 * HOLO_PROF_CAP; ++i) cudaEventDestroy(c->prof_ev[i]);
         delete[] c->prof_ev;
@@ -318,12 +318,20 @@ extern "C" int holo_raw_covariance(holo_ctx* c, const uint16_t* frames_dev, void
     return holo_launch_sum_gram(c, frames_dev, (float2*)C_dev, (cudaStream_t)stream);
 }
 
+// mode 3: a window that takes the eigen-basis form needs its image workspace (allocated once, here: never inside a
+// compute call)
+static int mode3_prepare(holo_ctx* c, int k_lo, int k_hi) {
+    if (holo_mode3_eigen_form(c, k_lo, k_hi) && !c->eig_img)
+        HOLO_CUDA_OK(cudaMalloc(&c->eig_img, (size_t)c->T * c->npix * sizeof(float)));
+    return HOLO_OK;
+}
+
 extern "C" int holo_set_mode(holo_ctx* c, int mode) {
     CHECK_CTX_QUIET(c);
     if (mode < 1 || mode > 3) { holo_set_error("mode must be 1 (covariance of the hologram stack), 2 (of the raw frames) or 3 (2 + image without the hologram stack)"); return HOLO_ERR_ARG; }
     if (c->pend_image || c->pend3_image || c->proj_recorded[0] || c->proj_recorded[1]) { holo_set_error("holo_flush the open holo_submit sequence before changing the mode"); return HOLO_ERR_STATE; }
     if (mode == 3) {
-        if ((c->k_lo - 1) + (c->T - c->k_hi) > 4) { holo_set_error("mode 3 removes at most 4 components (k_lo - 1 + T - k_hi <= 4)"); return HOLO_ERR_STATE; }
+        { const int rc3 = mode3_prepare(c, c->k_lo, c->k_hi); if (rc3) return rc3; }
         if (!c->defl_img) {                                  // first use: the mode's own workspace (allocation, may synchronise)
             HOLO_CUDA_OK(cudaMalloc(&c->defl_img, (size_t)4 * c->npix * sizeof(float)));
             HOLO_CUDA_OK(cudaMalloc(&c->defl_coef, (size_t)HOLO_MAX_T * 4 * sizeof(float)));
@@ -446,8 +454,12 @@ extern "C" int holo_submit(holo_ctx* c, const uint16_t* frames_dev, float* image
     const int s = (int)(c->nsubmit & 1);
     float2* H = s ? c->H1 : c->H;
     float2* C = s ? c->C1 : c->C;
-    const int split = c->tune[HOLO_TUNE_SPLIT_SMS];
-    if (split > 0) { if ((rc = join_side(c, st, s))) return rc; }      // H / V of slot s are free once the projection of stack i-2 is done
+    // the SM split pairs the HBM-bound DEFLATION projection with the ALU-bound covariance; a wide rejection set takes the
+    // direct (tensor-core) projection, which needs the whole GPU: stream order then
+    const int nS_now = c->k_hi - c->k_lo + 1;
+    const bool deflating = c->tune[HOLO_TUNE_PROJ_COMPLEMENT] && 2 * (c->T - nS_now) <= nS_now;
+    const int split = deflating ? c->tune[HOLO_TUNE_SPLIT_SMS] : 0;
+    if (c->tune[HOLO_TUNE_SPLIT_SMS] > 0) { if ((rc = join_side(c, st, s))) return rc; }      // H / V of slot s are free once the projection of stack i-2 is done
     if ((rc = holo_launch_fresnel(c, frames_dev, H, st))) return rc;
     if ((rc = project_pending(c, st))) return rc;
     c->cov_grid_cap = split > 0 ? c->num_sms - split : 0;
@@ -725,7 +737,7 @@ extern "C" int holo_set_range(holo_ctx* c, int k_lo, int k_hi) {
         holo_set_error("a holo_push sequence is open: its window's complement must stay at most half of the window");
         return HOLO_ERR_STATE;
     }
-    if (c->mode == 3 && (k_lo - 1) + (c->T - k_hi) > 4) { holo_set_error("mode 3 removes at most 4 components (k_lo - 1 + T - k_hi <= 4)"); return HOLO_ERR_STATE; }
+    if (c->mode == 3) { const int rc3 = mode3_prepare(c, k_lo, k_hi); if (rc3) return rc3; }
     c->k_lo = k_lo; c->k_hi = k_hi;
     return HOLO_OK;
 }
@@ -786,7 +798,9 @@ extern "C" int holo_launches_per_process(holo_ctx* c) {
     CHECK_CTX_QUIET(c);
     if (c->mode == 3) {
         const int ndefl = (c->k_lo - 1) + (c->T - c->k_hi);
-        return 2 /*sum + Gram, reduce + finish*/ + 1 /*eig*/ + (ndefl ? 1 : 0) + 2 /*row pass, column energy*/ + (holo_mode3_splits(c) > 1 ? 1 : 0);
+        const bool eigen = holo_mode3_eigen_form(c, c->k_lo, c->k_hi);
+        return 2 /*sum + Gram, reduce + finish*/ + 1 /*eig*/ + ((eigen || ndefl) ? 1 : 0) + 2 /*row pass, column energy*/
+             + (holo_mode3_splits(c, eigen ? c->k_hi - c->k_lo + 1 : c->T) > 1 ? 1 : 0);
     }
     if (c->mode == 2) return 2 /*sum + Gram, finish*/ + (holo_fresnel_launch_count(c) - 1) + 1 /*eig*/ + 1 /*project*/;
     return holo_fresnel_launch_count(c) + 2 /*cov partial + reduce*/ + 1 /*eig*/ + 1 /*project*/;

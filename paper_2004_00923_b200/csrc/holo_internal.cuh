@@ -74,6 +74,7 @@ struct holo_ctx {
     float* defl_img;        // mode 3: [4][ny][nx] raw-domain images of the rejected components (allocated at first use)
     float* defl_coef;       // mode 3: [T][4] their eigenvector entries
     float* energy_parts;    // mode 3: [splits][ny][nx] partial energy images
+    float* eig_img;         // mode 3, eigen-basis form: [T][ny][nx] raw-domain images of the kept components (allocated when a window needs it)
     uint32_t* sum1;         // mode 3, streaming form: frame sum of the second slot
     const uint16_t* pend3_frames; float* pend3_image; int pend3_slot;   // mode 3, streaming form: the stack whose image is owed
     unsigned long long* gram_X;   // [128][128] int64 byte-plane Gram of the raw frames (mode 2, rawgram.cu)
@@ -164,7 +165,8 @@ int holo_launch_project_tc(holo_ctx* c, const float2* H, const float2* V, int k_
 int holo_fresnel_launch_count(holo_ctx* c);
 // mode 3: image = sum_t |FFT2[q (d_t - sum_{k rejected} e_k V_tk)]|^2 without storing the hologram stack (c->sum and V must be ready)
 int holo_launch_energy_image(holo_ctx* c, const uint16_t* frames, const float2* V, int k_lo, int k_hi, float* image, cudaStream_t st);
-int holo_mode3_splits(const holo_ctx* c);
+int holo_mode3_splits(const holo_ctx* c, int nframes);
+bool holo_mode3_eigen_form(const holo_ctx* c, int k_lo, int k_hi);
 // display.cu: PAPER.md:86 normalisation, quadrant swap, Eq. 3 SVD filter
 int holo_launch_normalize(holo_ctx* c, float* image, cudaStream_t st);
 int holo_launch_fftshift(holo_ctx* c, const float* in, float* out, cudaStream_t st);
