@@ -407,7 +407,8 @@ def test_eig_degenerate_inputs(torch_cuda):
 # ------------------------------------------------------------------ A5/A6 holo_project (isolated)
 @pytest.mark.parametrize("T,n,k_lo,k_hi,unitary", [(16, 64, 2, 16, True), (16, 64, 2, 16, False), (32, 64, 13, 32, True),
                                                    (32, 32, 5, 9, True), (8, 32, 3, 3, False), (8, 32, 1, 8, True),
-                                                   (64, 32, 3, 64, True), (64, 32, 1, 40, False), (5, 16, 2, 4, True)])
+                                                   (64, 32, 3, 64, True), (64, 32, 1, 40, False), (5, 16, 2, 4, True),
+                                                   (32, 64, 1, 32, False), (7, 32, 1, 6, False), (17, 16, 3, 17, False), (32, 16, 9, 13, True)])
 def test_project_parity_isolated(torch_cuda, T, n, k_lo, k_hi, unitary):
     torch = torch_cuda
     rng = np.random.default_rng(T + n + k_lo)
@@ -422,6 +423,12 @@ def test_project_parity_isolated(torch_cuda, T, n, k_lo, k_hi, unitary):
     Mo = oracle.envelope(oracle.project(H32.astype(np.complex128), V32.astype(np.complex128)), k_lo, k_hi)
     err = rel_l2(M.cpu().numpy(), Mo)
     assert err <= TOL_M and err <= FP32_M, err
+    # the FP32 kernel and the tensor-core kernel (3 x TF32; direct form with more than 4 components at T <= 32) agree
+    h.tune(12, 0)
+    M0 = torch.empty_like(M)
+    h.project(_to_dev(torch, H32), _to_dev(torch, V32), M0)
+    assert rel_l2(M0.cpu().numpy(), Mo) <= FP32_M
+    assert rel_l2(M0.cpu().numpy(), M.cpu().numpy()) <= 5e-6
     h.close()
 
 
