@@ -165,21 +165,27 @@ __device__ __forceinline__ void exchange_read_twiddle(const XAddr& x, cpk* v, co
 // Warps are autonomous (row pairs drawn from a ticket, warp-private exchange slice, no CTA-wide step).
 // ------------------------------------------------------------------------------------------------
 struct R2Args {
-    const uint16_t* frames;   // [T][N][N]
+    const uint16_t* frames;   // [T][ny][nx]
     const uint32_t* sum;      // S = sum_t I_t
     const float2* qxs;        // chirp along x, scaled by 1/T
     const float2* qy;
-    const float2* tw;         // [32][32] inter-pass twiddles
-    const float* defl_img;    // [ndefl][N][N]  eT_k
+    const float2* tw;         // [32][32] inter-pass twiddles of the 1024-point transform
+    const float2* tw2048;     // NX = 2048: exp(-2 pi i n / 2048), n < 1024
+    const float* defl_img;    // [ndefl][ny][nx]  eT_k
     const float* defl_coef;   // [T][ndefl]
-    float2* out;              // [T][N][N] row-pass output
+    float2* out;              // [T][ny][nx] row-pass output
     unsigned int* ticket;     // zeroed by an earlier kernel of the stream
-    int T, ndefl;
+    int T, ndefl, ny;
 };
 
 constexpr int R2_WARPS = 12;
-constexpr int R2_SMEM = 1024 + (R2_WARPS / 4) * F2_TILE + 2 * F2N * 8;
+template <int NX> constexpr int r2_smem() { return 1024 + (R2_WARPS / 4) * F2_TILE + F2N * 8 + NX * 8 + (NX == 2048 ? F2N * 8 : 0); }
 
+// NX = 1024: a warp transforms row y of the two frames (f, f + 1): the packed pair is (frame f, frame f + 1).
+// NX = 2048: a warp transforms ONE row of 2048 points: a radix-2 decimation-in-frequency step in the prologue,
+//   y0(n) = x(n) + x(n + 1024),  y1(n) = (x(n) - x(n + 1024)) W_2048^n,   X(2k) = FFT1024[y0](k), X(2k + 1) = FFT1024[y1](k),
+// makes the packed pair (y0, y1); the two results of a register slot are adjacent outputs: one 16-byte store.
+template <int NX>
 __global__ void __launch_bounds__(R2_WARPS * 32, 1) k_rows2(const R2Args a) {
     extern __shared__ unsigned char smraw_[];
     const uint32_t s0 = smem_u32(smraw_);
@@ -188,13 +194,16 @@ __global__ void __launch_bounds__(R2_WARPS * 32, 1) k_rows2(const R2Args a) {
     const uint32_t bufs = s0 + pad;
     float2* tw_s = reinterpret_cast<float2*>(base + (R2_WARPS / 4) * F2_TILE);
     float2* qx_s = tw_s + F2N;
+    float2* w2_s = qx_s + NX;                                  // NX = 2048 only
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    for (int i = tid; i < F2N; i += R2_WARPS * 32) { tw_s[i] = a.tw[i]; qx_s[i] = a.qxs[i]; }
+    for (int i = tid; i < F2N; i += R2_WARPS * 32) tw_s[i] = a.tw[i];
+    for (int i = tid; i < NX; i += R2_WARPS * 32) qx_s[i] = a.qxs[i];
+    if constexpr (NX == 2048) for (int i = tid; i < F2N; i += R2_WARPS * 32) w2_s[i] = a.tw2048[i];
     __syncthreads();
     const uint32_t buf = bufs + (uint32_t)(warp >> 2) * F2_TILE;
     const XAddr xa = make_xaddr(buf, warp & 3, lane);
-    const long long npix = (long long)F2N * F2N;
-    const unsigned int npairs = (unsigned int)(a.T / 2) * F2N;
+    const long long npix = (long long)NX * a.ny;
+    const unsigned int ntasks = NX == 1024 ? (unsigned int)(a.T / 2) * (unsigned int)a.ny : (unsigned int)a.T * (unsigned int)a.ny;
     const float Tf = (float)a.T;
     // tickets are drawn two tasks ahead (the atomic's round trip is hidden) and the frame rows of the NEXT task are pulled
     // into L2 while the current one computes (ncu: 14 % of the warp time waited for the ticket, 30 % for the loads)
@@ -203,42 +212,61 @@ __global__ void __launch_bounds__(R2_WARPS * 32, 1) k_rows2(const R2Args a) {
     tk0 = __shfl_sync(0xffffffffu, tk0, 0); tk1 = __shfl_sync(0xffffffffu, tk1, 0);
     for (;;) {
         const unsigned int tk = tk0;
-        if (tk >= npairs) break;
+        if (tk >= ntasks) break;
         unsigned int tk2 = 0u;
         if (lane == 0) tk2 = atomicAdd(a.ticket, 1u);
-        if (tk1 < npairs) {
-            const int f1 = 2 * (int)(tk1 / F2N), y1 = (int)(tk1 % F2N);
-            const uint16_t* pf = a.frames + (long long)(f1 + (lane >> 4)) * npix + (long long)y1 * F2N + (lane & 15) * 64;
+        if (tk1 < ntasks) {
+            const int f1 = (NX == 1024 ? 2 : 1) * (int)(tk1 / (unsigned int)a.ny), y1 = (int)(tk1 % (unsigned int)a.ny);
+            const uint16_t* pf = NX == 1024 ? a.frames + (long long)(f1 + (lane >> 4)) * npix + (long long)y1 * NX + (lane & 15) * 64
+                                            : a.frames + (long long)f1 * npix + (long long)y1 * NX + lane * 64;
             asm volatile("prefetch.global.L2 [%0];" ::"l"(pf));
         }
-        const int f = 2 * (int)(tk / F2N), y = (int)(tk % F2N);
-        const uint16_t* Ia = a.frames + (long long)f * npix + (long long)y * F2N + lane;
-        const uint32_t* Sp = a.sum + (long long)y * F2N + lane;
+        const int f = (NX == 1024 ? 2 : 1) * (int)(tk / (unsigned int)a.ny), y = (int)(tk % (unsigned int)a.ny);
+        const uint16_t* Ia = a.frames + (long long)f * npix + (long long)y * NX + lane;
+        const uint32_t* Sp = a.sum + (long long)y * NX + lane;
         const float2 qyv = __ldg(a.qy + y);
         cpk v[32];
-        // d = T I - S exactly (integers below 2^23); the pair (frame f, frame f + 1) in the two halves of a packed value
+        // second element of the pair: the same position of frame f + 1 (NX = 1024) / position n + 1024 of the same row
+        const long long poff = NX == 1024 ? npix : 1024;
+        // d = T I - S exactly (integers below 2^23)
 #pragma unroll
         for (int m = 0; m < 32; ++m) {
-            const float ia = (float)__ldg(Ia + 32 * m), ib = (float)__ldg(Ia + npix + 32 * m);
-            const float sv = (float)__ldg(Sp + 32 * m);
-            v[m].re = make_float2(fmaf(Tf, ia, -sv), fmaf(Tf, ib, -sv));
+            const float ia = (float)__ldg(Ia + 32 * m), ib = (float)__ldg(Ia + poff + 32 * m);
+            const float sa = (float)__ldg(Sp + 32 * m);
+            const float sb = NX == 1024 ? sa : (float)__ldg(Sp + 1024 + 32 * m);
+            v[m].re = make_float2(fmaf(Tf, ia, -sa), fmaf(Tf, ib, -sb));
         }
-        const float* ep = a.defl_img + (long long)y * F2N + lane;
+        const float* ep = a.defl_img + (long long)y * NX + lane;
         for (int kk = 0; kk < a.ndefl; ++kk) {
-            const float2 cf = make_float2(-__ldg(a.defl_coef + f * a.ndefl + kk), -__ldg(a.defl_coef + (f + 1) * a.ndefl + kk));
-            float e[32];
+            const float ca = -__ldg(a.defl_coef + f * a.ndefl + kk);
+            const float2 cf = make_float2(ca, NX == 1024 ? -__ldg(a.defl_coef + (f + 1) * a.ndefl + kk) : ca);
+            float e[32], e2[NX == 1024 ? 1 : 32];
 #pragma unroll
-            for (int m = 0; m < 32; ++m) e[m] = __ldg(ep + 32 * m);
+            for (int m = 0; m < 32; ++m) { e[m] = __ldg(ep + 32 * m); if constexpr (NX == 2048) e2[m] = __ldg(ep + 1024 + 32 * m); }
 #pragma unroll
-            for (int m = 0; m < 32; ++m) v[m].re = __ffma2_rn(make_float2(e[m], e[m]), cf, v[m].re);
+            for (int m = 0; m < 32; ++m) v[m].re = __ffma2_rn(make_float2(e[m], NX == 1024 ? e[m] : e2[m]), cf, v[m].re);
             ep += npix;
         }
+        if constexpr (NX == 1024) {
 #pragma unroll
-        for (int m = 0; m < 32; ++m) {
-            const float2 q = cmul(qx_s[lane + 32 * m], qyv);
-            const float2 d = v[m].re;
-            v[m].re = __fmul2_rn(d, make_float2(q.x, q.x));
-            v[m].im = __fmul2_rn(d, make_float2(q.y, q.y));
+            for (int m = 0; m < 32; ++m) {
+                const float2 q = cmul(qx_s[lane + 32 * m], qyv);
+                const float2 d = v[m].re;
+                v[m].re = __fmul2_rn(d, make_float2(q.x, q.x));
+                v[m].im = __fmul2_rn(d, make_float2(q.y, q.y));
+            }
+        } else {
+#pragma unroll
+            for (int m = 0; m < 32; ++m) {
+                const int n = lane + 32 * m;
+                const float2 qa = cmul(qx_s[n], qyv), qb = cmul(qx_s[n + 1024], qyv);
+                const float2 d = v[m].re;
+                const float2 xa2 = make_float2(d.x * qa.x, d.x * qa.y), xb2 = make_float2(d.y * qb.x, d.y * qb.y);
+                const float2 y0 = make_float2(xa2.x + xb2.x, xa2.y + xb2.y);
+                const float2 y1 = cmul(make_float2(xa2.x - xb2.x, xa2.y - xb2.y), w2_s[n]);
+                v[m].re = make_float2(y0.x, y1.x);
+                v[m].im = make_float2(y0.y, y1.y);
+            }
         }
         P2S<0, 5>::run(v);
         exchange_write(xa, v);
@@ -248,12 +276,19 @@ __global__ void __launch_bounds__(R2_WARPS * 32, 1) k_rows2(const R2Args a) {
         P2S<0, 4>::run(v);
         float4 o[32];
         P2Last<0>::run(v, o);
-        // X[lane + 32 kk] of frame f in (o.x, o.y), of frame f + 1 in (o.z, o.w); kk = brev(register slot)
-        float2* out0 = a.out + (long long)f * npix + (long long)y * F2N + lane;
+        if constexpr (NX == 1024) {
+            // X[lane + 32 kk] of frame f in (o.x, o.y), of frame f + 1 in (o.z, o.w); kk = brev(register slot)
+            float2* out0 = a.out + (long long)f * npix + (long long)y * NX + lane;
 #pragma unroll
-        for (int p2 = 0; p2 < 32; ++p2) __stcs(out0 + 32 * brev<32>(p2), make_float2(o[p2].x, o[p2].y));
+            for (int p2 = 0; p2 < 32; ++p2) __stcs(out0 + 32 * brev<32>(p2), make_float2(o[p2].x, o[p2].y));
 #pragma unroll
-        for (int p2 = 0; p2 < 32; ++p2) __stcs(out0 + npix + 32 * brev<32>(p2), make_float2(o[p2].z, o[p2].w));
+            for (int p2 = 0; p2 < 32; ++p2) __stcs(out0 + npix + 32 * brev<32>(p2), make_float2(o[p2].z, o[p2].w));
+        } else {
+            // (X[2 k], X[2 k + 1]) with k = lane + 32 kk: adjacent outputs, one 16-byte store
+            float4* out0 = reinterpret_cast<float4*>(a.out + (long long)f * npix + (long long)y * NX) + lane;
+#pragma unroll
+            for (int p2 = 0; p2 < 32; ++p2) __stcs(out0 + 32 * brev<32>(p2), o[p2]);
+        }
         tk0 = tk1;
         tk1 = __shfl_sync(0xffffffffu, tk2, 0);
     }
@@ -262,18 +297,24 @@ __global__ void __launch_bounds__(R2_WARPS * 32, 1) k_rows2(const R2Args a) {
 }  // namespace
 
 
-// mode 3 row pass in the packed form: supported for 1024 x 1024 frames and even T
-bool holo_rows2_supported(const holo_ctx* c) { return c->nx == F2N && c->ny == F2N && (c->T % 2) == 0; }
+// mode 3 row pass in the packed form: rows of 1024 points (even T: frame pairs) or of 2048 points (even / odd halves)
+bool holo_rows2_supported(const holo_ctx* c) { return (c->nx == 1024 && (c->T % 2) == 0) || c->nx == 2048; }
 
 int holo_launch_rows2(holo_ctx* c, const uint16_t* frames, float2* out, int ndefl, cudaStream_t st) {
     R2Args a{};
     a.frames = frames; a.sum = c->sum; a.qxs = c->qxs; a.qy = c->qy; a.tw = c->px.tw1;
+    a.tw2048 = c->nx == 2048 ? c->px.tw2 + 1024 : nullptr;       // row r = 1 of the pass-2 table [2][1024]: exp(-2 pi i b / 2048)
     a.defl_img = c->defl_img; a.defl_coef = c->defl_coef; a.out = out; a.ticket = c->counters + 1001;
-    a.T = c->T; a.ndefl = ndefl;
+    a.T = c->T; a.ndefl = ndefl; a.ny = c->ny;
     int rc;
-    if ((rc = holo_ensure_smem_attr((const void*)k_rows2, c->device, R2_SMEM))) return rc;
     HoloProf prof(c, HOLO_K_FFT_ROWS, st);
-    k_rows2<<<c->num_sms, R2_WARPS * 32, R2_SMEM, st>>>(a);
+    if (c->nx == 1024) {
+        if ((rc = holo_ensure_smem_attr((const void*)k_rows2<1024>, c->device, r2_smem<1024>()))) return rc;
+        k_rows2<1024><<<c->num_sms, R2_WARPS * 32, r2_smem<1024>(), st>>>(a);
+    } else {
+        if ((rc = holo_ensure_smem_attr((const void*)k_rows2<2048>, c->device, r2_smem<2048>()))) return rc;
+        k_rows2<2048><<<c->num_sms, R2_WARPS * 32, r2_smem<2048>(), st>>>(a);
+    }
     HOLO_CUDA_OK(cudaGetLastError());
     return HOLO_OK;
 }
