@@ -192,9 +192,10 @@ def run_reference(args, cfg):
 KCLASS = ["sum", "fft_rows", "fft_cols", "cov_partial", "cov_reduce", "eig", "project"]
 
 
-def kernel_name(cls, fused_fft, cov_real, mode, T=32):
+def kernel_name(cls, fused_fft, cov_real, mode, T=32, n=1024):
     if mode == 3:
-        return {"sum": "k_sum_gram + k_deflate_images", "fft_rows": "k_fft<rows, deflating prologue>", "fft_cols": "k_col_energy",
+        rows = "k_rows2" if (n == 1024 and T % 2 == 0) or n == 2048 else "k_fft<rows, deflating prologue>"
+        return {"sum": "k_sum_gram + k_deflate_images", "fft_rows": rows, "fft_cols": "k_col_energy",
                 "cov_reduce": "k_gram_reduce_finish", "eig": "k_eig_real", "project": "k_sum_partial_images"}[cls]
     return {"sum": "k_frame_sum" if mode == 1 else "k_sum_gram", "fft_rows": "k_fresnel" if fused_fft else "k_fft<rows>",
             "fft_cols": "k_fft<cols>", "cov_partial": ("k_cov_tf32" if T > 32 else "k_cov_partial_real") if cov_real else "k_cov_partial",
@@ -361,7 +362,7 @@ def run_ours(args, cfg):
         if cnt == 0:
             continue
         us = ms_k / cnt * 1e3
-        stages[name] = {"kernel": kernel_name(name, fused_fft, cov_real, mode, T), "us_per_launch": round(us, 2),
+        stages[name] = {"kernel": kernel_name(name, fused_fft, cov_real, mode, T, n), "us_per_launch": round(us, 2),
                         "launches_per_step": cnt / prof_steps, "share": round(ms_k / tot_ms, 4),
                         "GBps": round(per_launch_bytes[name] / (us * 1e-6) / 1e9, 1)}
     cov_flops = (2 if cov_real else 4) * T * (T + 1) * npix
