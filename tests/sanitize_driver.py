@@ -1,7 +1,8 @@
 #!/usr/bin/env python
 """Workload for compute-sanitizer (SURVEY.md sections 4-5): BASELINE.json configs[0] (256 x 256 x 16) through every
-chained entry point of the C ABI -- holo_process, holo_submit x 3 + holo_flush, holo_push x 4 + holo_flush -- and the
-per-stage calls.  Run ONE tool per process (and per gpurun call, B200_PROFILING.md):
+chained entry point of the C ABI -- holo_process, holo_submit x 3 + holo_flush, holo_push x 4 + holo_flush, the same in
+modes 2 and 3 (tensor-core integer Gram, deflating row pass, column energy, eigen-basis form), the host entry -- and the
+per-stage calls (incl. the tensor-core Gram and projection, SVD filter, normalisation, fftshift).  Run ONE tool per process (and per gpurun call, B200_PROFILING.md):
 
     compute-sanitizer --tool memcheck  python tests/sanitize_driver.py
     compute-sanitizer --tool racecheck python tests/sanitize_driver.py
@@ -72,10 +73,43 @@ def main():
         h.covariance(H, C, st)
         h.eig(C, ev, V, st)
         h.project(H, V, M, st)
-        h.fourier_demod(H, 4, 12, M, st)
+        h.fourier_demod(H, 4, 12, M, st)                 # 9 kept components: tensor-core projection
+        h.raw_covariance(dev, C, st)
+        h.svd_filter(H, V, H, st)
+        h.normalize(M, st)
+        M2 = img()
+        h.fftshift(M, M2, st)
     st.synchronize()
     rc, status = h.status(st)
     assert rc == 0, status
+
+    # modes 2 and 3 (and the tensor-core covariance of mode 1), serial, streamed and through host buffers
+    host = [torch.from_numpy(stream[:T].view(np.int16).copy()).pin_memory() for _ in range(3)]
+    for mode, tf32, window in ((1, 3, None), (2, 0, None), (3, 0, None), (3, 0, (6, 12))):
+        h.set_mode(mode)
+        h.tune(13, tf32)
+        if window:
+            h.set_range(*window)                         # 9 rejected components: eigen-basis form
+        r = img()
+        h.process(dev, r, st)
+        outs = [img() for _ in range(3)]
+        for o in outs:
+            h.submit(dev, o, st)
+        h.flush(st)
+        hout = [torch.zeros((n, n), dtype=torch.float32).pin_memory() for _ in range(3)]
+        for f, o in zip(host, hout):
+            h.submit_host(f, o, st)
+        h.flush_host(st)
+        st.synchronize()
+        assert bool(torch.isfinite(r).all()) and float(r.sum()) > 0
+        if not window:
+            assert float((r - ref).norm() / ref.norm()) <= 2e-5
+        for o in outs + [x.cuda() for x in hout]:
+            assert float((o - r).norm() / r.norm()) <= 2e-5
+        rc, status = h.status(st)
+        assert rc == 0, status
+        h.set_range(cfg.k_lo, cfg.k_hi)
+    h.set_mode(1)
     h.close()
     torch.cuda.synchronize()
     print("sanitize_driver ok:", cfg.name, "sweeps", status[1])
