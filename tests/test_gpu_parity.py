@@ -284,8 +284,7 @@ def test_process_mode3_eigen_basis_windows(torch_cuda, n, T, k_lo, k_hi):
     assert rc == 0, st
     out = oracle.process(fr, LAM, PITCH, Z, k_lo, k_hi)
     err = rel_l2(M.cpu().numpy(), out["M"])
-    gmin = min([gaps[k_lo - 2]] if k_lo > 1 else [1.0]) if True else 1.0
-    gmin = min(gmin, gaps[k_hi - 1] if k_hi < T else 1.0)
+    gmin = min(gaps[k_lo - 2] if k_lo > 1 else 1.0, gaps[k_hi - 1] if k_hi < T else 1.0)
     # FP32 eigenvectors mix across a boundary by ~eps / gap: the bound follows the gap (R10)
     assert err <= TOL_M and err <= max(FP32_M, 2e-6 / max(gmin, 1e-3)), (err, gmin, k_lo, k_hi)
     # streaming form and a change of window in the middle of a sequence
@@ -1008,4 +1007,98 @@ def test_process_graph_capture_replay(torch_cuda):
     torch.cuda.synchronize()
     assert torch.equal(M0, M1)
     del g
+    h.close()
+
+
+# ------------------------------------------------------------------ random mixes of entry points, modes and windows
+@pytest.mark.parametrize("seed", [0, 1, 2])
+def test_random_call_sequences(torch_cuda, seed):
+    """State machine soak: random sequences of holo_set_mode / holo_set_range / holo_process / holo_submit ... holo_flush /
+    holo_submit_host ... holo_flush_host / holo_push on ONE handle; every image that comes out is compared with the oracle's
+    image of its stack (or window) and component range."""
+    torch = torch_cuda
+    rs = np.random.default_rng(100 + seed)
+    cfg = G.small_config(n=64, T=16)
+    n, T = cfg.n, cfg.T
+    scene = G.make_scene(G.Config(cfg.name, n, T, T + 5 * 8, 8, cfg.n_stripes, cfg.sigma_psi, cfg.self_beating, cfg.k_lo, cfg.k_hi), 7 + seed)
+    stream = G.frames_np(scene, 0, T + 5 * 8)
+    stacks = [np.ascontiguousarray(stream[8 * i: 8 * i + T]) for i in range(4)]          # overlapping windows of the stream
+    dev_stream = _to_dev(torch, stream)
+    devs = [dev_stream[8 * i: 8 * i + T] for i in range(4)]
+    hosts = [torch.from_numpy(sf.view(np.int16).copy()).pin_memory() for sf in stacks]
+    windows = []
+    for (a, b) in ((2, 16), (1, 16), (3, 15), (2, 12), (7, 16), (5, 9)):
+        ok = True
+        for sf in stacks:
+            ev, gaps = eig_gaps(sf)
+            if (a > 1 and gaps[a - 2] < 0.03) or (b < T and gaps[b - 1] < 0.03):
+                ok = False
+        if ok:
+            windows.append((a, b))
+    assert len(windows) >= 2
+    ref = {}
+
+    def oracle_M(i, w):
+        if (i, w) not in ref:
+            ref[(i, w)] = oracle.process(stacks[i], cfg.lam, cfg.pitch, cfg.z, w[0], w[1])["M"]
+        return ref[(i, w)]
+
+    def check(img, i, w):
+        err = rel_l2(img.cpu().numpy(), oracle_M(i, w))
+        assert err <= TOL_M, (err, i, w)
+
+    h = _holo(n, n, T, 2, 16)
+    st = torch.cuda.Stream()
+    mode, win = 1, (2, 16)
+    deflatable = lambda w: 2 * (T - (w[1] - w[0] + 1)) <= (w[1] - w[0] + 1)
+    for step in range(40):
+        op = rs.integers(0, 6)
+        if op == 0:
+            mode = int(rs.integers(1, 4))
+            h.flush(st)
+            h.set_mode(mode)
+        elif op == 1:
+            win = windows[int(rs.integers(0, len(windows)))]
+            h.set_range(*win)
+        elif op == 2:
+            i = int(rs.integers(0, 4))
+            M = torch.zeros((n, n), dtype=torch.float32, device="cuda")
+            h.process(devs[i], M, st)
+            st.synchronize()
+            check(M, i, win)
+        elif op == 3:
+            ids = [int(x) for x in rs.integers(0, 4, int(rs.integers(1, 5)))]
+            outs = [torch.zeros((n, n), dtype=torch.float32, device="cuda") for _ in ids]
+            wins = []
+            for i, o in zip(ids, outs):
+                if rs.random() < 0.3:
+                    win = windows[int(rs.integers(0, len(windows)))]
+                    h.set_range(*win)                     # an image still owed keeps the window of its own submit
+                wins.append(win)
+                h.submit(devs[i], o, st)
+            h.flush(st)
+            st.synchronize()
+            for i, o, w in zip(ids, outs, wins):
+                check(o, i, w)
+        elif op == 4:
+            ids = [int(x) for x in rs.integers(0, 4, int(rs.integers(1, 5)))]
+            outs = [torch.zeros((n, n), dtype=torch.float32).pin_memory() for _ in ids]
+            for i, o in zip(ids, outs):
+                h.submit_host(hosts[i], o, st)
+            h.flush_host(st)
+            for i, o in zip(ids, outs):
+                check(o, i, win)
+        elif op == 5 and deflatable(win):
+            # sliding window: first window, then up to three pushes of 8 new frames (always as in mode 1)
+            k = int(rs.integers(1, 4))
+            outs = [torch.zeros((n, n), dtype=torch.float32, device="cuda") for _ in range(k + 1)]
+            h.push(dev_stream.data_ptr(), T, outs[0], st)
+            for q in range(k):
+                h.push(dev_stream.data_ptr() + (T + 8 * q) * n * n * 2, 8, outs[q + 1], st)
+            h.flush(st)
+            st.synchronize()
+            for q in range(k + 1):
+                check(outs[q], q, win)
+        rc, status = h.status(st)
+        assert rc == 0, status
     h.close()
