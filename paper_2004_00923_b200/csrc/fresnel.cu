@@ -699,7 +699,9 @@ int holo_launch_fresnel(holo_ctx* c, const uint16_t* frames, float2* H, cudaStre
         if (p.L < 1) p.L = 1;
         p.RT = c->ny / Bq; p.CT = c->nx / Bq;
         HoloProf prof(c, HOLO_K_FFT_ROWS, st);
-        return launch_fresnel_fused(c->nx, p, c->num_sms, c->device, st);
+        // fresnel_sm_reserve: SMs left to a side-stream kernel that must run UNDER this persistent launch (mode 2: the
+        // eigensolver of the same stack; a persistent kernel that fills every SM would make it wait for the end)
+        return launch_fresnel_fused(c->nx, p, c->num_sms - c->fresnel_sm_reserve, c->device, st);
     }
     // A1 + A2, frame groups so that the row->column intermediate stays in L2
     const int G = c->scratch_frames;

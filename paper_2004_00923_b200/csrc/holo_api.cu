@@ -438,13 +438,18 @@ extern "C" int holo_submit(holo_ctx* c, const uint16_t* frames_dev, float* image
         // frames), so the projection follows in stream order and the image is complete when this call's work is done
         if ((rc = submit_init(c, /*second_stack=*/false))) return rc;
         c->push_ready = 0;
-        if ((rc = holo_launch_sum_gram(c, frames_dev, c->C, st, /*finish=*/false))) return rc;
+        // the Gram finish (260 small CTAs) stays on the main stream; only the single-CTA eigensolver goes to the side stream,
+        // and the persistent Fresnel launch leaves one SM to it (otherwise it fills every SM and the eigensolver waits for
+        // its end: measured 324 vs 281 us per stack)
+        if ((rc = holo_launch_sum_gram(c, frames_dev, c->C, st, /*finish=*/true))) return rc;
         HOLO_CUDA_OK(cudaEventRecord(c->ev_cov[0], st));
         HOLO_CUDA_OK(cudaStreamWaitEvent(c->side, c->ev_cov[0], 0));
-        if ((rc = holo_launch_gram_finish(c, c->C, c->side))) return rc;
         if ((rc = holo_launch_eig(c, c->C, c->evals, c->V, c->side, true))) return rc;
         HOLO_CUDA_OK(cudaEventRecord(c->ev_eig[0], c->side));
-        if ((rc = holo_launch_fresnel(c, frames_dev, c->H, st, /*with_sum=*/false, -1, /*counters_zeroed=*/true))) return rc;
+        c->fresnel_sm_reserve = 1;
+        rc = holo_launch_fresnel(c, frames_dev, c->H, st, /*with_sum=*/false, -1, /*counters_zeroed=*/true);
+        c->fresnel_sm_reserve = 0;
+        if (rc) return rc;
         HOLO_CUDA_OK(cudaStreamWaitEvent(st, c->ev_eig[0], 0));
         c->nsubmit++;
         return holo_launch_project(c, c->H, c->V, c->k_lo, c->k_hi, c->tune[HOLO_TUNE_PROJ_COMPLEMENT], image_dev, st);

@@ -7,7 +7,7 @@
 #include "../../include/holo.h"
 
 #define HOLO_MAX_T 64
-#define HOLO_NUM_TUNE 16
+#define HOLO_NUM_TUNE 20
 #define HOLO_NORM_PARTS 1024
 
 // tuning keys (holo_tune); not part of the stable ABI
@@ -78,6 +78,7 @@ struct holo_ctx {
     uint32_t* sum1;         // mode 3, streaming form: frame sum of the second slot
     const uint16_t* pend3_frames; float* pend3_image; int pend3_slot;   // mode 3, streaming form: the stack whose image is owed
     unsigned long long* gram_X;   // [128][128] int64 byte-plane Gram of the raw frames (mode 2, rawgram.cu)
+    int fresnel_sm_reserve;       // SMs the fused Fresnel launch leaves free (set around the launch by mode 2's holo_submit)
     int gram_nparts;              // CTAs of the last k_sum_gram launch
     unsigned long long* gram_Xp;  // [N (N + 1) / 2][3 num_sms] per-CTA partials of it (N = 64 or 128)
     int mode;               // 1: covariance from the hologram stack (Eq. 4 as written); 2: from the raw frames
