@@ -461,7 +461,7 @@ def run_ours(args, cfg):
     torch.cuda.empty_cache()
     if side is not None:
         # (config, api, steps, resident stacks): streams of >= 3x L2, kept short so that the default run ends in minutes
-        for cn, sapi, ssteps, sstacks, smode in ((3, "submit", 512, 0, 3), (2, "submit", 256, 24, 1), (2, "submit", 256, 24, 3), (4, "push", 256, 16, 1),
+        for cn, sapi, ssteps, sstacks, smode in ((3, "submit", 512, 0, 2), (3, "submit", 512, 0, 3), (2, "submit", 256, 24, 1), (2, "submit", 256, 24, 3), (4, "push", 256, 16, 1),
                                                  (5, "submit", 24, 3, 1), (5, "submit", 24, 3, 3)):
             c2 = G.CONFIGS[cn]
             p2 = shard_plan(c2, rank, world, stacks=sstacks or None)
@@ -478,7 +478,7 @@ def run_ours(args, cfg):
                 dt2, err2 = R2.oracle_check(sapi)
                 ent["oracle_rel_l2_M_first_stack"] = err2
                 ent["oracle_s_per_stack"] = round(dt2, 2)
-            side[c2.name + ("_mode3" if smode == 3 else "")] = ent
+            side[c2.name + (f"_mode{smode}" if smode != 1 else "")] = ent
             R2.close()
             del R2
             torch.cuda.empty_cache()
