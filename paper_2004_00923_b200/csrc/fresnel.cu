@@ -797,7 +797,8 @@ int holo_launch_energy_image(holo_ctx* c, const uint16_t* frames, const float2* 
     a.T = T;
     a.defl_img = c->defl_img; a.defl_coef = c->defl_coef; a.ndefl = ndefl;
     a.eimg = c->eig_img;
-    a.ticket = c->counters + 1001;                        // zeroed by k_sum_gram, which always precedes this call in stream order
+    a.ticket = c->counters + 1001;
+    HOLO_CUDA_OK(cudaMemsetAsync(c->counters + 1001, 0, sizeof(unsigned int), st));     // row ticket (k_sum_gram may run on another stream)
     if (eigen) { HoloProf prof(c, HOLO_K_FFT_ROWS, st); rc = launch_fft<false, true, 2>(c->nx, a, c->num_sms, c->device, st); }
     else if (c->tune[HOLO_TUNE_ROWS2] && holo_rows2_supported(c)) rc = holo_launch_rows2(c, frames, c->H, ndefl, st);
     else
