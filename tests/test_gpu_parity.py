@@ -873,9 +873,19 @@ def test_process_cfg5_full_size(torch_cuda):
     rc, st = h.status()
     assert rc == 0, st
     res, out = _compare_full(torch, cfg, fr, h, M.cpu().numpy())
+    # the same stack through modes 2 and 3 (integer Gram at T = 64, packed 2048-point row pass, three-pass column energy)
+    errs = {}
+    for mode in (2, 3):
+        h.set_mode(mode)
+        Mm = torch.empty_like(M)
+        h.process(stream, Mm)
+        rc, st = h.status()
+        assert rc == 0, st
+        errs[mode] = rel_l2(Mm.cpu().numpy(), out["M"])
     h.close()
     assert res["M"] <= TOL_M and res["ev"] <= TOL_EV and res["C"] <= TOL_STAGE and res["H"] <= TOL_STAGE, res
     assert res["M"] <= FP32_M and res["ev"] <= FP32_EV and res["C"] <= FP32_C and res["H"] <= FP32_H, res
+    assert errs[2] <= FP32_M and errs[3] <= FP32_M, errs
 
 
 def test_process_cfg2_full_size(torch_cuda):
