@@ -743,6 +743,7 @@ int holo_launch_fresnel(holo_ctx* c, const uint16_t* frames, float2* H, cudaStre
 //   3. k_col_energy: column transform reduced to sum_t |.|^2, frame splits -> k_sum_partial_images
 // ------------------------------------------------------------------------------------------------
 int holo_mode3_splits(const holo_ctx* c, int nframes) {
+    if (c->tune[HOLO_TUNE_COLS2048] && holo_cols2048_supported(c)) return nframes >= 4 ? 4 : 1;   // packed kernel: (tile, quarter of the frames) units
     const int ct = c->nx / fft_batch(c->ny);
     int ns = (2 * c->num_sms) / (ct > 0 ? ct : 1);
     if (ns < 1) ns = 1;
@@ -814,8 +815,12 @@ int holo_launch_energy_image(holo_ctx* c, const uint16_t* frames, const float2* 
     b.ntiles = b.tiles_per_frame;
     b.T = T;
     const int ns = holo_mode3_splits(c, nframes);
-    { HoloProf prof(c, HOLO_K_FFT_COLS, st);
-      rc = launch_col_energy(c->ny, b, ns > 1 ? c->energy_parts : image, c->npix, nframes, ns, c->device, st); }
+    if (c->tune[HOLO_TUNE_COLS2048] && holo_cols2048_supported(c)) {
+        rc = holo_launch_cols2048(c, c->H, ns > 1 ? c->energy_parts : image, nframes, ns, st);
+    } else {
+        HoloProf prof(c, HOLO_K_FFT_COLS, st);
+        rc = launch_col_energy(c->ny, b, ns > 1 ? c->energy_parts : image, c->npix, nframes, ns, c->device, st);
+    }
     if (rc) return rc;
     if (ns > 1) {
         HoloProf prof(c, HOLO_K_PROJECT, st);

@@ -294,6 +294,85 @@ __global__ void __launch_bounds__(R2_WARPS * 32, 1) k_rows2(const R2Args a) {
     }
 }
 
+// ------------------------------------------------------------------------------------------------
+// Mode 3 column pass for 2048-point columns, packed form: a CTA owns a tile of 8 columns (64-byte row segments); thread
+// (j, c) holds elements n = j + 32 r and n + 1024 of column c, takes the radix-2 decimation-in-frequency step in registers
+// (as k_rows2<2048>) and transforms the pair (y0, y1) with packed butterflies; the exchange goes through a padded CTA-wide
+// buffer of 16-byte entries.  Outputs X(2k), X(2k+1) are two pixels: two accumulators per register slot.  Work units =
+// (column tile, quarter of the frames), one CTA per SM; the quarters' partial images are added by k_sum_partial_images.
+// Replaces the scalar three-pass kernel (4-column tiles, 32-byte segments, two exchanges) at N = 2048.
+// ------------------------------------------------------------------------------------------------
+struct C2Args {
+    const float2* G;          // row-pass output [T][2048][nx]
+    const float2* tw;         // [32][32] inter-pass twiddles of the 1024-point transform
+    const float2* tw2048;     // exp(-2 pi i n / 2048), n < 1024
+    float* out;               // [nsplit][2048][nx] partial images
+    int nx, T, nsplit;
+};
+constexpr int C2_B = 8;
+constexpr int C2_SMEM = (F2N + F2N / 32) * C2_B * 16 + F2N * 8;
+
+__global__ void __launch_bounds__(256, 1) k_cols2048(const C2Args a) {
+    extern __shared__ __align__(16) unsigned char smc_[];
+    float4* ex = reinterpret_cast<float4*>(smc_);
+    float2* tw_s = reinterpret_cast<float2*>(smc_ + (F2N + F2N / 32) * C2_B * 16);
+    const int tid = threadIdx.x, j = tid / C2_B, c = tid % C2_B;
+    for (int i = tid; i < F2N; i += 256) tw_s[i] = a.tw[i];
+    auto sidx = [&](int i) -> int { return (i + i / 32) * C2_B + c; };
+    const long long npix = 2048ll * a.nx;
+    const int ntiles = a.nx / C2_B;
+    const int per = (a.T + a.nsplit - 1) / a.nsplit;
+    for (int unit = blockIdx.x; unit < ntiles * a.nsplit; unit += gridDim.x) {
+        const int split = unit / ntiles, tile = unit - split * ntiles;       // split-major: concurrent CTAs walk adjacent tiles of the same frames
+        const int t0 = split * per, t1 = t0 + per < a.T ? t0 + per : a.T;
+        const float2* src0 = a.G + (long long)j * a.nx + (long long)tile * C2_B + c;
+        float2 acc[32];
+#pragma unroll
+        for (int r = 0; r < 32; ++r) acc[r] = make_float2(0.f, 0.f);
+        for (int t = t0; t < t1; ++t) {
+            const float2* sa = src0 + (long long)t * npix;
+            cpk v[32];
+#pragma unroll
+            for (int r = 0; r < 32; ++r) {
+                const float2 xa = __ldcs(sa + (long long)(32 * r) * a.nx);
+                const float2 xb = __ldcs(sa + (long long)(32 * r + 1024) * a.nx);
+                v[r].re = make_float2(xa.x, xb.x); v[r].im = make_float2(xa.y, xb.y);       // (x(n), x(n + 1024)) for now
+            }
+#pragma unroll
+            for (int r = 0; r < 32; ++r) {                     // y0 = x(n) + x(n + 1024), y1 = (x(n) - x(n + 1024)) W^n
+                const float2 w = __ldg(a.tw2048 + j + 32 * r);
+                const float sr = v[r].re.x + v[r].re.y, si = v[r].im.x + v[r].im.y;
+                const float dr = v[r].re.x - v[r].re.y, di = v[r].im.x - v[r].im.y;
+                v[r].re = make_float2(sr, fmaf(dr, w.x, -di * w.y));
+                v[r].im = make_float2(si, fmaf(dr, w.y, di * w.x));
+            }
+            P2S<0, 5>::run(v);
+            __syncthreads();                                   // the previous frame's exchange reads are over
+#pragma unroll
+            for (int r = 0; r < 32; ++r) { const cpk e = v[brev<32>(r)]; ex[sidx(j * 32 + r)] = make_float4(e.re.x, e.re.y, e.im.x, e.im.y); }
+            __syncthreads();
+#pragma unroll
+            for (int r = 0; r < 32; ++r) { const float4 e = ex[sidx(j + 32 * r)]; v[r].re = make_float2(e.x, e.y); v[r].im = make_float2(e.z, e.w); }
+#pragma unroll
+            for (int r = 1; r < 32; ++r) {
+                const float2 w = tw_s[r * 32 + j];
+                const float2 re = pfma(w.x, v[r].re, pneg(__fmul2_rn(make_float2(w.y, w.y), v[r].im)));
+                const float2 im = pfma(w.x, v[r].im, __fmul2_rn(make_float2(w.y, w.y), v[r].re));
+                v[r].re = re; v[r].im = im;
+            }
+            P2S<0, 5>::run(v);
+#pragma unroll
+            for (int r = 0; r < 32; ++r) {                     // k = j + 32 r: rows 2 k (first of the pair) and 2 k + 1
+                const cpk x = v[brev<32>(r)];
+                acc[r] = __ffma2_rn(x.re, x.re, __ffma2_rn(x.im, x.im, acc[r]));
+            }
+        }
+        float* op = a.out + (long long)split * npix + (long long)(2 * j) * a.nx + (long long)tile * C2_B + c;
+#pragma unroll
+        for (int r = 0; r < 32; ++r) { op[(long long)(64 * r) * a.nx] = acc[r].x; op[(long long)(64 * r + 1) * a.nx] = acc[r].y; }
+    }
+}
+
 }  // namespace
 
 
@@ -315,6 +394,21 @@ int holo_launch_rows2(holo_ctx* c, const uint16_t* frames, float2* out, int ndef
         if ((rc = holo_ensure_smem_attr((const void*)k_rows2<2048>, c->device, r2_smem<2048>()))) return rc;
         k_rows2<2048><<<c->num_sms, R2_WARPS * 32, r2_smem<2048>(), st>>>(a);
     }
+    HOLO_CUDA_OK(cudaGetLastError());
+    return HOLO_OK;
+}
+
+// mode 3 column-energy pass in the packed form: columns of 2048 points.  `out` = image (nsplit = 1) or the partial images
+bool holo_cols2048_supported(const holo_ctx* c) { return c->ny == 2048 && c->nx % C2_B == 0; }
+
+int holo_launch_cols2048(holo_ctx* c, const float2* G, float* out, int nframes, int nsplit, cudaStream_t st) {
+    C2Args a{};
+    a.G = G; a.tw = c->py.tw1; a.tw2048 = c->py.tw2 + 1024; a.out = out; a.nx = c->nx; a.T = nframes; a.nsplit = nsplit;
+    int rc;
+    if ((rc = holo_ensure_smem_attr((const void*)k_cols2048, c->device, C2_SMEM))) return rc;
+    const int units = (c->nx / C2_B) * nsplit;
+    HoloProf prof(c, HOLO_K_FFT_COLS, st);
+    k_cols2048<<<units < c->num_sms ? units : c->num_sms, 256, C2_SMEM, st>>>(a);
     HOLO_CUDA_OK(cudaGetLastError());
     return HOLO_OK;
 }

@@ -149,6 +149,7 @@ static int create_impl(holo_ctx* c) {
     c->tune[HOLO_TUNE_COV_TF32] = (T > 32 && np % 256 == 0) ? (np >= (1ll << 20) ? 1 : 3) : 0;
     c->tune[HOLO_TUNE_COV_TF32_DRAIN] = 4;
     c->tune[HOLO_TUNE_PROJ_TC] = 1;
+    c->tune[HOLO_TUNE_COLS2048] = 1;
     c->tune[HOLO_TUNE_ROWS2] = 1;                // packed two-frame row pass of mode 3 (1024^2, even T): 79 vs 84 us
     c->scratch_frames = (int)grp;
     c->cov_parts_cap = 4 * c->num_sms;
