@@ -248,8 +248,10 @@ int holo_launches_per_process(holo_ctx* ctx);
  *   13 real covariance of holo_process / holo_submit on the tensor cores (tcgen05.mma kind::tf32 on values
  *   rounded to nearest, FP64 partials): 0 = FP32 FFMA kernel (default at T <= 32), 1 = TF32 (default at T > 32), 3 = 3 x TF32,
  *   14 operand stages accumulated in TMEM between two FP64 drains of key 13 (default 4 = 512 products),
- *   15 mode 3: packed two-frame row pass (FFMA2 / FADD2 on the same row of two consecutive frames) where supported
- *   (1024 x 1024, even T; default 1). */
+ *   15 mode 3: packed row pass (FFMA2 / FADD2 on pairs: the same row of two consecutive frames at nx = 1024 with even T,
+ *   the even / odd halves of one row at nx = 2048; default 1), 16 packed 2048-point column passes (mode 3 column energy;
+ *   at 2048 x 2048 also the Fresnel stage of modes 1 / 2 as packed row pass + packed column pass instead of the fused
+ *   kernel; default 1). */
 int holo_tune(holo_ctx* ctx, int key, int value);
 
 /* Measurement hooks used by bench.py (not needed for normal use).

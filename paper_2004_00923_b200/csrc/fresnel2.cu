@@ -174,8 +174,9 @@ struct R2Args {
     const float* defl_img;    // [ndefl][ny][nx]  eT_k
     const float* defl_coef;   // [T][ndefl]
     float2* out;              // [T][ny][nx] row-pass output
-    unsigned int* ticket;     // zeroed by an earlier kernel of the stream
+    unsigned int* ticket;     // zeroed by an earlier operation of the stream
     int T, ndefl, ny;
+    int nframes;              // frames to transform (T, or fewer: sliding window); T itself enters d = T I - S
 };
 
 constexpr int R2_WARPS = 12;
@@ -203,7 +204,7 @@ __global__ void __launch_bounds__(R2_WARPS * 32, 1) k_rows2(const R2Args a) {
     const uint32_t buf = bufs + (uint32_t)(warp >> 2) * F2_TILE;
     const XAddr xa = make_xaddr(buf, warp & 3, lane);
     const long long npix = (long long)NX * a.ny;
-    const unsigned int ntasks = NX == 1024 ? (unsigned int)(a.T / 2) * (unsigned int)a.ny : (unsigned int)a.T * (unsigned int)a.ny;
+    const unsigned int ntasks = NX == 1024 ? (unsigned int)(a.nframes / 2) * (unsigned int)a.ny : (unsigned int)a.nframes * (unsigned int)a.ny;
     const float Tf = (float)a.T;
     // tickets are drawn two tasks ahead (the atomic's round trip is hidden) and the frame rows of the NEXT task are pulled
     // into L2 while the current one computes (ncu: 14 % of the warp time waited for the ticket, 30 % for the loads)
@@ -306,12 +307,14 @@ struct C2Args {
     const float2* G;          // row-pass output [T][2048][nx]
     const float2* tw;         // [32][32] inter-pass twiddles of the 1024-point transform
     const float2* tw2048;     // exp(-2 pi i n / 2048), n < 1024
-    float* out;               // [nsplit][2048][nx] partial images
+    float* out;               // ENERGY: [nsplit][2048][nx] partial images
+    float2* H;                // !ENERGY: the hologram stack [T][2048][nx]
     int nx, T, nsplit;
 };
 constexpr int C2_B = 8;
 constexpr int C2_SMEM = (F2N + F2N / 32) * C2_B * 16 + F2N * 8;
 
+template <bool ENERGY>
 __global__ void __launch_bounds__(256, 1) k_cols2048(const C2Args a) {
     extern __shared__ __align__(16) unsigned char smc_[];
     float4* ex = reinterpret_cast<float4*>(smc_);
@@ -326,9 +329,11 @@ __global__ void __launch_bounds__(256, 1) k_cols2048(const C2Args a) {
         const int split = unit / ntiles, tile = unit - split * ntiles;       // split-major: concurrent CTAs walk adjacent tiles of the same frames
         const int t0 = split * per, t1 = t0 + per < a.T ? t0 + per : a.T;
         const float2* src0 = a.G + (long long)j * a.nx + (long long)tile * C2_B + c;
-        float2 acc[32];
+        float2 acc[ENERGY ? 32 : 1];
+        if constexpr (ENERGY) {
 #pragma unroll
-        for (int r = 0; r < 32; ++r) acc[r] = make_float2(0.f, 0.f);
+            for (int r = 0; r < 32; ++r) acc[r] = make_float2(0.f, 0.f);
+        }
         for (int t = t0; t < t1; ++t) {
             const float2* sa = src0 + (long long)t * npix;
             cpk v[32];
@@ -361,15 +366,27 @@ __global__ void __launch_bounds__(256, 1) k_cols2048(const C2Args a) {
                 v[r].re = re; v[r].im = im;
             }
             P2S<0, 5>::run(v);
+            if constexpr (ENERGY) {
 #pragma unroll
-            for (int r = 0; r < 32; ++r) {                     // k = j + 32 r: rows 2 k (first of the pair) and 2 k + 1
-                const cpk x = v[brev<32>(r)];
-                acc[r] = __ffma2_rn(x.re, x.re, __ffma2_rn(x.im, x.im, acc[r]));
+                for (int r = 0; r < 32; ++r) {                 // k = j + 32 r: rows 2 k (first of the pair) and 2 k + 1
+                    const cpk x = v[brev<32>(r)];
+                    acc[r] = __ffma2_rn(x.re, x.re, __ffma2_rn(x.im, x.im, acc[r]));
+                }
+            } else {
+                float2* hp = a.H + (long long)t * npix + (long long)(2 * j) * a.nx + (long long)tile * C2_B + c;
+#pragma unroll
+                for (int r = 0; r < 32; ++r) {
+                    const cpk x = v[brev<32>(r)];
+                    __stcs(hp + (long long)(64 * r) * a.nx, make_float2(x.re.x, x.im.x));
+                    __stcs(hp + (long long)(64 * r + 1) * a.nx, make_float2(x.re.y, x.im.y));
+                }
             }
         }
-        float* op = a.out + (long long)split * npix + (long long)(2 * j) * a.nx + (long long)tile * C2_B + c;
+        if constexpr (ENERGY) {
+            float* op = a.out + (long long)split * npix + (long long)(2 * j) * a.nx + (long long)tile * C2_B + c;
 #pragma unroll
-        for (int r = 0; r < 32; ++r) { op[(long long)(64 * r) * a.nx] = acc[r].x; op[(long long)(64 * r + 1) * a.nx] = acc[r].y; }
+            for (int r = 0; r < 32; ++r) { op[(long long)(64 * r) * a.nx] = acc[r].x; op[(long long)(64 * r + 1) * a.nx] = acc[r].y; }
+        }
     }
 }
 
@@ -379,8 +396,9 @@ __global__ void __launch_bounds__(256, 1) k_cols2048(const C2Args a) {
 // mode 3 row pass in the packed form: rows of 1024 points (even T: frame pairs) or of 2048 points (even / odd halves)
 bool holo_rows2_supported(const holo_ctx* c) { return (c->nx == 1024 && (c->T % 2) == 0) || c->nx == 2048; }
 
-int holo_launch_rows2(holo_ctx* c, const uint16_t* frames, float2* out, int ndefl, cudaStream_t st) {
+int holo_launch_rows2(holo_ctx* c, const uint16_t* frames, float2* out, int ndefl, cudaStream_t st, int nframes) {
     R2Args a{};
+    a.nframes = nframes > 0 ? nframes : c->T;
     a.frames = frames; a.sum = c->sum; a.qxs = c->qxs; a.qy = c->qy; a.tw = c->px.tw1;
     a.tw2048 = c->nx == 2048 ? c->px.tw2 + 1024 : nullptr;       // row r = 1 of the pass-2 table [2][1024]: exp(-2 pi i b / 2048)
     a.defl_img = c->defl_img; a.defl_coef = c->defl_coef; a.out = out; a.ticket = c->counters + 1001;
@@ -389,10 +407,10 @@ int holo_launch_rows2(holo_ctx* c, const uint16_t* frames, float2* out, int ndef
     HoloProf prof(c, HOLO_K_FFT_ROWS, st);
     if (c->nx == 1024) {
         if ((rc = holo_ensure_smem_attr((const void*)k_rows2<1024>, c->device, r2_smem<1024>()))) return rc;
-        k_rows2<1024><<<c->num_sms, R2_WARPS * 32, r2_smem<1024>(), st>>>(a);
+        k_rows2<1024><<<c->num_sms - c->fresnel_sm_reserve, R2_WARPS * 32, r2_smem<1024>(), st>>>(a);
     } else {
         if ((rc = holo_ensure_smem_attr((const void*)k_rows2<2048>, c->device, r2_smem<2048>()))) return rc;
-        k_rows2<2048><<<c->num_sms, R2_WARPS * 32, r2_smem<2048>(), st>>>(a);
+        k_rows2<2048><<<c->num_sms - c->fresnel_sm_reserve, R2_WARPS * 32, r2_smem<2048>(), st>>>(a);
     }
     HOLO_CUDA_OK(cudaGetLastError());
     return HOLO_OK;
@@ -405,10 +423,24 @@ int holo_launch_cols2048(holo_ctx* c, const float2* G, float* out, int nframes, 
     C2Args a{};
     a.G = G; a.tw = c->py.tw1; a.tw2048 = c->py.tw2 + 1024; a.out = out; a.nx = c->nx; a.T = nframes; a.nsplit = nsplit;
     int rc;
-    if ((rc = holo_ensure_smem_attr((const void*)k_cols2048, c->device, C2_SMEM))) return rc;
+    if ((rc = holo_ensure_smem_attr((const void*)k_cols2048<true>, c->device, C2_SMEM))) return rc;
     const int units = (c->nx / C2_B) * nsplit;
     HoloProf prof(c, HOLO_K_FFT_COLS, st);
-    k_cols2048<<<units < c->num_sms ? units : c->num_sms, 256, C2_SMEM, st>>>(a);
+    k_cols2048<true><<<units < c->num_sms ? units : c->num_sms, 256, C2_SMEM, st>>>(a);
+    HOLO_CUDA_OK(cudaGetLastError());
+    return HOLO_OK;
+}
+
+// the same column pass with the hologram stack as output (unfused Fresnel stage at 2048 x 2048)
+int holo_launch_cols2048_store(holo_ctx* c, const float2* G, float2* H, int nframes, cudaStream_t st) {
+    C2Args a{};
+    a.G = G; a.tw = c->py.tw1; a.tw2048 = c->py.tw2 + 1024; a.H = H; a.nx = c->nx; a.T = nframes; a.nsplit = nframes >= 4 ? 4 : 1;
+    int rc;
+    if ((rc = holo_ensure_smem_attr((const void*)k_cols2048<false>, c->device, C2_SMEM))) return rc;
+    const int units = (c->nx / C2_B) * a.nsplit;
+    HoloProf prof(c, HOLO_K_FFT_COLS, st);
+    const int sms = c->num_sms - c->fresnel_sm_reserve;    // (mode 2: one SM for the side-stream eigensolver)
+    k_cols2048<false><<<units < sms ? units : sms, 256, C2_SMEM, st>>>(a);
     HOLO_CUDA_OK(cudaGetLastError());
     return HOLO_OK;
 }

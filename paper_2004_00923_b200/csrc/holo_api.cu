@@ -75,7 +75,7 @@ static void free_ctx(holo_ctx* c) {
     if (!c) return;
     cudaFree(c->qx); cudaFree(c->qy); cudaFree(c->qxs); cudaFree(c->Wdft); cudaFree(c->Fmat); cudaFree(c->norm_partials);
     holo_fft_plan_free(&c->px); holo_fft_plan_free(&c->py);
-    cudaFree(c->sum); cudaFree(c->scratch); cudaFree(c->H); cudaFree(c->cov_partials);
+    cudaFree(c->sum); cudaFree(c->scratch); cudaFree(c->H); cudaFree(c->rowout); cudaFree(c->cov_partials);
     cudaFree(c->C); cudaFree(c->evals); cudaFree(c->V); cudaFree(c->status);
     if (c->noconv_host) cudaFreeHost(c->noconv_host);
     cudaFree(c->counters); cudaFree(c->gram_X); cudaFree(c->gram_Xp);
@@ -157,6 +157,7 @@ static int create_impl(holo_ctx* c) {
     HOLO_CUDA_OK(cudaMalloc(&c->sum, np * sizeof(uint32_t)));
     HOLO_CUDA_OK(cudaMalloc(&c->scratch, (size_t)c->scratch_frames * np * sizeof(float2)));
     HOLO_CUDA_OK(cudaMalloc(&c->H, (size_t)T * np * sizeof(float2)));
+    if (c->nx == 2048 && c->ny == 2048) HOLO_CUDA_OK(cudaMalloc(&c->rowout, (size_t)T * np * sizeof(float2)));
     HOLO_CUDA_OK(cudaMalloc(&c->cov_partials, (size_t)c->cov_parts_cap * T8 * T8 * sizeof(float2)));
     HOLO_CUDA_OK(cudaMalloc(&c->C, (size_t)T * T * sizeof(float2)));
     HOLO_CUDA_OK(cudaMalloc(&c->evals, T * sizeof(float)));

@@ -63,6 +63,7 @@ struct holo_ctx {
     double* norm_partials;  // [HOLO_NORM_PARTS] partial sums of holo_normalize
     // workspace
     uint32_t* sum;          // [ny][nx]
+    float2* rowout;         // 2048 x 2048 frames: row-pass output of the whole stack [T][ny][nx] (unfused packed Fresnel stage)
     float2* scratch;        // FFT row->column intermediate, fft_group frames
     int scratch_frames;
     float2* H;              // [T][ny][nx]
@@ -180,6 +181,7 @@ int holo_launch_gram_finish(holo_ctx* c, float2* C, cudaStream_t st);
 bool holo_rows2_supported(const holo_ctx* c);
 bool holo_cols2048_supported(const holo_ctx* c);
 int holo_launch_cols2048(holo_ctx* c, const float2* G, float* out, int nframes, int nsplit, cudaStream_t st);
-int holo_launch_rows2(holo_ctx* c, const uint16_t* frames, float2* out, int ndefl, cudaStream_t st);
+int holo_launch_cols2048_store(holo_ctx* c, const float2* G, float2* H, int nframes, cudaStream_t st);
+int holo_launch_rows2(holo_ctx* c, const uint16_t* frames, float2* out, int ndefl, cudaStream_t st, int nframes = 0);
 int holo_fft_plan_init(FftPlan* p, int N);
 void holo_fft_plan_free(FftPlan* p);

@@ -914,14 +914,23 @@ def test_fresnel_fused_square_sizes(torch_cuda, n, T):
     rng = np.random.default_rng(n + T)
     fr = _rand_frames(rng, T, n, n, 0, 65536 if T == 3 else 4096)
     h = _holo(n, n, T, 1, T)
-    assert h.launches_per_process() == 6
+    # 2048 x 2048 takes the packed row pass + packed column pass by default (one more launch); tune 16 = 0: fused kernel
+    assert h.launches_per_process() == (7 if n == 2048 else 6)
     H = torch.empty((T, n, n), dtype=torch.complex64, device="cuda")
     h.fresnel(_to_dev(torch, fr), H)
     torch.cuda.synchronize()
     Ho = oracle.fresnel(fr, LAM, PITCH, Z)
     err = max(rel_l2(H[t].cpu().numpy(), Ho[t]) for t in range(T))
-    h.close()
     assert err <= FP32_H, err
+    if n == 2048:
+        h.tune(16, 0)
+        assert h.launches_per_process() == 6
+        H.zero_()
+        h.fresnel(_to_dev(torch, fr), H)
+        torch.cuda.synchronize()
+        err = max(rel_l2(H[t].cpu().numpy(), Ho[t]) for t in range(T))
+        assert err <= FP32_H, err
+    h.close()
 
 
 def test_push_cfg4_full_size(torch_cuda):
