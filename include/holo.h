@@ -251,7 +251,9 @@ int holo_launches_per_process(holo_ctx* ctx);
  *   15 mode 3: packed row pass (FFMA2 / FADD2 on pairs: the same row of two consecutive frames at nx = 1024 with even T,
  *   the even / odd halves of one row at nx = 2048; default 1), 16 packed 2048-point column passes (mode 3 column energy;
  *   at 2048 x 2048 also the Fresnel stage of modes 1 / 2 as packed row pass + packed column pass instead of the fused
- *   kernel; default 1). */
+ *   kernel; default 1), 17 mode 3 at 1024 x 1024: width w of the column blocks in which the packed row pass stores its
+ *   output, [frame][x / w][y][x % w] (8, 16, 32; 0 = row-major; default 8 = the column tile of the energy pass, which
+ *   then reads one contiguous 64 KB block per tile and frame). */
 int holo_tune(holo_ctx* ctx, int key, int value);
 
 /* Measurement hooks used by bench.py (not needed for normal use).

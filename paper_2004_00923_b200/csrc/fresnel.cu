@@ -74,7 +74,11 @@ struct NoHook { __device__ __forceinline__ void operator()() const {} };
 // index `frame` selects the V row); 2 = the input is a real float image (a.eimg: eigen-images of mode 3), d = eimg.
 // ENERGY: nothing is stored; |X|^2 of output slot s (the s-th value this thread would store, see tile_out_offset) is added
 // to acc[s] instead.
-template <int N, int E, int R1, int R2, int B, bool COL, bool PRO, int LDC = 0, class Mid = NoHook, int DEFL = 0, bool ENERGY = false>
+// TILED = w > 0 (column tiles without prologue): the input is stored in column blocks of w >= B columns,
+// [frame][x / w][row][x % w] (the packed row pass writes it so): the tiles of w / B neighbouring CTAs are ONE contiguous block
+// of N * w elements instead of N row segments one row pitch apart.
+template <int N, int E, int R1, int R2, int B, bool COL, bool PRO, int LDC = 0, class Mid = NoHook, int DEFL = 0, bool ENERGY = false,
+          int TILED = 0>
 __device__ __forceinline__ void fft_tile(const FftArgs& a, long long in_foff, long long out_foff, int tile_in_frame, float2* sm,
                                          Mid mid = Mid(), int frame = 0, float* acc = nullptr, int seq_override = -1) {
     constexpr int TPS = N / E;
@@ -158,9 +162,16 @@ __device__ __forceinline__ void fft_tile(const FftArgs& a, long long in_foff, lo
                 }
             }
         } else {
+            if constexpr (TILED != 0) {
+                const int x = tile_in_frame * B + c;
+                const float2* ip = a.in + in_foff + (long long)(x / TILED) * (N * TILED) + x % TILED;
+#pragma unroll
+                for (int r = 0; r < E; ++r) v[r] = __ldcg(ip + (j + r * TPS) * TILED);
+            } else {
             const float2* ip = a.in + ibase;
 #pragma unroll
             for (int r = 0; r < E; ++r) v[r] = FUSED ? ldcg_hint(ip + (j + r * TPS) * estride, pol_in) : __ldcg(ip + (j + r * TPS) * estride);   // L2-coherent: written earlier in this kernel
+            }
         }
         fft_reg<E>(v);
         float2* op = a.out + obase;
@@ -273,18 +284,18 @@ __device__ __forceinline__ int tile_out_offset(int slot) {
 // already removed in the raw domain by the row pass), so that sum over all t is the image of Eq. 7 (R12
 // identity: sum_{k in S}|P_k|^2 = sum_t |H_t - sum_{k not in S} P_k conj(V_tk)|^2 for unitary V).  The hologram stack is
 // never written.  grid = (column tiles, frame splits); split s writes out + s * npix (a plain store: deterministic).
-template <int N, int E, int R1, int R2, int B>
+template <int N, int E, int R1, int R2, int B, int TILED = 0>
 __global__ void __launch_bounds__((N / E) * B, 512 / ((N / E) * B) > 0 ? 512 / ((N / E) * B) : 1)
 k_col_energy(const FftArgs a, float* __restrict__ out, long long npix, int nframes, int nsplit) {
     extern __shared__ float2 sm[];
     const int tile = blockIdx.x, split = blockIdx.y;
-    const int per = (nframes + nsplit - 1) / nsplit;
-    const int t0 = split * per, t1 = t0 + per < nframes ? t0 + per : nframes;
     float acc[E];
 #pragma unroll
     for (int s = 0; s < E; ++s) acc[s] = 0.f;
-    for (int t = t0; t < t1; ++t)
-        fft_tile<N, E, R1, R2, B, true, false, 0, NoHook, 0, true>(a, (long long)t * a.in_fstride, 0, tile, sm, NoHook(), 0, acc);
+    // split s takes the frames nframes-1-s, nframes-1-s-nsplit, ...: all splits start with the frames the row pass wrote
+    // LAST, which are still in L2 (the row-pass output is larger than L2), and walk down together
+    for (int t = nframes - 1 - split; t >= 0; t -= nsplit)
+        fft_tile<N, E, R1, R2, B, true, false, 0, NoHook, 0, true, TILED>(a, (long long)t * a.in_fstride, 0, tile, sm, NoHook(), 0, acc);
     const int c = (int)threadIdx.x % B;
     float* op = out + (long long)split * npix + (long long)tile * B + c;
 #pragma unroll
@@ -591,17 +602,25 @@ static int launch_fft(int N, const FftArgs& a, int num_sms, int device, cudaStre
     return HOLO_ERR_ARG;
 }
 
-template <int N, int E, int R1, int R2, int B>
+template <int N, int E, int R1, int R2, int B, int TILED = 0>
 static int launch_col_energy_t(const FftArgs& a, float* out, long long npix, int nframes, int nsplit, int device, cudaStream_t st) {
     constexpr int threads = (N / E) * B;
     constexpr size_t smem = (R1 > 1) ? sizeof(float2) * (size_t)(N + N / E) * B : 0;
-    auto kern = k_col_energy<N, E, R1, R2, B>;
+    auto kern = k_col_energy<N, E, R1, R2, B, TILED>;
     { const int rc = holo_ensure_smem_attr((const void*)kern, device, smem); if (rc) return rc; }
     kern<<<dim3((unsigned)a.tiles_per_frame, (unsigned)nsplit), threads, smem, st>>>(a, out, npix, nframes, nsplit);
     HOLO_CUDA_OK(cudaGetLastError());
     return HOLO_OK;
 }
-static int launch_col_energy(int N, const FftArgs& a, float* out, long long npix, int nframes, int nsplit, int device, cudaStream_t st) {
+static int launch_col_energy(int N, const FftArgs& a, float* out, long long npix, int nframes, int nsplit, int device, cudaStream_t st,
+                             int tiled = 0) {
+    if (tiled) {
+        if (N == 1024 && tiled == 8) return launch_col_energy_t<1024, 32, 32, 1, 8, 8>(a, out, npix, nframes, nsplit, device, st);
+        if (N == 1024 && tiled == 16) return launch_col_energy_t<1024, 32, 32, 1, 8, 16>(a, out, npix, nframes, nsplit, device, st);
+        if (N == 1024 && tiled == 32) return launch_col_energy_t<1024, 32, 32, 1, 8, 32>(a, out, npix, nframes, nsplit, device, st);
+        holo_set_error("tiled column input: unsupported length %d", N);
+        return HOLO_ERR_ARG;
+    }
     switch (N) {
         case 16:   return launch_col_energy_t<16, 16, 1, 1, 16>(a, out, npix, nframes, nsplit, device, st);
         case 32:   return launch_col_energy_t<32, 32, 1, 1, 16>(a, out, npix, nframes, nsplit, device, st);
@@ -809,8 +828,12 @@ int holo_launch_energy_image(holo_ctx* c, const uint16_t* frames, const float2* 
     a.eimg = c->eig_img;
     a.ticket = c->counters + 1001;
     HOLO_CUDA_OK(cudaMemsetAsync(c->counters + 1001, 0, sizeof(unsigned int), st));     // row ticket (k_sum_gram may run on another stream)
+    // the packed row pass can write its output column tile by column tile (the layout is private to this function): the
+    // column pass then reads one contiguous 64 KB block per tile and frame instead of 1024 segments of 64 bytes
+    const bool rows2 = !eigen && c->tune[HOLO_TUNE_ROWS2] && holo_rows2_supported(c);
+    const int tiled = rows2 && c->nx == 1024 && c->ny == 1024 ? c->tune[HOLO_TUNE_TILED_G] : 0;
     if (eigen) { HoloProf prof(c, HOLO_K_FFT_ROWS, st); rc = launch_fft<false, true, 2>(c->nx, a, c->num_sms, c->device, st); }
-    else if (c->tune[HOLO_TUNE_ROWS2] && holo_rows2_supported(c)) rc = holo_launch_rows2(c, frames, c->H, ndefl, st);
+    else if (rows2) rc = holo_launch_rows2(c, frames, c->H, ndefl, st, 0, tiled);
     else
     { HoloProf prof(c, HOLO_K_FFT_ROWS, st);
       rc = ndefl ? launch_fft<false, true, 1>(c->nx, a, c->num_sms, c->device, st) : launch_fft<false, true, 0>(c->nx, a, c->num_sms, c->device, st); }
@@ -828,7 +851,7 @@ int holo_launch_energy_image(holo_ctx* c, const uint16_t* frames, const float2* 
         rc = holo_launch_cols2048(c, c->H, ns > 1 ? c->energy_parts : image, nframes, ns, st);
     } else {
         HoloProf prof(c, HOLO_K_FFT_COLS, st);
-        rc = launch_col_energy(c->ny, b, ns > 1 ? c->energy_parts : image, c->npix, nframes, ns, c->device, st);
+        rc = launch_col_energy(c->ny, b, ns > 1 ? c->energy_parts : image, c->npix, nframes, ns, c->device, st, tiled);
     }
     if (rc) return rc;
     if (ns > 1) {

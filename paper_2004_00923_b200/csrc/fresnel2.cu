@@ -177,6 +177,7 @@ struct R2Args {
     unsigned int* ticket;     // zeroed by an earlier operation of the stream
     int T, ndefl, ny;
     int nframes;              // frames to transform (T, or fewer: sliding window); T itself enters d = T I - S
+    int tile_w;               // NX = 1024: 0 = row-major output; w = output stored [frame][x / w][y][x % w] (w divides 32)
 };
 
 constexpr int R2_WARPS = 12;
@@ -279,16 +280,20 @@ __global__ void __launch_bounds__(R2_WARPS * 32, 1) k_rows2(const R2Args a) {
         P2Last<0>::run(v, o);
         if constexpr (NX == 1024) {
             // X[lane + 32 kk] of frame f in (o.x, o.y), of frame f + 1 in (o.z, o.w); kk = brev(register slot)
-            float2* out0 = a.out + (long long)f * npix + (long long)y * NX + lane;
+            // (plain stores: the column pass finds the last frames in L2).  Tiled output: x = lane + 32 kk lies in column tile
+            // x / w = lane / w + kk (32 / w), so the stride between a lane's stores is 32 ny elements for every w
+            const int w = a.tile_w;
+            float2* out0 = a.out + (long long)f * npix + (w ? (long long)(lane / w) * a.ny * w + (long long)y * w + lane % w : (long long)y * NX + lane);
+            const int es = w ? 32 * a.ny : 32;
 #pragma unroll
-            for (int p2 = 0; p2 < 32; ++p2) __stcs(out0 + 32 * brev<32>(p2), make_float2(o[p2].x, o[p2].y));
+            for (int p2 = 0; p2 < 32; ++p2) out0[brev<32>(p2) * es] = make_float2(o[p2].x, o[p2].y);
 #pragma unroll
-            for (int p2 = 0; p2 < 32; ++p2) __stcs(out0 + npix + 32 * brev<32>(p2), make_float2(o[p2].z, o[p2].w));
+            for (int p2 = 0; p2 < 32; ++p2) out0[npix + brev<32>(p2) * es] = make_float2(o[p2].z, o[p2].w);
         } else {
             // (X[2 k], X[2 k + 1]) with k = lane + 32 kk: adjacent outputs, one 16-byte store
             float4* out0 = reinterpret_cast<float4*>(a.out + (long long)f * npix + (long long)y * NX) + lane;
 #pragma unroll
-            for (int p2 = 0; p2 < 32; ++p2) __stcs(out0 + 32 * brev<32>(p2), o[p2]);
+            for (int p2 = 0; p2 < 32; ++p2) out0[32 * brev<32>(p2)] = o[p2];
         }
         tk0 = tk1;
         tk1 = __shfl_sync(0xffffffffu, tk2, 0);
@@ -396,8 +401,9 @@ __global__ void __launch_bounds__(256, 1) k_cols2048(const C2Args a) {
 // mode 3 row pass in the packed form: rows of 1024 points (even T: frame pairs) or of 2048 points (even / odd halves)
 bool holo_rows2_supported(const holo_ctx* c) { return (c->nx == 1024 && (c->T % 2) == 0) || c->nx == 2048; }
 
-int holo_launch_rows2(holo_ctx* c, const uint16_t* frames, float2* out, int ndefl, cudaStream_t st, int nframes) {
+int holo_launch_rows2(holo_ctx* c, const uint16_t* frames, float2* out, int ndefl, cudaStream_t st, int nframes, int tile_w) {
     R2Args a{};
+    a.tile_w = c->nx == 1024 ? tile_w : 0;
     a.nframes = nframes > 0 ? nframes : c->T;
     a.frames = frames; a.sum = c->sum; a.qxs = c->qxs; a.qy = c->qy; a.tw = c->px.tw1;
     a.tw2048 = c->nx == 2048 ? c->px.tw2 + 1024 : nullptr;       // row r = 1 of the pass-2 table [2][1024]: exp(-2 pi i b / 2048)

@@ -29,6 +29,7 @@ enum {
     HOLO_TUNE_COV_TF32_DRAIN = 14,
     HOLO_TUNE_PROJ_TC = 12,        // direct projection of more than 4 components on the tensor cores (T <= 32; default 1)
     HOLO_TUNE_ROWS2 = 15,          // mode 3: packed two-frame row pass where supported (1024^2, even T) // stages accumulated in TMEM before the accumulators are added to FP64 (default 4)
+    HOLO_TUNE_TILED_G = 17,        // mode 3, 1024 x 1024: the row pass writes its output column tile by column tile (default 1)
     HOLO_TUNE_COLS2048 = 16,       // mode 3: packed column-energy pass for 2048-point columns (default 1)
     HOLO_TUNE_FFT_LAG = 6,         // frames between the row pass and the column pass in the fused kernel (0 = auto)
 };
@@ -182,6 +183,6 @@ bool holo_rows2_supported(const holo_ctx* c);
 bool holo_cols2048_supported(const holo_ctx* c);
 int holo_launch_cols2048(holo_ctx* c, const float2* G, float* out, int nframes, int nsplit, cudaStream_t st);
 int holo_launch_cols2048_store(holo_ctx* c, const float2* G, float2* H, int nframes, cudaStream_t st);
-int holo_launch_rows2(holo_ctx* c, const uint16_t* frames, float2* out, int ndefl, cudaStream_t st, int nframes = 0);
+int holo_launch_rows2(holo_ctx* c, const uint16_t* frames, float2* out, int ndefl, cudaStream_t st, int nframes = 0, int tile_w = 0);
 int holo_fft_plan_init(FftPlan* p, int N);
 void holo_fft_plan_free(FftPlan* p);
