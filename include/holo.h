@@ -253,7 +253,9 @@ int holo_launches_per_process(holo_ctx* ctx);
  *   at 2048 x 2048 also the Fresnel stage of modes 1 / 2 as packed row pass + packed column pass instead of the fused
  *   kernel; default 1), 17 mode 3 at 1024 x 1024: width w of the column blocks in which the packed row pass stores its
  *   output, [frame][x / w][y][x % w] (8, 16, 32; 0 = row-major; default 8 = the column tile of the energy pass, which
- *   then reads one contiguous 64 KB block per tile and frame). */
+ *   then reads one contiguous 64 KB block per tile and frame), 18 programmatic dependent launches between the kernels of a
+ *   chain (each such kernel waits with griddepcontrol.wait before it touches data; PROCESS-WIDE; default 1, 0 = plain
+ *   launches; results are bit-identical either way). */
 int holo_tune(holo_ctx* ctx, int key, int value);
 
 /* Measurement hooks used by bench.py (not needed for normal use).

@@ -226,6 +226,8 @@ k_cov_partial_real(const __grid_constant__ CUtensorMap tmH, float2* __restrict__
         for (int s = 0; s < nstages; ++s) { mbar_init(full + s, 1); mbar_init(empty + s, (uint32_t)njobs); }   // nstages is a multiple of ngroups: a stage always serves the same group
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
+    pdl_trigger();                                        // (k_cov_reduce)
+    pdl_wait();                                           // the holograms are complete
     __syncthreads();
     int ps = 0; uint32_t pph = 0;
     long long pchunk = blockIdx.x;
@@ -325,6 +327,8 @@ k_cov_partial_real(const __grid_constant__ CUtensorMap tmH, float2* __restrict__
 __global__ void __launch_bounds__(256) k_cov_reduce(const float2* __restrict__ partials, int nparts, int T, int T8, float2* __restrict__ C,
                                                     double2* __restrict__ Cd) {
     const int w = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+    pdl_trigger();                                        // (the single-CTA eigensolver)
+    pdl_wait();
     if (w >= T * T) return;
     const int t = w / T, s = w - t * T;
     if (s > t) return;
@@ -498,7 +502,8 @@ static int launch_cov_real(holo_ctx* c, const float2* H, float2* C, cudaStream_t
     { const int rc = holo_make_tensor_map(&tmH, H, c->npix, c->ring_nrb ? 8 * c->ring_nrb : T, COV_P); if (rc) return rc; }
     {
         HoloProf prof(c, HOLO_K_COV_PARTIAL, st);
-        k_cov_partial_real<<<dim3(gx, gy), COV_NW * 32, smem, st>>>(tmH, c->cov_partials, c->npix, T8, nstages, nslots, ngroups, ahead, plan, c->ring_rb0, c->ring_nrb);
+        HOLO_CUDA_OK(holo_launch_pdl(k_cov_partial_real, dim3(gx, gy), dim3(COV_NW * 32), smem, st, tmH, c->cov_partials, c->npix, T8, nstages, nslots,
+                                     ngroups, ahead, plan, c->ring_rb0, c->ring_nrb));
     }
     HOLO_CUDA_OK(cudaGetLastError());
     c->cov_nparts = gx * ngroups;
@@ -518,7 +523,8 @@ static int launch_cov_real(holo_ctx* c, const float2* H, float2* C, cudaStream_t
 int holo_launch_cov_reduce(holo_ctx* c, int nparts, float2* C, cudaStream_t st) {
     const int T = c->T, T8 = (T + 7) / 8 * 8, n = T * T;
     HoloProf prof(c, HOLO_K_COV_REDUCE, st);
-    k_cov_reduce<<<(n * 32 + 255) / 256, 256, 0, st>>>(c->cov_partials, nparts, T, T8, C, c->center_gram ? c->Cd : nullptr);
+    HOLO_CUDA_OK(holo_launch_pdl(k_cov_reduce, dim3((n * 32 + 255) / 256), dim3(256), 0, st, (const float2*)c->cov_partials, nparts, T, T8, C,
+                                 c->center_gram ? c->Cd : (double2*)nullptr));
     HOLO_CUDA_OK(cudaGetLastError());
     if (c->center_gram) {                                  // holo_push: C <- J Gamma J
         k_center_gram<<<1, 256, 0, st>>>(c->Cd, T, C, c->ring_nrb ? c->Gs : nullptr, 8 * c->ring_nrb, 8 * c->ring_rb0, 1);

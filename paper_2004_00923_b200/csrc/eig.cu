@@ -64,6 +64,7 @@ __global__ void __launch_bounds__((TP / 2) * (TP / 2) < 32 ? 32 : (TP / 2) * (TP
 k_eig(const float2* __restrict__ C, int T, float* __restrict__ evals, float2* __restrict__ Vout,
       int32_t* __restrict__ status, int max_sweeps, int32_t* __restrict__ noconv) {
     extern __shared__ __align__(16) unsigned char raw[];
+    pdl_wait();
     constexpr int Tp = TP, LD = TP + 2, half = TP / 2, m = TP - 1;   // LD even: rows 16-byte aligned for LDS.128
     float2* A0 = reinterpret_cast<float2*>(raw);
     float2* A1 = A0 + Tp * LD;
@@ -285,6 +286,7 @@ __global__ void __launch_bounds__((TP / 2) * (TP / 2) < 32 ? 32 : (TP / 2) * (TP
 k_eig_real(const float2* __restrict__ C, int T, float* __restrict__ evals, float2* __restrict__ Vout,
            int32_t* __restrict__ status, int max_sweeps, int32_t* __restrict__ noconv) {
     extern __shared__ __align__(16) unsigned char raw[];
+    pdl_wait();                                                     // (launched as a programmatic dependent of the reduction)
     constexpr int Tp = TP, LD = TP + 2, half = TP / 2, m = TP - 1;   // LD even: pairs 8-byte aligned
     float* A0 = reinterpret_cast<float*>(raw);
     float* A1 = A0 + Tp * LD;
@@ -445,7 +447,7 @@ static int launch_eig_real_t(holo_ctx* c, const float2* C, float* evals, float2*
     { const int rc = holo_ensure_smem_attr((const void*)k_eig_real<TP>, c->device, smem); if (rc) return rc; }
     constexpr int threads = (TP / 2) * (TP / 2) < 32 ? 32 : (TP / 2) * (TP / 2);
     HoloProf prof(c, HOLO_K_EIG, st);
-    k_eig_real<TP><<<1, threads, smem, st>>>(C, T, evals, V, c->status, c->tune[HOLO_TUNE_EIG_MAX_SWEEPS], c->noconv_dev);
+    HOLO_CUDA_OK(holo_launch_pdl(k_eig_real<TP>, dim3(1), dim3(threads), smem, st, C, T, evals, V, c->status, c->tune[HOLO_TUNE_EIG_MAX_SWEEPS], c->noconv_dev));
     HOLO_CUDA_OK(cudaGetLastError());
     return HOLO_OK;
 }
@@ -460,7 +462,7 @@ static int launch_eig_t(holo_ctx* c, const float2* C, float* evals, float2* V, c
     { const int rc = holo_ensure_smem_attr((const void*)k_eig<TP>, c->device, smem); if (rc) return rc; }
     constexpr int threads = (TP / 2) * (TP / 2) < 32 ? 32 : (TP / 2) * (TP / 2);
     HoloProf prof(c, HOLO_K_EIG, st);
-    k_eig<TP><<<1, threads, smem, st>>>(C, T, evals, V, c->status, c->tune[HOLO_TUNE_EIG_MAX_SWEEPS], c->noconv_dev);
+    HOLO_CUDA_OK(holo_launch_pdl(k_eig<TP>, dim3(1), dim3(threads), smem, st, C, T, evals, V, c->status, c->tune[HOLO_TUNE_EIG_MAX_SWEEPS], c->noconv_dev));
     HOLO_CUDA_OK(cudaGetLastError());
     return HOLO_OK;
 }

@@ -14,6 +14,7 @@
 // ------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256) k_frame_sum(const uint16_t* __restrict__ frames, uint32_t* __restrict__ sum,
                                                    long long npix, int T, unsigned int* __restrict__ counters) {
+    pdl_trigger();                                        // (the Fresnel kernel may become resident while this one drains)
     if (blockIdx.x == 0 && threadIdx.x < 2 * T + 1) counters[threadIdx.x] = 0u;   // ticket / completion counters of the fused Fresnel kernel
     long long v = (long long)blockIdx.x * blockDim.x + threadIdx.x;      // one uint4 = 8 pixels per thread
     long long nvec = npix >> 3;
@@ -288,6 +289,8 @@ template <int N, int E, int R1, int R2, int B, int TILED = 0>
 __global__ void __launch_bounds__((N / E) * B, 512 / ((N / E) * B) > 0 ? 512 / ((N / E) * B) : 1)
 k_col_energy(const FftArgs a, float* __restrict__ out, long long npix, int nframes, int nsplit) {
     extern __shared__ float2 sm[];
+    pdl_trigger();                                        // (k_sum_partial_images may become resident)
+    pdl_wait();                                           // the row pass is complete
     const int tile = blockIdx.x, split = blockIdx.y;
     float acc[E];
 #pragma unroll
@@ -306,6 +309,7 @@ k_col_energy(const FftArgs a, float* __restrict__ out, long long npix, int nfram
 __global__ void __launch_bounds__(256) k_sum_partial_images(const float* __restrict__ part, int nsplit, long long npix, float* __restrict__ out) {
     const long long n4 = npix >> 2;                         // npix is a multiple of 256
     const float4* p4 = reinterpret_cast<const float4*>(part);
+    pdl_wait();
     for (long long p = (long long)blockIdx.x * 256 + threadIdx.x; p < n4; p += (long long)gridDim.x * 256) {
         float4 s = __ldg(p4 + p);
         for (int k = 1; k < nsplit; ++k) { const float4 w = __ldg(p4 + (long long)k * n4 + p); s.x += w.x; s.y += w.y; s.z += w.z; s.w += w.w; }
@@ -376,6 +380,7 @@ __global__ void __launch_bounds__(256) k_deflate_images(const uint16_t* __restri
                                                         const float2* __restrict__ V, long long npix, int T,
                                                         int c0_lo, int c0_n, int c1_lo, float* __restrict__ img, float* __restrict__ coef) {
     __shared__ float Vs[HOLO_MAX_T * NDEFL];
+    pdl_trigger();                                        // (the row pass may load its tables while this kernel drains)
     for (int i = threadIdx.x; i < T * NDEFL; i += blockDim.x) {
         const int t = i / NDEFL, kk = i - t * NDEFL;
         const int col = kk < c0_n ? c0_lo + kk : c1_lo + (kk - c0_n);
@@ -468,6 +473,8 @@ __global__ void __launch_bounds__((N / E) * B, 512 / ((N / E) * B) > 0 ? 512 / (
     extern __shared__ float2 sm[];
     __shared__ unsigned int s_ticket[2];
     __shared__ int s_ready[2];
+    pdl_trigger();                                        // (covariance / projection CTAs: one per SM, as SMs drain)
+    pdl_wait();                                           // S and the zeroed counters are complete
     const unsigned int total = (unsigned int)p.T * (unsigned int)(p.RT + p.CT);
     if (threadIdx.x == 0) { s_ticket[0] = atomicAdd(p.counters, 1u); s_ready[0] = 0; }
     __syncthreads();
@@ -608,8 +615,7 @@ static int launch_col_energy_t(const FftArgs& a, float* out, long long npix, int
     constexpr size_t smem = (R1 > 1) ? sizeof(float2) * (size_t)(N + N / E) * B : 0;
     auto kern = k_col_energy<N, E, R1, R2, B, TILED>;
     { const int rc = holo_ensure_smem_attr((const void*)kern, device, smem); if (rc) return rc; }
-    kern<<<dim3((unsigned)a.tiles_per_frame, (unsigned)nsplit), threads, smem, st>>>(a, out, npix, nframes, nsplit);
-    HOLO_CUDA_OK(cudaGetLastError());
+    HOLO_CUDA_OK(holo_launch_pdl(kern, dim3((unsigned)a.tiles_per_frame, (unsigned)nsplit), dim3(threads), smem, st, a, out, npix, nframes, nsplit));
     return HOLO_OK;
 }
 static int launch_col_energy(int N, const FftArgs& a, float* out, long long npix, int nframes, int nsplit, int device, cudaStream_t st,
@@ -653,7 +659,7 @@ static int launch_fresnel_t(const FresnelArgs& p, int num_sms, int device, cudaS
     const long long total = (long long)p.T * (p.RT + p.CT);
     long long grid = (long long)num_sms * blocks_per_sm;      // one wave of persistent CTAs
     if (grid > total) grid = total;
-    kern<<<(int)grid, threads, smem, st>>>(p);
+    HOLO_CUDA_OK(holo_launch_pdl(kern, dim3((unsigned)grid), dim3(threads), smem, st, p));
     HOLO_CUDA_OK(cudaGetLastError());
     return HOLO_OK;
 }
@@ -794,6 +800,9 @@ int holo_launch_energy_image(holo_ctx* c, const uint16_t* frames, const float2* 
     if (eigen && !c->eig_img) { holo_set_error("internal: eigen-image workspace missing (holo_set_mode / holo_set_range allocate it)"); return HOLO_ERR_STATE; }
     int rc = HOLO_OK;
     const int nframes = eigen ? nS : T;
+    // row ticket (k_sum_gram may run on another stream).  First in the chain: the kernels below follow one another as
+    // programmatic dependent launches (deflation images -> row pass -> column pass -> sum of the partial images)
+    HOLO_CUDA_OK(cudaMemsetAsync(c->counters + 1001, 0, sizeof(unsigned int), st));
     if (eigen) {
         HoloProf prof(c, HOLO_K_SUM, st);
         const int px = T <= 32 ? 4 : 2;
@@ -827,7 +836,6 @@ int holo_launch_energy_image(holo_ctx* c, const uint16_t* frames, const float2* 
     a.defl_img = c->defl_img; a.defl_coef = c->defl_coef; a.ndefl = ndefl;
     a.eimg = c->eig_img;
     a.ticket = c->counters + 1001;
-    HOLO_CUDA_OK(cudaMemsetAsync(c->counters + 1001, 0, sizeof(unsigned int), st));     // row ticket (k_sum_gram may run on another stream)
     // the packed row pass can write its output column tile by column tile (the layout is private to this function): the
     // column pass then reads one contiguous 64 KB block per tile and frame instead of 1024 segments of 64 bytes
     const bool rows2 = !eigen && c->tune[HOLO_TUNE_ROWS2] && holo_rows2_supported(c);
@@ -857,8 +865,8 @@ int holo_launch_energy_image(holo_ctx* c, const uint16_t* frames, const float2* 
     if (ns > 1) {
         HoloProf prof(c, HOLO_K_PROJECT, st);
         const long long want = ((c->npix >> 2) + 255) / 256;
-        k_sum_partial_images<<<(int)(want < 8ll * c->num_sms ? want : 8ll * c->num_sms), 256, 0, st>>>(c->energy_parts, ns, c->npix, image);
-        HOLO_CUDA_OK(cudaGetLastError());
+        HOLO_CUDA_OK(holo_launch_pdl(k_sum_partial_images, dim3((unsigned)(want < 8ll * c->num_sms ? want : 8ll * c->num_sms)), dim3(256), 0, st,
+                                     (const float*)c->energy_parts, ns, c->npix, image));
     }
     return HOLO_OK;
 }

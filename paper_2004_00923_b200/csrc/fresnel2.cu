@@ -201,6 +201,9 @@ __global__ void __launch_bounds__(R2_WARPS * 32, 1) k_rows2(const R2Args a) {
     for (int i = tid; i < F2N; i += R2_WARPS * 32) tw_s[i] = a.tw[i];
     for (int i = tid; i < NX; i += R2_WARPS * 32) qx_s[i] = a.qxs[i];
     if constexpr (NX == 2048) for (int i = tid; i < F2N; i += R2_WARPS * 32) w2_s[i] = a.tw2048[i];
+    // (no early trigger here: column CTAs made resident while this kernel drains pile up three deep on the SMs that finish
+    //  first and leave the others empty: 224 vs 206 us per stack)
+    pdl_wait();                                                // the tables above never change; everything below depends on earlier kernels
     __syncthreads();
     const uint32_t buf = bufs + (uint32_t)(warp >> 2) * F2_TILE;
     const XAddr xa = make_xaddr(buf, warp & 3, lane);
@@ -413,10 +416,10 @@ int holo_launch_rows2(holo_ctx* c, const uint16_t* frames, float2* out, int ndef
     HoloProf prof(c, HOLO_K_FFT_ROWS, st);
     if (c->nx == 1024) {
         if ((rc = holo_ensure_smem_attr((const void*)k_rows2<1024>, c->device, r2_smem<1024>()))) return rc;
-        k_rows2<1024><<<c->num_sms - c->fresnel_sm_reserve, R2_WARPS * 32, r2_smem<1024>(), st>>>(a);
+        HOLO_CUDA_OK(holo_launch_pdl(k_rows2<1024>, dim3(c->num_sms - c->fresnel_sm_reserve), dim3(R2_WARPS * 32), r2_smem<1024>(), st, a));
     } else {
         if ((rc = holo_ensure_smem_attr((const void*)k_rows2<2048>, c->device, r2_smem<2048>()))) return rc;
-        k_rows2<2048><<<c->num_sms - c->fresnel_sm_reserve, R2_WARPS * 32, r2_smem<2048>(), st>>>(a);
+        HOLO_CUDA_OK(holo_launch_pdl(k_rows2<2048>, dim3(c->num_sms - c->fresnel_sm_reserve), dim3(R2_WARPS * 32), r2_smem<2048>(), st, a));
     }
     HOLO_CUDA_OK(cudaGetLastError());
     return HOLO_OK;

@@ -9,6 +9,7 @@
 #include <vector>
 
 static thread_local char g_err[512] = "";
+int holo_pdl_enabled = 1;
 
 void holo_set_error(const char* fmt, ...) {
     va_list ap;
@@ -151,6 +152,7 @@ static int create_impl(holo_ctx* c) {
     c->tune[HOLO_TUNE_PROJ_TC] = 1;
     c->tune[HOLO_TUNE_COLS2048] = 1;
     c->tune[HOLO_TUNE_TILED_G] = 8;
+    c->tune[HOLO_TUNE_PDL] = holo_pdl_enabled;
     c->tune[HOLO_TUNE_ROWS2] = 1;                // packed two-frame row pass of mode 3 (1024^2, even T): 79 vs 84 us
     c->scratch_frames = (int)grp;
     c->cov_parts_cap = 4 * c->num_sms;
@@ -836,6 +838,7 @@ extern "C" int holo_tune(holo_ctx* c, int key, int value) {
         for (int i = 0; i < 2 * HOLO_PROF_CAP; ++i) HOLO_CUDA_OK(cudaEventCreate(&c->prof_ev[i]));
         c->prof_n = 0;
     }
+    if (key == HOLO_TUNE_PDL) holo_pdl_enabled = value != 0;
     if (key == HOLO_TUNE_TILED_G && value != 0 && value != 8 && value != 16 && value != 32) { holo_set_error("tile width must be 0, 8, 16 or 32"); return HOLO_ERR_ARG; }
     if (key == HOLO_TUNE_COV_GRIDX && (value < 1 || value > c->cov_parts_cap)) { holo_set_error("cov grid out of range"); return HOLO_ERR_ARG; }
     c->tune[key] = value;

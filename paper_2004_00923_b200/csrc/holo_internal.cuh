@@ -30,6 +30,7 @@ enum {
     HOLO_TUNE_PROJ_TC = 12,        // direct projection of more than 4 components on the tensor cores (T <= 32; default 1)
     HOLO_TUNE_ROWS2 = 15,          // mode 3: packed two-frame row pass where supported (1024^2, even T) // stages accumulated in TMEM before the accumulators are added to FP64 (default 4)
     HOLO_TUNE_TILED_G = 17,        // mode 3, 1024 x 1024: the row pass writes its output column tile by column tile (default 1)
+    HOLO_TUNE_PDL = 18,            // programmatic dependent launches between the kernels of a chain (process-wide; default 1)
     HOLO_TUNE_COLS2048 = 16,       // mode 3: packed column-energy pass for 2048-point columns (default 1)
     HOLO_TUNE_FFT_LAG = 6,         // frames between the row pass and the column pass in the fused kernel (0 = auto)
 };
@@ -125,6 +126,24 @@ struct holo_ctx {
 };
 
 void holo_set_error(const char* fmt, ...);
+// Programmatic dependent launch: a kernel launched with holo_launch_pdl may be made resident while the kernel before it in
+// the stream is still running (after every CTA of that one has called pdl_trigger or exited), which hides its launch
+// latency; it must call pdl_wait() before it reads or writes anything another kernel touches (pdl_wait returns when the
+// kernels before it are complete and their writes visible; a no-op in a plain launch).
+extern int holo_pdl_enabled;      // process-wide (holo_tune key 18): 0 = plain launches everywhere
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+template <class... KArgs, class... Args>
+static inline cudaError_t holo_launch_pdl(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args... args) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at; cfg.numAttrs = holo_pdl_enabled ? 1 : 0;
+    return cudaLaunchKernelEx(&cfg, kern, KArgs(args)...);
+}
+
 #define HOLO_CUDA_OK(expr)                                                              \
     do {                                                                                \
         cudaError_t _e = (expr);                                                        \

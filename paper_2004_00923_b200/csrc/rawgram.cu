@@ -214,6 +214,7 @@ __global__ void __launch_bounds__(256) k_gram_reduce_finish(const long long* __r
     __shared__ long long r[HOLO_MAX_T];
     __shared__ long long tau_lo; __shared__ long long tau_hi;   // tau as a 128-bit value
     __shared__ int s_last;
+    pdl_trigger();                                        // (the single-CTA eigensolver that follows waits for this whole kernel)
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int entry = blockIdx.x * 8 + warp;
     const int nent = N * (N + 1) / 2;

@@ -338,6 +338,12 @@ def test_process_mode3_matches_oracle_on_configs(torch_cuda, cfgn):
             Mw = torch.empty_like(M)
             h.process(dev, Mw)
             assert torch.equal(Mw, M), w
+        # plain launches instead of programmatic dependent ones: the same kernels on the same data
+        h.tune(18, 0)
+        Mp = torch.empty_like(M)
+        h.process(dev, Mp)
+        h.tune(18, 1)
+        assert torch.equal(Mp, M)
         # the scalar row pass (one frame per warp) instead of the packed two-frame one: same image up to FP32 rounding
         h.tune(15, 0)
         Ms = torch.empty_like(M)
@@ -840,6 +846,12 @@ def test_process_cfg3_full_size(torch_cuda):
     assert rc == 0, st
     Mg = M.cpu().numpy()
     res, out = _compare_full(torch, cfg, fr, h, Mg)
+    # plain launches instead of programmatic dependent ones (tune key 18): the same kernels on the same data
+    h.tune(18, 0)
+    Mp = torch.empty_like(M)
+    h.process(stream, Mp)
+    h.tune(18, 1)
+    assert torch.equal(Mp, M)
     h.close()
     assert res["M"] <= TOL_M and res["ev"] <= TOL_EV and res["C"] <= TOL_STAGE and res["H"] <= TOL_STAGE, res
     assert res["M"] <= FP32_M and res["ev"] <= FP32_EV and res["C"] <= FP32_C and res["H"] <= FP32_H, res
