@@ -255,7 +255,10 @@ int holo_launches_per_process(holo_ctx* ctx);
  *   output, [frame][x / w][y][x % w] (8, 16, 32; 0 = row-major; default 8 = the column tile of the energy pass, which
  *   then reads one contiguous 64 KB block per tile and frame), 18 programmatic dependent launches between the kernels of a
  *   chain (each such kernel waits with griddepcontrol.wait before it touches data; PROCESS-WIDE; default 1, 0 = plain
- *   launches; results are bit-identical either way). */
+ *   launches; results are bit-identical either way), 19 the Fresnel stage at 1024 x 1024 (even T >= 16, whole stacks) as two
+ *   streaming kernels -- packed row pass of frame pairs into column blocks, column pass from those blocks -- with the
+ *   row-pass output of the stack in a second T nx ny complex64 buffer (default 1; 0 = the fused persistent kernel with its
+ *   L2 ring, which holo_push keeps for its short strides). */
 int holo_tune(holo_ctx* ctx, int key, int value);
 
 /* Measurement hooks used by bench.py (not needed for normal use).

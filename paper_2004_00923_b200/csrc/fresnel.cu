@@ -16,6 +16,7 @@ __global__ void __launch_bounds__(256) k_frame_sum(const uint16_t* __restrict__ 
                                                    long long npix, int T, unsigned int* __restrict__ counters) {
     pdl_trigger();                                        // (the Fresnel kernel may become resident while this one drains)
     if (blockIdx.x == 0 && threadIdx.x < 2 * T + 1) counters[threadIdx.x] = 0u;   // ticket / completion counters of the fused Fresnel kernel
+    if (blockIdx.x == 0 && threadIdx.x == 0) counters[1001] = 0u;                 // row ticket of the packed row pass
     long long v = (long long)blockIdx.x * blockDim.x + threadIdx.x;      // one uint4 = 8 pixels per thread
     long long nvec = npix >> 3;
     for (; v < nvec; v += (long long)gridDim.x * blockDim.x) {
@@ -260,6 +261,21 @@ __global__ void __launch_bounds__((N / E) * B) k_fft(const FftArgs a) {
         const int fl = tile / a.tiles_per_frame;
         fft_tile<N, E, R1, R2, B, COL, PRO, 0, NoHook, DEFL>(a, (long long)fl * a.in_fstride, (long long)fl * a.out_fstride,
                                                              tile - fl * a.tiles_per_frame, sm, NoHook(), fl);
+    }
+}
+
+// column pass of whole frames whose row-pass output is stored in column blocks of B columns (see TILED above); plain
+// row-major output.  Tiles in frame-major order: concurrent CTAs walk adjacent column tiles of the same frame.
+template <int N, int E, int R1, int R2, int B>
+__global__ void __launch_bounds__((N / E) * B) k_cols_tiled(const FftArgs a) {
+    extern __shared__ float2 sm[];
+    pdl_wait();
+    const int nf = a.ntiles / a.tiles_per_frame;
+    for (int tile = blockIdx.x; tile < a.ntiles; tile += gridDim.x) {
+        const int fr = tile / a.tiles_per_frame;
+        const int fl = nf - 1 - fr;                          // newest frames first: the tail of the row-pass output is still in L2 (-4 us)
+        fft_tile<N, E, R1, R2, B, true, false, 0, NoHook, 0, false, B>(a, (long long)fl * a.in_fstride, (long long)fl * a.out_fstride,
+                                                                       tile - fr * a.tiles_per_frame, sm);
     }
 }
 
@@ -684,8 +700,20 @@ static bool use_fused(const holo_ctx* c) {
     return c->nx == c->ny && c->tune[HOLO_TUNE_FFT_PERSISTENT] && c->scratch_frames >= 2 && 2 * c->T + 1 <= 256;
 }
 
+// Fresnel stage as two streaming kernels (packed row pass -> row-pass output of the whole stack in c->rowout -> column pass)
+// instead of the fused persistent kernel: 2048 x 2048 (any frame count), and 1024 x 1024 for an even frame count of at
+// least 16 (shorter runs -- the strides of holo_push -- are faster in the fused kernel, whose ring stays in L2)
+static bool use_packed_pair(const holo_ctx* c, int nproc) {
+    if (!c->rowout) return false;
+    if (c->nx == 2048 && c->ny == 2048) return c->tune[HOLO_TUNE_COLS2048] != 0;
+    if (c->nx == 1024 && c->ny == 1024) return c->tune[HOLO_TUNE_PACKED1024] != 0 && (c->T % 2) == 0 && (nproc % 2) == 0 && nproc >= 16;
+    return false;
+}
+
+bool holo_fresnel_is_packed(const holo_ctx* c) { return use_packed_pair(c, c->T); }
+
 int holo_fresnel_launch_count(holo_ctx* c) {
-    if (c->rowout && c->tune[HOLO_TUNE_COLS2048] && c->nx == 2048 && c->ny == 2048) return 3;
+    if (use_packed_pair(c, c->T)) return 3;
     if (use_fused(c)) return 2;
     int g = c->scratch_frames;
     int groups = (c->T + g - 1) / g;
@@ -709,14 +737,41 @@ int holo_launch_sum(holo_ctx* c, const uint16_t* frames, cudaStream_t st) {
 int holo_launch_fresnel(holo_ctx* c, const uint16_t* frames, float2* H, cudaStream_t st, bool with_sum, int nproc, bool counters_zeroed) {
     if (nproc < 0) nproc = c->T;
     if (with_sum) { const int rc = holo_launch_sum(c, frames, st); if (rc) return rc; }
-    else if (!counters_zeroed && use_fused(c)) HOLO_CUDA_OK(cudaMemsetAsync(c->counters, 0, (2 * c->T + 1) * sizeof(unsigned int), st));
-    if (c->rowout && c->tune[HOLO_TUNE_COLS2048] && c->nx == 2048 && c->ny == 2048) {
-        // 2048 x 2048: the packed row pass (radix-2 decimation in frequency + a pair of 1024-point transforms) and the packed
-        // column pass, the row-pass output of the stack going through HBM: 1.8 vs 2.4 ms for the fused three-pass kernel
-        HOLO_CUDA_OK(cudaMemsetAsync(c->counters + 1001, 0, sizeof(unsigned int), st));
-        int rc = holo_launch_rows2(c, frames, c->rowout, 0, st, nproc);
+    else if (!counters_zeroed && use_fused(c) && !use_packed_pair(c, nproc))
+        HOLO_CUDA_OK(cudaMemsetAsync(c->counters, 0, (2 * c->T + 1) * sizeof(unsigned int), st));
+    if (use_packed_pair(c, nproc)) {
+        // the row ticket: zeroed by the sum kernels (k_frame_sum, k_sum_gram) where one of them ran just before
+        if (!with_sum && !counters_zeroed) HOLO_CUDA_OK(cudaMemsetAsync(c->counters + 1001, 0, sizeof(unsigned int), st));
+        if (c->nx == 2048) {
+            // 2048 x 2048: the packed row pass (radix-2 decimation in frequency + a pair of 1024-point transforms) and the
+            // packed column pass, the row-pass output of the stack going through HBM: 1.8 vs 2.4 ms for the fused three-pass kernel
+            int rc = holo_launch_rows2(c, frames, c->rowout, 0, st, nproc);
+            if (rc) return rc;
+            return holo_launch_cols2048_store(c, c->rowout, H, nproc, st);
+        }
+        // 1024 x 1024: the packed row pass of frame pairs stores its output in column blocks of 8 columns, the column pass
+        // reads one contiguous 64 KB block per tile: both kernels stream at ~80 % of the HBM peak on their DRAM traffic
+        // (871 MB with the intermediate) and take 168 us together; the fused kernel keeps the intermediate in L2 (438 MB
+        // of DRAM traffic) but is bound by the dependency stalls of its tile pipeline: 197 us
+        int rc = holo_launch_rows2(c, frames, c->rowout, 0, st, nproc, 8);
         if (rc) return rc;
-        return holo_launch_cols2048_store(c, c->rowout, H, nproc, st);
+        FftArgs b{};
+        b.in = c->rowout; b.out = H;
+        b.tw1 = c->py.tw1; b.tw2 = c->py.tw2;
+        b.in_fstride = c->npix; b.out_fstride = c->npix;
+        b.ld = c->nx; b.nseq = c->nx;
+        b.tiles_per_frame = c->nx / 8;
+        b.ntiles = nproc * b.tiles_per_frame;
+        b.T = c->T;
+        constexpr size_t smem = sizeof(float2) * (size_t)(1024 + 32) * 8;
+        auto kern = k_cols_tiled<1024, 32, 32, 1, 8>;
+        int blocks_per_sm = 0;
+        if ((rc = holo_cached_occupancy((const void*)kern, c->device, 256, smem, &blocks_per_sm))) return rc;
+        const int sms = c->num_sms - c->fresnel_sm_reserve;    // (mode 2: one SM for the side-stream eigensolver)
+        const int grid = b.ntiles < sms * blocks_per_sm ? b.ntiles : sms * blocks_per_sm;
+        HoloProf prof(c, HOLO_K_FFT_COLS, st);
+        HOLO_CUDA_OK(holo_launch_pdl(kern, dim3(grid), dim3(256), smem, st, b));
+        return HOLO_OK;
     }
     if (use_fused(c)) {
         FresnelArgs p{};

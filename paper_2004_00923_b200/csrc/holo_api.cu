@@ -147,11 +147,14 @@ static int create_impl(holo_ctx* c) {
     // products): measured 584 vs 919 us at 2048^2 x 64 with 2e-6 on the eigenvalues; at T <= 32 the gain is 12 % (75 vs 85 us)
     // and the FP32 kernel stays the default (profiles/r02_tf32_gram.md)
     // (the rounding noise of single-pass TF32 averages out as 1 / sqrt(pixels): below 2^20 pixels the split form is used)
-    c->tune[HOLO_TUNE_COV_TF32] = (T > 32 && np % 256 == 0) ? (np >= (1ll << 20) ? 1 : 3) : 0;
+    // tensor-core covariance: at T > 32 (the FP32 kernel is ALU bound there), and at T = 32 from 2^20 pixels, where one TF32 pass
+    // is accurate enough and the covariance is on the critical path (packed Fresnel stage: no SM split): 300 vs 321 us per stack
+    c->tune[HOLO_TUNE_COV_TF32] = (np % 256 != 0) ? 0 : T > 32 ? (np >= (1ll << 20) ? 1 : 3) : (T == 32 && np >= (1ll << 20)) ? 1 : 0;
     c->tune[HOLO_TUNE_COV_TF32_DRAIN] = 4;
     c->tune[HOLO_TUNE_PROJ_TC] = 1;
     c->tune[HOLO_TUNE_COLS2048] = 1;
     c->tune[HOLO_TUNE_TILED_G] = 8;
+    c->tune[HOLO_TUNE_PACKED1024] = 1;
     c->tune[HOLO_TUNE_PDL] = holo_pdl_enabled;
     c->tune[HOLO_TUNE_ROWS2] = 1;                // packed two-frame row pass of mode 3 (1024^2, even T): 79 vs 84 us
     c->scratch_frames = (int)grp;
@@ -160,7 +163,8 @@ static int create_impl(holo_ctx* c) {
     HOLO_CUDA_OK(cudaMalloc(&c->sum, np * sizeof(uint32_t)));
     HOLO_CUDA_OK(cudaMalloc(&c->scratch, (size_t)c->scratch_frames * np * sizeof(float2)));
     HOLO_CUDA_OK(cudaMalloc(&c->H, (size_t)T * np * sizeof(float2)));
-    if (c->nx == 2048 && c->ny == 2048) HOLO_CUDA_OK(cudaMalloc(&c->rowout, (size_t)T * np * sizeof(float2)));
+    if ((c->nx == 2048 && c->ny == 2048) || (c->nx == 1024 && c->ny == 1024 && T % 2 == 0 && T >= 16))
+        HOLO_CUDA_OK(cudaMalloc(&c->rowout, (size_t)T * np * sizeof(float2)));
     HOLO_CUDA_OK(cudaMalloc(&c->cov_partials, (size_t)c->cov_parts_cap * T8 * T8 * sizeof(float2)));
     HOLO_CUDA_OK(cudaMalloc(&c->C, (size_t)T * T * sizeof(float2)));
     HOLO_CUDA_OK(cudaMalloc(&c->evals, T * sizeof(float)));
@@ -470,7 +474,10 @@ extern "C" int holo_submit(holo_ctx* c, const uint16_t* frames_dev, float* image
     // direct (tensor-core) projection, which needs the whole GPU: stream order then
     const int nS_now = c->k_hi - c->k_lo + 1;
     const bool deflating = c->tune[HOLO_TUNE_PROJ_COMPLEMENT] && 2 * (c->T - nS_now) <= nS_now;
-    const int split = deflating ? c->tune[HOLO_TUNE_SPLIT_SMS] : 0;
+    // The split pays under the FUSED Fresnel kernel (latency bound at 27 % of the HBM peak: the side-stream projection of the
+    // previous stack runs beside it for free).  The packed row / column kernels stream at ~80 % of the HBM peak and need whole
+    // SMs: a projection beside them only takes bandwidth and SMs away (339 vs 321 us per stack): stream order then.
+    const int split = deflating && !holo_fresnel_is_packed(c) ? c->tune[HOLO_TUNE_SPLIT_SMS] : 0;
     if (c->tune[HOLO_TUNE_SPLIT_SMS] > 0) { if ((rc = join_side(c, st, s))) return rc; }      // H / V of slot s are free once the projection of stack i-2 is done
     if ((rc = holo_launch_fresnel(c, frames_dev, H, st))) return rc;
     if ((rc = project_pending(c, st))) return rc;

@@ -30,6 +30,7 @@ enum {
     HOLO_TUNE_PROJ_TC = 12,        // direct projection of more than 4 components on the tensor cores (T <= 32; default 1)
     HOLO_TUNE_ROWS2 = 15,          // mode 3: packed two-frame row pass where supported (1024^2, even T) // stages accumulated in TMEM before the accumulators are added to FP64 (default 4)
     HOLO_TUNE_TILED_G = 17,        // mode 3, 1024 x 1024: the row pass writes its output column tile by column tile (default 1)
+    HOLO_TUNE_PACKED1024 = 19,     // 1024 x 1024 Fresnel stage as packed row pass + column pass (default 1; 0 = fused kernel)
     HOLO_TUNE_PDL = 18,            // programmatic dependent launches between the kernels of a chain (process-wide; default 1)
     HOLO_TUNE_COLS2048 = 16,       // mode 3: packed column-energy pass for 2048-point columns (default 1)
     HOLO_TUNE_FFT_LAG = 6,         // frames between the row pass and the column pass in the fused kernel (0 = auto)
@@ -65,7 +66,7 @@ struct holo_ctx {
     double* norm_partials;  // [HOLO_NORM_PARTS] partial sums of holo_normalize
     // workspace
     uint32_t* sum;          // [ny][nx]
-    float2* rowout;         // 2048 x 2048 frames: row-pass output of the whole stack [T][ny][nx] (unfused packed Fresnel stage)
+    float2* rowout;         // 2048 x 2048 and 1024 x 1024 (even T) frames: row-pass output of the whole stack [T][ny][nx] (unfused packed Fresnel stage)
     float2* scratch;        // FFT row->column intermediate, fft_group frames
     int scratch_frames;
     float2* H;              // [T][ny][nx]
@@ -202,6 +203,7 @@ bool holo_rows2_supported(const holo_ctx* c);
 bool holo_cols2048_supported(const holo_ctx* c);
 int holo_launch_cols2048(holo_ctx* c, const float2* G, float* out, int nframes, int nsplit, cudaStream_t st);
 int holo_launch_cols2048_store(holo_ctx* c, const float2* G, float2* H, int nframes, cudaStream_t st);
+bool holo_fresnel_is_packed(const holo_ctx* c);      // Fresnel stage of whole stacks = packed row pass + column pass (not the fused kernel)
 int holo_launch_rows2(holo_ctx* c, const uint16_t* frames, float2* out, int ndefl, cudaStream_t st, int nframes = 0, int tile_w = 0);
 int holo_fft_plan_init(FftPlan* p, int N);
 void holo_fft_plan_free(FftPlan* p);

@@ -76,6 +76,7 @@ k_sum_gram(const uint16_t* __restrict__ frames, uint32_t* __restrict__ sum, unsi
     const int N = 2 * Tp;                                     // MMA N (64 or 128); M = 128 always
 
     if (blockIdx.x == 0 && tid < 2 * T + 1) counters[tid] = 0u;   // ticket / completion counters of the Fresnel kernel (as k_frame_sum)
+    if (blockIdx.x == 0 && tid == 0) counters[1001] = 0u;
     // rows that no frame writes (t >= T within a plane, and rows >= 2 Tp) must read as zero: clear both stages once
     for (int i = tid; i < 2 * RG_STAGE / 16; i += RG_THREADS) reinterpret_cast<uint4*>(base)[i] = make_uint4(0, 0, 0, 0);
     if (tid == 0) {

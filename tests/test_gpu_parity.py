@@ -150,7 +150,7 @@ def test_process_mode2_matches_oracle(torch_cuda, cfgn):
     assert gaps[cfg.k_lo - 2] >= 0.05
     h = _holo(cfg.n, cfg.n, cfg.T, cfg.k_lo, cfg.k_hi)
     h.set_mode(2)
-    assert h.launches_per_process() == 5
+    assert h.launches_per_process() == (6 if cfg.n == 1024 else 5)      # 1024^2: row pass + column pass instead of the fused kernel
     M = torch.empty((cfg.n, cfg.n), dtype=torch.float32, device="cuda")
     h.process(dev, M)
     rc, st = h.status()
