@@ -132,7 +132,7 @@ def stage_bytes(cfg, mode=1):
     """Algorithmic (compulsory) bytes per stack and stage, SURVEY.md 8(d) / DESIGN.md.  mode 2 (Gram from the raw
     frames, SURVEY.md 8(f)-2 stage 1) has no covariance read of the hologram stack: 20 T N_p + 12 N_p.  mode 3 (stage 2:
     no hologram stack) reads the frames three times (Gram + sum, deflation images, row pass), writes and reads the
-    row-pass output once and writes the image: 22 T N_p + (20 + 8 n_rej) N_p with n_rej rejected components."""
+    row-pass output once and writes the image: 22 T N_p + (16 + 8 n_rej) N_p with n_rej rejected components."""
     npix, T = cfg.n * cfg.n, cfg.T
     if mode == 3:
         nrej = (cfg.k_lo - 1) + (T - cfg.k_hi)
