@@ -102,9 +102,10 @@ int holo_process(holo_ctx* ctx, const uint16_t* frames_dev, float* image_dev, ho
  * enqueues on `stream` the Fresnel stage of stack i, then the projection of stack i-1 into the image_dev
  * given to submit(i-1), then the covariance of stack i, and forks the single-CTA eigensolver of stack i
  * to a side stream owned by the handle, where it runs under the Fresnel kernels of stack i+1.
- * By default (T <= 32) the projection of stack i follows its eigensolver on the side stream and runs on about a
- * quarter of the SMs, next to the (ALU-bound) covariance of stack i+1 on the others (that covariance then sums over
- * fewer CTAs: images equal those of holo_process up to FP32 summation order, and are bit-reproducible).
+ * Where the Fresnel stage is the fused persistent kernel (T <= 32; frame sizes other than 1024 x 1024 and 2048 x 2048,
+ * or holo_tune key 19 = 0) the projection of stack i instead follows its eigensolver on the side stream and runs on
+ * about a quarter of the SMs beside the kernels of stack i+1, whose covariance then sums over fewer CTAs: images equal
+ * those of holo_process up to FP32 summation order, and are bit-reproducible.
  * Contract: the image passed to submit(i) is complete, in `stream` order, after holo_flush, or after the
  * holo_submit after next (i+2); frames_dev may be reused as soon as `stream` has passed the submit.  The handle
  * allocates a second hologram stack (8*T*nx*ny bytes) at the first call.  holo_process / holo_flush
@@ -246,7 +247,8 @@ int holo_launches_per_process(holo_ctx* ctx);
  *   10 pipelined ring form of holo_push (default 1), 11 incremental Gram update in that form (default 1),
  *   12 direct projection of more than 4 components on the tensor cores (3 x TF32, T <= 32; default 1; 0 = FP32 kernel),
  *   13 real covariance of holo_process / holo_submit on the tensor cores (tcgen05.mma kind::tf32 on values
- *   rounded to nearest, FP64 partials): 0 = FP32 FFMA kernel (default at T <= 32), 1 = TF32 (default at T > 32), 3 = 3 x TF32,
+ *   rounded to nearest, FP64 partials): 0 = FP32 FFMA kernel (default below T = 32, and at T = 32 below 2^20 pixels),
+ *   1 = TF32 (default at T > 32 and at T = 32 from 2^20 pixels; 3 x TF32 below 2^20 pixels at T > 32), 3 = 3 x TF32,
  *   14 operand stages accumulated in TMEM between two FP64 drains of key 13 (default 4 = 512 products),
  *   15 mode 3: packed row pass (FFMA2 / FADD2 on pairs: the same row of two consecutive frames at nx = 1024 with even T,
  *   the even / odd halves of one row at nx = 2048; default 1), 16 packed 2048-point column passes (mode 3 column energy;
