@@ -952,6 +952,45 @@ def test_fresnel_fused_square_sizes(torch_cuda, n, T):
     h.close()
 
 
+@pytest.mark.parametrize("T", [16, 17, 22])
+def test_fresnel_1024_packed_and_fused(torch_cuda, T):
+    """1024 x 1024: whole stacks of an even T >= 16 take the packed row pass + the column pass from 8-column blocks
+    (holo_tune key 19, default 1); an odd T, key 19 = 0 and the short strides of holo_push take the fused persistent
+    kernel.  Both against the oracle on full-range uint16 values, frame by frame."""
+    from paper_2004_00923_b200 import HOLO_WS_SUM
+    torch = torch_cuda
+    n = 1024
+    rng = np.random.default_rng(1024 + T)
+    fr = _rand_frames(rng, T, n, n, 0, 65536)
+    Ho = oracle.fresnel(fr, LAM, PITCH, Z)
+    h = _holo(n, n, T, 1, T)
+    packed = T % 2 == 0
+    assert h.launches_per_process() == (7 if packed else 6)
+    H = torch.empty((T, n, n), dtype=torch.complex64, device="cuda")
+    dev = _to_dev(torch, fr)
+    h.fresnel(dev, H)
+    torch.cuda.synchronize()
+    err = max(rel_l2(H[t].cpu().numpy(), Ho[t]) for t in range(T))
+    assert err <= FP32_H, err
+    S = h.workspace_tensor(HOLO_WS_SUM).cpu().numpy()
+    assert np.array_equal(S.astype(np.int64), fr.astype(np.int64).sum(0))
+    if packed:
+        H1 = H.clone()
+        h.fresnel(dev, H)                                   # the row ticket is zeroed by the sum kernel of every call
+        torch.cuda.synchronize()
+        assert torch.equal(H.view(torch.float32), H1.view(torch.float32))
+        h.tune(19, 0)
+        assert h.launches_per_process() == 6
+        H.zero_()
+        h.fresnel(dev, H)
+        torch.cuda.synchronize()
+        err = max(rel_l2(H[t].cpu().numpy(), Ho[t]) for t in range(T))
+        assert err <= FP32_H, err
+        # the two forms differ only by FP32 rounding order
+        assert max(rel_l2(H[t].cpu().numpy(), H1[t].cpu().numpy()) for t in (0, T - 1)) <= 2e-6
+    h.close()
+
+
 def test_push_cfg4_full_size(torch_cuda):
     """holo_push at 1024x1024x32, stride 8 (BASELINE.json configs[3]), the launch configuration `bench.py --api push`
     times: first window, a window after seven pushes (the 48-slot ring has wrapped), a re-reference in mid-sequence
