@@ -1061,14 +1061,18 @@ def test_submit_cfg3_default_split_vs_oracle(torch_cuda):
     h.close()
 
 
-def test_process_graph_capture_replay(torch_cuda):
-    """include/holo.h: holo_process only enqueues on the caller's stream, so it can be captured into a CUDA graph;
-    the replayed graph must reproduce the eager image bit for bit."""
+@pytest.mark.parametrize("n,T,mode", [(128, 16, 1), (128, 16, 2), (128, 16, 3), (1024, 16, 1), (1024, 16, 3)])
+def test_process_graph_capture_replay(torch_cuda, n, T, mode):
+    """include/holo.h: holo_process only enqueues on the caller's stream, so it can be captured into a CUDA graph
+    (every mode; at 1024 x 1024 the capture holds the packed row / column kernels, their ticket reset and the
+    programmatic dependent launches); the replayed graph must reproduce the eager image bit for bit."""
     torch = torch_cuda
-    cfg = G.small_config(n=128, T=16)
+    cfg = G.small_config(n=n, T=T)
     d = _to_dev(torch, G.stack_np(cfg, 11))
-    h = _holo(128, 128, 16, 2, 16)
-    M0 = torch.empty((128, 128), dtype=torch.float32, device="cuda")
+    h = _holo(n, n, T, 2, T)
+    if mode != 1:
+        h.set_mode(mode)
+    M0 = torch.empty((n, n), dtype=torch.float32, device="cuda")
     M1 = torch.zeros_like(M0)
     st = torch.cuda.Stream()
     h.process(d, M0, st)                                   # eager (also the warm-up: attributes, lazy state)
