@@ -247,8 +247,8 @@ int holo_launches_per_process(holo_ctx* ctx);
  *   10 pipelined ring form of holo_push (default 1), 11 incremental Gram update in that form (default 1),
  *   12 direct projection of more than 4 components on the tensor cores (3 x TF32, T <= 32; default 1; 0 = FP32 kernel),
  *   13 real covariance of holo_process / holo_submit on the tensor cores (tcgen05.mma kind::tf32 on values
- *   rounded to nearest, FP64 partials): 0 = FP32 FFMA kernel (default below T = 32, and at T = 32 below 2^20 pixels),
- *   1 = TF32 (default at T > 32 and at T = 32 from 2^20 pixels; 3 x TF32 below 2^20 pixels at T > 32), 3 = 3 x TF32,
+ *   rounded to nearest, FP64 partials): 0 = FP32 FFMA kernel (default below T = 32, and at T = 32 below 2^18 pixels),
+ *   1 = TF32 (default at T = 32 from 2^18 pixels and at T > 32 from 2^20 pixels; T > 32 below that: 3 x TF32), 3 = 3 x TF32,
  *   14 operand stages accumulated in TMEM between two FP64 drains of key 13 (default 4 = 512 products),
  *   15 mode 3: packed row pass (FFMA2 / FADD2 on pairs: the same row of two consecutive frames at nx = 1024 with even T,
  *   the even / odd halves of one row at nx = 2048; default 1), 16 packed 2048-point column passes (mode 3 column energy;

@@ -147,9 +147,11 @@ static int create_impl(holo_ctx* c) {
     // products): measured 584 vs 919 us at 2048^2 x 64 with 2e-6 on the eigenvalues; at T <= 32 the gain is 12 % (75 vs 85 us)
     // and the FP32 kernel stays the default (profiles/r02_tf32_gram.md)
     // (the rounding noise of single-pass TF32 averages out as 1 / sqrt(pixels): below 2^20 pixels the split form is used)
-    // tensor-core covariance: at T > 32 (the FP32 kernel is ALU bound there), and at T = 32 from 2^20 pixels, where one TF32 pass
-    // is accurate enough and the covariance is on the critical path (packed Fresnel stage: no SM split): 300 vs 321 us per stack
-    c->tune[HOLO_TUNE_COV_TF32] = (np % 256 != 0) ? 0 : T > 32 ? (np >= (1ll << 20) ? 1 : 3) : (T == 32 && np >= (1ll << 20)) ? 1 : 0;
+    // tensor-core covariance: at T > 32 (the FP32 kernel is ALU bound there; 3 x TF32 below 2^20 pixels, where the rounding noise
+    // of a single pass has too few products to average over), and at T = 32 from 2^18 pixels in a single pass (measured against
+    // the oracle: C 3.3e-6 / eigenvalues 2.4e-6 / image 2.5e-7 at 512^2, 2.7e-6 / 2.5e-6 / 2.6e-7 at 1024^2; the FP32 kernel:
+    // 2e-7 / 2e-7 / 2.1e-7): 300 vs 321 us per stack at 1024^2, 99 vs 108 us at 512^2
+    c->tune[HOLO_TUNE_COV_TF32] = (np % 256 != 0) ? 0 : T > 32 ? (np >= (1ll << 20) ? 1 : 3) : (T == 32 && np >= (1ll << 18)) ? 1 : 0;
     c->tune[HOLO_TUNE_COV_TF32_DRAIN] = 4;
     c->tune[HOLO_TUNE_PROJ_TC] = 1;
     c->tune[HOLO_TUNE_COLS2048] = 1;
