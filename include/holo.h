@@ -25,7 +25,9 @@
  *   - `stream` is a cudaStream_t cast to void* (NULL = legacy default stream).  Every call only
  *     ENQUEUES work: no host synchronisation and no host<->device copy except in the *_host entry
  *     points, holo_status, holo_profile_read and holo_tune(key 0), which say so.
- *     Allocation: holo_create allocates the workspace of holo_process and of the per-stage calls.
+ *     Allocation: holo_create allocates the workspace of holo_process and of the per-stage calls
+ *     (about 8 T nx ny bytes for the hologram stack; at 1024 x 1024 with an even T >= 16 and at
+ *     2048 x 2048 the same again for the row-pass output of the packed Fresnel stage).
  *     The following calls allocate more at their FIRST use on a handle (cudaMalloc, which may
  *     synchronise the device) and never afterwards: holo_submit (second hologram stack, second
  *     C / V / evals / status slot, a side stream and six events), holo_push (FP64 Gram store, and in
