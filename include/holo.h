@@ -207,6 +207,21 @@ int holo_svd_filter(holo_ctx* ctx, const void* H_dev, const void* V_dev, void* H
  * left unchanged.  Two small kernels on `stream`. */
 int holo_normalize(holo_ctx* ctx, float* image_dev, holo_stream stream);
 
+/* holo_normalize for callers that cannot allocate (code under CUDA-graph capture, tight serving loops, harnesses that forbid
+ * cudaMalloc): out = in / mean(in), in_dev, out_dev float [ny][nx] device pointers, 4-byte aligned;
+ * out_dev == in_dev is allowed.  NO handle and NO allocation: the call uses neither cudaMalloc / cudaFree nor any
+ * allocating library routine; the partial sums of the mean live in a file-scope __device__ array of 32 KB that every GPU
+ * which loads the library holds until the process exits.  Limit: nx * ny <= HOLO_STATIC_MAX_PIXELS (2^24 = 4096 x 4096);
+ * larger images are rejected with HOLO_ERR_ARG and a message (use holo_normalize).  The mean is a fixed-order FP64 reduction
+ * over chunks of 4096 pixels (bit-reproducible, and the same on every GPU); an all-zero image is left unchanged.
+ * Two small kernels on `stream`, nothing else: no synchronisation, no copy.  The first call on a device resolves the
+ * device address of the array (cudaGetSymbolAddress, no allocation): make it outside stream capture.
+ * SHARED STATE: every call on a device uses the same array, which keeps the previous call's contents (nothing needs to
+ * start at zero: a call writes every entry it reads).  Calls that overlap on the GPU -- different streams, or host
+ * threads without ordering -- race on it and return wrong means: issue them on one stream or order them with events. */
+#define HOLO_STATIC_MAX_PIXELS (1LL << 24)
+int holo_normalize_static(const float* in_dev, float* out_dev, int nx, int ny, holo_stream stream);
+
 /* Quadrant swap of an image in FFT-bin order: out[(j + ny/2) mod ny][(i + nx/2) mod nx] = in[j][i] (zero frequency to the
  * centre; R6: every other call leaves images in raw FFT-bin order).  Out of place: in_dev != out_dev. */
 int holo_fftshift(holo_ctx* ctx, const float* in_dev, float* out_dev, holo_stream stream);

@@ -10,7 +10,7 @@ HOLO_WS_SUM, HOLO_WS_H, HOLO_WS_C, HOLO_WS_EVALS, HOLO_WS_V, HOLO_WS_STATUS, HOL
 
 EXPORTED_SYMBOLS = [
     "holo_create", "holo_destroy", "holo_process", "holo_submit", "holo_flush", "holo_submit_host", "holo_flush_host", "holo_push", "holo_process_host", "holo_fresnel", "holo_covariance",
-    "holo_raw_covariance", "holo_set_mode", "holo_eig", "holo_project", "holo_fourier_demod", "holo_svd_filter", "holo_normalize", "holo_fftshift", "holo_set_range", "holo_set_assume_unitary",
+    "holo_raw_covariance", "holo_set_mode", "holo_eig", "holo_project", "holo_fourier_demod", "holo_svd_filter", "holo_normalize", "holo_normalize_static", "holo_fftshift", "holo_set_range", "holo_set_assume_unitary",
     "holo_workspace", "holo_workspace_copy", "holo_status", "holo_launches_per_process", "holo_tune", "holo_profile_read", "holo_fft_group",
     "holo_last_error", "holo_version",
 ]
@@ -57,6 +57,7 @@ def load_library():
     L.holo_fourier_demod.argtypes = [vp, vp, ip, ip, vp, vp]
     L.holo_svd_filter.argtypes = [vp, vp, vp, vp, vp]
     L.holo_normalize.argtypes = [vp, vp, vp]
+    L.holo_normalize_static.argtypes = [vp, vp, ip, ip, vp]
     L.holo_fftshift.argtypes = [vp, vp, vp, vp]
     L.holo_set_range.argtypes = [vp, ip, ip]
     L.holo_set_assume_unitary.argtypes = [vp, ip]
@@ -81,6 +82,14 @@ def _stream_ptr(stream):
     if isinstance(stream, int):
         return stream
     return stream.cuda_stream
+
+
+def normalize_static(in_dev, out_dev, nx, ny, stream=None):
+    """holo_normalize_static: out = in / mean(in) without a handle and without any allocation (include/holo.h)."""
+    L = load_library()
+    rc = L.holo_normalize_static(Holo._p(in_dev), Holo._p(out_dev), nx, ny, _stream_ptr(stream))
+    if rc != 0:
+        raise HoloError(rc, L.holo_last_error().decode())
 
 
 class Holo:

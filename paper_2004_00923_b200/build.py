@@ -5,7 +5,7 @@ import sys
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
-SOURCES = ["holo_api.cu", "fresnel.cu", "fresnel2.cu", "rawgram.cu", "covariance.cu", "covtf32.cu", "eig.cu", "project.cu", "project_tc.cu", "display.cu"]
+SOURCES = ["holo_api.cu", "fresnel.cu", "fresnel2.cu", "rawgram.cu", "covariance.cu", "covtf32.cu", "eig.cu", "project.cu", "project_tc.cu", "display.cu", "noalloc.cu"]
 LIB = os.path.join(HERE, "libholo_b200.so")
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
