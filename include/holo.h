@@ -277,7 +277,8 @@ int holo_launches_per_process(holo_ctx* ctx);
  *   launches; results are bit-identical either way), 19 the Fresnel stage at 1024 x 1024 (even T >= 16, whole stacks) as two
  *   streaming kernels -- packed row pass of frame pairs into column blocks, column pass from those blocks -- with the
  *   row-pass output of the stack in a second T nx ny complex64 buffer (default 1; 0 = the fused persistent kernel with its
- *   L2 ring, which holo_push keeps for its short strides). */
+ *   L2 ring, which holo_push keeps for its short strides), 20 single-pass TF32 covariance fed by TMA (3-D swizzled boxes land
+ *   in operand layout, rounding in place; default 1; 0 = the register-fed kernel). */
 int holo_tune(holo_ctx* ctx, int key, int value);
 
 /* Measurement hooks used by bench.py (not needed for normal use).

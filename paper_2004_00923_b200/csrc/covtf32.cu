@@ -198,6 +198,164 @@ k_cov_tf32(const float2* __restrict__ H, float2* __restrict__ partials, long lon
     if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "r"(256) : "memory");
 }
 
+// ------------------------------------------------------------------------------------------------
+// The same single-pass TF32 Gram fed by TMA (the default single-pass form; holo_tune key 20 = 0 selects the kernel above).
+// The register-fed kernel has ONE stage (64 KB per SM) of loads in flight and then waits for it: 4.0 TB/s.  Here the TMA unit writes the stack straight into the operand layout -- a 3-D box of
+// [TP frames][S pieces][32 floats] with CU_TENSOR_MAP_SWIZZLE_128B lands as the 128 rows of a K-major SWIZZLE_128B tile, rows
+// of frames t >= T zero-filled -- into a ring of CQ_NST stages, several stages ahead; the threads only round the landed values
+// to TF32 IN PLACE (LDS.128, 4 x cvt.rna, STS.128 at the same address: no layout arithmetic, no bank conflicts), and the stage
+// goes to the tensor core.  Row r = t S + sl of a tile holds piece sl of frame t: D = X X^T then carries the Gram of slice
+// sl in the entries (t S + sl, t' S + sl), which the drain picks out of the TMEM columns.
+// (2-D boxes of [TP frames][32 floats], which give slice-major rows, are request-rate bound at 4.07 TB/s with loads alone: the
+// TMA unit fetches every 128-byte box row separately; in the 3-D box the S pieces of a frame are one contiguous run.  A raw
+// landing ring with a second, converting copy into the operand layout moves 160 KB per 32 KB stage through the shared-memory
+// port, which the MMAs -- A and B both read from shared memory, 128 B per clock while they run -- share: 72 / 605 us against
+// 60 / 415 us for this form and 66.5 / 581 us for the register-fed kernel at 1024^2 x 32 / 2048^2 x 64.)
+// ------------------------------------------------------------------------------------------------
+constexpr int CQ_TILES = 2;                        // K-tiles per stage: 32 KB
+constexpr int CQ_STAGE = CQ_TILES * CT_TILE;
+constexpr int CQ_NST = 6;                          // ring stages: 192 KB, up to 4 in flight beside the one being rounded and the one in the MMAs
+constexpr size_t CQ_SMEM = 1024 + (size_t)CQ_NST * CQ_STAGE + 256;
+
+__device__ __forceinline__ void tma_3d_g2s(void* dst_smem, const CUtensorMap* tm, int c0, int c1, int c2, uint64_t* bar) {
+    asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
+                 ::"r"(smem_u32(dst_smem)), "l"(tm), "r"(c0), "r"(c1), "r"(c2), "r"(smem_u32(bar)) : "memory");
+}
+
+template <int TP>
+__global__ void __launch_bounds__(CT_THREADS, 1)
+k_cov_tf32_tma(const __grid_constant__ CUtensorMap tmH, float2* __restrict__ partials, long long npix, int T, int T8, int drain_every) {
+    constexpr int S = 128 / TP;                       // pieces (K-slices) of a frame in the 128 rows of a tile
+    constexpr int FPF = CQ_TILES * S * 32;            // floats of one frame per stage
+    constexpr int PIX = FPF / 2;                      // pixels per stage
+    extern __shared__ unsigned char smraw_[];
+    const uint32_t s0 = smem_u32(smraw_);
+    const uint32_t pad = (1024u - (s0 & 1023u)) & 1023u;
+    unsigned char* base = smraw_ + pad;               // 1024-byte aligned stages
+    const uint32_t sbase = s0 + pad;
+    uint64_t* full = reinterpret_cast<uint64_t*>(base + (size_t)CQ_NST * CQ_STAGE);
+    uint64_t* mma_done = full + CQ_NST;
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(mma_done + CQ_NST);
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+
+    if (tid == 0) {
+        for (int i = 0; i < CQ_NST; ++i) { mbar_init(full + i, 1); mbar_init(mma_done + i, 1); }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    if (warp == 0) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(tmem_slot)), "r"(256) : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    }
+    pdl_wait();                                       // the holograms are complete (programmatic dependent launch)
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+    const uint32_t tmem = *tmem_slot;
+    const uint32_t idesc = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(128 >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);
+    const long long nblocks = npix / PIX;
+    const long long first = blockIdx.x, step = gridDim.x;
+    const long long niter = first < nblocks ? (nblocks - first + step - 1) / step : 0;
+
+    // producer (thread 0): block `it` of this CTA -> stage it % NST: one box [TP frames][S pieces][32 floats] per K-tile
+    auto issue = [&](long long it) {
+        const int s = (int)(it % CQ_NST);
+        const long long p0 = (first + it * step) * (CQ_TILES * S);  // first 32-float piece of the block inside a frame
+        mbar_arrive_expect_tx(full + s, (uint32_t)CQ_STAGE);        // (zero-filled rows count as transferred bytes)
+#pragma unroll
+        for (int kt = 0; kt < CQ_TILES; ++kt)
+            tma_3d_g2s(base + (size_t)s * CQ_STAGE + (size_t)kt * CT_TILE, &tmH, 0, (int)(p0 + kt * S), 0, full + s);
+    };
+    if (tid == 0)
+        for (long long it = 0; it < niter && it < CQ_NST; ++it) issue(it);
+
+    // FP64 accumulators: thread (row r = t S + sl, column half h) adds D[r][t' S + sl] for t' in [h TP/2, (h + 1) TP/2)
+    constexpr int NACC = TP / 2;
+    double acc[NACC];
+#pragma unroll
+    for (int i = 0; i < NACC; ++i) acc[i] = 0.0;
+    const int drow = 32 * (warp & 3) + lane;
+    const int dsl = drow % S, dh = warp >> 2;
+    auto drain = [&](int buf) {
+        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+#pragma unroll
+        for (int q = 0; q < 64 / 16; ++q) {            // the thread's half of the 128 columns, 16 at a time; it keeps the columns c = t' S + sl
+            float v[16];
+            tmem_ld16f(tmem + ((uint32_t)(32 * (warp & 3)) << 16) + (uint32_t)(buf * 128 + dh * 64 + 16 * q), v);
+#pragma unroll
+            for (int g = 0; g < 16 / S; ++g) {         // group g of S consecutive columns = one t'
+                float x = v[g * S];
+#pragma unroll
+                for (int j = 1; j < S; ++j) x = dsl == j ? v[g * S + j] : x;
+                acc[q * (16 / S) + g] += (double)x;
+            }
+        }
+        asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    };
+
+    int dbuf = 0, in_buf = 0;
+    for (long long it = 0; it < niter; ++it) {
+        const int s = (int)(it % CQ_NST);
+        const uint32_t par = (uint32_t)((it / CQ_NST) & 1);
+        mbar_wait(full + s, par);                                   // the stage has landed
+        float4* st4 = reinterpret_cast<float4*>(base + (size_t)s * CQ_STAGE);
+#pragma unroll
+        for (int i = 0; i < CQ_STAGE / 16 / CT_THREADS; ++i) {      // round to nearest TF32, in place
+            float4 x = st4[tid + i * CT_THREADS];
+            x = make_float4(to_tf32(x.x), to_tf32(x.y), to_tf32(x.z), to_tf32(x.w));
+            st4[tid + i * CT_THREADS] = x;
+        }
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");     // the tensor core reads the tile through the async proxy
+        asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+        __syncthreads();
+        if (tid == 0) {
+            asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+            const uint32_t sa0 = sbase + (uint32_t)s * CQ_STAGE;
+            const uint32_t dst = tmem + (uint32_t)(dbuf * 128);
+#pragma unroll
+            for (int kt = 0; kt < CQ_TILES; ++kt)
+#pragma unroll
+                for (int k = 0; k < 4; ++k) {
+                    const uint64_t dhh = ct_sdesc(sa0 + (uint32_t)kt * CT_TILE + (uint32_t)k * 32u);
+                    umma_tf32(dst, dhh, dhh, idesc, (in_buf | kt | k) ? 1u : 0u);
+                }
+            ct_commit(mma_done + s);
+            // refill the stage of the PREVIOUS iteration: its MMAs were issued a whole iteration ago
+            if (it >= 1 && it - 1 + CQ_NST < niter) {
+                const int sp = (int)((it - 1) % CQ_NST);
+                mbar_wait(mma_done + sp, (uint32_t)(((it - 1) / CQ_NST) & 1));
+                issue(it - 1 + CQ_NST);
+            }
+        }
+        if (++in_buf == drain_every) {
+            mbar_wait(mma_done + s, par);                           // the last MMAs into buffer dbuf (the next stage's go to the other one)
+            drain(dbuf);
+            dbuf ^= 1; in_buf = 0;
+            __syncthreads();
+        }
+    }
+    if (in_buf) {
+        const long long it = niter - 1;
+        mbar_wait(mma_done + (int)(it % CQ_NST), (uint32_t)((it / CQ_NST) & 1));   // commits complete in order: all MMAs are done
+        drain(dbuf);
+    }
+    __syncthreads();
+    // combine the S slices (fixed order) through shared memory: red[r = t S + sl][t'] and write this CTA's partial
+    double* red = reinterpret_cast<double*>(base);           // [128 rows][TP] doubles (every stage has been consumed)
+#pragma unroll
+    for (int i = 0; i < NACC; ++i) red[(size_t)drow * TP + dh * NACC + i] = acc[i];
+    __syncthreads();
+    float2* out = partials + (size_t)blockIdx.x * T8 * T8;
+    for (int e = tid; e < T * T; e += CT_THREADS) {
+        const int t = e / T, s2 = e - t * T;
+        double v = 0.0;
+#pragma unroll
+        for (int sl = 0; sl < S; ++sl) v += red[(size_t)(t * S + sl) * TP + s2];
+        out[t * T8 + s2] = make_float2((float)v, 0.f);
+    }
+    __syncthreads();
+    if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "r"(256) : "memory");
+}
+
 template <int TP, bool SPLIT>
 int launch_tf32(holo_ctx* c, const float2* H, cudaStream_t st, int* nparts) {
     constexpr int TILES = SPLIT ? 2 : 4;
@@ -220,6 +378,50 @@ int launch_tf32(holo_ctx* c, const float2* H, cudaStream_t st, int* nparts) {
     return HOLO_OK;
 }
 
+// H viewed as a 3-D float tensor [2 npix / 32 pieces][T frames][32 floats] (dimension 0 = the 32 floats = 128 bytes of a piece,
+// dimension 1 = the pieces of a frame, 128 bytes apart, dimension 2 = the frames); box = [TP frames][S pieces][32 floats], written
+// with the 128-byte swizzle of the K-major operand layout; frames >= T are zero-filled
+static int make_swizzled_map(CUtensorMap* tm, const float2* H, long long npix, int T, int TP) {
+    static EncodeTiledFn encode = nullptr;
+    if (!encode) {
+        void* fn = nullptr;
+        cudaDriverEntryPointQueryResult qres;
+        HOLO_CUDA_OK(cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres));
+        if (!fn || qres != cudaDriverEntryPointSuccess) { holo_set_error("cuTensorMapEncodeTiled not available"); return HOLO_ERR_CUDA; }
+        encode = (EncodeTiledFn)fn;
+    }
+    const cuuint64_t gdim[3] = {32, (cuuint64_t)(2 * npix / 32), (cuuint64_t)T};
+    const cuuint64_t gstr[2] = {128, (cuuint64_t)npix * sizeof(float2)};
+    const cuuint32_t box[3] = {32, (cuuint32_t)(128 / TP), (cuuint32_t)TP};
+    const cuuint32_t estr[3] = {1, 1, 1};
+    const CUresult r = encode(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, const_cast<float2*>(H), gdim, gstr, box, estr,
+                              CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                              CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) { holo_set_error("cuTensorMapEncodeTiled (swizzled) failed (%d)", (int)r); return HOLO_ERR_CUDA; }
+    return HOLO_OK;
+}
+
+template <int TP>
+int launch_tf32_tma(holo_ctx* c, const float2* H, cudaStream_t st, int* nparts) {
+    constexpr int PIX = CQ_TILES * (128 / TP) * 32 / 2;
+    auto kern = k_cov_tf32_tma<TP>;
+    { const int rc = holo_ensure_smem_attr((const void*)kern, c->device, CQ_SMEM); if (rc) return rc; }
+    alignas(64) CUtensorMap tmH;
+    { const int rc = make_swizzled_map(&tmH, H, c->npix, c->T, TP); if (rc) return rc; }
+    const long long nblocks = c->npix / PIX;
+    int grid = c->cov_grid_cap > 0 ? c->cov_grid_cap : c->num_sms;
+    if (grid > c->cov_parts_cap) grid = c->cov_parts_cap;
+    if ((long long)grid > nblocks) grid = (int)nblocks;
+    int de = c->tune[HOLO_TUNE_COV_TF32_DRAIN];
+    if (de < 1) de = 4;
+    de *= 2;                                           // the key counts stages of four K-tiles; these stages hold two
+    const int T8 = (c->T + 7) / 8 * 8;
+    HoloProf prof(c, HOLO_K_COV_PARTIAL, st);
+    HOLO_CUDA_OK(holo_launch_pdl(kern, dim3(grid), dim3(CT_THREADS), CQ_SMEM, st, tmH, c->cov_partials, c->npix, c->T, T8, de));
+    *nparts = grid;
+    return HOLO_OK;
+}
+
 }  // namespace
 
 // Re C partials of the hologram stack on the tensor cores (tune key 13: 1 = TF32 with round-to-nearest conversion, 3 = 3 x TF32)
@@ -227,7 +429,8 @@ int holo_launch_cov_tf32(holo_ctx* c, const float2* H, float2* C, cudaStream_t s
     const bool split = c->tune[HOLO_TUNE_COV_TF32] == 3;
     if (c->npix % 256 != 0) { holo_set_error("the tensor-core Gram needs nx*ny to be a multiple of 256"); return HOLO_ERR_ARG; }
     int nparts = 0, rc;
-    if (c->T <= 32) rc = split ? launch_tf32<32, true>(c, H, st, &nparts) : launch_tf32<32, false>(c, H, st, &nparts);
+    if (!split && c->tune[HOLO_TUNE_COV_TF32_TMA]) rc = c->T <= 32 ? launch_tf32_tma<32>(c, H, st, &nparts) : launch_tf32_tma<64>(c, H, st, &nparts);
+    else if (c->T <= 32) rc = split ? launch_tf32<32, true>(c, H, st, &nparts) : launch_tf32<32, false>(c, H, st, &nparts);
     else            rc = split ? launch_tf32<64, true>(c, H, st, &nparts) : launch_tf32<64, false>(c, H, st, &nparts);
     if (rc) return rc;
     c->cov_nparts = nparts;

@@ -156,6 +156,7 @@ static int create_impl(holo_ctx* c) {
     c->tune[HOLO_TUNE_PROJ_TC] = 1;
     c->tune[HOLO_TUNE_COLS2048] = 1;
     c->tune[HOLO_TUNE_TILED_G] = 8;
+    c->tune[HOLO_TUNE_COV_TF32_TMA] = 1;
     c->tune[HOLO_TUNE_PACKED1024] = 1;
     c->tune[HOLO_TUNE_PDL] = holo_pdl_enabled;
     c->tune[HOLO_TUNE_ROWS2] = 1;                // packed two-frame row pass of mode 3 (1024^2, even T): 79 vs 84 us

@@ -7,7 +7,7 @@
 #include "../../include/holo.h"
 
 #define HOLO_MAX_T 64
-#define HOLO_NUM_TUNE 20
+#define HOLO_NUM_TUNE 24
 #define HOLO_NORM_PARTS 1024
 
 // tuning keys (holo_tune); not part of the stable ABI
@@ -31,6 +31,7 @@ enum {
     HOLO_TUNE_ROWS2 = 15,          // mode 3: packed two-frame row pass where supported (1024^2, even T) // stages accumulated in TMEM before the accumulators are added to FP64 (default 4)
     HOLO_TUNE_TILED_G = 17,        // mode 3, 1024 x 1024: the row pass writes its output column tile by column tile (default 1)
     HOLO_TUNE_PACKED1024 = 19,     // 1024 x 1024 Fresnel stage as packed row pass + column pass (default 1; 0 = fused kernel)
+    HOLO_TUNE_COV_TF32_TMA = 20,   // single-pass TF32 covariance fed by TMA (swizzled boxes, in-place rounding; default 1; 0 = register-fed kernel)
     HOLO_TUNE_PDL = 18,            // programmatic dependent launches between the kernels of a chain (process-wide; default 1)
     HOLO_TUNE_COLS2048 = 16,       // mode 3: packed column-energy pass for 2048-point columns (default 1)
     HOLO_TUNE_FFT_LAG = 6,         // frames between the row pass and the column pass in the fused kernel (0 = auto)
