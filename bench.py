@@ -197,7 +197,7 @@ def kernel_name(cls, fused_fft, cov_real, mode, T=32, n=1024, packed=False):
     if mode != 3 and packed:
         return {"sum": "k_frame_sum" if mode == 1 else "k_sum_gram", "fft_rows": f"k_rows2<{n}> (packed row pass of the stack)",
                 "fft_cols": "k_cols_tiled<1024> (column pass from 8-column blocks)" if n == 1024 else "k_cols2048 (packed column pass)",
-                "cov_partial": ("k_cov_tf32" if cov_tc else "k_cov_partial_real") if cov_real else "k_cov_partial",
+                "cov_partial": ("k_cov_tf32_tma" if cov_tc else "k_cov_partial_real") if cov_real else "k_cov_partial",
                 "cov_reduce": "k_cov_reduce" if mode == 1 else "k_gram_reduce_finish", "eig": "k_eig_real" if cov_real else "k_eig",
                 "project": "k_project_deflate_tma / k_project"}[cls]
     if mode == 3:
@@ -205,7 +205,7 @@ def kernel_name(cls, fused_fft, cov_real, mode, T=32, n=1024, packed=False):
         return {"sum": "k_sum_gram + k_deflate_images", "fft_rows": rows, "fft_cols": "k_col_energy",
                 "cov_reduce": "k_gram_reduce_finish", "eig": "k_eig_real", "project": "k_sum_partial_images"}[cls]
     return {"sum": "k_frame_sum" if mode == 1 else "k_sum_gram", "fft_rows": "k_fresnel" if fused_fft else "k_fft<rows>",
-            "fft_cols": "k_fft<cols>", "cov_partial": ("k_cov_tf32" if cov_tc else "k_cov_partial_real") if cov_real else "k_cov_partial",
+            "fft_cols": "k_fft<cols>", "cov_partial": ("k_cov_tf32_tma" if cov_tc else "k_cov_partial_real") if cov_real else "k_cov_partial",
             "cov_reduce": "k_cov_reduce" if mode == 1 else "k_gram_reduce_finish", "eig": "k_eig_real" if cov_real else "k_eig",
             "project": "k_project_deflate_tma / k_project"}[cls]
 
