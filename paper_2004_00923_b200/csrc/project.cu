@@ -159,8 +159,11 @@ __global__ void __launch_bounds__(256) k_project_deflate(const ProjArgs a, int n
 // free: 32 consecutive float2).  Bound by HBM; measured 4.7 -> see profiles/ TB/s.
 // PROJ_P pixels per stage (256 up to T = 32, 128 above so that >= 2 stages fit); PROJ_P / 32 consumer warps
 #define PROJ_MAX_STAGES 8
-template <int TMAX, int PROJ_P>
-__global__ void __launch_bounds__(PROJ_P, 1)
+// HS = 2 (T > 32): TWO lanes per pixel, lanes l and l + 16 of a warp hold frames [0, TMAX/2) and [TMAX/2, TMAX) of pixel l & 15;
+// the partial projections, means and energies are combined by one butterfly shuffle.  Twice the warps per stage (a single
+// warp per scheduler at 255 registers was latency bound: 507 us at 2048^2 x 64) at half the registers.
+template <int TMAX, int PROJ_P, int HS>
+__global__ void __launch_bounds__(PROJ_P * HS, 1)
 k_project_deflate_tma(const __grid_constant__ CUtensorMap tmH, const ProjArgs a, int nc, int nstages, int rb0, int nrb) {
     extern __shared__ __align__(128) unsigned char smraw[];
     uint64_t* full = reinterpret_cast<uint64_t*>(smraw);
@@ -178,7 +181,7 @@ k_project_deflate_tma(const __grid_constant__ CUtensorMap tmH, const ProjArgs a,
         Vd[i] = t < a.T ? a.V[t * a.T + col] : make_float2(0.f, 0.f);
     }
     if (tid == 0) {
-        for (int s = 0; s < nstages; ++s) { mbar_init(full + s, 1); mbar_init(empty + s, PROJ_P / 32); }
+        for (int s = 0; s < nstages; ++s) { mbar_init(full + s, 1); mbar_init(empty + s, PROJ_P * HS / 32); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
@@ -204,34 +207,40 @@ k_project_deflate_tma(const __grid_constant__ CUtensorMap tmH, const ProjArgs a,
     int s = 0; uint32_t ph = 0;
     for (long long chunk = blockIdx.x; chunk < nchunks; chunk += gridDim.x) {
         mbar_wait(full + s, ph);
-        const float2* src = ring + (size_t)s * stage_elems + (warp >> 2) * (TMAX * 128) + (warp & 3) * 32 + lane;
-        float2 h[TMAX];
+        constexpr int TH = TMAX / HS;                     // frames per thread
+        // HS = 1: pixel = 32 warp + lane; HS = 2: pixel = 16 warp + (lane & 15), frames [TH (lane >> 4), + TH)
+        const int pix = HS == 1 ? warp * 32 + lane : warp * 16 + (lane & 15);
+        const int tb = HS == 1 ? 0 : (lane >> 4) * TH;
+        const float2* src = ring + (size_t)s * stage_elems + (pix >> 7) * (TMAX * 128) + (pix & 127) + tb * 128;
+        float2 h[TH];
 #pragma unroll
-        for (int t = 0; t < TMAX; ++t) h[t] = src[t * 128];
+        for (int t = 0; t < TH; ++t) h[t] = src[t * 128];
         __syncwarp();
         if (lane == 0) mbar_arrive(empty + s);           // the stage is in registers: hand it back at once
         if (warp == 0) issue();
         if (a.center) {                                   // rows t >= T are zero (TMA fill): they do not enter the mean
             float2 m = make_float2(0.f, 0.f);
 #pragma unroll
-            for (int t = 0; t < TMAX; ++t) { m.x += h[t].x; m.y += h[t].y; }
+            for (int t = 0; t < TH; ++t) { m.x += h[t].x; m.y += h[t].y; }
+            if constexpr (HS == 2) { m.x += __shfl_xor_sync(0xffffffffu, m.x, 16); m.y += __shfl_xor_sync(0xffffffffu, m.y, 16); }
             const float inv = 1.f / (float)a.T;
             m.x *= inv; m.y *= inv;
 #pragma unroll
-            for (int t = 0; t < TMAX; ++t) if (t < a.T) { h[t].x -= m.x; h[t].y -= m.y; }
+            for (int t = 0; t < TH; ++t) if (tb + t < a.T) { h[t].x -= m.x; h[t].y -= m.y; }
         }
 #pragma unroll 1
         for (int c = 0; c < nc; ++c) {
-            const float2* v = Vd + c * TMAX;
+            const float2* v = Vd + c * TMAX + tb;
             float2 P = make_float2(0.f, 0.f);
 #pragma unroll
-            for (int t = 0; t < TMAX; ++t) {                      // P += h_t * v_t
+            for (int t = 0; t < TH; ++t) {                        // P += h_t * v_t
                 const float2 w = v[t];
                 P.x = fmaf(h[t].x, w.x, fmaf(-h[t].y, w.y, P.x));
                 P.y = fmaf(h[t].x, w.y, fmaf(h[t].y, w.x, P.y));
             }
+            if constexpr (HS == 2) { P.x += __shfl_xor_sync(0xffffffffu, P.x, 16); P.y += __shfl_xor_sync(0xffffffffu, P.y, 16); }
 #pragma unroll
-            for (int t = 0; t < TMAX; ++t) {                      // h_t -= P * conj(v_t)
+            for (int t = 0; t < TH; ++t) {                        // h_t -= P * conj(v_t)
                 const float2 w = v[t];
                 h[t].x = fmaf(-P.x, w.x, fmaf(-P.y, w.y, h[t].x));
                 h[t].y = fmaf(-P.y, w.x, fmaf(P.x, w.y, h[t].y));
@@ -239,14 +248,16 @@ k_project_deflate_tma(const __grid_constant__ CUtensorMap tmH, const ProjArgs a,
         }
         float sum = 0.f;
 #pragma unroll
-        for (int t = 0; t < TMAX; ++t) sum = fmaf(h[t].x, h[t].x, fmaf(h[t].y, h[t].y, sum));
-        a.M[chunk * PROJ_P + warp * 32 + lane] = sum;
+        for (int t = 0; t < TH; ++t) sum = fmaf(h[t].x, h[t].x, fmaf(h[t].y, h[t].y, sum));
+        if constexpr (HS == 2) sum += __shfl_xor_sync(0xffffffffu, sum, 16);
+        if (HS == 1 || lane < 16) a.M[chunk * PROJ_P + pix] = sum;
         if (++s == nstages) { s = 0; ph ^= 1u; }
     }
 }
 
 template <int TMAX> static int launch_deflate(holo_ctx* c, const ProjArgs& a, int nc, cudaStream_t st) {
     constexpr int PROJ_P = TMAX <= 32 ? 256 : 128;
+    constexpr int HS = TMAX <= 32 ? 1 : 2;             // lanes per pixel (T > 32: the frames of a pixel are split over two lanes)
     const int vbytes = ((nc > 0 ? nc : 1) * TMAX * (int)sizeof(float2) + 127) & ~127;
     const size_t stage_bytes = (size_t)TMAX * PROJ_P * sizeof(float2);
     int nstages = (int)((200 * 1024 - vbytes) / stage_bytes);
@@ -256,14 +267,14 @@ template <int TMAX> static int launch_deflate(holo_ctx* c, const ProjArgs& a, in
     }
     if (c->tune[HOLO_TUNE_PROJ_TMA] && nstages >= 2 && a.npix % PROJ_P == 0) {
         const size_t smem = 128 + vbytes + (size_t)nstages * stage_bytes;
-        { const int rc = holo_ensure_smem_attr((const void*)k_project_deflate_tma<TMAX, PROJ_P>, c->device, 200 * 1024 + 128); if (rc) return rc; }
+        { const int rc = holo_ensure_smem_attr((const void*)k_project_deflate_tma<TMAX, PROJ_P, HS>, c->device, 200 * 1024 + 128); if (rc) return rc; }
         alignas(64) CUtensorMap tmH;
         { const int rc = holo_make_tensor_map(&tmH, a.H, a.npix, c->ring_nrb ? 8 * c->ring_nrb : a.T, 128); if (rc) return rc; }
         const long long nchunks = a.npix / PROJ_P;
         const int cap = c->proj_grid_cap > 0 ? c->proj_grid_cap : c->num_sms;
         const int grid = (int)(nchunks < cap ? nchunks : cap);
         HoloProf prof(c, HOLO_K_PROJECT, st);
-        k_project_deflate_tma<TMAX, PROJ_P><<<grid, PROJ_P, smem, st>>>(tmH, a, nc, nstages, c->ring_rb0, c->ring_nrb);
+        k_project_deflate_tma<TMAX, PROJ_P, HS><<<grid, PROJ_P * HS, smem, st>>>(tmH, a, nc, nstages, c->ring_rb0, c->ring_nrb);
         HOLO_CUDA_OK(cudaGetLastError());
         return HOLO_OK;
     }
