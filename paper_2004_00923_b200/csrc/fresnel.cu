@@ -12,6 +12,8 @@
 // ------------------------------------------------------------------------------------------------
 // A0: per-pixel temporal sum  S(p) = sum_t I_t(p)   (uint32: exact, T*65535 < 2^32)
 // ------------------------------------------------------------------------------------------------
+// Batches of SUM_U frames are loaded into registers before any of them is added: left to itself the compiler keeps two loads
+// in flight per thread (16 round trips to DRAM at T = 32): 17.9 -> 13.4 us at 512 x 512 x 32, 20.0 -> 17.3 us at 1024 x 1024 x 32.
 __global__ void __launch_bounds__(256) k_frame_sum(const uint16_t* __restrict__ frames, uint32_t* __restrict__ sum,
                                                    long long npix, int T, unsigned int* __restrict__ counters) {
     pdl_trigger();                                        // (the Fresnel kernel may become resident while this one drains)
@@ -22,14 +24,22 @@ __global__ void __launch_bounds__(256) k_frame_sum(const uint16_t* __restrict__ 
     for (; v < nvec; v += (long long)gridDim.x * blockDim.x) {
         uint32_t s[8] = {0, 0, 0, 0, 0, 0, 0, 0};
         const uint4* src = reinterpret_cast<const uint4*>(frames) + v;
-#pragma unroll 8
-        for (int t = 0; t < T; ++t) {
-            uint4 w = __ldg(src + (long long)t * nvec);
+        auto add = [&](const uint4& w) {
             s[0] += w.x & 0xffffu; s[1] += w.x >> 16;
             s[2] += w.y & 0xffffu; s[3] += w.y >> 16;
             s[4] += w.z & 0xffffu; s[5] += w.z >> 16;
             s[6] += w.w & 0xffffu; s[7] += w.w >> 16;
+        };
+        constexpr int SUM_U = 16;
+        int t = 0;
+        for (; t + SUM_U <= T; t += SUM_U) {
+            uint4 w[SUM_U];
+#pragma unroll
+            for (int j = 0; j < SUM_U; ++j) w[j] = __ldg(src + (long long)(t + j) * nvec);
+#pragma unroll
+            for (int j = 0; j < SUM_U; ++j) add(w[j]);
         }
+        for (; t < T; ++t) add(__ldg(src + (long long)t * nvec));
         uint4* dst = reinterpret_cast<uint4*>(sum) + 2 * v;
         dst[0] = make_uint4(s[0], s[1], s[2], s[3]);
         dst[1] = make_uint4(s[4], s[5], s[6], s[7]);
@@ -416,9 +426,7 @@ __global__ void __launch_bounds__(256) k_deflate_images(const uint16_t* __restri
 #pragma unroll
             for (int x = 0; x < 8; ++x) e[kk][x] = 0.f;
         const uint4* src = reinterpret_cast<const uint4*>(frames) + q;
-#pragma unroll 8
-        for (int t = 0; t < T; ++t) {
-            const uint4 w = __ldg(src + (long long)t * nvec);
+        auto accumulate = [&](const uint4& w, int t) {
             const uint32_t ws[4] = {w.x, w.y, w.z, w.w};
             float d[8];
 #pragma unroll
@@ -432,7 +440,18 @@ __global__ void __launch_bounds__(256) k_deflate_images(const uint16_t* __restri
 #pragma unroll
                 for (int x = 0; x < 8; ++x) e[kk][x] = fmaf(d[x], v, e[kk][x]);
             }
+        };
+        // batches of DEFL_U frames in registers before the arithmetic (as k_frame_sum: the loads of a batch are all in flight)
+        constexpr int DEFL_U = 16;
+        int t = 0;
+        for (; t + DEFL_U <= T; t += DEFL_U) {
+            uint4 w[DEFL_U];
+#pragma unroll
+            for (int j = 0; j < DEFL_U; ++j) w[j] = __ldg(src + (long long)(t + j) * nvec);
+#pragma unroll
+            for (int j = 0; j < DEFL_U; ++j) accumulate(w[j], t + j);
         }
+        for (; t < T; ++t) accumulate(__ldg(src + (long long)t * nvec), t);
 #pragma unroll
         for (int kk = 0; kk < NDEFL; ++kk) {
             float4* dst = reinterpret_cast<float4*>(img + (long long)kk * npix) + 2 * q;
