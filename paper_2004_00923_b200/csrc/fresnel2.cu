@@ -221,12 +221,19 @@ __global__ void __launch_bounds__(R2_WARPS * 32, 1) k_rows2(const R2Args a) {
         unsigned int tk2 = 0u;
         if (lane == 0) tk2 = atomicAdd(a.ticket, 1u);
         if (tk1 < ntasks) {
-            const int f1 = (NX == 1024 ? 2 : 1) * (int)(tk1 / (unsigned int)a.ny), y1 = (int)(tk1 % (unsigned int)a.ny);
+            const int f1 = NX == 1024 ? 2 * (int)(tk1 / (unsigned int)a.ny) : (int)(tk1 % (unsigned int)a.nframes);
+            const int y1 = NX == 1024 ? (int)(tk1 % (unsigned int)a.ny) : (int)(tk1 / (unsigned int)a.nframes);
             const uint16_t* pf = NX == 1024 ? a.frames + (long long)(f1 + (lane >> 4)) * npix + (long long)y1 * NX + (lane & 15) * 64
                                             : a.frames + (long long)f1 * npix + (long long)y1 * NX + lane * 64;
             asm volatile("prefetch.global.L2 [%0];" ::"l"(pf));
         }
-        const int f = (NX == 1024 ? 2 : 1) * (int)(tk / (unsigned int)a.ny), y = (int)(tk % (unsigned int)a.ny);
+        // task order.  NX = 1024: row-minor (consecutive tickets = consecutive rows of a frame pair: the frames are written one after
+        // the other and the column pass finds the last ones in L2).  NX = 2048: FRAME-minor (consecutive tickets = the same row of
+        // consecutive frames): the twelve warps of a CTA then share the row of S and of the deflation images through L1 instead
+        // of fetching 8 + 8 n_rej KB per task from L2 (mode 3 at 2048^2 x 64: row pass 965 -> 686 us; mode 1: 622 -> 580 us; at
+        // 1024 points the same order measured 1 - 2 us slower in both passes)
+        const int f = NX == 1024 ? 2 * (int)(tk / (unsigned int)a.ny) : (int)(tk % (unsigned int)a.nframes);
+        const int y = NX == 1024 ? (int)(tk % (unsigned int)a.ny) : (int)(tk / (unsigned int)a.nframes);
         const uint16_t* Ia = a.frames + (long long)f * npix + (long long)y * NX + lane;
         const uint32_t* Sp = a.sum + (long long)y * NX + lane;
         const float2 qyv = __ldg(a.qy + y);
